@@ -1,0 +1,223 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU).
+
+The paper prints no worked numerical example, so the oracle is pinned by:
+  F   Fock-space brute force of Eq. 2/7/13-15 on micro inputs (tests/fock_bruteforce.py:
+      no determinants, no inverses, no Wick's theorem)
+  P10 Eq. 2 == Eq. 3 + Eq. 4 as operators (fixes the index reading A2/A3)
+  P1  reference ratio / 1-determinant overlap = det * det (Eq. 13)
+  P2  single-determinant trial -> SD-AFQMC closed form (closed shell)
+  P4  gauge invariance psi -> psi A
+  P5  tr G = n, idempotency of single-determinant G
+  P6  O0 == O1 == O2
+  P7  walker = reference determinant: ovlp = c_0, Hartree-Fock closed form
+  P9  variational energy c^T H c / c^T c from local energies at basis determinants
+  P11 determinant-order invariance, linearity in c
+"""
+import numpy as np
+import pytest
+
+import msd_inputs as mi
+from fock_bruteforce import Fock, brute_force
+from oracle import msd_oracle as mo
+from oracle import o2
+
+
+def _args(x, sl=None):
+    pa, pb = (x.phi_a, x.phi_b) if sl is None else (x.phi_a[sl], x.phi_b[sl])
+    return (x.h1, x.L, x.e0, x.occa, x.occb, x.ci, pa, pb)
+
+
+@pytest.mark.parametrize("name", ["micro", "micro-cs"])
+def test_fock_bruteforce_pins_all_tiers(name):
+    x = mi.generate(name)
+    tiers = {"o0": mo.o0_pure_determinants(*_args(x)), "o1": mo.o1_definition(*_args(x)), "o2": o2.o2(*_args(x))}
+    for w in range(x.n_w):
+        bf = brute_force(x.h1, x.L, x.e0, x.occa, x.occb, x.ci, x.phi_a[w], x.phi_b[w])
+        for t, o in tiers.items():
+            assert abs(o["ovlp"][w] - bf["ovlp"]) <= 1e-13 * abs(bf["ovlp"]), t
+            assert np.abs(o["G"][w] - bf["G"]).max() < 1e-12, t
+            assert np.abs(o["fb"][w] - bf["fb"]).max() < 1e-12, t
+            assert np.abs(o["E"][w] - bf["E"]).max() < 1e-11, t
+
+
+def test_eq2_equals_eq3_plus_eq4():
+    """P10: H of Eq. 2 with (ps|qr) = sum_g L_ps L_qr equals Eq. 3 with h' of Eq. 4."""
+    x = mi.generate("micro")
+    for w in range(x.n_w):
+        a = brute_force(*_args(x)[:6], x.phi_a[w], x.phi_b[w], hamiltonian="eq2")
+        b = brute_force(*_args(x)[:6], x.phi_a[w], x.phi_b[w], hamiltonian="eq3")
+        assert abs(a["E"][0] - b["E"][0]) < 1e-12
+
+
+def test_single_determinant_overlap_and_reference_ratio():
+    """P1: a 1-determinant trial gives det(psi_a[occ0]) det(psi_b[occ0]) (Eq. 13)."""
+    x = mi.generate("tiny").subset_dets([0])
+    x.ci[:] = 1.0
+    r = o2.run(x, want=("ovlp",))
+    for w in range(x.n_w):
+        ref = np.linalg.det(x.phi_a[w][:2, :]) * np.linalg.det(x.phi_b[w][:2, :])
+        assert abs(r["ovlp"][w] - ref) < 1e-15
+
+
+def test_single_determinant_closed_shell_closed_form():
+    """P2: SD-AFQMC closed-shell expression with Eq. 14's G (alpha = beta walker)."""
+    x = mi.generate("small").subset_dets([0])
+    x.ci[:] = 1.0
+    pa = x.phi_a[:3]
+    x = x.with_walkers(pa, pa.copy())
+    r = o2.run(x)
+    n = x.n_alpha
+    for w in range(3):
+        psi = pa[w]
+        theta = psi @ np.linalg.inv(psi[:n, :])
+        G = np.zeros((x.N, x.N), complex)
+        G[:n, :] = theta.T                                     # G[p][q] = <a+_p a_q>
+        X = np.einsum("gpq,pq->g", x.L, 2 * G)
+        ex = np.einsum("gpq,grs,ps,rq->g", x.L, x.L, G, G, optimize=True)
+        E = 2 * np.sum(x.h1 * G) + 0.5 * np.sum(X * X - 2 * ex)
+        assert abs(r["E"][w, 0] - (x.e0 + E)) < 1e-11
+        assert np.abs(r["fb"][w] - X).max() < 1e-12
+        assert np.abs(r["G"][w, 0] - G).max() < 1e-12
+
+
+def test_gauge_invariance():
+    """P4: psi -> psi A multiplies ovlp by det A_a det A_b and leaves G, fb, E unchanged."""
+    x = mi.generate("tiny")
+    rng = np.random.default_rng(11)
+    Aa = rng.standard_normal((2, 2)) + 1j * rng.standard_normal((2, 2))
+    Ab = rng.standard_normal((2, 2)) + 1j * rng.standard_normal((2, 2))
+    y = x.with_walkers(x.phi_a @ Aa, x.phi_b @ Ab)
+    for f in (mo.o1_definition, o2.o2):
+        r0, r1 = f(*_args(x)), f(*_args(y))
+        fac = np.linalg.det(Aa) * np.linalg.det(Ab)
+        assert np.abs(r1["ovlp"] - fac * r0["ovlp"]).max() < 1e-13
+        assert np.abs(r1["G"] - r0["G"]).max() < 1e-11
+        assert np.abs(r1["fb"] - r0["fb"]).max() < 1e-11
+        assert np.abs(r1["E"] - r0["E"]).max() < 1e-10
+
+
+def test_trace_and_idempotency():
+    """P5: tr G^s = n_s for the MSD Green's function; G_I G_I = G_I for each single determinant."""
+    x = mi.generate("open-shell")
+    r = o2.run(x)
+    tr = np.einsum("wspp->ws", r["G"])
+    assert np.abs(tr[:, 0] - x.n_alpha).max() < 1e-11 and np.abs(tr[:, 1] - x.n_beta).max() < 1e-11
+    d, G = mo.sd_overlap_and_greens(x.phi_a[0], x.occa[7])
+    # G[p][q] = Theta[q,l] on rows occ: as a matrix in (p,q) it is the transpose of the projector
+    assert np.abs(G.T @ G.T - G.T).max() < 1e-12
+
+
+@pytest.mark.parametrize("name", ["tiny", "open-shell"])
+def test_tiers_agree(name):
+    """P6: O0 (determinants only) == O1 (dense G) == O2 (C, non-zero rows)."""
+    x = mi.generate(name)
+    sl = slice(0, 3)
+    a = mo.o1_definition(*_args(x, sl))
+    b = o2.o2(*_args(x, sl))
+    for k in ("ovlp", "G", "fb", "E"):
+        assert np.abs(a[k] - b[k]).max() < 1e-11, k
+    if name == "tiny":
+        c = mo.o0_pure_determinants(*_args(x, slice(0, 2)))
+        for k in ("ovlp", "G", "fb", "E"):
+            assert np.abs(a[k][:2] - c[k]).max() < 1e-11, k
+
+
+def test_o2_matches_o1_on_small_one_walker():
+    x = mi.generate("small")
+    a = mo.o1_definition(*_args(x, slice(5, 6)))
+    b = o2.o2(*_args(x, slice(5, 6)))
+    assert abs(a["ovlp"][0] - b["ovlp"][0]) < 1e-12 * abs(a["ovlp"][0])
+    assert np.abs(a["fb"] - b["fb"]).max() < 1e-11 and np.abs(a["E"] - b["E"]).max() < 1e-10
+
+
+def _reference_walkers(x, n_w=1):
+    pa = np.zeros((n_w, x.N, x.n_alpha), complex)
+    pb = np.zeros((n_w, x.N, x.n_beta), complex)
+    pa[:, x.occ_ref_a, np.arange(x.n_alpha)] = 1.0
+    pb[:, x.occ_ref_b, np.arange(x.n_beta)] = 1.0
+    return x.with_walkers(pa, pb)
+
+
+def test_walker_equals_reference():
+    """P7: psi = D_0: ovlp = c_0 (other determinants are orthogonal), E from O0 equals the
+    Fock-space <Psi_T|H|D_0>/c_0; for a 1-determinant trial the Hartree-Fock closed form."""
+    x = _reference_walkers(mi.generate("micro-cs"))
+    r = mo.o0_pure_determinants(*_args(x))
+    assert abs(r["ovlp"][0] - x.ci[0]) < 1e-15
+    bf = brute_force(*_args(x)[:6], x.phi_a[0], x.phi_b[0])
+    assert np.abs(r["E"][0] - bf["E"]).max() < 1e-12
+    y = _reference_walkers(mi.generate("small").subset_dets([0]))
+    n = y.n_alpha
+    h, L = y.h1, y.L
+    hf = 2 * np.trace(h[:n, :n]) + 0.5 * np.sum((2 * np.einsum("gii->g", L[:, :n, :n])) ** 2
+                                                - 2 * np.einsum("gij,gji->g", L[:, :n, :n], L[:, :n, :n]))
+    r = o2.run(y)
+    assert abs(r["E"][0, 0] - hf) < 1e-11
+    assert abs(r["ovlp"][0] - y.ci[0]) < 1e-15
+
+
+def test_variational_energy_from_local_energies():
+    """P9: E_var = c^T H c / c^T c with H built operator-by-operator in Fock space equals
+    sum_J c_J [ovlp_J E_L(D_J)] / sum_J c_J^2, the local energies taken at the basis determinants
+    (O0: the only tier that survives singular O_I)."""
+    x = mi.generate("micro-cs")
+    # exact H in the trial's determinant basis from the brute force: H_IJ = <D_I|H|D_J>
+    nd = x.n_det
+    num = 0.0
+    for J in range(nd):
+        pa = np.zeros((1, x.N, x.n_alpha), complex)
+        pb = np.zeros((1, x.N, x.n_beta), complex)
+        pa[0, x.occa[J], np.arange(x.n_alpha)] = 1.0
+        pb[0, x.occb[J], np.arange(x.n_beta)] = 1.0
+        r = mo.o0_pure_determinants(x.h1, x.L, x.e0, x.occa, x.occb, x.ci, pa, pb)
+        assert abs(r["ovlp"][0] - x.ci[J]) < 1e-14
+        num += x.ci[J] * r["ovlp"][0] * r["E"][0, 0]
+    evar = num / np.sum(x.ci ** 2)
+    # independent: apply H to the trial vector in Fock space
+    F = Fock(x.N)
+    T = F.trial(x.ci, x.occa, x.occb)
+    eri = np.einsum("gps,gqr->psqr", x.L, x.L)
+    HT = np.zeros_like(T)
+    for s in range(2):
+        for p in range(x.N):
+            for q in range(x.N):
+                HT += x.h1[p, q] * F.create(F.so(p, s), F.annihilate(F.so(q, s), T))
+    for s in range(2):
+        for t in range(2):
+            for p in range(x.N):
+                for q in range(x.N):
+                    for r_ in range(x.N):
+                        for ss in range(x.N):
+                            v = F.annihilate(F.so(r_, t), F.annihilate(F.so(ss, s), T))
+                            if v.any():
+                                HT += 0.5 * eri[p, ss, q, r_] * F.create(F.so(p, s), F.create(F.so(q, t), v))
+    ref = x.e0 + np.vdot(T, HT) / np.vdot(T, T)
+    assert abs(evar - ref) < 1e-11
+    assert abs(evar.imag) < 1e-12
+
+
+def test_order_invariance_and_linearity():
+    """P11: permuting determinants changes nothing; scaling c scales ovlp only."""
+    x = mi.generate("open-shell")
+    perm = np.random.default_rng(5).permutation(x.n_det)
+    y = x.subset_dets(perm)
+    a, b = o2.run(x), o2.run(y)
+    for k in ("ovlp", "fb", "E"):
+        assert np.abs(a[k] - b[k]).max() < 1e-11 * max(1.0, np.abs(a[k]).max()), k
+    z = x.subset_dets(np.arange(x.n_det))
+    z.ci *= -2.5
+    c = o2.run(z)
+    assert np.abs(c["ovlp"] + 2.5 * a["ovlp"]).max() < 1e-13 * np.abs(a["ovlp"]).max()
+    assert np.abs(c["E"] - a["E"]).max() < 1e-11
+
+
+def test_generator_roundtrip_and_shapes():
+    for name in ("tiny", "small", "open-shell"):
+        x = mi.generate(name)
+        occ = mi.tables_to_occ(x.exc_off_a, x.holes_a, x.parts_a, x.occ_ref_a, x.n_det)
+        assert (occ == x.occa).all()
+        assert len(np.unique(np.concatenate([x.occa, x.occb], axis=1), axis=0)) == x.n_det
+        assert abs(np.sum(x.ci ** 2) - 1.0) < 1e-12
+        assert np.abs(np.einsum("wpi,wpj->wij", x.phi_a.conj(), x.phi_a) - np.eye(x.n_alpha)).max() < 1e-12
+        assert np.abs(x.L - x.L.transpose(0, 2, 1)).max() == 0.0
+    assert mi.generate("tiny").n_det == 36 and mi.generate("tiny-full").n_det == 199
