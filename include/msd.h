@@ -1,0 +1,138 @@
+/* msd.h -- C ABI of the B200-native MSD-AFQMC Wick's-theorem hot path.
+ *
+ * Paper: "GPU-accelerated Auxiliary-field quantum Monte Carlo with multi-Slater determinant
+ * trial states", arXiv 2406.08314 (text at /root/reference/PAPER.md; cited below as PAPER.md:L<line>).
+ *
+ * For a batch of walkers (single Slater determinants) against a multi-Slater-determinant
+ * trial |Psi_T> = sum_I c_I |D_I> (Eq. 15; orthogonal CI expansion only) the library
+ * evaluates, by the generalized Wick's theorem:
+ *     the overlap <Psi_T|psi_w>                                              (Eq. 13 + Eq. 15)
+ *     the mixed Green's function G^s_pq = <Psi_T|a+_p a_q|psi_w>/<Psi_T|psi_w>   (Eq. 14 generalised)
+ *     the force bias v_g = sum_s sum_pq L^g_pq G^s_pq                            (Eq. 7 without -sqrt(dtau))
+ *     the local (mixed) energy E = e0 + <Psi_T|H|psi_w>/<Psi_T|psi_w>, H of Eq. 2 with
+ *         (pq|rs) = sum_g L^g_pq L^g_rs.
+ *
+ * Conventions:
+ *   - a determinant is the ASCENDING-ordered string of its occupied orbitals, alpha string first;
+ *     <D_I|psi> = det psi_a[occ_I^a,:] * det psi_b[occ_I^b,:].  The caller never supplies phases: the
+ *     library computes the in-place -> sorted permutation parity itself.
+ *   - G[p][q] = <a+_p a_q> = [phi (Psi_T^+ phi)^-1 Psi_T^+]_{qp}.
+ *   - h1 is Eq. 2's h (NOT Eq. 3-4's h'); the two-body term is normal ordered.
+ *   - CI coefficients are real.
+ *
+ * All arithmetic is float64 / complex128.  A complex128 is two consecutive doubles (re, im), i.e. the
+ * memory of a contiguous torch.complex128 / numpy.complex128 array.
+ *
+ * Pointers marked HOST are read during the call and may be freed afterwards; pointers marked DEVICE must
+ * be CUDA device memory on the context's device and stay valid until the work enqueued on `stream`
+ * has completed.  `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ * The three hot calls enqueue kernels on `stream` and return without synchronising the host (the first
+ * call for a larger n_w than seen before allocates workspace with cudaMalloc, which synchronises).
+ *
+ * Errors: every function returning int returns MSD_OK (0) or a negative code; no exceptions cross the
+ * ABI.  msd_last_error() gives a human-readable message for the last failure on that context (or the
+ * last msd_setup failure if ctx is NULL).  Data-dependent singularities are NOT errors: a walker whose
+ * reference overlap matrix is exactly singular (det O0 = 0) or whose W = sum_I c~_I R_I^a R_I^b is exactly
+ * zero gets flags[w] != 0 (MSD_FLAG_*) and NaN outputs; the call still returns MSD_OK.
+ */
+#ifndef MSD_H
+#define MSD_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MSD_OK            0
+#define MSD_EINVAL       -1   /* bad argument or invalid excitation table */
+#define MSD_ENOMEM       -2   /* host or device allocation failed */
+#define MSD_ECUDA        -3   /* a CUDA runtime call or kernel launch failed */
+#define MSD_EUNSUPPORTED -4   /* size outside what the kernels support (see msd_setup) */
+
+#define MSD_FLAG_SINGULAR_REFERENCE 1   /* det psi[occ_ref,:] == 0 for a spin */
+#define MSD_FLAG_ZERO_OVERLAP       2   /* W == 0 */
+
+typedef struct msd_ctx msd_ctx;   /* opaque; owns every device copy made at setup and all workspace */
+
+/* msd_setup: build the trial (PAPER.md:L222-254 inputs h1e, chol, e0, (coeff, occa, occb) in
+ * hole/particle form; S0 "pack" of SURVEY.md 8(a)).  Runs the excitation-table packer kernels
+ * (validate, phases, level sort into contiguous buckets) and packs the rows of L and h1 that the path touches.
+ *   N, n_alpha, n_beta, n_chol, n_det : sizes.  Limits: 1 <= N <= 1024, 0 <= n_s <= 64, n_s <= N,
+ *       n_chol >= 1, n_det >= 1, per-spin excitation level <= 16, active window (distinct hole
+ *       orbitals n_o, distinct particle orbitals n_v per spin) n_o*n_v <= 65535; else MSD_EUNSUPPORTED.
+ *   h1   HOST [N][N] row-major, real symmetric.
+ *   L    HOST [n_chol][N][N], each slice real symmetric.
+ *   e0   constant added to every energy.
+ *   occ_ref_a/b  HOST [n_alpha]/[n_beta], strictly ascending reference occupation.
+ *   exc_off_s HOST [n_det+1] CSR offsets; determinant I has level k = off[I+1]-off[I] in spin s;
+ *   holes_s / parts_s HOST [off[n_det]]: holes are in occ_ref_s, particles are not; distinct within a
+ *       determinant; any order (the a-th smallest hole is paired with the a-th smallest particle).
+ *   ci   HOST [n_det] real coefficients in the ascending-string convention.
+ *   stream: setup work is enqueued there and synchronised before returning.
+ * On success *out is a new context (destroy with msd_destroy).  Invalid tables -> MSD_EINVAL. */
+int msd_setup(msd_ctx** out, int N, int n_alpha, int n_beta, int n_chol, int64_t n_det,
+              const double* h1, const double* L, double e0,
+              const int32_t* occ_ref_a, const int32_t* occ_ref_b,
+              const int64_t* exc_off_a, const int32_t* holes_a, const int32_t* parts_a,
+              const int64_t* exc_off_b, const int32_t* holes_b, const int32_t* parts_b,
+              const double* ci, void* stream);
+
+/* Convenience for the paper's (coeff, occa, occb) format: occa HOST [n_det][n_alpha],
+ * occb HOST [n_det][n_beta] occupation lists (any order inside a row); determinant 0 is the reference. */
+int msd_setup_from_occ(msd_ctx** out, int N, int n_alpha, int n_beta, int n_chol, int64_t n_det,
+                       const double* h1, const double* L, double e0,
+                       const int32_t* occa, const int32_t* occb, const double* ci, void* stream);
+
+/* Walkers: phi_a DEVICE [n_w][N][n_alpha] complex128 row-major, phi_b DEVICE [n_w][N][n_beta]; columns need
+ * not be orthonormal.  flags DEVICE [n_w] int32 or NULL.  n_w >= 0 (0 is a no-op). */
+
+/* ovlp DEVICE [n_w] complex128 = <Psi_T|psi_w>  (S1, S2, S4 of SURVEY.md 8(a)). */
+int msd_overlap(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
+                void* ovlp, int32_t* flags, void* stream);
+
+/* fb DEVICE [n_w][n_chol] complex128 = sum_s sum_pq L^g_pq G^s_pq[w]   (Eq. 7 without -sqrt(dtau); the caller
+ * scales: reading A4).  S1-S6. */
+int msd_force_bias(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
+                   void* fb, int32_t* flags, void* stream);
+
+/* e DEVICE [n_w][3] complex128 = (E, E1, E2): E = e0 + E1 + E2, E1 one-body, E2 two-body.  S1-S9. */
+int msd_local_energy(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
+                     void* e, int32_t* flags, void* stream);
+
+/* G DEVICE [n_w][2][N][N] complex128, G[w][s][p][q] = <a+_p a_q>.  Test hook (S5). */
+int msd_greens(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
+               void* G, int32_t* flags, void* stream);
+
+/* Introspection of the packed trial (host-side copies made at setup; for tests of the packer).
+ * msd_get_info fills: info[0]=n_o_alpha, [1]=n_v_alpha, [2]=n_o_beta, [3]=n_v_beta, [4]=number of level
+ * buckets, [5]=max level alpha, [6]=max level beta, [7]=walker tile width.
+ * msd_get_packed copies, in the packer's sorted order, perm[n_det] (original index of each packed
+ * determinant), coef[n_det] (c_I * phase_a * phase_b), level_a[n_det], level_b[n_det]; any may be NULL. HOST. */
+int msd_get_info(const msd_ctx* ctx, int64_t* info8);
+int msd_get_packed(const msd_ctx* ctx, int64_t* perm, double* coef, int32_t* level_a, int32_t* level_b);
+
+/* Set an upper bound (bytes) on the workspace the hot calls may allocate (default: 70 % of free device
+ * memory at the first call); walkers are processed in chunks that fit. */
+int msd_set_workspace_limit(msd_ctx* ctx, int64_t bytes);
+
+/* Number of kernels the library launched on this context since setup (for bench.py's gpu_launches). */
+int64_t msd_launch_count(const msd_ctx* ctx);
+
+/* Per-phase device timings of the most recent hot call when profiling is enabled with
+ * msd_set_profiling(ctx, 1): fills ms[0..n-1] for phases (reference, dets, greens/fb, dense, vgemm, assemble);
+ * synchronises the stream.  Off by default (no events recorded). */
+int msd_set_profiling(msd_ctx* ctx, int on);
+int msd_get_phase_ms(msd_ctx* ctx, float* ms, int n);
+
+/* Measured FP64 peak of this device (TFLOP/s) from a register-resident DMMA loop run for ~`ms` ms;
+ * used as the roofline denominator by bench.py (MEASURED_PEAKS.json has no FP64 entry). */
+double msd_probe_fp64_tflops(int use_dmma, double ms, void* stream);
+
+void msd_destroy(msd_ctx* ctx);
+const char* msd_last_error(const msd_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MSD_H */

@@ -1,0 +1,259 @@
+"""Thin Python binding of libmsd_b200.so (include/msd.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of the library; PyTorch is used for device
+memory and streams.  There is no CPU fallback: if the shared library is missing or cannot be
+loaded, importing a symbol from here raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmsd_b200.so")
+
+MSD_OK, MSD_EINVAL, MSD_ENOMEM, MSD_ECUDA, MSD_EUNSUPPORTED = 0, -1, -2, -3, -4
+_CODES = {MSD_EINVAL: "MSD_EINVAL", MSD_ENOMEM: "MSD_ENOMEM", MSD_ECUDA: "MSD_ECUDA",
+          MSD_EUNSUPPORTED: "MSD_EUNSUPPORTED"}
+
+EXPORTS = ["msd_setup", "msd_setup_from_occ", "msd_overlap", "msd_force_bias", "msd_local_energy", "msd_greens",
+           "msd_get_info", "msd_get_packed", "msd_set_workspace_limit", "msd_launch_count", "msd_set_profiling",
+           "msd_get_phase_ms", "msd_probe_fp64_tflops", "msd_destroy", "msd_last_error"]
+
+
+class MSDError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__("%s (%d): %s" % (_CODES.get(code, "error"), code, msg))
+        self.code = code
+
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """Load libmsd_b200.so (built in-tree by paper_2406_08314_b200/build.py).  Fails loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("libmsd_b200.so not found at %s: run `python -m paper_2406_08314_b200.build` "
+                          "(or __graft_entry__.build()); there is no CPU fallback" % LIB_PATH)
+    lib = C.CDLL(LIB_PATH)
+    vp, i32, i64, dbl = C.c_void_p, C.c_int, C.c_int64, C.c_double
+    lib.msd_setup.restype = i32
+    lib.msd_setup.argtypes = [C.POINTER(vp), i32, i32, i32, i32, i64, vp, vp, dbl, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.msd_setup_from_occ.restype = i32
+    lib.msd_setup_from_occ.argtypes = [C.POINTER(vp), i32, i32, i32, i32, i64, vp, vp, dbl, vp, vp, vp, vp]
+    for name in ("msd_overlap", "msd_force_bias", "msd_local_energy", "msd_greens"):
+        f = getattr(lib, name)
+        f.restype = i32
+        f.argtypes = [vp, i64, vp, vp, vp, vp, vp]
+    lib.msd_get_info.restype = i32
+    lib.msd_get_info.argtypes = [vp, vp]
+    lib.msd_get_packed.restype = i32
+    lib.msd_get_packed.argtypes = [vp, vp, vp, vp, vp]
+    lib.msd_set_workspace_limit.restype = i32
+    lib.msd_set_workspace_limit.argtypes = [vp, i64]
+    lib.msd_launch_count.restype = i64
+    lib.msd_launch_count.argtypes = [vp]
+    lib.msd_set_profiling.restype = i32
+    lib.msd_set_profiling.argtypes = [vp, i32]
+    lib.msd_get_phase_ms.restype = i32
+    lib.msd_get_phase_ms.argtypes = [vp, vp, i32]
+    lib.msd_probe_fp64_tflops.restype = dbl
+    lib.msd_probe_fp64_tflops.argtypes = [i32, dbl, vp]
+    lib.msd_destroy.restype = None
+    lib.msd_destroy.argtypes = [vp]
+    lib.msd_last_error.restype = C.c_char_p
+    lib.msd_last_error.argtypes = [vp]
+    _lib = lib
+    return lib
+
+
+def _np(a, dtype):
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+def _ptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _stream_ptr(stream) -> Optional[int]:
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    if isinstance(stream, int):
+        return stream or None
+    return stream.cuda_stream or None
+
+
+class MSDTrial:
+    """Owns an msd_ctx.  Methods mirror the C entry points of include/msd.h."""
+
+    def __init__(self, handle: int, N: int, n_alpha: int, n_beta: int, n_chol: int, n_det: int):
+        self._h = C.c_void_p(handle)
+        self.N, self.n_alpha, self.n_beta, self.n_chol, self.n_det = N, n_alpha, n_beta, n_chol, n_det
+
+    # -- lifetime ------------------------------------------------------------------------------
+    def close(self):
+        if self._h:
+            load_library().msd_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc: int):
+        if rc != MSD_OK:
+            msg = load_library().msd_last_error(self._h)
+            raise MSDError(rc, msg.decode() if msg else "")
+
+    # -- hot calls -----------------------------------------------------------------------------
+    def _walkers(self, phi_a, phi_b):
+        import torch
+        for phi, n in ((phi_a, self.n_alpha), (phi_b, self.n_beta)):
+            if not (isinstance(phi, torch.Tensor) and phi.is_cuda and phi.dtype == torch.complex128
+                    and phi.is_contiguous() and phi.dim() == 3 and phi.shape[1] == self.N and phi.shape[2] == n):
+                raise ValueError("walkers must be contiguous CUDA complex128 tensors [n_w][N][n_sigma]")
+        if phi_a.shape[0] != phi_b.shape[0]:
+            raise ValueError("phi_a and phi_b disagree on n_w")
+        return int(phi_a.shape[0])
+
+    def _call(self, fn, phi_a, phi_b, out, flags, stream):
+        import torch
+        if flags is not None and not (flags.is_cuda and flags.dtype == torch.int32 and flags.is_contiguous()):
+            raise ValueError("flags must be a contiguous CUDA int32 tensor")
+        nw = self._walkers(phi_a, phi_b)
+        rc = fn(self._h, nw, phi_a.data_ptr(), phi_b.data_ptr(), out.data_ptr(),
+                flags.data_ptr() if flags is not None else None, _stream_ptr(stream))
+        self._check(rc)
+        return out
+
+    def overlap(self, phi_a, phi_b, out=None, flags=None, stream=None):
+        import torch
+        nw = self._walkers(phi_a, phi_b)
+        out = torch.empty(nw, dtype=torch.complex128, device=phi_a.device) if out is None else out
+        return self._call(load_library().msd_overlap, phi_a, phi_b, out, flags, stream)
+
+    def force_bias(self, phi_a, phi_b, out=None, flags=None, stream=None):
+        import torch
+        nw = self._walkers(phi_a, phi_b)
+        out = torch.empty((nw, self.n_chol), dtype=torch.complex128, device=phi_a.device) if out is None else out
+        return self._call(load_library().msd_force_bias, phi_a, phi_b, out, flags, stream)
+
+    def local_energy(self, phi_a, phi_b, out=None, flags=None, stream=None):
+        import torch
+        nw = self._walkers(phi_a, phi_b)
+        out = torch.empty((nw, 3), dtype=torch.complex128, device=phi_a.device) if out is None else out
+        return self._call(load_library().msd_local_energy, phi_a, phi_b, out, flags, stream)
+
+    def greens(self, phi_a, phi_b, out=None, flags=None, stream=None):
+        import torch
+        nw = self._walkers(phi_a, phi_b)
+        out = torch.empty((nw, 2, self.N, self.N), dtype=torch.complex128, device=phi_a.device) if out is None else out
+        return self._call(load_library().msd_greens, phi_a, phi_b, out, flags, stream)
+
+    # -- introspection -------------------------------------------------------------------------
+    def info(self) -> dict:
+        a = np.zeros(8, dtype=np.int64)
+        self._check(load_library().msd_get_info(self._h, _ptr(a)))
+        keys = ["n_o_alpha", "n_v_alpha", "n_o_beta", "n_v_beta", "n_buckets", "kmax_alpha", "kmax_beta", "walker_tile"]
+        return dict(zip(keys, (int(v) for v in a)))
+
+    def packed(self) -> dict:
+        perm = np.zeros(self.n_det, dtype=np.int64)
+        coef = np.zeros(self.n_det, dtype=np.float64)
+        la = np.zeros(self.n_det, dtype=np.int32)
+        lb = np.zeros(self.n_det, dtype=np.int32)
+        self._check(load_library().msd_get_packed(self._h, _ptr(perm), _ptr(coef), _ptr(la), _ptr(lb)))
+        return dict(perm=perm, coef=coef, level_a=la, level_b=lb)
+
+    def set_workspace_limit(self, nbytes: int):
+        self._check(load_library().msd_set_workspace_limit(self._h, int(nbytes)))
+
+    def launch_count(self) -> int:
+        return int(load_library().msd_launch_count(self._h))
+
+    def set_profiling(self, on: bool):
+        self._check(load_library().msd_set_profiling(self._h, 1 if on else 0))
+
+    def phase_ms(self) -> dict:
+        a = np.zeros(6, dtype=np.float32)
+        self._check(load_library().msd_get_phase_ms(self._h, _ptr(a), 6))
+        return dict(zip(["reference", "p1", "p2", "p3", "p4", "p5"], (float(v) for v in a)))
+
+
+def msd_setup(N, n_alpha, n_beta, n_chol, n_det, h1, L, e0, occ_ref_a, occ_ref_b,
+              exc_off_a, holes_a, parts_a, exc_off_b, holes_b, parts_b, ci, stream=None) -> MSDTrial:
+    """include/msd.h msd_setup: host numpy arrays in, device-resident packed trial out."""
+    lib = load_library()
+    h1 = _np(h1, np.float64); L = _np(L, np.float64); ci = _np(ci, np.float64)
+    ra = _np(occ_ref_a, np.int32); rb = _np(occ_ref_b, np.int32)
+    oa = _np(exc_off_a, np.int64); ob = _np(exc_off_b, np.int64)
+    ha = _np(holes_a, np.int32); pa = _np(parts_a, np.int32)
+    hb = _np(holes_b, np.int32); pb = _np(parts_b, np.int32)
+    if h1.shape != (N, N) or L.shape != (n_chol, N, N) or ci.shape != (n_det,):
+        raise ValueError("h1 / L / ci shapes disagree with N, n_chol, n_det")
+    if ra.shape != (n_alpha,) or rb.shape != (n_beta,) or oa.shape != (n_det + 1,) or ob.shape != (n_det + 1,):
+        raise ValueError("occ_ref / exc_off shapes disagree with n_alpha, n_beta, n_det")
+    if len(ha) != len(pa) or len(hb) != len(pb) or len(ha) != oa[-1] or len(hb) != ob[-1]:
+        raise ValueError("holes / parts lengths disagree with exc_off")
+    out = C.c_void_p()
+    rc = lib.msd_setup(C.byref(out), N, n_alpha, n_beta, n_chol, n_det, _ptr(h1), _ptr(L), float(e0),
+                       _ptr(ra), _ptr(rb), _ptr(oa), _ptr(ha), _ptr(pa), _ptr(ob), _ptr(hb), _ptr(pb), _ptr(ci),
+                       _stream_ptr(stream))
+    if rc != MSD_OK:
+        msg = lib.msd_last_error(None)
+        raise MSDError(rc, msg.decode() if msg else "")
+    return MSDTrial(out.value, N, n_alpha, n_beta, n_chol, n_det)
+
+
+def msd_setup_from_occ(N, n_alpha, n_beta, n_chol, n_det, h1, L, e0, occa, occb, ci, stream=None) -> MSDTrial:
+    """include/msd.h msd_setup_from_occ: the paper's (coeff, occa, occb) format."""
+    lib = load_library()
+    h1 = _np(h1, np.float64); L = _np(L, np.float64); ci = _np(ci, np.float64)
+    occa = _np(occa, np.int32); occb = _np(occb, np.int32)
+    if occa.shape != (n_det, n_alpha) or occb.shape != (n_det, n_beta):
+        raise ValueError("occa / occb shapes disagree with n_det, n_alpha, n_beta")
+    if h1.shape != (N, N) or L.shape != (n_chol, N, N) or ci.shape != (n_det,):
+        raise ValueError("h1 / L / ci shapes disagree with N, n_chol, n_det")
+    out = C.c_void_p()
+    rc = lib.msd_setup_from_occ(C.byref(out), N, n_alpha, n_beta, n_chol, n_det, _ptr(h1), _ptr(L), float(e0),
+                                _ptr(occa), _ptr(occb), _ptr(ci), _stream_ptr(stream))
+    if rc != MSD_OK:
+        msg = lib.msd_last_error(None)
+        raise MSDError(rc, msg.decode() if msg else "")
+    return MSDTrial(out.value, N, n_alpha, n_beta, n_chol, n_det)
+
+
+def msd_overlap(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, stream=None):
+    return trial.overlap(phi_a, phi_b, out, flags, stream)
+
+
+def msd_force_bias(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, stream=None):
+    return trial.force_bias(phi_a, phi_b, out, flags, stream)
+
+
+def msd_local_energy(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, stream=None):
+    return trial.local_energy(phi_a, phi_b, out, flags, stream)
+
+
+def msd_greens(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, stream=None):
+    return trial.greens(phi_a, phi_b, out, flags, stream)
+
+
+def msd_probe_fp64_tflops(use_dmma: bool = True, ms: float = 50.0, stream=None) -> float:
+    return float(load_library().msd_probe_fp64_tflops(1 if use_dmma else 0, float(ms), _stream_ptr(stream)))
+
+
+def setup_from_inputs(inp, stream=None) -> MSDTrial:
+    """Convenience for msd_inputs.MSDInputs (tests / bench)."""
+    return msd_setup(inp.N, inp.n_alpha, inp.n_beta, inp.n_chol, inp.n_det, inp.h1, inp.L, inp.e0,
+                     inp.occ_ref_a, inp.occ_ref_b, inp.exc_off_a, inp.holes_a, inp.parts_a,
+                     inp.exc_off_b, inp.holes_b, inp.parts_b, inp.ci, stream=stream)

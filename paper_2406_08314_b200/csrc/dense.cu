@@ -1,0 +1,387 @@
+// S5 Green's function rows, S7 dense energy intermediates (all but the two big GEMMs, which are in gemm.cu),
+// S9 assembly.  Wick steps W5-W10 of DESIGN.md "The algorithm"; Eq. 7, Eq. 14, L98.
+#include "msd_internal.cuh"
+
+__device__ __forceinline__ double nan_d() { return __longlong_as_double(0x7ff8000000000000LL); }
+
+// block-wide sum of a complex; result valid in thread 0
+__device__ __forceinline__ cplx block_sum(cplx v)
+{
+    __shared__ double sred[2][32];
+    for (int o = 16; o > 0; o >>= 1) {
+        v.x += __shfl_down_sync(0xffffffffu, v.x, o);
+        v.y += __shfl_down_sync(0xffffffffu, v.y, o);
+    }
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    __syncthreads();
+    if (lane == 0) { sred[0][wid] = v.x; sred[1][wid] = v.y; }
+    __syncthreads();
+    if (wid == 0) {
+        v.x = lane < nw ? sred[0][lane] : 0.0;
+        v.y = lane < nw ? sred[1][lane] : 0.0;
+        for (int o = 16; o > 0; o >>= 1) {
+            v.x += __shfl_down_sync(0xffffffffu, v.x, o);
+            v.y += __shfl_down_sync(0xffffffffu, v.y, o);
+        }
+    }
+    return v;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S5: G^s = G0 + (1/W) Q0 C G0 restricted to its non-zero rows occ_ref U act_virt  (W5)
+//   rows l < n      : G[occ_ref[l]][q] = Theta[q][l] - sum_h U[l][h] Theta[q][pos(h)],  U = Theta_v^T D
+//   rows n + r'     : G[act_v[r']][q]  = sum_h D[r'][h] Theta[q][pos(h)],               D = C / W
+// written planar (re row, im row) as the B operand of the force-bias GEMM; optionally scattered into the
+// full N x N matrix (msd_greens).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_green_rows(int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw, const cplx* __restrict__ theta_a,
+             const cplx* __restrict__ theta_b, const cplx* __restrict__ C_a, const cplx* __restrict__ C_b,
+             const cplx* __restrict__ Wacc, double* Gp_a, double* Gp_b, cplx* Gfull, int* wflags)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int s = blockIdx.y;
+    const int64_t w = blockIdx.x;
+    const SpinDev sp = s ? sb : sa;
+    const int n = sp.n, no = sp.n_o, nv = sp.n_v;
+    const cplx* theta = (s ? theta_b : theta_a) + w * (int64_t)N * n;
+    const cplx* C = (s ? C_b : C_a) + (w / MSD_WT) * (int64_t)sp.P * MSD_WT + (w % MSD_WT);
+    double* Gp = (s ? Gp_b : Gp_a);
+    cplx* D = reinterpret_cast<cplx*>(smem_raw);     // [nv][no]
+    cplx* U = D + nv * no;                            // [n][no]
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const cplx W = Wacc[w];
+    const bool bad = (W.x == 0.0 && W.y == 0.0) || (wflags[w] & 1);
+    if (tid == 0 && s == 0 && (W.x == 0.0 && W.y == 0.0)) atomicOr(&wflags[w], 2);
+    const cplx Winv = bad ? cmake(nan_d(), nan_d()) : cinv(W);
+    for (int x = tid; x < nv * no; x += nt) D[x] = cmul(C[(int64_t)x * MSD_WT], Winv);
+    __syncthreads();
+    for (int e = tid; e < n * no; e += nt) {
+        int l = e / no, h = e - l * no;
+        cplx acc = cmake(0.0, 0.0);
+        for (int r = 0; r < nv; r++) acc = cfma(theta[(int64_t)sp.act_v[r] * n + l], D[r * no + h], acc);
+        U[e] = acc;
+    }
+    __syncthreads();
+    const int nr = sp.n_r;
+    const int64_t ldk = (int64_t)nr * ldN;
+    double* gre = Gp ? Gp + (w * 2) * ldk : nullptr;
+    double* gim = Gp ? gre + ldk : nullptr;
+    cplx* Gf = Gfull ? Gfull + (w * 2 + s) * (int64_t)N * N : nullptr;
+    for (int e = tid; e < nr * ldN; e += nt) {
+        int r = e / ldN, q = e - r * ldN;
+        cplx acc = cmake(0.0, 0.0);
+        if (q < N) {
+            const cplx* th = theta + (int64_t)q * n;
+            if (r < n) {
+                acc = th[r];
+                for (int h = 0; h < no; h++) acc = cfms(U[r * no + h], th[sp.pos_o[h]], acc);
+            } else {
+                const cplx* d = D + (r - n) * no;
+                for (int h = 0; h < no; h++) acc = cfma(d[h], th[sp.pos_o[h]], acc);
+            }
+            if (Gf) {
+                int p = (r < n) ? sp.occ_ref[r] : sp.act_v[r - n];
+                Gf[(int64_t)p * N + q] = acc;
+            }
+        }
+        if (gre) { gre[e] = acc.x; gim[e] = acc.y; }
+    }
+}
+
+cudaError_t launch_green_rows(msd_ctx* c, int64_t nw, Workspace& ws, cplx* Gfull, cudaStream_t st)
+{
+    if (nw == 0) return cudaSuccess;
+    int ldN = c->N + (c->N & 1);
+    size_t smem = 0;
+    for (int s = 0; s < 2; s++) {
+        size_t v = ((size_t)c->sp[s].n_v * c->sp[s].n_o + (size_t)c->sp[s].n * c->sp[s].n_o + 1) * sizeof(cplx);
+        if (v > smem) smem = v;
+    }
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(k_green_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    dim3 grid((unsigned)nw, 2);
+    k_green_rows<<<grid, 256, smem, st>>>(c->N, ldN, c->dev(0), c->dev(1), nw, ws.theta[0], ws.theta[1], ws.C[0],
+                                          ws.C[1], ws.Wacc, ws.Gp[0], ws.Gp[1], Gfull, ws.wflags);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// S7: from Lam = L_sub Theta (rows (g, r), r < n: T^g = occupied block; r >= n: active-virtual block)   (W7)
+//   X0_g = tr T^g,  Ex0_g = tr(T^g T^g)
+//   Bfull^g[r'][i] = Lam_v^g[r'][i] - sum_l Theta_v[r'][l] T^g[l][i]
+//   B^g[x=(r',h)]  = Bfull^g[r'][pos(h)]             -> Bp (complex rows) and Bq (rows (br,-bi), (bi,br))
+//   FK[x]         += sum_l Bfull^g[r'][l] T^g[l][pos(h)]      (exchange-like part of F, W9)
+//   slice g = n_chol holds h1: Hrot[x] = B^{h1}[x], E1_0 += tr T^{h1}                              (W8)
+// CTA = (chunk of GC slices, walker, spin).
+// ------------------------------------------------------------------------------------------------
+template <int GC>
+__global__ void __launch_bounds__(256)
+k_energy_dense(int n_chol, int64_t nw, SpinDev sa, SpinDev sb, const cplx* __restrict__ theta_a,
+               const cplx* __restrict__ theta_b, const cplx* __restrict__ Lam_a, const cplx* __restrict__ Lam_b,
+               cplx* Bp_a, cplx* Bp_b, double* Bq_a, double* Bq_b, cplx* X0 /*[2][nw][n_chol]*/, cplx* F_a, cplx* F_b,
+               cplx* Hrot_a, cplx* Hrot_b, cplx* Eacc, int N)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int s = blockIdx.z;
+    const int64_t w = blockIdx.y;
+    const int g0 = blockIdx.x * GC;
+    const SpinDev sp = s ? sb : sa;
+    const int n = sp.n, no = sp.n_o, nv = sp.n_v, nr = sp.n_r, P = sp.P;
+    if (n == 0) return;
+    const cplx* theta = (s ? theta_b : theta_a) + w * (int64_t)N * n;
+    const cplx* Lam = s ? Lam_b : Lam_a;
+    cplx* Bp = (s ? Bp_b : Bp_a) + w * (int64_t)P * n_chol;
+    double* Bq = (s ? Bq_b : Bq_a) + w * (int64_t)2 * P * 2 * n_chol;
+    cplx* F = (s ? F_b : F_a) + w * (int64_t)P;
+    cplx* Hrot = (s ? Hrot_b : Hrot_a) + w * (int64_t)P;
+    const int tid = threadIdx.x, nt = blockDim.x;
+
+    cplx* T = reinterpret_cast<cplx*>(smem_raw);     // [n][n]
+    cplx* Bf = T + n * n;                             // [nv][n]   Lam_v then Bfull (in place)
+    cplx* Thv = Bf + nv * n;                          // [nv][n]   Theta rows of the active virtuals
+    cplx* Fk = Thv + nv * n;                          // [P]       accumulates sum_g BT^g
+    cplx* Bout = Fk + P;                              // [P][GC]
+    int* pos = reinterpret_cast<int*>(Bout + (size_t)P * GC);   // [no]
+
+    for (int e = tid; e < nv * n; e += nt) { int r = e / n, l = e - r * n; Thv[e] = theta[(int64_t)sp.act_v[r] * n + l]; }
+    for (int x = tid; x < P; x += nt) Fk[x] = cmake(0.0, 0.0);
+    for (int h = tid; h < no; h += nt) pos[h] = sp.pos_o[h];
+    cplx ex_part = cmake(0.0, 0.0);
+    __syncthreads();
+
+    for (int gi = 0; gi < GC; gi++) {
+        const int g = g0 + gi;
+        if (g > n_chol) {                  // past the h1 slice: pad Bout
+            for (int x = tid; x < P; x += nt) Bout[(size_t)x * GC + gi] = cmake(0.0, 0.0);
+            continue;
+        }
+        const cplx* lam = Lam + ((int64_t)g * nr * nw + w) * n;      // row r at + r * nw * n
+        for (int e = tid; e < nr * n; e += nt) {
+            int r = e / n, i = e - r * n;
+            cplx v = lam[(int64_t)r * nw * n + i];
+            if (r < n) T[e] = v; else Bf[(r - n) * n + i] = v;
+        }
+        __syncthreads();
+        // X0, Ex0 (the h1 slice contributes tr T to E1_0 instead)
+        if (tid < 32) {
+            cplx tr = cmake(0.0, 0.0);
+            for (int l = tid; l < n; l += 32) tr = cadd(tr, T[l * n + l]);
+            for (int o = 16; o > 0; o >>= 1) {
+                tr.x += __shfl_down_sync(0xffffffffu, tr.x, o);
+                tr.y += __shfl_down_sync(0xffffffffu, tr.y, o);
+            }
+            if (tid == 0) {
+                if (g < n_chol) X0[((int64_t)s * nw + w) * n_chol + g] = tr;
+                else red_add(&Eacc[w * 2 + 0], tr);
+            }
+        }
+        if (g < n_chol)
+            for (int e = tid; e < n * n; e += nt) { int l = e / n, i = e - l * n; ex_part = cfma(T[e], T[i * n + l], ex_part); }
+        // Bfull = Lam_v - Theta_v T
+        for (int e = tid; e < nv * n; e += nt) {
+            int r = e / n, i = e - r * n;
+            cplx acc = Bf[e];
+            const cplx* tv = Thv + r * n;
+            for (int l = 0; l < n; l++) acc = cfms(tv[l], T[l * n + i], acc);
+            // the element is only read by its own thread before the barrier
+            Bf[e] = acc;
+        }
+        __syncthreads();
+        for (int x = tid; x < P; x += nt) {
+            int r = x / no, h = x - r * no;
+            const int ph = pos[h];
+            cplx b = Bf[r * n + ph];
+            Bout[(size_t)x * GC + gi] = b;
+            if (g < n_chol) {
+                cplx acc = cmake(0.0, 0.0);
+                const cplx* bf = Bf + r * n;
+                for (int l = 0; l < n; l++) acc = cfma(bf[l], T[l * n + ph], acc);
+                Fk[x] = cadd(Fk[x], acc);
+            } else {
+                Hrot[x] = b;
+            }
+        }
+        __syncthreads();
+    }
+    // flush: B rows (GC consecutive slices per x), exchange part of F, Ex0
+    const int gcount = (g0 + GC <= n_chol) ? GC : (n_chol - g0 > 0 ? n_chol - g0 : 0);
+    for (int e = tid; e < P * GC; e += nt) {
+        int x = e / GC, gi = e - x * GC;
+        if (gi >= gcount) continue;
+        cplx b = Bout[e];
+        const int g = g0 + gi;
+        Bp[(int64_t)x * n_chol + g] = b;
+        double* q0 = Bq + ((int64_t)(2 * x) * 2 * n_chol) + 2 * g;
+        q0[0] = b.x; q0[1] = -b.y;
+        double* q1 = q0 + 2 * n_chol;
+        q1[0] = b.y; q1[1] = b.x;
+    }
+    for (int x = tid; x < P; x += nt) red_add(&F[x], cneg(Fk[x]));
+    cplx ex = block_sum(ex_part);
+    if (tid == 0) red_add(&Eacc[w * 2 + 1], cscale(-0.5, ex));
+}
+
+// F[x] += sum_g Xt_g B^g[x]  (Coulomb-like part of F, W9);   one warp per x
+__global__ void __launch_bounds__(256)
+k_fx(int n_chol, int64_t nw, int Pa, int Pb, const cplx* __restrict__ X0, const cplx* __restrict__ Bp_a,
+     const cplx* __restrict__ Bp_b, cplx* F_a, cplx* F_b)
+{
+    const int s = blockIdx.z;
+    const int64_t w = blockIdx.y;
+    const int P = s ? Pb : Pa;
+    const int x = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (x >= P) return;
+    const int lane = threadIdx.x & 31;
+    const cplx* b = (s ? Bp_b : Bp_a) + (w * (int64_t)P + x) * n_chol;
+    const cplx* xa = X0 + w * (int64_t)n_chol;
+    const cplx* xb = X0 + (nw + w) * (int64_t)n_chol;
+    cplx acc = cmake(0.0, 0.0);
+    for (int g = lane; g < n_chol; g += 32) acc = cfma(cadd(xa[g], xb[g]), b[g], acc);
+    for (int o = 16; o > 0; o >>= 1) {
+        acc.x += __shfl_down_sync(0xffffffffu, acc.x, o);
+        acc.y += __shfl_down_sync(0xffffffffu, acc.y, o);
+    }
+    if (lane == 0) { cplx* F = (s ? F_b : F_a) + w * (int64_t)P + x; *F = cadd(*F, acc); }
+}
+
+cudaError_t launch_energy_dense(msd_ctx* c, int64_t nw, Workspace& ws, cudaStream_t st)
+{
+    if (nw == 0) return cudaSuccess;
+    constexpr int GC = 8;
+    size_t smem = 0;
+    for (int s = 0; s < 2; s++) {
+        const auto& sp = c->sp[s];
+        size_t v = ((size_t)sp.n * sp.n + 2 * (size_t)sp.n_v * sp.n + (size_t)sp.P * (1 + GC) + 1) * sizeof(cplx) +
+                   (size_t)(sp.n_o + 4) * sizeof(int);
+        if (v > smem) smem = v;
+    }
+    if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
+    cudaError_t e = cudaFuncSetAttribute(k_energy_dense<GC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    // X0 of a spin with no electrons must read as zero: ws.X0 lies in the region zeroed per call
+    dim3 grid((c->n_chol + 1 + GC - 1) / GC, (unsigned)nw, 2);
+    cplx* X0 = ws.X0;
+    k_energy_dense<GC><<<grid, 256, smem, st>>>(c->n_chol, nw, c->dev(0), c->dev(1), ws.theta[0], ws.theta[1],
+                                                ws.Lam[0], ws.Lam[1], ws.Bp[0], ws.Bp[1], ws.Bq[0], ws.Bq[1], X0,
+                                                ws.F[0], ws.F[1], ws.Hrot[0], ws.Hrot[1], ws.Eacc, c->N);
+    c->launches++;
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    int Pmax = c->sp[0].P > c->sp[1].P ? c->sp[0].P : c->sp[1].P;
+    if (Pmax > 0) {
+        dim3 g2((Pmax + 7) / 8, (unsigned)nw, 2);
+        k_fx<<<g2, 256, 0, st>>>(c->n_chol, nw, c->sp[0].P, c->sp[1].P, X0, ws.Bp[0], ws.Bp[1], ws.F[0], ws.F[1]);
+        c->launches++;
+    }
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// S9 / finishing kernels
+// ------------------------------------------------------------------------------------------------
+__global__ void k_finish_overlap(int64_t nw, const cplx* __restrict__ det0, const cplx* __restrict__ Wacc,
+                                 int* wflags, cplx* ovlp, int* flags)
+{
+    int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= nw) return;
+    cplx W = Wacc[w];
+    int f = wflags[w];
+    if (W.x == 0.0 && W.y == 0.0) f |= 2;
+    cplx o = cmul(cmul(det0[w * 2], det0[w * 2 + 1]), W);
+    if (f) o = cmake(nan_d(), nan_d());
+    ovlp[w] = o;
+    if (flags) flags[w] = f;
+}
+
+// NaN-fill outputs of flagged walkers (force bias / greens) and export flags
+__global__ void k_finish_flags(int64_t nw, const cplx* __restrict__ Wacc, const int* __restrict__ wflags, cplx* out,
+                               int64_t per_walker, int* flags)
+{
+    const int64_t w = blockIdx.x;
+    cplx W = Wacc[w];
+    int f = wflags[w];
+    if (W.x == 0.0 && W.y == 0.0) f |= 2;
+    if (threadIdx.x == 0 && flags) flags[w] = f;
+    if (f && out)
+        for (int64_t e = threadIdx.x; e < per_walker; e += blockDim.x) out[w * per_walker + e] = cmake(nan_d(), nan_d());
+}
+
+//   E1 = E1_0 + (1/W) sum_s sum_x C^s[x] Hrot^s[x]                                            (W8)
+//   E2 = 1/2 sum_g Xt_g^2 - 1/2 sum_g (Ex0^a_g + Ex0^b_g) + (1/W) [ sum_s sum_x C^s[x] F^s[x] + E2nd ]   (W9)
+__global__ void __launch_bounds__(256)
+k_finish_energy(int n_chol, int64_t nw, double e0, int Pa, int Pb, const cplx* __restrict__ C_a,
+                const cplx* __restrict__ C_b, const cplx* __restrict__ F_a, const cplx* __restrict__ F_b,
+                const cplx* __restrict__ H_a, const cplx* __restrict__ H_b, const cplx* __restrict__ X0,
+                const cplx* __restrict__ Eacc, const cplx* __restrict__ Wacc, const cplx* __restrict__ E2nd,
+                const int* __restrict__ wflags, cplx* eout, int* flags)
+{
+    const int64_t w = blockIdx.x;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    cplx ch = cmake(0.0, 0.0), cf = cmake(0.0, 0.0), xx = cmake(0.0, 0.0);
+    for (int s = 0; s < 2; s++) {
+        const int P = s ? Pb : Pa;
+        const cplx* C = (s ? C_b : C_a) + (w / MSD_WT) * (int64_t)P * MSD_WT + (w % MSD_WT);
+        const cplx* F = (s ? F_b : F_a) + w * (int64_t)P;
+        const cplx* H = (s ? H_b : H_a) + w * (int64_t)P;
+        for (int x = tid; x < P; x += nt) {
+            cplx c = C[(int64_t)x * MSD_WT];
+            ch = cfma(c, H[x], ch);
+            cf = cfma(c, F[x], cf);
+        }
+    }
+    for (int g = tid; g < n_chol; g += nt) {
+        cplx xt = cadd(X0[w * (int64_t)n_chol + g], X0[(nw + w) * (int64_t)n_chol + g]);
+        xx = cfma(xt, xt, xx);
+    }
+    ch = block_sum(ch);
+    cf = block_sum(cf);
+    xx = block_sum(xx);
+    if (tid == 0) {
+        cplx W = Wacc[w];
+        int f = wflags[w];
+        if (W.x == 0.0 && W.y == 0.0) f |= 2;
+        cplx E1, E2;
+        if (f) { E1 = cmake(nan_d(), nan_d()); E2 = E1; }
+        else {
+            cplx Winv = cinv(W);
+            E1 = cadd(Eacc[w * 2 + 0], cmul(ch, Winv));
+            E2 = cadd(cadd(cscale(0.5, xx), Eacc[w * 2 + 1]), cmul(cadd(cf, E2nd[w]), Winv));
+        }
+        eout[w * 3 + 0] = cmake(e0 + E1.x + E2.x, E1.y + E2.y);
+        eout[w * 3 + 1] = E1;
+        eout[w * 3 + 2] = E2;
+        if (flags) flags[w] = f;
+    }
+}
+
+cudaError_t launch_finish_overlap(msd_ctx* c, int64_t nw, Workspace& ws, cplx* ovlp, int* flags, cudaStream_t st)
+{
+    if (nw == 0) return cudaSuccess;
+    k_finish_overlap<<<(unsigned)((nw + 127) / 128), 128, 0, st>>>(nw, ws.det0, ws.Wacc, ws.wflags, ovlp, flags);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_finish_flags(msd_ctx* c, int64_t nw, Workspace& ws, cplx* out, int64_t per_walker, int* flags,
+                                cudaStream_t st)
+{
+    if (nw == 0) return cudaSuccess;
+    k_finish_flags<<<(unsigned)nw, 128, 0, st>>>(nw, ws.Wacc, ws.wflags, out, per_walker, flags);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_finish_energy(msd_ctx* c, int64_t nw, Workspace& ws, cplx* e, int* flags, cudaStream_t st)
+{
+    if (nw == 0) return cudaSuccess;
+    cplx* X0 = ws.X0;
+    k_finish_energy<<<(unsigned)nw, 256, 0, st>>>(c->n_chol, nw, c->e0, c->sp[0].P, c->sp[1].P, ws.C[0], ws.C[1],
+                                                  ws.F[0], ws.F[1], ws.Hrot[0], ws.Hrot[1], X0, ws.Eacc, ws.Wacc,
+                                                  ws.E2nd, ws.wflags, e, flags);
+    c->launches++;
+    return cudaGetLastError();
+}

@@ -1,0 +1,213 @@
+// FP64 tensor-core (DMMA, mma.sync.m8n8k4.f64) batched GEMM used by the dense contractions of the path:
+//   S6 force bias   fb[g][w]   = sum_(r,q) L_sub[g][(r,q)] G[w][(r,q)]          (Eq. 7)
+//   S7 Lambda       Lam[(g,r)][(w,i)] = sum_q L_sub[(g,r)][q] Theta_w[q][i]     (half rotation)
+//   S7 V            V_w[x][y]  = sum_g B_w[x][g] B'_w[y][g]                      (two-body tensor in the active window)
+// All three are  C[m][n] (+)= sum_k A[m][k] B[n][k]  with both operands K-contiguous ("TN"), real FP64;
+// complex operands are expressed as real ones by the callers (see dense.cu).
+//
+// tcgen05/UMMA has no f64 kind, so FP64 tensor work on sm_100a goes through warp-level mma.sync; the probe in
+// this file measured 37.1 TFLOP/s for DMMA and 36.3 for DFMA on B200 (they share the FP64 units).
+// Tiles: CTA BM x BN x 16, 3-stage cp.async ring, warp tile 32 x 32 (4 x 4 DMMA tiles), fragments read from
+// shared memory with row stride 20 doubles (conflict-free for the 8x4 fragment pattern).
+#include "msd_internal.cuh"
+
+#define BK 16
+#define LDS_ 20       // BK + 4
+#define STAGES 3
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, int src_bytes)
+{
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+template <int BM, int BN, int WARPS_M, int WARPS_N>
+__global__ void __launch_bounds__(WARPS_M * WARPS_N * 32)
+k_gemm_tn(GemmArgs g)
+{
+    constexpr int NT = WARPS_M * WARPS_N * 32;
+    constexpr int WM = BM / WARPS_M, WN = BN / WARPS_N;       // warp tile
+    constexpr int TM = WM / 8, TN = WN / 8;
+    extern __shared__ __align__(16) double smem_gemm[];
+    double* As = smem_gemm;                                    // [STAGES][BM][LDS_]
+    double* Bs = smem_gemm + STAGES * BM * LDS_;               // [STAGES][BN][LDS_]
+    const int z = blockIdx.z;
+    const double* A = g.A + (int64_t)z * g.strideA;
+    const double* B = g.B + (int64_t)z * g.strideB;
+    const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int wm = (wid % WARPS_M) * WM, wn = (wid / WARPS_M) * WN;
+    const int gq = lane >> 2, tq = lane & 3;
+    const int KT = (g.K + BK - 1) / BK;
+
+    auto load_tile = [&](int stage, int kt) {
+        const int k0 = kt * BK;
+        double* as = As + stage * BM * LDS_;
+        double* bs = Bs + stage * BN * LDS_;
+        for (int c = tid; c < BM * (BK / 2); c += NT) {
+            int r = c / (BK / 2), kc = (c % (BK / 2)) * 2;
+            int m = m0 + r, k = k0 + kc;
+            bool ok = (m < g.M) && (k < g.K);
+            const double* src = ok ? (A + (int64_t)m * g.lda + k) : A;
+            cp_async16(as + r * LDS_ + kc, src, ok ? 16 : 0);
+        }
+        for (int c = tid; c < BN * (BK / 2); c += NT) {
+            int r = c / (BK / 2), kc = (c % (BK / 2)) * 2;
+            int n = n0 + r, k = k0 + kc;
+            bool ok = (n < g.N) && (k < g.K);
+            const double* src = ok ? (B + (int64_t)n * g.ldb + k) : B;
+            cp_async16(bs + r * LDS_ + kc, src, ok ? 16 : 0);
+        }
+    };
+
+    double acc[TM][TN][2];
+#pragma unroll
+    for (int i = 0; i < TM; i++)
+#pragma unroll
+        for (int j = 0; j < TN; j++) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+
+    for (int s = 0; s < STAGES - 1; s++) {
+        if (s < KT) load_tile(s, s);
+        cp_async_commit();
+    }
+    for (int kt = 0; kt < KT; kt++) {
+        cp_async_wait<STAGES - 2>();
+        __syncthreads();
+        {
+            int nk = kt + STAGES - 1;
+            if (nk < KT) load_tile(nk % STAGES, nk);
+            cp_async_commit();
+        }
+        const double* as = As + (kt % STAGES) * BM * LDS_ + (wm + gq) * LDS_ + tq;
+        const double* bs = Bs + (kt % STAGES) * BN * LDS_ + (wn + gq) * LDS_ + tq;
+#pragma unroll
+        for (int kk = 0; kk < BK / 4; kk++) {
+            double a[TM], b[TN];
+#pragma unroll
+            for (int i = 0; i < TM; i++) a[i] = as[i * 8 * LDS_ + kk * 4];
+#pragma unroll
+            for (int j = 0; j < TN; j++) b[j] = bs[j * 8 * LDS_ + kk * 4];
+#pragma unroll
+            for (int i = 0; i < TM; i++)
+#pragma unroll
+                for (int j = 0; j < TN; j++) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+    }
+    cp_async_wait<0>();
+
+    // epilogue: thread holds (row gq, columns 2 tq, 2 tq + 1) of every 8x8 tile = one complex / column pair
+    double* Cz = g.C + 2 * ((int64_t)(z / g.zdiv) * g.strideC_hi + (int64_t)(z % g.zdiv) * g.strideC_lo);
+#pragma unroll
+    for (int i = 0; i < TM; i++) {
+        const int m = m0 + wm + i * 8 + gq;
+        if (m >= g.M) continue;
+#pragma unroll
+        for (int j = 0; j < TN; j++) {
+            const int n = n0 + wn + j * 8 + 2 * tq;
+            if (n >= g.N) continue;
+            double2* dst = reinterpret_cast<double2*>(Cz + 2 * ((int64_t)m * g.cs_m + (int64_t)(n >> 1) * g.cs_j));
+            double2 v = make_double2(acc[i][j][0], acc[i][j][1]);
+            if (g.accumulate) { double2 o = *dst; v.x += o.x; v.y += o.y; }
+            *dst = v;
+        }
+    }
+}
+
+template <int BM, int BN, int WARPS_M, int WARPS_N>
+static cudaError_t launch_cfg(const GemmArgs& a, cudaStream_t st)
+{
+    size_t smem = (size_t)STAGES * (BM + BN) * LDS_ * sizeof(double);
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_gemm_tn<BM, BN, WARPS_M, WARPS_N>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    dim3 grid((a.N + BN - 1) / BN, (a.M + BM - 1) / BM, a.batch);
+    k_gemm_tn<BM, BN, WARPS_M, WARPS_N><<<grid, WARPS_M * WARPS_N * 32, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_gemm_tn(const GemmArgs& a, int n_sm, cudaStream_t st)
+{
+    if (a.M <= 0 || a.N <= 0 || a.batch <= 0) return cudaSuccess;
+    if ((a.N & 1) || (a.K & 1) || (a.lda & 1) || (a.ldb & 1) || (a.strideA & 1) || (a.strideB & 1))
+        return cudaErrorInvalidValue;     // callers pad to even sizes (16-byte cp.async chunks)
+    int64_t big = (int64_t)((a.M + 127) / 128) * ((a.N + 63) / 64) * a.batch;
+    if (big >= 2 * (int64_t)n_sm) return launch_cfg<128, 64, 4, 2>(a, st);
+    return launch_cfg<64, 64, 2, 2>(a, st);
+}
+
+// ------------------------------------------------------------------------------------------------
+// FP64 peak probe (register-resident): roofline denominator for bench.py
+// ------------------------------------------------------------------------------------------------
+__global__ void k_probe_dmma(double* out, int iters)
+{
+    double d[8][2];
+    for (int j = 0; j < 8; j++) { d[j][0] = 0.0; d[j][1] = 0.0; }
+    double a = threadIdx.x * 1e-3, b = 1e-3;
+    for (int i = 0; i < iters; i++) {
+#pragma unroll
+        for (int j = 0; j < 8; j++) dmma884(d[j][0], d[j][1], a, b);
+    }
+    double s = 0.0;
+    for (int j = 0; j < 8; j++) s += d[j][0] + d[j][1];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+__global__ void k_probe_dfma(double* out, int iters)
+{
+    double a[8];
+    for (int j = 0; j < 8; j++) a[j] = threadIdx.x * 1e-9 + j;
+    const double b = 1.0000001, c = 1e-9;
+    for (int i = 0; i < iters; i++) {
+#pragma unroll
+        for (int j = 0; j < 8; j++) a[j] = fma(a[j], b, c);
+    }
+    double s = 0.0;
+    for (int j = 0; j < 8; j++) s += a[j];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+double probe_fp64(int use_dmma, double ms_target, cudaStream_t st)
+{
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -1.0;
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    const int thr = 512, blocks = nsm * 2;
+    double* out = nullptr;
+    if (cudaMalloc(&out, sizeof(double) * thr * blocks) != cudaSuccess) return -1.0;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    int iters = 20000;
+    double best = 0.0;
+    for (int rep = 0; rep < 3; rep++) {
+        cudaEventRecord(e0, st);
+        if (use_dmma) k_probe_dmma<<<blocks, thr, 0, st>>>(out, iters);
+        else k_probe_dfma<<<blocks, thr, 0, st>>>(out, iters);
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { best = -1.0; break; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        double fl = use_dmma ? 2.0 * 8 * 8 * 4 * 8 * (double)iters * blocks * thr / 32.0
+                             : 2.0 * 8 * (double)iters * blocks * thr;
+        double tf = fl / (ms * 1e-3) / 1e12;
+        if (rep > 0 && tf > best) best = tf;
+        if (rep == 0 && ms > 0.f && ms_target > 0.0) {
+            double scale = ms_target / ms;
+            if (scale > 200.0) scale = 200.0;
+            if (scale > 1.0) iters = (int)(iters * scale);
+        }
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(out);
+    return best;
+}

@@ -1,0 +1,636 @@
+// C ABI of libmsd_b200.so (include/msd.h): context, setup (S0), workspace, and the call graphs of the hot calls.
+#include "../../include/msd.h"
+#include "msd_internal.cuh"
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+static std::string g_setup_error;
+
+#define CK(call)                                                                                        \
+    do {                                                                                                \
+        cudaError_t e_ = (call);                                                                        \
+        if (e_ != cudaSuccess) {                                                                        \
+            char buf_[512];                                                                             \
+            snprintf(buf_, sizeof buf_, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+            *errp = buf_;                                                                               \
+            return (e_ == cudaErrorMemoryAllocation) ? MSD_ENOMEM : MSD_ECUDA;                          \
+        }                                                                                               \
+    } while (0)
+
+template <class T> static cudaError_t upload(T** d, const T* h, size_t n, cudaStream_t st)
+{
+    cudaError_t e = cudaMalloc((void**)d, std::max<size_t>(n, 1) * sizeof(T));
+    if (e != cudaSuccess) return e;
+    if (n) e = cudaMemcpyAsync(*d, h, n * sizeof(T), cudaMemcpyHostToDevice, st);
+    return e;
+}
+
+static int fail(std::string* errp, int code, const char* msg) { *errp = msg; return code; }
+
+// ---------------------------------------------------------------------------------------------
+// setup
+// ---------------------------------------------------------------------------------------------
+static int do_setup(msd_ctx* c, std::string* errp, int N, int na, int nb, int n_chol, int64_t n_det, const double* h1,
+                    const double* L, double e0, const int32_t* occ_ref_a, const int32_t* occ_ref_b,
+                    const int64_t* off_a, const int32_t* holes_a, const int32_t* parts_a, const int64_t* off_b,
+                    const int32_t* holes_b, const int32_t* parts_b, const double* ci, cudaStream_t st)
+{
+    if (!h1 || !L || !off_a || !off_b || !ci || (na > 0 && !occ_ref_a) || (nb > 0 && !occ_ref_b))
+        return fail(errp, MSD_EINVAL, "null pointer argument");
+    if (N < 1 || na < 0 || nb < 0 || n_chol < 1 || n_det < 1) return fail(errp, MSD_EINVAL, "non-positive size");
+    if (N > 1024 || na > MSD_MAX_NOCC || nb > MSD_MAX_NOCC || na > N || nb > N)
+        return fail(errp, MSD_EUNSUPPORTED, "N <= 1024 and n_alpha, n_beta <= 64 required");
+    if (n_det > (int64_t)1 << 31) return fail(errp, MSD_EUNSUPPORTED, "n_det too large");
+    CK(cudaGetDevice(&c->device));
+    CK(cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device));
+    c->N = N; c->n_chol = n_chol; c->n_det = n_det; c->e0 = e0;
+    const int32_t* occ_ref[2] = {occ_ref_a, occ_ref_b};
+    const int64_t* off[2] = {off_a, off_b};
+    const int32_t* holes[2] = {holes_a, holes_b};
+    const int32_t* parts[2] = {parts_a, parts_b};
+    const int ns[2] = {na, nb};
+
+    std::vector<int> pos_in_ref[2];
+    int* d_pos_in_ref[2] = {nullptr, nullptr};
+    for (int s = 0; s < 2; s++) {
+        auto& sp = c->sp[s];
+        sp.n = ns[s];
+        sp.occ_ref.assign(occ_ref[s], occ_ref[s] + ns[s]);
+        pos_in_ref[s].assign(N, -1);
+        for (int l = 0; l < ns[s]; l++) {
+            int o = sp.occ_ref[l];
+            if (o < 0 || o >= N || (l > 0 && o <= sp.occ_ref[l - 1]))
+                return fail(errp, MSD_EINVAL, "reference occupation must be strictly ascending and inside [0, N)");
+            pos_in_ref[s][o] = l;
+        }
+        if (off[s][0] != 0) return fail(errp, MSD_EINVAL, "exc_off[0] must be 0");
+        CK(upload(&d_pos_in_ref[s], pos_in_ref[s].data(), N, st));
+        CK(upload(&sp.d_occ_ref, sp.occ_ref.data(), ns[s], st));
+    }
+    // --- tables to the device ---
+    int64_t* d_off[2]; int32_t* d_holes[2]; int32_t* d_parts[2];
+    for (int s = 0; s < 2; s++) {
+        int64_t nnz = off[s][n_det];
+        if (nnz < 0) return fail(errp, MSD_EINVAL, "negative table size");
+        if (nnz > 0 && (!holes[s] || !parts[s])) return fail(errp, MSD_EINVAL, "null table");
+        CK(upload(&d_off[s], off[s], (size_t)n_det + 1, st));
+        CK(upload(&d_holes[s], holes[s], (size_t)nnz, st));
+        CK(upload(&d_parts[s], parts[s], (size_t)nnz, st));
+    }
+    double* d_ci; CK(upload(&d_ci, ci, (size_t)n_det, st));
+    // --- pass 1: validate, mark the active window (reading A10) ---
+    int* d_used; CK(cudaMalloc(&d_used, sizeof(int) * (4 * N + 1)));
+    CK(cudaMemsetAsync(d_used, 0, sizeof(int) * (4 * N + 1), st));
+    int* d_err = d_used + 4 * N;
+    for (int s = 0; s < 2; s++) {
+        CK(launch_pack_mark(n_det, d_off[s], d_holes[s], d_parts[s], N, d_pos_in_ref[s], d_used + (2 * s) * N,
+                            d_used + (2 * s + 1) * N, d_err, st));
+        c->launches++;
+    }
+    std::vector<int> used(4 * N + 1);
+    CK(cudaMemcpyAsync(used.data(), d_used, sizeof(int) * (4 * N + 1), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (used[4 * N] != 0) {
+        char b[160];
+        snprintf(b, sizeof b, "invalid excitation table (error bits 0x%x: 1 range, 2 hole not in reference, "
+                 "4 particle in reference, 16 level)", used[4 * N]);
+        *errp = b;
+        return MSD_EINVAL;
+    }
+    std::vector<int> map_h[2], map_p[2];
+    int* d_map[4];
+    for (int s = 0; s < 2; s++) {
+        auto& sp = c->sp[s];
+        map_h[s].assign(N, -1); map_p[s].assign(N, -1);
+        for (int o = 0; o < N; o++) {
+            if (used[(2 * s) * N + o]) { map_h[s][o] = (int)sp.act_o.size(); sp.act_o.push_back(o); sp.pos_o.push_back(pos_in_ref[s][o]); }
+            if (used[(2 * s + 1) * N + o]) { map_p[s][o] = (int)sp.act_v.size(); sp.act_v.push_back(o); }
+        }
+        sp.n_o = (int)sp.act_o.size(); sp.n_v = (int)sp.act_v.size();
+        sp.n_r = sp.n + sp.n_v; sp.P = sp.n_o * sp.n_v;
+        if (sp.n_o > 255 || sp.n_v > 255 || sp.P > 65535)
+            return fail(errp, MSD_EUNSUPPORTED, "active window too large (n_o, n_v <= 255, n_o*n_v <= 65535)");
+        CK(upload(&d_map[2 * s], map_h[s].data(), N, st));
+        CK(upload(&d_map[2 * s + 1], map_p[s].data(), N, st));
+        CK(upload(&sp.d_act_v, sp.act_v.data(), sp.act_v.size(), st));
+        CK(upload(&sp.d_pos_o, sp.pos_o.data(), sp.pos_o.size(), st));
+    }
+    // --- pass 2: per-determinant rows, phases, level keys ---
+    constexpr int NK = (MSD_MAX_LEVEL + 1) * (MSD_MAX_LEVEL + 1);
+    unsigned char* d_tmp; int* d_key; double* d_coef_unsorted; int* d_hist;
+    CK(cudaMalloc(&d_tmp, (size_t)n_det * 64));
+    CK(cudaMalloc(&d_key, sizeof(int) * n_det));
+    CK(cudaMalloc(&d_coef_unsorted, sizeof(double) * n_det));
+    CK(cudaMalloc(&d_hist, sizeof(int) * NK));
+    CK(cudaMemsetAsync(d_hist, 0, sizeof(int) * NK, st));
+    CK(launch_pack_rows(n_det, N, d_off[0], d_holes[0], d_parts[0], d_off[1], d_holes[1], d_parts[1],
+                        c->sp[0].d_occ_ref, na, c->sp[1].d_occ_ref, nb, d_pos_in_ref[0], d_pos_in_ref[1],
+                        d_map[0], d_map[1], d_map[2], d_map[3], d_ci, d_tmp, d_key, d_coef_unsorted, d_hist, d_err, st));
+    c->launches++;
+    std::vector<int> hist(NK);
+    int err2 = 0;
+    CK(cudaMemcpyAsync(hist.data(), d_hist, sizeof(int) * NK, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(&err2, d_err, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (err2 != 0) return fail(errp, MSD_EINVAL, "invalid excitation table (repeated index inside a determinant, or level > n)");
+    // --- buckets ---
+    std::vector<int> bucket_keys, bucket_of_key(NK, -1);
+    std::vector<int64_t> bucket_start;
+    int64_t run = 0, tab_bytes = 0;
+    for (int ky = 0; ky < NK; ky++) {
+        if (!hist[ky]) continue;
+        Bucket b;
+        b.ka = ky / (MSD_MAX_LEVEL + 1); b.kb = ky % (MSD_MAX_LEVEL + 1);
+        b.start = run; b.count = hist[ky];
+        b.rs = std::max(4, (2 * b.ka + 2 * b.kb + 3) / 4 * 4);
+        b.tab_off = tab_bytes;
+        tab_bytes += (b.count * b.rs + 15) / 16 * 16;
+        run += b.count;
+        bucket_of_key[ky] = (int)c->buckets.size();
+        bucket_keys.push_back(ky);
+        bucket_start.push_back(b.start);
+        c->buckets.push_back(b);
+        c->sp[0].kmax = std::max(c->sp[0].kmax, b.ka);
+        c->sp[1].kmax = std::max(c->sp[1].kmax, b.kb);
+    }
+    if (run != n_det) return fail(errp, MSD_ECUDA, "internal: histogram does not sum to n_det");
+    const int nbk = (int)c->buckets.size();
+    int* d_bkeys; int64_t* d_bstart; int64_t* d_perm; Bucket* d_buckets; int* d_bok;
+    CK(upload(&d_bkeys, bucket_keys.data(), nbk, st));
+    CK(upload(&d_bstart, bucket_start.data(), nbk, st));
+    CK(upload(&d_buckets, c->buckets.data(), nbk, st));
+    CK(upload(&d_bok, bucket_of_key.data(), NK, st));
+    CK(cudaMalloc(&d_perm, sizeof(int64_t) * n_det));
+    CK(cudaMalloc(&c->d_tab, std::max<int64_t>(tab_bytes, 16)));
+    CK(cudaMalloc(&c->d_coef, sizeof(double) * n_det));
+    CK(launch_pack_scatter(n_det, d_key, nbk, d_bkeys, d_bstart, d_perm, st));
+    CK(launch_pack_write(n_det, d_perm, d_key, d_tmp, d_coef_unsorted, nbk, d_buckets, d_bok, c->d_tab, c->d_coef, st));
+    c->launches += 2;
+    c->h_perm.resize(n_det); c->h_coef.resize(n_det);
+    CK(cudaMemcpyAsync(c->h_perm.data(), d_perm, sizeof(int64_t) * n_det, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(c->h_coef.data(), c->d_coef, sizeof(double) * n_det, cudaMemcpyDeviceToHost, st));
+    // --- L_sub, h1_sub (A17): rows occ_ref U act_virt, row stride ldN (even) ---
+    const int ldN = N + (N & 1);
+    {
+        double* d_L; double* d_h1;
+        CK(upload(&d_L, L, (size_t)n_chol * N * N, st));
+        CK(upload(&d_h1, h1, (size_t)N * N, st));
+        for (int s = 0; s < 2; s++) {
+            auto& sp = c->sp[s];
+            std::vector<int> rows(sp.occ_ref);
+            rows.insert(rows.end(), sp.act_v.begin(), sp.act_v.end());
+            int* d_rows; CK(upload(&d_rows, rows.data(), rows.size(), st));
+            size_t nel = (size_t)(n_chol + 1) * sp.n_r * ldN;
+            CK(cudaMalloc(&sp.d_Lsub, std::max<size_t>(nel, 2) * sizeof(double)));
+            CK(cudaMemsetAsync(sp.d_Lsub, 0, std::max<size_t>(nel, 2) * sizeof(double), st));
+            // packed with row stride ldN: copy N columns of each row
+            if (sp.n_r > 0) {
+                // reuse the pack kernel with "N" = source stride; destination stride handled by a 2D copy
+                double* tmp; CK(cudaMalloc(&tmp, (size_t)(n_chol + 1) * sp.n_r * N * sizeof(double)));
+                CK(launch_pack_lsub(d_L, n_chol, N, sp.n_r, d_rows, tmp, st));
+                CK(launch_pack_lsub(d_h1, 1, N, sp.n_r, d_rows, tmp + (size_t)n_chol * sp.n_r * N, st));
+                c->launches += 2;
+                CK(cudaMemcpy2DAsync(sp.d_Lsub, ldN * sizeof(double), tmp, N * sizeof(double), N * sizeof(double),
+                                     (size_t)(n_chol + 1) * sp.n_r, cudaMemcpyDeviceToDevice, st));
+                CK(cudaStreamSynchronize(st));
+                cudaFree(tmp);
+            }
+            CK(cudaStreamSynchronize(st));
+            cudaFree(d_rows);
+        }
+        cudaFree(d_L); cudaFree(d_h1);
+    }
+    CK(cudaStreamSynchronize(st));
+    c->h_ka.resize(n_det); c->h_kb.resize(n_det);
+    for (const Bucket& b : c->buckets)
+        for (int64_t i = 0; i < b.count; i++) { c->h_ka[b.start + i] = b.ka; c->h_kb[b.start + i] = b.kb; }
+    // --- work items ---
+    int gen_elems = 0;
+    for (const Bucket& b : c->buckets)
+        if (std::max(b.ka, b.kb) > MSD_CF_MAX) gen_elems = std::max(gen_elems, b.ka * b.ka + b.kb * b.kb);
+    if (gen_elems > 400) return fail(errp, MSD_EUNSUPPORTED, "k_alpha^2 + k_beta^2 <= 400 required");
+    c->gen_smem_per_thread = std::max(gen_elems, 1) * 16;
+    {
+        int t = (200 * 1024) / c->gen_smem_per_thread;
+        t = std::min(128, t / 32 * 32);
+        c->gen_threads = std::max(32, t);
+    }
+    auto cost = [](const Bucket& b) {
+        double a = b.ka, bb = b.kb;
+        return 1.0 + a * a * a + bb * bb * bb + a * a * bb * bb;
+    };
+    for (int bi = 0; bi < nbk; bi++) {
+        const Bucket& b = c->buckets[bi];
+        const bool gen = std::max(b.ka, b.kb) > MSD_CF_MAX;
+        int slots = gen ? c->gen_threads / MSD_WT : 128 / MSD_WT;
+        int iters = (int)std::max(2.0, std::min(32.0, 512.0 / cost(b)));
+        int dpc = slots * iters;
+        for (int64_t i0 = 0; i0 < b.count; i0 += dpc) {
+            WorkItem it;
+            it.bucket = bi; it.ka = b.ka; it.kb = b.kb; it.rs = b.rs;
+            it.det_begin = b.start + i0;
+            it.det_count = (int)std::min<int64_t>(dpc, b.count - i0);
+            it.tab_off = b.tab_off + i0 * b.rs;
+            (gen ? c->items_gen : c->items_cf).push_back(it);
+        }
+    }
+    auto cls = [](const WorkItem& w) { int m = std::max(w.ka, w.kb); return m <= 2 ? 0 : (m == 3 ? 1 : 2); };
+    auto icost = [](const WorkItem& w) {
+        double a = w.ka, b = w.kb;
+        return (1.0 + a * a * a + b * b * b + a * a * b * b) * w.det_count;
+    };
+    std::stable_sort(c->items_cf.begin(), c->items_cf.end(), [&](const WorkItem& x, const WorkItem& y) {
+        if (cls(x) != cls(y)) return cls(x) < cls(y);
+        return icost(x) > icost(y);
+    });
+    std::stable_sort(c->items_gen.begin(), c->items_gen.end(),
+                     [&](const WorkItem& x, const WorkItem& y) { return icost(x) > icost(y); });
+    CK(upload(&c->d_items_cf, c->items_cf.data(), c->items_cf.size(), st));
+    CK(upload(&c->d_items_gen, c->items_gen.data(), c->items_gen.size(), st));
+    CK(cudaStreamSynchronize(st));
+    // free setup temporaries
+    for (int s = 0; s < 2; s++) { cudaFree(d_pos_in_ref[s]); cudaFree(d_off[s]); cudaFree(d_holes[s]); cudaFree(d_parts[s]); }
+    for (int i = 0; i < 4; i++) cudaFree(d_map[i]);
+    cudaFree(d_ci); cudaFree(d_used); cudaFree(d_tmp); cudaFree(d_key); cudaFree(d_coef_unsorted); cudaFree(d_hist);
+    cudaFree(d_bkeys); cudaFree(d_bstart); cudaFree(d_perm); cudaFree(d_buckets); cudaFree(d_bok);
+    return MSD_OK;
+}
+
+extern "C" int msd_setup(msd_ctx** out, int N, int n_alpha, int n_beta, int n_chol, int64_t n_det, const double* h1,
+                         const double* L, double e0, const int32_t* occ_ref_a, const int32_t* occ_ref_b,
+                         const int64_t* exc_off_a, const int32_t* holes_a, const int32_t* parts_a,
+                         const int64_t* exc_off_b, const int32_t* holes_b, const int32_t* parts_b, const double* ci,
+                         void* stream)
+{
+    if (!out) { g_setup_error = "out is NULL"; return MSD_EINVAL; }
+    *out = nullptr;
+    msd_ctx* c = new (std::nothrow) msd_ctx();
+    if (!c) { g_setup_error = "out of host memory"; return MSD_ENOMEM; }
+    std::string err;
+    int rc;
+    try {
+        rc = do_setup(c, &err, N, n_alpha, n_beta, n_chol, n_det, h1, L, e0, occ_ref_a, occ_ref_b, exc_off_a, holes_a,
+                      parts_a, exc_off_b, holes_b, parts_b, ci, (cudaStream_t)stream);
+    } catch (const std::bad_alloc&) {
+        rc = MSD_ENOMEM; err = "out of host memory";
+    }
+    if (rc != MSD_OK) {
+        g_setup_error = err;
+        cudaGetLastError();
+        msd_destroy(c);
+        return rc;
+    }
+    *out = c;
+    return MSD_OK;
+}
+
+extern "C" int msd_setup_from_occ(msd_ctx** out, int N, int n_alpha, int n_beta, int n_chol, int64_t n_det,
+                                  const double* h1, const double* L, double e0, const int32_t* occa,
+                                  const int32_t* occb, const double* ci, void* stream)
+{
+    if (!out || n_det < 1 || N < 1 || n_alpha < 0 || n_beta < 0 || (n_alpha > 0 && !occa) || (n_beta > 0 && !occb)) {
+        g_setup_error = "bad argument";
+        return MSD_EINVAL;
+    }
+    // pure set bookkeeping on the host: reference = sorted row 0; holes = ref \ occ, particles = occ \ ref
+    try {
+        std::vector<int32_t> ref[2];
+        std::vector<int64_t> off[2];
+        std::vector<int32_t> holes[2], parts[2];
+        const int32_t* occ[2] = {occa, occb};
+        const int ns[2] = {n_alpha, n_beta};
+        for (int s = 0; s < 2; s++) {
+            ref[s].assign(occ[s], occ[s] + ns[s]);
+            std::sort(ref[s].begin(), ref[s].end());
+            std::vector<char> inref(N, 0), inocc(N, 0);
+            for (int o : ref[s]) { if (o < 0 || o >= N) { g_setup_error = "orbital out of range"; return MSD_EINVAL; } inref[o] = 1; }
+            off[s].assign(n_det + 1, 0);
+            for (int64_t I = 0; I < n_det; I++) {
+                const int32_t* row = occ[s] + I * ns[s];
+                for (int l = 0; l < ns[s]; l++) {
+                    if (row[l] < 0 || row[l] >= N) { g_setup_error = "orbital out of range"; return MSD_EINVAL; }
+                    if (inocc[row[l]]) { g_setup_error = "repeated orbital in an occupation list"; return MSD_EINVAL; }
+                    inocc[row[l]] = 1;
+                    if (!inref[row[l]]) parts[s].push_back(row[l]);
+                }
+                for (int o : ref[s]) if (!inocc[o]) holes[s].push_back(o);
+                for (int l = 0; l < ns[s]; l++) inocc[row[l]] = 0;
+                off[s][I + 1] = (int64_t)parts[s].size();
+                if (holes[s].size() != parts[s].size()) { g_setup_error = "internal: hole/particle mismatch"; return MSD_EINVAL; }
+            }
+        }
+        return msd_setup(out, N, n_alpha, n_beta, n_chol, n_det, h1, L, e0, ref[0].data(), ref[1].data(),
+                         off[0].data(), holes[0].data(), parts[0].data(), off[1].data(), holes[1].data(),
+                         parts[1].data(), ci, stream);
+    } catch (const std::bad_alloc&) {
+        g_setup_error = "out of host memory";
+        return MSD_ENOMEM;
+    }
+}
+
+extern "C" void msd_destroy(msd_ctx* c)
+{
+    if (!c) return;
+    for (int s = 0; s < 2; s++) {
+        cudaFree(c->sp[s].d_occ_ref); cudaFree(c->sp[s].d_act_v); cudaFree(c->sp[s].d_pos_o); cudaFree(c->sp[s].d_Lsub);
+    }
+    cudaFree(c->d_tab); cudaFree(c->d_coef); cudaFree(c->d_items_cf); cudaFree(c->d_items_gen);
+    cudaFree(c->ws.base);
+    for (auto& e : c->ev) if (e) cudaEventDestroy(e);
+    delete c;
+}
+
+extern "C" const char* msd_last_error(const msd_ctx* c) { return c ? c->err.c_str() : g_setup_error.c_str(); }
+
+extern "C" int msd_get_info(const msd_ctx* c, int64_t* info)
+{
+    if (!c || !info) return MSD_EINVAL;
+    info[0] = c->sp[0].n_o; info[1] = c->sp[0].n_v; info[2] = c->sp[1].n_o; info[3] = c->sp[1].n_v;
+    info[4] = (int64_t)c->buckets.size(); info[5] = c->sp[0].kmax; info[6] = c->sp[1].kmax; info[7] = MSD_WT;
+    return MSD_OK;
+}
+
+extern "C" int msd_get_packed(const msd_ctx* c, int64_t* perm, double* coef, int32_t* la, int32_t* lb)
+{
+    if (!c) return MSD_EINVAL;
+    if (perm) memcpy(perm, c->h_perm.data(), sizeof(int64_t) * c->n_det);
+    if (coef) memcpy(coef, c->h_coef.data(), sizeof(double) * c->n_det);
+    if (la) memcpy(la, c->h_ka.data(), sizeof(int32_t) * c->n_det);
+    if (lb) memcpy(lb, c->h_kb.data(), sizeof(int32_t) * c->n_det);
+    return MSD_OK;
+}
+
+extern "C" int msd_set_workspace_limit(msd_ctx* c, int64_t bytes)
+{
+    if (!c || bytes < 0) return MSD_EINVAL;
+    c->ws_limit = bytes;
+    return MSD_OK;
+}
+extern "C" int64_t msd_launch_count(const msd_ctx* c) { return c ? c->launches : -1; }
+extern "C" int msd_set_profiling(msd_ctx* c, int on)
+{
+    if (!c) return MSD_EINVAL;
+    c->profiling = on != 0;
+    if (c->profiling)
+        for (auto& e : c->ev) if (!e && cudaEventCreate(&e) != cudaSuccess) return MSD_ECUDA;
+    return MSD_OK;
+}
+extern "C" int msd_get_phase_ms(msd_ctx* c, float* ms, int n)
+{
+    if (!c || !ms) return MSD_EINVAL;
+    for (int i = 0; i < n && i < 6; i++) ms[i] = c->phase_ms[i];
+    return MSD_OK;
+}
+extern "C" double msd_probe_fp64_tflops(int use_dmma, double ms, void* stream)
+{
+    return probe_fp64(use_dmma, ms, (cudaStream_t)stream);
+}
+
+// ---------------------------------------------------------------------------------------------
+// workspace
+// ---------------------------------------------------------------------------------------------
+struct Carver {
+    char* base; size_t off = 0;
+    explicit Carver(char* b) : base(b) {}
+    template <class T> T* take(size_t n) {
+        off = (off + 255) / 256 * 256;
+        T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+        off += std::max<size_t>(n, 1) * sizeof(T);
+        return p;
+    }
+};
+
+// lays the workspace out for wc walkers at `level`; with base == nullptr only measures
+static size_t carve(const msd_ctx* c, Workspace& ws, char* base, int64_t wc, int level)
+{
+    Carver k(base);
+    const int N = c->N, ldN = N + (N & 1), ng = c->n_chol;
+    const int64_t nt = wc / MSD_WT;
+    // zero region first
+    char* z0 = base ? base : nullptr;
+    for (int s = 0; s < 2; s++) ws.C[s] = k.take<cplx>((size_t)nt * c->sp[s].P * MSD_WT);
+    ws.Wacc = k.take<cplx>(wc);
+    ws.E2nd = k.take<cplx>(wc);
+    ws.wflags = k.take<int>(wc);
+    if (level >= 3) {
+        for (int s = 0; s < 2; s++) ws.F[s] = k.take<cplx>((size_t)wc * c->sp[s].P);
+        ws.Eacc = k.take<cplx>((size_t)wc * 2);
+    }
+    if (level >= 3) ws.X0 = k.take<cplx>((size_t)2 * wc * ng);   // zero for a spin without electrons
+    k.off = (k.off + 255) / 256 * 256;
+    ws.zero_begin = z0;
+    ws.zero_bytes = k.off;
+    for (int s = 0; s < 2; s++) {
+        ws.theta[s] = k.take<cplx>((size_t)wc * N * c->sp[s].n);
+        ws.g[s] = k.take<cplx>((size_t)nt * c->sp[s].P * MSD_WT);
+    }
+    ws.det0 = k.take<cplx>((size_t)wc * 2);
+    if (level == 2) {
+        for (int s = 0; s < 2; s++) ws.Gp[s] = k.take<double>((size_t)wc * 2 * c->sp[s].n_r * ldN);
+    }
+    if (level >= 3) {
+        for (int s = 0; s < 2; s++) {
+            const auto& sp = c->sp[s];
+            ws.thetaT[s] = k.take<double>((size_t)wc * sp.n * 2 * ldN);
+            ws.Lam[s] = k.take<cplx>((size_t)(ng + 1) * sp.n_r * wc * sp.n);
+            ws.Bp[s] = k.take<cplx>((size_t)wc * sp.P * ng);
+            ws.Bq[s] = k.take<double>((size_t)wc * 2 * sp.P * 2 * ng);
+            ws.Vss[s] = k.take<cplx>((size_t)nt * sp.P * sp.P * MSD_WT);
+            ws.Hrot[s] = k.take<cplx>((size_t)wc * sp.P);
+        }
+        ws.Vab = k.take<cplx>((size_t)nt * c->sp[0].P * c->sp[1].P * MSD_WT);
+    }
+    return k.off + 256;
+}
+
+// level: 1 overlap, 2 force bias / greens, 3 energy.  A separate workspace layout per level (the buffers differ);
+// reallocated only when the level or the walker capacity changes.
+static int ensure_workspace(msd_ctx* c, int level, int64_t nw, std::string* errp)
+{
+    int64_t want = (nw + MSD_WT - 1) / MSD_WT * MSD_WT;
+    if (want == 0) want = MSD_WT;
+    Workspace& ws = c->ws;
+    if (ws.base && ws.level == level && ws.want == want) return MSD_OK;     // fast path: no CUDA call at all
+    int64_t limit = c->ws_limit;
+    if (limit == 0) {
+        if (c->ws_limit_auto == 0) {
+            size_t fr = 0, tot = 0;
+            CK(cudaMemGetInfo(&fr, &tot));
+            c->ws_limit_auto = (int64_t)((fr + ws.bytes) * 0.7);
+        }
+        limit = c->ws_limit_auto;
+    }
+    Workspace probe;
+    int64_t wc = want;
+    while (wc > MSD_WT && (int64_t)carve(c, probe, nullptr, wc, level) > limit) wc = (wc / 2 + MSD_WT - 1) / MSD_WT * MSD_WT;
+    size_t need = carve(c, probe, nullptr, wc, level);
+    if ((int64_t)need > limit) return fail(errp, MSD_ENOMEM, "workspace for one walker tile exceeds the limit");
+    if (ws.base && ws.bytes >= need) {
+        // re-carve inside the existing allocation
+        ws.level = level; ws.wc = wc; ws.want = want;
+        carve(c, ws, ws.base, wc, level);
+        return MSD_OK;
+    }
+    if (ws.base) { CK(cudaDeviceSynchronize()); cudaFree(ws.base); ws.base = nullptr; ws.bytes = 0; }
+    char* p = nullptr;
+    CK(cudaMalloc(&p, need));
+    ws.base = p; ws.bytes = need; ws.level = level; ws.wc = wc; ws.want = want;
+    carve(c, ws, ws.base, wc, level);
+    return MSD_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// hot calls
+// ---------------------------------------------------------------------------------------------
+enum { CALL_OVERLAP = 1, CALL_FB = 2, CALL_GREENS = 4, CALL_ENERGY = 8 };
+
+static void mark(msd_ctx* c, int i, cudaStream_t st) { if (c->profiling) cudaEventRecord(c->ev[i], st); }
+
+static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, const cplx* phi_a, const cplx* phi_b,
+                      cplx* out, int* flags, cudaStream_t st)
+{
+    const int level = (call == CALL_OVERLAP) ? 1 : (call == CALL_ENERGY ? 3 : 2);
+    if (call == CALL_ENERGY && std::max(c->sp[0].P, c->sp[1].P) > 4096)
+        return fail(errp, MSD_EUNSUPPORTED, "local energy requires n_o*n_v <= 4096 per spin");
+    int rc = ensure_workspace(c, level, n_w, errp);
+    if (rc != MSD_OK) return rc;
+    Workspace& ws = c->ws;
+    const int N = c->N, ldN = N + (N & 1), ng = c->n_chol;
+    for (int i = 0; i < 6; i++) c->phase_ms[i] = 0.f;
+    for (int64_t w0 = 0; w0 < n_w; w0 += ws.wc) {
+        const int64_t nw = std::min<int64_t>(ws.wc, n_w - w0);
+        const cplx* pa = phi_a + w0 * (int64_t)N * c->sp[0].n;
+        const cplx* pb = phi_b + w0 * (int64_t)N * c->sp[1].n;
+        int* fl = flags ? flags + w0 : nullptr;
+        CK(cudaMemsetAsync(ws.zero_begin, 0, ws.zero_bytes, st));
+        mark(c, 0, st);
+        CK(launch_reference(N, ldN, c->dev(0), c->dev(1), nw, pa, pb, ws, level >= 3, st));
+        c->launches++;
+        mark(c, 1, st);
+        if (call == CALL_OVERLAP) {
+            CK(launch_dets(c, 0, nw, ws, st));
+            mark(c, 2, st);
+            CK(launch_finish_overlap(c, nw, ws, out + w0, fl, st));
+            mark(c, 3, st); mark(c, 4, st); mark(c, 5, st);
+        } else if (call == CALL_FB || call == CALL_GREENS) {
+            CK(launch_dets(c, 1, nw, ws, st));
+            mark(c, 2, st);
+            if (call == CALL_GREENS) {
+                cplx* G = out + w0 * (int64_t)2 * N * N;
+                CK(cudaMemsetAsync(G, 0, sizeof(cplx) * (size_t)nw * 2 * N * N, st));
+                double* keep[2] = {ws.Gp[0], ws.Gp[1]};
+                ws.Gp[0] = ws.Gp[1] = nullptr;
+                cudaError_t e = launch_green_rows(c, nw, ws, G, st);
+                ws.Gp[0] = keep[0]; ws.Gp[1] = keep[1];
+                CK(e);
+                mark(c, 3, st);
+                CK(launch_finish_flags(c, nw, ws, G, (int64_t)2 * N * N, fl, st));
+            } else {
+                CK(launch_green_rows(c, nw, ws, nullptr, st));
+                cplx* fb = out + w0 * (int64_t)ng;
+                CK(cudaMemsetAsync(fb, 0, sizeof(cplx) * (size_t)nw * ng, st));
+                for (int s = 0; s < 2; s++) {
+                    const auto& sp = c->sp[s];
+                    if (sp.n_r == 0) continue;
+                    GemmArgs a;
+                    a.A = sp.d_Lsub; a.B = ws.Gp[s]; a.C = reinterpret_cast<double*>(fb);
+                    a.M = ng; a.N = (int)(2 * nw); a.K = sp.n_r * ldN;
+                    a.lda = (int64_t)sp.n_r * ldN; a.ldb = (int64_t)sp.n_r * ldN;
+                    a.strideA = 0; a.strideB = 0; a.batch = 1;
+                    a.zdiv = 1; a.strideC_hi = 0; a.strideC_lo = 0; a.cs_m = 1; a.cs_j = ng;
+                    a.accumulate = 1;
+                    CK(launch_gemm_tn(a, c->n_sm, st));
+                    c->launches++;
+                }
+                mark(c, 3, st);
+                CK(launch_finish_flags(c, nw, ws, fb, ng, fl, st));
+            }
+            mark(c, 4, st); mark(c, 5, st);
+        } else {   // energy
+            // Lambda = L_sub Theta for every slice (incl. h1), both spins
+            for (int s = 0; s < 2; s++) {
+                const auto& sp = c->sp[s];
+                if (sp.n == 0 || sp.n_r == 0) continue;
+                GemmArgs a;
+                a.A = sp.d_Lsub; a.B = ws.thetaT[s]; a.C = reinterpret_cast<double*>(ws.Lam[s]);
+                a.M = (ng + 1) * sp.n_r; a.N = (int)(2 * sp.n * nw); a.K = ldN;
+                a.lda = ldN; a.ldb = ldN; a.strideA = 0; a.strideB = 0; a.batch = 1;
+                a.zdiv = 1; a.strideC_hi = 0; a.strideC_lo = 0; a.cs_m = (int64_t)nw * sp.n; a.cs_j = 1;
+                a.accumulate = 0;
+                CK(launch_gemm_tn(a, c->n_sm, st));
+                c->launches++;
+            }
+            mark(c, 2, st);
+            CK(launch_energy_dense(c, nw, ws, st));
+            mark(c, 3, st);
+            // V GEMMs: ab, aa, bb
+            for (int pr = 0; pr < 3; pr++) {
+                const int s1 = (pr == 2) ? 1 : 0, s2 = (pr == 0) ? 1 : s1;
+                const auto& A_ = c->sp[s1]; const auto& B_ = c->sp[s2];
+                if (A_.P == 0 || B_.P == 0) continue;
+                if (pr > 0 && A_.kmax < 2) continue;          // same-spin V only feeds levels >= 2
+                GemmArgs a;
+                a.A = reinterpret_cast<const double*>(ws.Bp[s1]); a.B = ws.Bq[s2];
+                a.C = reinterpret_cast<double*>(pr == 0 ? ws.Vab : ws.Vss[s1]);
+                a.M = A_.P; a.N = 2 * B_.P; a.K = 2 * ng;
+                a.lda = 2 * ng; a.ldb = 2 * ng;
+                a.strideA = (int64_t)A_.P * 2 * ng; a.strideB = (int64_t)2 * B_.P * 2 * ng; a.batch = (int)nw;
+                a.zdiv = MSD_WT; a.strideC_hi = (int64_t)A_.P * B_.P * MSD_WT; a.strideC_lo = 1;
+                a.cs_m = (int64_t)B_.P * MSD_WT; a.cs_j = MSD_WT;
+                a.accumulate = 0;
+                CK(launch_gemm_tn(a, c->n_sm, st));
+                c->launches++;
+            }
+            mark(c, 4, st);
+            CK(launch_dets(c, 2, nw, ws, st));
+            mark(c, 5, st);
+            CK(launch_finish_energy(c, nw, ws, out + w0 * 3, fl, st));
+        }
+        if (c->profiling) {
+            cudaEventRecord(c->ev[6], st);
+            CK(cudaEventSynchronize(c->ev[6]));
+            for (int i = 0; i < 6; i++) {
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 1]);
+                c->phase_ms[i] += ms;
+            }
+        }
+    }
+    return MSD_OK;
+}
+
+static int hot_call(msd_ctx* c, int call, int64_t n_w, const void* phi_a, const void* phi_b, void* out, int32_t* flags,
+                    void* stream)
+{
+    if (!c) return MSD_EINVAL;
+    if (n_w < 0 || (n_w > 0 && (!out || (c->sp[0].n > 0 && !phi_a) || (c->sp[1].n > 0 && !phi_b)))) {
+        c->err = "bad argument";
+        return MSD_EINVAL;
+    }
+    if (n_w == 0) return MSD_OK;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != c->device) { c->err = "context used on another device"; return MSD_EINVAL; }
+    std::string err;
+    int rc = run_chunks(c, &err, call, n_w, (const cplx*)phi_a, (const cplx*)phi_b, (cplx*)out, flags, (cudaStream_t)stream);
+    if (rc != MSD_OK) { c->err = err; cudaGetLastError(); }
+    return rc;
+}
+
+extern "C" int msd_overlap(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* ovlp, int32_t* flags,
+                           void* stream)
+{ return hot_call(c, CALL_OVERLAP, n_w, phi_a, phi_b, ovlp, flags, stream); }
+
+extern "C" int msd_force_bias(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* fb, int32_t* flags,
+                              void* stream)
+{ return hot_call(c, CALL_FB, n_w, phi_a, phi_b, fb, flags, stream); }
+
+extern "C" int msd_local_energy(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* e, int32_t* flags,
+                                void* stream)
+{ return hot_call(c, CALL_ENERGY, n_w, phi_a, phi_b, e, flags, stream); }
+
+extern "C" int msd_greens(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* G, int32_t* flags,
+                          void* stream)
+{ return hot_call(c, CALL_GREENS, n_w, phi_a, phi_b, G, flags, stream); }

@@ -1,0 +1,193 @@
+// Internal declarations shared by the translation units of libmsd_b200.so.
+// Not part of the C ABI (include/msd.h).  sm_100a only.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#define MSD_WT 8            // walkers per tile: lanes of a warp = 4 determinants x 8 walkers
+#define MSD_MAX_LEVEL 16    // per-spin excitation level limit
+#define MSD_MAX_NOCC 64     // electrons per spin limit
+#define MSD_CF_MAX 4        // closed-form (register) minors up to this level; above: in-smem Gauss-Jordan
+
+typedef double2 cplx;
+
+__host__ __device__ __forceinline__ cplx cmake(double r, double i) { return make_double2(r, i); }
+__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ cplx csub(cplx a, cplx b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ cplx cneg(cplx a) { return make_double2(-a.x, -a.y); }
+__device__ __forceinline__ cplx cmul(cplx a, cplx b) {
+    return make_double2(fma(a.x, b.x, -a.y * b.y), fma(a.x, b.y, a.y * b.x));
+}
+__device__ __forceinline__ cplx cscale(double s, cplx a) { return make_double2(s * a.x, s * a.y); }
+// acc + a*b
+__device__ __forceinline__ cplx cfma(cplx a, cplx b, cplx acc) {
+    acc.x = fma(a.x, b.x, acc.x); acc.x = fma(-a.y, b.y, acc.x);
+    acc.y = fma(a.x, b.y, acc.y); acc.y = fma(a.y, b.x, acc.y);
+    return acc;
+}
+// acc - a*b
+__device__ __forceinline__ cplx cfms(cplx a, cplx b, cplx acc) {
+    acc.x = fma(-a.x, b.x, acc.x); acc.x = fma(a.y, b.y, acc.x);
+    acc.y = fma(-a.x, b.y, acc.y); acc.y = fma(-a.y, b.x, acc.y);
+    return acc;
+}
+__device__ __forceinline__ double cabs2(cplx a) { return a.x * a.x + a.y * a.y; }
+__device__ __forceinline__ cplx cinv(cplx a) {
+    // Smith-free: fine for the magnitudes here (no over/underflow guard needed for |a|^2 in range)
+    double d = 1.0 / cabs2(a);
+    return make_double2(a.x * d, -a.y * d);
+}
+__device__ __forceinline__ cplx cdiv(cplx a, cplx b) { return cmul(a, cinv(b)); }
+__device__ __forceinline__ void red_add(cplx* p, cplx v) {
+    atomicAdd(&p->x, v.x);
+    atomicAdd(&p->y, v.y);
+}
+
+// ---------------------------------------------------------------------------------------------
+// packed trial (device pointers live in the context; this POD is passed to kernels by value)
+// ---------------------------------------------------------------------------------------------
+struct SpinDev {
+    int n;                 // electrons of this spin
+    int n_o, n_v;          // active occupied / active virtual orbitals (reading A10)
+    int n_r;               // n + n_v : rows of L_sub
+    int P;                 // n_o * n_v pair indices  x = p_loc * n_o + h_loc
+    const int* occ_ref;    // [n]
+    const int* act_v;      // [n_v] orbital index of active virtual r'
+    const int* pos_o;      // [n_o] position in occ_ref of active occupied h_loc
+    const double* Lsub;    // [(n_chol+1)][n_r][N]; slice n_chol holds the same rows of h1
+};
+
+struct Bucket {            // one (k_alpha, k_beta) level pair: determinants [start, start+count) of the sorted list
+    int ka, kb;
+    int64_t start, count;
+    int64_t tab_off;       // byte offset of the bucket's rows in the table
+    int rs;                // row stride in bytes (multiple of 4): [hA(ka) pA(ka) hB(kb) pB(kb)] local indices, uint8
+};
+
+struct WorkItem {          // a chunk of one bucket, processed by one CTA per walker tile
+    int bucket;
+    int ka, kb, rs;
+    int64_t det_begin;     // in the sorted list
+    int det_count;
+    int64_t tab_off;       // byte offset of the chunk's first row
+};
+
+struct Workspace {
+    int64_t wc = 0;        // walker capacity of one chunk (multiple of MSD_WT)
+    int64_t want = 0;      // padded n_w the layout was made for
+    int level = 0;         // 1 overlap, 2 force bias/greens, 3 energy : which buffers exist
+    char* base = nullptr;  // one cudaMalloc
+    size_t bytes = 0;
+    // views
+    cplx* theta[2] = {nullptr, nullptr};      // [wc][N][n]
+    double* thetaT[2] = {nullptr, nullptr};   // [wc][n][2][N]  rows (w,i,c), K = N contiguous
+    cplx* det0 = nullptr;                     // [wc][2]
+    cplx* g[2] = {nullptr, nullptr};          // [nt][P][WT]
+    cplx* C[2] = {nullptr, nullptr};          // [nt][P][WT]      (zeroed every call)
+    cplx* Wacc = nullptr;                     // [wc]             (zeroed)
+    cplx* E2nd = nullptr;                     // [wc]             (zeroed)
+    int* wflags = nullptr;                    // [wc]
+    double* Gp[2] = {nullptr, nullptr};       // [wc][2][n_r*N]   planar rows (w,c)
+    cplx* Lam[2] = {nullptr, nullptr};        // [(n_chol+1)*n_r][wc][n]
+    cplx* Bp[2] = {nullptr, nullptr};         // [wc][P][n_chol]
+    double* Bq[2] = {nullptr, nullptr};       // [wc][2P][2 n_chol]
+    cplx* Vab = nullptr;                      // [nt][Pa][Pb][WT]
+    cplx* Vss[2] = {nullptr, nullptr};        // [nt][P][P][WT]
+    cplx* F[2] = {nullptr, nullptr};          // [wc][P]          (zeroed)
+    cplx* Hrot[2] = {nullptr, nullptr};       // [wc][P]
+    cplx* Eacc = nullptr;                     // [wc][2]: (E1_0, E2_0)  (zeroed)
+    cplx* X0 = nullptr;                       // [2][nw][n_chol] tr T^g per spin (zeroed)
+    char* zero_begin = nullptr;               // region memset to 0 at the start of every chunk
+    size_t zero_bytes = 0;
+};
+
+struct msd_ctx {
+    int device = 0;
+    int N = 0, n_chol = 0;
+    int64_t n_det = 0;
+    double e0 = 0.0;
+    int n_sm = 148;
+    struct SpinHost {
+        int n = 0, n_o = 0, n_v = 0, n_r = 0, P = 0, kmax = 0;
+        std::vector<int> occ_ref, act_o, act_v, pos_o;
+        int* d_occ_ref = nullptr; int* d_act_v = nullptr; int* d_pos_o = nullptr;
+        double* d_Lsub = nullptr;
+    } sp[2];
+    // packed determinant list
+    unsigned char* d_tab = nullptr;
+    double* d_coef = nullptr;
+    std::vector<Bucket> buckets;
+    std::vector<WorkItem> items_cf, items_gen;
+    WorkItem* d_items_cf = nullptr; WorkItem* d_items_gen = nullptr;
+    int gen_smem_per_thread = 0;              // bytes of shared memory per thread of the generic kernel
+    int gen_threads = 0;
+    // host copies for introspection
+    std::vector<int64_t> h_perm; std::vector<double> h_coef; std::vector<int> h_ka, h_kb;
+    Workspace ws;
+    int64_t ws_limit = 0;
+    int64_t ws_limit_auto = 0;
+    int64_t launches = 0;
+    bool profiling = false;
+    cudaEvent_t ev[8] = {};
+    float phase_ms[6] = {};
+    std::string err;
+    SpinDev dev(int s) const {
+        SpinDev d; d.n = sp[s].n; d.n_o = sp[s].n_o; d.n_v = sp[s].n_v; d.n_r = sp[s].n_r; d.P = sp[s].P;
+        d.occ_ref = sp[s].d_occ_ref; d.act_v = sp[s].d_act_v; d.pos_o = sp[s].d_pos_o; d.Lsub = sp[s].d_Lsub;
+        return d;
+    }
+};
+
+// ---------------------------------------------------------------------------------------------
+// launchers (each returns cudaGetLastError() after its launches and bumps *launches)
+// ---------------------------------------------------------------------------------------------
+// pack.cu
+cudaError_t launch_pack_mark(int64_t n_det, const int64_t* off, const int32_t* holes, const int32_t* parts, int N,
+                             const int* pos_in_ref, int* used_h, int* used_p, int* err, cudaStream_t st);
+cudaError_t launch_pack_rows(int64_t n_det, int N,
+                             const int64_t* off_a, const int32_t* holes_a, const int32_t* parts_a,
+                             const int64_t* off_b, const int32_t* holes_b, const int32_t* parts_b,
+                             const int* occ_ref_a, int na, const int* occ_ref_b, int nb,
+                             const int* pos_in_ref_a, const int* pos_in_ref_b,
+                             const int* map_h_a, const int* map_p_a, const int* map_h_b, const int* map_p_b,
+                             const double* ci, unsigned char* tmp_rows /*[n_det][64]*/, int* key, double* coef,
+                             int* hist /*[17*17]*/, int* err, cudaStream_t st);
+cudaError_t launch_pack_scatter(int64_t n_det, const int* key, int n_buckets, const int* bucket_keys,
+                                const int64_t* bucket_start, int64_t* perm, cudaStream_t st);
+cudaError_t launch_pack_write(int64_t n_det, const int64_t* perm, const int* key, const unsigned char* tmp_rows,
+                              const double* coef, int n_buckets, const Bucket* buckets, const int* bucket_of_key,
+                              unsigned char* tab, double* coef_sorted, cudaStream_t st);
+cudaError_t launch_pack_lsub(const double* L_or_h1, int n_slices, int N, int n_r, const int* rows,
+                             double* out, cudaStream_t st);
+
+// reference.cu
+cudaError_t launch_reference(int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw,
+                             const cplx* phi_a, const cplx* phi_b, Workspace& ws, bool want_thetaT, cudaStream_t st);
+
+// dets.cu   mode: 0 overlap, 1 + CI matrix, 2 + second-order energy
+cudaError_t launch_dets(msd_ctx* c, int mode, int64_t nw, Workspace& ws, cudaStream_t st);
+
+// dense.cu
+cudaError_t launch_green_rows(msd_ctx* c, int64_t nw, Workspace& ws, cplx* Gfull /*or null*/, cudaStream_t st);
+cudaError_t launch_energy_dense(msd_ctx* c, int64_t nw, Workspace& ws, cudaStream_t st);
+cudaError_t launch_finish_overlap(msd_ctx* c, int64_t nw, Workspace& ws, cplx* ovlp, int* flags, cudaStream_t st);
+cudaError_t launch_finish_energy(msd_ctx* c, int64_t nw, Workspace& ws, cplx* e, int* flags, cudaStream_t st);
+cudaError_t launch_finish_flags(msd_ctx* c, int64_t nw, Workspace& ws, cplx* out, int64_t per_walker, int* flags,
+                                cudaStream_t st);
+
+// gemm.cu : C[m][n] (+)= sum_k A[m][k] * B[n][k]   (both K-contiguous, FP64 DMMA m8n8k4)
+struct GemmArgs {
+    const double* A; const double* B; double* C;
+    int M, N, K;
+    int64_t lda, ldb;           // row strides (doubles)
+    int64_t strideA, strideB;   // per-batch strides (doubles); 0 = shared operand
+    int batch;
+    // output addressing: column pair (2j, 2j+1) of row m is one complex at
+    //   C + 2*( (z / zdiv)*strideC_hi + (z % zdiv)*strideC_lo + m*cs_m + j*cs_j )   [complex units inside]
+    int zdiv; int64_t strideC_hi, strideC_lo, cs_m, cs_j;
+    int accumulate;             // 1: C += result
+};
+cudaError_t launch_gemm_tn(const GemmArgs& a, int n_sm, cudaStream_t st);
+double probe_fp64(int use_dmma, double ms, cudaStream_t st);
