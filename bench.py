@@ -1,0 +1,326 @@
+#!/usr/bin/env python
+"""bench.py -- walker x determinant local-energy + force-bias evaluations per second (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path over one walker batch: msd_force_bias + msd_local_energy
+(S1-S9 of SURVEY.md 8(a)) on synthetic inputs shaped like the paper's Fe2S2 workload (BASELINE.json configs[3],
+the largest fully specified single-GPU config; stands in for PAPER.md:L315, whose integrals are unavailable).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config fe2s2] [--impl ours|reference]
+
+N > 1 (torchrun): replicas only -- walkers are independent, every rank holds the trial and its
+own walker batch (seed + rank), no data-path collective; value = units of all ranks / max-over-ranks time.
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "walker x determinant local-energy + force-bias evaluations per second"
+UNIT = "walker*det/s"
+FP64_PEAK_DERIVED = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 FP64 FMA/clk x 2 flop x 1.965 GHz = 37.2 TF
+
+
+def shard_info(n_gpus: int):
+    """(rank, world, local_rank) from the torchrun environment; (0, 1, 0) when run as a plain script."""
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != max(1, n_gpus) and world > 1:
+        raise SystemExit("WORLD_SIZE %d does not match --gpus %d" % (world, n_gpus))
+    return rank, world, local
+
+
+def reduce_max_time(ms: float, world: int, device=None) -> float:
+    """max over ranks of a per-rank duration (the job is as slow as its slowest replica)."""
+    if world == 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def total_units(n_w: int, n_det: int, steps: int, world: int) -> float:
+    return float(n_w) * float(n_det) * steps * world
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        def pump():
+            for line in self.proc.stdout:
+                self.rows.append(line.strip())
+        self.thread = threading.Thread(target=pump, daemon=True)
+        self.thread.start()
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [t.strip() for t in r.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def cpu_oracle_sample(inp, n_det_sample: int, steps: int = 1, warmup: int = 0):
+    """The oracle as it stands (tier O2, oracle/o2.c) on walker 0 and the first n_det_sample determinants
+    (force bias + local energy).  Returns (walker*det/s, seconds per step, threads)."""
+    from oracle import o2
+    sub = inp.subset_dets(np.arange(min(n_det_sample, inp.n_det)))
+    for _ in range(warmup):
+        o2.run(sub, walkers=[0], return_G=False)
+    ts = []
+    for _ in range(steps):
+        t = time.perf_counter()
+        o2.run(sub, walkers=[0], return_G=False)
+        ts.append(time.perf_counter() - t)
+    sec = sum(ts) / len(ts)
+    return sub.n_det / sec, sec, o2.threads()
+
+
+def run_reference(args, rank):
+    """--impl reference: the CPU oracle, timed on the host cores on a bounded sample of the same workload."""
+    if rank != 0:
+        return
+    import msd_inputs as mi
+    inp = mi.generate(args.config)
+    nsamp = args.oracle_dets
+    thr, sec, cores = cpu_oracle_sample(inp, nsamp, steps=args.steps, warmup=min(args.warmup, 1))
+    sample = "walker 0 x first %d of %d determinants of '%s' per step (force bias + local energy, tier O2)" % (
+        min(nsamp, inp.n_det), inp.n_det, args.config)
+    line = {"impl": "reference", "metric": METRIC, "value": thr, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64 (complex128)", "data": "synthetic",
+            "config": {"workload": args.config, "N": inp.N, "n_alpha": inp.n_alpha, "n_beta": inp.n_beta,
+                       "n_chol": inp.n_chol, "n_det": inp.n_det, "n_w": inp.n_w, "sample": sample},
+            "cpu_baseline": {"value": thr, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": thr, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="fe2s2")
+    ap.add_argument("--oracle-dets", type=int, default=4000, help="determinants in the CPU-oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank, world, local = shard_info(args.gpus)
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    if args.warmup < 3:
+        args.warmup = 3
+
+    import torch
+    import msd_inputs as mi
+    import paper_2406_08314_b200 as msd
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    inp = mi.generate(args.config)
+    if rank > 0:   # replicas: same trial, a different walker batch per rank
+        rng = np.random.default_rng(inp.params["seed"] + 7919 * rank)
+        inp = inp.with_walkers(mi.walkers_from_rng(rng, inp.n_w, inp.N, inp.n_alpha),
+                               mi.walkers_from_rng(rng, inp.n_w, inp.N, inp.n_beta))
+    trial = msd.setup_from_inputs(inp)
+    info = trial.info()
+    stream = torch.cuda.current_stream()
+    h_a = torch.from_numpy(inp.phi_a).pin_memory()
+    h_b = torch.from_numpy(inp.phi_b).pin_memory()
+    d_a = h_a.to(dev)
+    d_b = h_b.to(dev)
+    fb = torch.empty((inp.n_w, inp.n_chol), dtype=torch.complex128, device=dev)
+    en = torch.empty((inp.n_w, 3), dtype=torch.complex128, device=dev)
+    h_fb = torch.empty((inp.n_w, inp.n_chol), dtype=torch.complex128).pin_memory()
+    h_en = torch.empty((inp.n_w, 3), dtype=torch.complex128).pin_memory()
+    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)   # > 126 MB L2
+
+    def step():
+        trial.force_bias(d_a, d_b, out=fb)
+        trial.local_energy(d_a, d_b, out=en)
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    # ---- timed region: K steps, CUDA events on the launching stream, L2 flushed between steps ----
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = trial.launch_count()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    for a, b in evs:
+        flush.zero_()
+        a.record(stream)
+        step()
+        b.record(stream)
+    barrier()
+    launches = trial.launch_count() - l0
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in evs]
+    total_ms = reduce_max_time(sum(step_ms), world, dev)
+    value = total_units(inp.n_w, inp.n_det, args.steps, world) / (total_ms * 1e-3)
+
+    # ---- end to end: host buffers, H2D + both calls + D2H inside the timed region ----
+    def e2e_step():
+        d_a.copy_(h_a, non_blocking=True)
+        d_b.copy_(h_b, non_blocking=True)
+        step()
+        h_fb.copy_(fb, non_blocking=True)
+        h_en.copy_(en, non_blocking=True)
+
+    e2e_step()
+    barrier()
+    ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n_e2e = max(3, min(args.steps, 10))
+    ea.record(stream)
+    for _ in range(n_e2e):
+        e2e_step()
+    eb.record(stream)
+    barrier()
+    e2e_ms = reduce_max_time(ea.elapsed_time(eb), world, dev)
+    e2e_val = total_units(inp.n_w, inp.n_det, n_e2e, world) / (e2e_ms * 1e-3)
+    h2d = h_a.numel() * 16 + h_b.numel() * 16
+    d2h = h_fb.numel() * 16 + h_en.numel() * 16
+
+    # ---- roofline of the dominant kernel (phase timings from CUDA events inside the library, same stream) ----
+    roofline = None
+    phases = None
+    if rank == 0:
+        peak = msd.msd_probe_fp64_tflops(True, 30.0)
+        trial.set_profiling(True)
+        acc = {}
+        reps = 3
+        for _ in range(reps):
+            flush.zero_()
+            trial.local_energy(d_a, d_b, out=en)
+            for k, v in trial.phase_ms().items():
+                acc[k] = acc.get(k, 0.0) + v / reps
+        fbacc = {}
+        for _ in range(reps):
+            flush.zero_()
+            trial.force_bias(d_a, d_b, out=fb)
+            for k, v in trial.phase_ms().items():
+                fbacc[k] = fbacc.get(k, 0.0) + v / reps
+        trial.set_profiling(False)
+        Pa = info["n_o_alpha"] * info["n_v_alpha"]
+        Pb = info["n_o_beta"] * info["n_v_beta"]
+        nr_a = inp.n_alpha + info["n_v_alpha"]
+        nr_b = inp.n_beta + info["n_v_beta"]
+        ng, nw, N = inp.n_chol, inp.n_w, inp.N
+        flops_v = 8.0 * ng * nw * (Pa * Pb + Pa * Pa + Pb * Pb)               # complex MAC = 8 flops
+        flops_lam = 4.0 * (ng + 1) * N * nw * (nr_a * inp.n_alpha + nr_b * inp.n_beta)   # real x complex MAC = 4
+        phases = {"energy_ms": {"reference": acc["reference"], "lambda_gemm": acc["p1"], "energy_dense": acc["p2"],
+                                "v_gemm": acc["p3"], "dets": acc["p4"], "assemble": acc["p5"]},
+                  "force_bias_ms": {"reference": fbacc["reference"], "dets": fbacc["p1"], "greens_fb_gemm": fbacc["p2"]}}
+        # dominant DMMA kernel: k_gemm_tn (V and Lambda launches); algorithmic flops / measured duration
+        gemm_ms = acc["p3"] + acc["p1"]
+        achieved = (flops_v + flops_lam) / (gemm_ms * 1e-3) / 1e12
+        roofline = {"kernel": "k_gemm_tn (FP64 DMMA: V and Lambda contractions, %d launches per step)" % 5,
+                    "bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                    "frac": achieved / peak if peak > 0 else None,
+                    "peak_source": "measured live: register-resident DMMA m8n8k4 loop (msd_probe_fp64_tflops); "
+                                   "MEASURED_PEAKS.json has no FP64 entry; derived 148 SM x 64 FMA/clk x 1.965 GHz = %.1f"
+                                   % FP64_PEAK_DERIVED,
+                    "traffic": None,
+                    "share_of_step": gemm_ms / (sum(step_ms) / len(step_ms)),
+                    "algorithmic_flops_per_step": flops_v + flops_lam}
+
+    if rank != 0:
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+
+    cpu_baseline = None
+    if not args.no_cpu_baseline:
+        thr, sec, cores = cpu_oracle_sample(inp, args.oracle_dets)
+        cpu_baseline = {"value": thr, "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "sample": "walker 0 x first %d of %d determinants (force bias + local energy, tier O2), %.1f s"
+                                  % (min(args.oracle_dets, inp.n_det), inp.n_det, sec)}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64 (complex128)", "data": "synthetic",
+            "config": {"workload": args.config, "N": inp.N, "n_alpha": inp.n_alpha, "n_beta": inp.n_beta,
+                       "n_chol": inp.n_chol, "n_det": inp.n_det, "n_w": inp.n_w, "active_window": info,
+                       "step": "msd_force_bias + msd_local_energy", "l2": "flushed between timed steps (256 MB write)",
+                       "parallelism": "replicas x%d" % world, "input_sha256": inp.sha256()[:16]},
+            "clocks": clocks,
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": n_e2e},
+            "gpu_launches": int(launches),
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "phases": phases,
+            "step_ms": {"min": min(step_ms), "median": statistics.median(step_ms), "max": max(step_ms)}}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

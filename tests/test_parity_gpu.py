@@ -1,0 +1,394 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on identical seeded inputs.
+
+Tolerances (BASELINE.json north_star; norms per DESIGN.md reading A13), written here:
+    overlap      |d| / |ovlp|                      <= 1e-10
+    force bias   max_g |d fb| / max_g |fb|  per walker <= 1e-10
+    Green's fn   max |dG| / max |G|          per walker <= 1e-10
+    energies     |dE|, |dE1|, |dE2|                <= 1e-8 Ha
+Summation order differs (atomics, reading A12), so nothing here is bit-exact by construction.
+"""
+import itertools
+import json
+import os
+
+import numpy as np
+import pytest
+
+import msd_inputs as mi
+from oracle import msd_oracle as mo
+from oracle import o2
+
+pytestmark = pytest.mark.gpu
+
+TOL_REL = 1e-10
+TOL_E = 1e-8
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    torch.cuda.set_device(0)
+    return torch
+
+
+def _msd():
+    import paper_2406_08314_b200 as msd
+    return msd
+
+
+def gpu_all(torch, x, trial=None, want_G=True):
+    msd = _msd()
+    own = trial is None
+    trial = msd.setup_from_inputs(x) if own else trial
+    pa = torch.tensor(x.phi_a, device="cuda")
+    pb = torch.tensor(x.phi_b, device="cuda")
+    fl = torch.full((x.n_w,), -1, dtype=torch.int32, device="cuda")
+    out = dict(ovlp=trial.overlap(pa, pb, flags=fl).cpu().numpy(),
+               fb=trial.force_bias(pa, pb).cpu().numpy(),
+               E=trial.local_energy(pa, pb).cpu().numpy())
+    if want_G:
+        out["G"] = trial.greens(pa, pb).cpu().numpy()
+    out["flags"] = fl.cpu().numpy()
+    torch.cuda.synchronize()
+    if own:
+        trial.close()
+    return out
+
+
+def assert_parity(got, ref, walkers=None, what=("ovlp", "fb", "E", "G")):
+    ws = np.arange(len(ref["ovlp"])) if walkers is None else np.asarray(walkers)
+    if "ovlp" in what:
+        err = np.abs(got["ovlp"][ws] - ref["ovlp"]) / np.abs(ref["ovlp"])
+        assert err.max() <= TOL_REL, "overlap rel err %.3e" % err.max()
+    if "fb" in what:
+        err = np.abs(got["fb"][ws] - ref["fb"]).max(axis=1) / np.abs(ref["fb"]).max(axis=1)
+        assert err.max() <= TOL_REL, "force bias rel err %.3e" % err.max()
+    if "E" in what:
+        err = np.abs(got["E"][ws] - ref["E"])
+        assert err.max() <= TOL_E, "energy abs err %.3e Ha" % err.max()
+    if "G" in what and "G" in ref and "G" in got:
+        err = np.abs(got["G"][ws] - ref["G"]).max(axis=(1, 2, 3)) / np.abs(ref["G"]).max(axis=(1, 2, 3))
+        assert err.max() <= TOL_REL, "greens rel err %.3e" % err.max()
+
+
+# ----------------------------------------------------------------------------------------------
+# element-by-element parity at sizes the oracle finishes in seconds (several tiles + ragged tails)
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["micro", "micro-cs", "tiny", "tiny-full", "open-shell", "small"])
+def test_parity_all_walkers(torch_cuda, name):
+    x = mi.generate(name)
+    got = gpu_all(torch_cuda, x)
+    ref = o2.run(x)
+    assert (got["flags"] == 0).all()
+    assert_parity(got, ref)
+
+
+def test_parity_tiny_against_o0_and_o1(torch_cuda):
+    """BASELINE configs[0] against the two numpy tiers as well (no inverse in O0)."""
+    x = mi.generate("tiny")
+    got = gpu_all(torch_cuda, x)
+    assert_parity(got, mo.run(x, "o1"))
+    assert_parity(got, mo.run(x, "o0", walkers=[0, 3, 7]), walkers=[0, 3, 7])
+
+
+@pytest.mark.parametrize("K", [1, 3, 6, 10])
+def test_parity_sweep_points(torch_cuda, K):
+    """BASELINE configs[4] (kernel sweep) at n_det = 1500: closed-form levels, the level-4/5 boundary and the
+    in-shared-memory Gauss-Jordan path up to 10-fold excitations."""
+    x = mi.generate("sweep", n_det=1500 if K > 1 else 300, max_level=K)
+    got = gpu_all(torch_cuda, x, want_G=False)
+    ws = [0, 7, 8, 63, 127]
+    assert_parity(got, o2.run(x, walkers=ws, return_G=False), walkers=ws)
+    assert_parity(got, o2.run(x, want=("ovlp",)), what=("ovlp",))
+
+
+def test_parity_cu2o2_full_size(torch_cuda):
+    """BASELINE configs[2] at full size, full batch on the GPU; oracle on sampled walkers (first, last, tile
+    boundaries 7|8 and 63|64) for energy and force bias, on every walker for the overlap."""
+    x = mi.generate("cu2o2")
+    got = gpu_all(torch_cuda, x, want_G=False)
+    assert (got["flags"] == 0).all()
+    ws = [0, 7, 8, 64, 199]
+    assert_parity(got, o2.run(x, walkers=ws, return_G=False), walkers=ws)
+    assert_parity(got, o2.run(x, want=("ovlp",)), what=("ovlp",))
+    ws2 = list(range(16, 32))
+    assert_parity(got, o2.run(x, walkers=ws2, want=("ovlp", "greens"), return_G=False), walkers=ws2, what=("ovlp", "fb"))
+
+
+@pytest.mark.parametrize("name", ["fe2s2", "cu2o2"])
+def test_parity_full_size_against_stored_oracle_values(torch_cuda, name):
+    """BASELINE configs[3] (the bench workload, same launch configuration) and configs[2] against oracle values
+    stored by tests/golden/make_golden.py (which calls only oracle/): the brute-force oracle needs ~10 minutes per
+    walker at the Fe2S2 size."""
+    path = os.path.join(GOLDEN, "%s_seed0.json" % name)
+    if not os.path.exists(path):
+        pytest.skip("golden file %s not generated yet" % path)
+    gold = json.load(open(path))
+    x = mi.generate(name)
+    msd = _msd()
+    torch = torch_cuda
+    trial = msd.setup_from_inputs(x)
+    pa = torch.tensor(x.phi_a, device="cuda")
+    pb = torch.tensor(x.phi_b, device="cuda")
+    ov = trial.overlap(pa, pb).cpu().numpy()
+    fb = trial.force_bias(pa, pb).cpu().numpy()
+    E = trial.local_energy(pa, pb).cpu().numpy()
+    trial.close()
+    ws = gold["walkers"]
+    c = lambda a: np.array(a)[..., 0] + 1j * np.array(a)[..., 1]
+    g_ov, g_E, g_fb = c(gold["ovlp"]), c(gold["E"]), c(gold["fb"])
+    gs = gold["fb_gamma_sample"]
+    assert (np.abs(ov[ws] - g_ov) / np.abs(g_ov)).max() <= TOL_REL
+    assert np.abs(E[ws] - g_E).max() <= TOL_E
+    fb_err = np.abs(fb[ws][:, gs] - g_fb).max(axis=1) / np.array(gold["fb_max_abs"])
+    assert fb_err.max() <= TOL_REL
+    if name == "fe2s2":   # overlap of a further walker sample, oracle run live (cheap: no L loop)
+        ws2 = [1, 8, 50, 98]
+        r = o2.run(x, walkers=ws2, want=("ovlp",))
+        assert (np.abs(ov[ws2] - r["ovlp"]) / np.abs(r["ovlp"])).max() <= TOL_REL
+
+
+# ----------------------------------------------------------------------------------------------
+# edge and degenerate cases
+# ----------------------------------------------------------------------------------------------
+def test_empty_and_ragged_batches(torch_cuda):
+    torch = torch_cuda
+    msd = _msd()
+    x = mi.generate("small", n_w=21)
+    trial = msd.setup_from_inputs(x)
+    pa = torch.tensor(x.phi_a, device="cuda")
+    pb = torch.tensor(x.phi_b, device="cuda")
+    assert trial.overlap(pa[:0], pb[:0]).shape == (0,)
+    assert trial.local_energy(pa[:0], pb[:0]).shape == (0, 3)
+    ref = o2.run(x, return_G=False)
+    for nw in (1, 5, 8, 9, 21):
+        got = dict(ovlp=trial.overlap(pa[:nw].contiguous(), pb[:nw].contiguous()).cpu().numpy(),
+                   fb=trial.force_bias(pa[:nw].contiguous(), pb[:nw].contiguous()).cpu().numpy(),
+                   E=trial.local_energy(pa[:nw].contiguous(), pb[:nw].contiguous()).cpu().numpy())
+        sub = {k: ref[k][:nw] for k in ("ovlp", "fb", "E")}
+        assert_parity(got, sub, what=("ovlp", "fb", "E"))
+    trial.close()
+
+
+def test_single_determinant_trial(torch_cuda):
+    """P1/P2: the MSD path with one determinant is SD-AFQMC (Eq. 13-14)."""
+    x = mi.generate("small", n_w=9).subset_dets([0])
+    x.ci[:] = 1.0
+    got = gpu_all(torch_cuda, x)
+    assert_parity(got, o2.run(x))
+    d = np.array([np.linalg.det(x.phi_a[w][:8]) * np.linalg.det(x.phi_b[w][:8]) for w in range(x.n_w)])
+    assert (np.abs(got["ovlp"] - d) / np.abs(d)).max() < 1e-12
+
+
+def _reference_walkers(x, n_w):
+    pa = np.zeros((n_w, x.N, x.n_alpha), complex)
+    pb = np.zeros((n_w, x.N, x.n_beta), complex)
+    pa[:, x.occ_ref_a, np.arange(x.n_alpha)] = 1.0
+    pb[:, x.occ_ref_b, np.arange(x.n_beta)] = 1.0
+    return x.with_walkers(pa, pb)
+
+
+@pytest.mark.parametrize("name", ["micro-cs", "tiny", "open-shell"])
+def test_walker_equals_reference_exact_singular_minors(torch_cuda, name):
+    """P7: psi = D_0 makes every minor exactly singular (g = 0); only division-free cofactors survive.
+    Oracle: O0 (determinants only; O1/O2 cannot invert O_I here)."""
+    x = _reference_walkers(mi.generate(name), 3)
+    got = gpu_all(torch_cuda, x)
+    ref = mo.run(x, "o0", walkers=[0])
+    assert (got["flags"] == 0).all()
+    for w in range(3):
+        assert abs(got["ovlp"][w] - x.ci[0]) <= 1e-15
+        assert np.abs(got["E"][w] - ref["E"][0]).max() <= TOL_E
+        assert np.abs(got["fb"][w] - ref["fb"][0]).max() <= TOL_REL * np.abs(ref["fb"][0]).max()
+        assert np.abs(got["G"][w] - ref["G"][0]).max() <= TOL_REL
+
+
+@pytest.mark.parametrize("eps", [1e-1, 1e-3, 1e-6])
+def test_near_reference_walkers(torch_cuda, eps):
+    """P8: psi = QR(D_0 + eps Z): the regime of real AFQMC walkers; stresses det*inverse cofactors at high levels."""
+    x = mi.generate("sweep", n_det=600, max_level=6, n_w=10)
+    pa, pb = mi.near_reference_walkers(x, eps, seed=4)
+    x = x.with_walkers(pa, pb)
+    got = gpu_all(torch_cuda, x, want_G=False)
+    assert_parity(got, o2.run(x, return_G=False), what=("ovlp", "fb", "E"))
+
+
+def test_singular_reference_and_zero_overlap_are_flagged(torch_cuda):
+    torch = torch_cuda
+    msd = _msd()
+    x = mi.generate("tiny")
+    pa = x.phi_a.copy()
+    pa[2][x.occ_ref_a, :] = 0.0                      # walker 2: psi[occ_ref,:] = 0 -> det O0 = 0
+    y = x.with_walkers(pa, x.phi_b)
+    got = gpu_all(torch, y)
+    assert got["flags"][2] & 1 and (np.delete(got["flags"], 2) == 0).all()
+    assert np.isnan(got["ovlp"][2]) and np.isnan(got["E"][2]).all() and np.isnan(got["fb"][2]).all()
+    ref = o2.run(y, walkers=[0, 1, 3, 7])
+    assert_parity(got, ref, walkers=[0, 1, 3, 7])
+    # a trial without its reference determinant, evaluated at the reference walker: every R_I = 0 -> W = 0
+    z = _reference_walkers(mi.generate("tiny").subset_dets(np.arange(1, 36)), 2)
+    trial = msd.setup_from_inputs(z)
+    fl = torch.zeros(2, dtype=torch.int32, device="cuda")
+    e = trial.local_energy(torch.tensor(z.phi_a, device="cuda"), torch.tensor(z.phi_b, device="cuda"), flags=fl)
+    assert (fl.cpu().numpy() & 2).all() and torch.isnan(e.real).all()
+    trial.close()
+
+
+def test_invalid_tables_are_rejected(torch_cuda):
+    msd = _msd()
+    x = mi.generate("tiny")
+
+    def setup(**kw):
+        a = dict(N=x.N, n_alpha=x.n_alpha, n_beta=x.n_beta, n_chol=x.n_chol, n_det=x.n_det, h1=x.h1, L=x.L, e0=0.0,
+                 occ_ref_a=x.occ_ref_a, occ_ref_b=x.occ_ref_b, exc_off_a=x.exc_off_a, holes_a=x.holes_a.copy(),
+                 parts_a=x.parts_a.copy(), exc_off_b=x.exc_off_b, holes_b=x.holes_b, parts_b=x.parts_b, ci=x.ci)
+        a.update(kw)
+        return msd.msd_setup(**a)
+
+    bad = x.holes_a.copy(); bad[0] = 5                     # hole not in the reference
+    with pytest.raises(msd.MSDError) as e:
+        setup(holes_a=bad)
+    assert e.value.code == -1
+    bad = x.parts_a.copy(); bad[0] = 1                     # particle inside the reference
+    with pytest.raises(msd.MSDError):
+        setup(parts_a=bad)
+    bad = x.parts_a.copy(); bad[0] = x.N + 3               # out of range
+    with pytest.raises(msd.MSDError):
+        setup(parts_a=bad)
+    with pytest.raises(msd.MSDError):                      # unsorted reference
+        setup(occ_ref_a=x.occ_ref_a[::-1].copy())
+    k = np.diff(x.exc_off_a)
+    I = int(np.argmax(k == 2))
+    bad = x.parts_a.copy(); bad[x.exc_off_a[I] + 1] = bad[x.exc_off_a[I]]   # repeated particle in one determinant
+    with pytest.raises(msd.MSDError):
+        setup(parts_a=bad)
+    setup().close()
+
+
+def test_setup_from_occ_and_unordered_tables(torch_cuda):
+    """The paper's (coeff, occa, occb) format and hole/particle lists in any order."""
+    torch = torch_cuda
+    msd = _msd()
+    x = mi.generate("open-shell")
+    ref = o2.run(x, return_G=False)
+    rng = np.random.default_rng(0)
+    occa = np.array([rng.permutation(r) for r in x.occa], dtype=np.int32)
+    occb = np.array([rng.permutation(r) for r in x.occb], dtype=np.int32)
+    t1 = msd.msd_setup_from_occ(x.N, x.n_alpha, x.n_beta, x.n_chol, x.n_det, x.h1, x.L, x.e0, occa, occb, x.ci)
+    assert_parity(gpu_all(torch, x, trial=t1, want_G=False), ref, what=("ovlp", "fb", "E"))
+    t1.close()
+    ha, pa = x.holes_a.copy(), x.parts_a.copy()
+    for I in range(x.n_det):
+        s = slice(x.exc_off_a[I], x.exc_off_a[I + 1])
+        ha[s] = ha[s][::-1]
+        pa[s] = rng.permutation(pa[s])
+    t2 = msd.msd_setup(x.N, x.n_alpha, x.n_beta, x.n_chol, x.n_det, x.h1, x.L, x.e0, x.occ_ref_a, x.occ_ref_b,
+                       x.exc_off_a, ha, pa, x.exc_off_b, x.holes_b, x.parts_b, x.ci)
+    assert_parity(gpu_all(torch, x, trial=t2, want_G=False), ref, what=("ovlp", "fb", "E"))
+    t2.close()
+
+
+def test_non_aufbau_reference(torch_cuda):
+    """Reference occupation that is not the lowest orbitals: particles may lie below occupied orbitals, so the
+    in-place -> sorted phases are non-trivial (reading A6)."""
+    torch = torch_cuda
+    rng = np.random.default_rng(3)
+    x = mi.generate("open-shell")
+    perm = rng.permutation(x.N)                      # relabel orbitals: same physics, scrambled reference
+    inv = np.argsort(perm)
+    h1 = x.h1[np.ix_(inv, inv)]
+    L = np.ascontiguousarray(x.L[:, inv][:, :, inv])
+    occa = np.sort(perm[x.occa], axis=1).astype(np.int32)
+    occb = np.sort(perm[x.occb], axis=1).astype(np.int32)
+    # relabelling permutes the rows of each determinant's string: the sign change is part of the physics of the
+    # relabelled problem, so compare against the oracle run on the relabelled inputs themselves
+    import dataclasses
+    ra, rb = occa[0].copy(), occb[0].copy()
+    ta, tb = mi.occ_to_tables(occa, ra), mi.occ_to_tables(occb, rb)
+    y = dataclasses.replace(x, h1=h1, L=L, occa=occa, occb=occb, occ_ref_a=ra, occ_ref_b=rb,
+                            exc_off_a=ta[0], holes_a=ta[1], parts_a=ta[2], exc_off_b=tb[0], holes_b=tb[1], parts_b=tb[2],
+                            phi_a=np.ascontiguousarray(x.phi_a[:, inv]), phi_b=np.ascontiguousarray(x.phi_b[:, inv]))
+    assert_parity(gpu_all(torch, y), o2.run(y))
+
+
+# ----------------------------------------------------------------------------------------------
+# properties that hold at any size, on the full batch (GPU self-consistency)
+# ----------------------------------------------------------------------------------------------
+def test_gauge_order_and_chunk_invariance(torch_cuda):
+    torch = torch_cuda
+    msd = _msd()
+    x = mi.generate("small")
+    base = gpu_all(torch, x, want_G=False)
+    rng = np.random.default_rng(9)
+    # P4 gauge: psi -> psi A
+    Aa = rng.standard_normal((8, 8)) + 1j * rng.standard_normal((8, 8))
+    Ab = rng.standard_normal((8, 8)) + 1j * rng.standard_normal((8, 8))
+    g = gpu_all(torch, x.with_walkers(x.phi_a @ Aa, x.phi_b @ Ab), want_G=False)
+    fac = np.linalg.det(Aa) * np.linalg.det(Ab)
+    assert (np.abs(g["ovlp"] - fac * base["ovlp"]) / np.abs(fac * base["ovlp"])).max() < 1e-9
+    assert np.abs(g["E"] - base["E"]).max() < TOL_E
+    assert (np.abs(g["fb"] - base["fb"]).max(axis=1) / np.abs(base["fb"]).max(axis=1)).max() < 1e-9
+    # P11 determinant order
+    p = gpu_all(torch, x.subset_dets(rng.permutation(x.n_det)), want_G=False)
+    assert (np.abs(p["ovlp"] - base["ovlp"]) / np.abs(base["ovlp"])).max() < TOL_REL
+    assert np.abs(p["E"] - base["E"]).max() < TOL_E
+    # walker chunking under a small workspace limit (results must not depend on chunking)
+    trial = msd.setup_from_inputs(x)
+    trial.set_workspace_limit(24 * 1024 * 1024)
+    c = gpu_all(torch, x, trial=trial, want_G=False)
+    trial.close()
+    assert (np.abs(c["ovlp"] - base["ovlp"]) / np.abs(base["ovlp"])).max() < TOL_REL
+    assert np.abs(c["E"] - base["E"]).max() < TOL_E
+    assert (np.abs(c["fb"] - base["fb"]).max(axis=1) / np.abs(base["fb"]).max(axis=1)).max() < TOL_REL
+
+
+# ----------------------------------------------------------------------------------------------
+# the packer (S0): integer / index work is bit-exact
+# ----------------------------------------------------------------------------------------------
+def _parity_bruteforce(occ_ref, holes, parts):
+    lst = list(occ_ref)
+    for h, p in zip(sorted(holes), sorted(parts)):
+        lst[lst.index(h)] = p
+    inv = sum(1 for i, j in itertools.combinations(range(len(lst)), 2) if lst[i] > lst[j])
+    return -1.0 if inv & 1 else 1.0
+
+
+@pytest.mark.parametrize("name", ["tiny-full", "open-shell", "small"])
+def test_packer_buckets_and_phases(torch_cuda, name):
+    msd = _msd()
+    x = mi.generate(name)
+    trial = msd.setup_from_inputs(x)
+    pk = trial.packed()
+    info = trial.info()
+    trial.close()
+    perm = pk["perm"]
+    assert sorted(perm.tolist()) == list(range(x.n_det))                      # a permutation
+    ka, kb = np.diff(x.exc_off_a)[perm], np.diff(x.exc_off_b)[perm]
+    assert (ka == pk["level_a"]).all() and (kb == pk["level_b"]).all()
+    key = ka * 17 + kb
+    assert (np.diff(key) >= 0).all()                                           # contiguous level buckets, ascending
+    for k in np.unique(key):                                                   # stable inside a bucket
+        assert (np.diff(perm[key == k]) > 0).all()
+    assert info["n_buckets"] == len(np.unique(key))
+    for s, I in enumerate(perm):
+        ph = _parity_bruteforce(x.occ_ref_a, x.holes_a[x.exc_off_a[I]:x.exc_off_a[I + 1]],
+                                x.parts_a[x.exc_off_a[I]:x.exc_off_a[I + 1]]) * \
+             _parity_bruteforce(x.occ_ref_b, x.holes_b[x.exc_off_b[I]:x.exc_off_b[I + 1]],
+                                x.parts_b[x.exc_off_b[I]:x.exc_off_b[I + 1]])
+        assert pk["coef"][s] == x.ci[I] * ph                                   # bit-exact
+    assert info["n_o_alpha"] == len(np.unique(x.holes_a)) and info["n_v_alpha"] == len(np.unique(x.parts_a))
+
+
+def test_native_library_is_the_path(torch_cuda):
+    """The kernels ran: launches counted, and the in-tree .so is mapped into this process."""
+    msd = _msd()
+    x = mi.generate("tiny")
+    trial = msd.setup_from_inputs(x)
+    n0 = trial.launch_count()
+    gpu_all(torch_cuda, x, trial=trial)
+    assert trial.launch_count() > n0 >= 5
+    trial.close()
+    maps = open("/proc/self/maps").read()
+    assert "libmsd_b200.so" in maps
