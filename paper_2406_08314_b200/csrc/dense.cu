@@ -36,7 +36,7 @@ __device__ __forceinline__ cplx block_sum(cplx v)
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 k_green_rows(int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw, const cplx* __restrict__ theta_a,
-             const cplx* __restrict__ theta_b, const cplx* __restrict__ C_a, const cplx* __restrict__ C_b,
+             const cplx* __restrict__ theta_b, const double* __restrict__ C_a, const double* __restrict__ C_b,
              const cplx* __restrict__ Wacc, double* Gp_a, double* Gp_b, cplx* Gfull, int* wflags)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -45,7 +45,7 @@ k_green_rows(int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw, const cplx* __r
     const SpinDev sp = s ? sb : sa;
     const int n = sp.n, no = sp.n_o, nv = sp.n_v;
     const cplx* theta = (s ? theta_b : theta_a) + w * (int64_t)N * n;
-    const cplx* C = (s ? C_b : C_a) + (w / MSD_WT) * (int64_t)sp.P * MSD_WT + (w % MSD_WT);
+    const double* C = (s ? C_b : C_a) + (w / MSD_WT) * (int64_t)sp.P * 2 * MSD_WT + (w % MSD_WT);
     double* Gp = (s ? Gp_b : Gp_a);
     cplx* D = reinterpret_cast<cplx*>(smem_raw);     // [nv][no]
     cplx* U = D + nv * no;                            // [n][no]
@@ -54,7 +54,7 @@ k_green_rows(int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw, const cplx* __r
     const bool bad = (W.x == 0.0 && W.y == 0.0) || (wflags[w] & 1);
     if (tid == 0 && s == 0 && (W.x == 0.0 && W.y == 0.0)) atomicOr(&wflags[w], 2);
     const cplx Winv = bad ? cmake(nan_d(), nan_d()) : cinv(W);
-    for (int x = tid; x < nv * no; x += nt) D[x] = cmul(C[(int64_t)x * MSD_WT], Winv);
+    for (int x = tid; x < nv * no; x += nt) D[x] = cmul(load_planar(C, x), Winv);
     __syncthreads();
     for (int e = tid; e < n * no; e += nt) {
         int l = e / no, h = e - l * no;
@@ -313,8 +313,8 @@ __global__ void k_finish_flags(int64_t nw, const cplx* __restrict__ Wacc, const 
 //   E1 = E1_0 + (1/W) sum_s sum_x C^s[x] Hrot^s[x]                                            (W8)
 //   E2 = 1/2 sum_g Xt_g^2 - 1/2 sum_g (Ex0^a_g + Ex0^b_g) + (1/W) [ sum_s sum_x C^s[x] F^s[x] + E2nd ]   (W9)
 __global__ void __launch_bounds__(256)
-k_finish_energy(int n_chol, int64_t nw, double e0, int Pa, int Pb, const cplx* __restrict__ C_a,
-                const cplx* __restrict__ C_b, const cplx* __restrict__ F_a, const cplx* __restrict__ F_b,
+k_finish_energy(int n_chol, int64_t nw, double e0, int Pa, int Pb, const double* __restrict__ C_a,
+                const double* __restrict__ C_b, const cplx* __restrict__ F_a, const cplx* __restrict__ F_b,
                 const cplx* __restrict__ H_a, const cplx* __restrict__ H_b, const cplx* __restrict__ X0,
                 const cplx* __restrict__ Eacc, const cplx* __restrict__ Wacc, const cplx* __restrict__ E2nd,
                 const int* __restrict__ wflags, cplx* eout, int* flags)
@@ -324,11 +324,11 @@ k_finish_energy(int n_chol, int64_t nw, double e0, int Pa, int Pb, const cplx* _
     cplx ch = cmake(0.0, 0.0), cf = cmake(0.0, 0.0), xx = cmake(0.0, 0.0);
     for (int s = 0; s < 2; s++) {
         const int P = s ? Pb : Pa;
-        const cplx* C = (s ? C_b : C_a) + (w / MSD_WT) * (int64_t)P * MSD_WT + (w % MSD_WT);
+        const double* C = (s ? C_b : C_a) + (w / MSD_WT) * (int64_t)P * 2 * MSD_WT + (w % MSD_WT);
         const cplx* F = (s ? F_b : F_a) + w * (int64_t)P;
         const cplx* H = (s ? H_b : H_a) + w * (int64_t)P;
         for (int x = tid; x < P; x += nt) {
-            cplx c = C[(int64_t)x * MSD_WT];
+            cplx c = load_planar(C, x);
             ch = cfma(c, H[x], ch);
             cf = cfma(c, F[x], cf);
         }

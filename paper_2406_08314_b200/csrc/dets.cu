@@ -18,7 +18,7 @@ struct DetsParams {
     const unsigned char* tab;
     const double* coef;
     const cplx* g[2];      // [nt][P][WT]
-    cplx* C[2];            // [nt][P][WT]
+    double* C[2];          // [nt][P][2][WT] planar
     const cplx* Vab;       // [nt][Pa][Pb][WT]
     const cplx* Vss[2];    // [nt][P][P][WT]
     cplx* Wacc;            // [nt*WT]
@@ -131,26 +131,28 @@ __device__ __forceinline__ cplx second_cofactor(const cplx (*M)[K > 0 ? K : 1], 
     return ((a + b + c + d) & 1) ? cneg(m) : m;
 }
 
-// one spin of one (determinant, walker): gather, det, adjugate, same-spin second-order sum
+// one spin of one (determinant, walker): gather from the shared-memory copy of g, det, adjugate,
+// same-spin second-order sum
 template <int K, int MODE>
 struct SpinEval {
-    cplx A[K > 0 ? K : 1][K > 0 ? K : 1];
-    int x[K > 0 ? K : 1][K > 0 ? K : 1];     // pair index x[a][b] = p_b * n_o + h_a
+    static constexpr int K1 = K > 0 ? K : 1;
+    cplx A[K1][K1];
+    int h[K1], pn[K1];                        // h_a and p_b * n_o: pair index x(a,b) = pn[b] + h[a]
     cplx R;
     cplx Ess;
-    __device__ __forceinline__ void run(const unsigned char* hp, const cplx* __restrict__ g, int no,
-                                        const cplx* __restrict__ Vss, int P)
+    __device__ __forceinline__ int x(int a, int b) const { return pn[b] + h[a]; }
+    __device__ __forceinline__ void run(const unsigned char* hp, const cplx* g /* smem tile + lane walker */, int no,
+                                        const cplx* __restrict__ Vss, unsigned P)
     {
         Ess = cmake(0.0, 0.0);
         if (K == 0) { R = cmake(1.0, 0.0); return; }
-        cplx M[K > 0 ? K : 1][K > 0 ? K : 1];
+        cplx M[K1][K1];
+#pragma unroll
+        for (int a = 0; a < K; a++) { h[a] = (int)hp[a]; pn[a] = (int)hp[K + a] * no; }
 #pragma unroll
         for (int a = 0; a < K; a++)
 #pragma unroll
-            for (int b = 0; b < K; b++) {
-                x[a][b] = (int)hp[K + b] * no + (int)hp[a];
-                M[a][b] = __ldg(&g[(int64_t)x[a][b] * MSD_WT]);
-            }
+            for (int b = 0; b < K; b++) M[a][b] = g[x(a, b) * MSD_WT];
         R = Closed<K>::det_adj(M, A);
         if (MODE == 2 && K >= 2) {
 #pragma unroll
@@ -162,49 +164,52 @@ struct SpinEval {
 #pragma unroll
                         for (int d = b + 1; d < K; d++) {
                             cplx t = second_cofactor<K>(M, a, c, b, d);
-                            cplx v1 = __ldg(&Vss[((int64_t)x[a][b] * P + x[c][d]) * MSD_WT]);
-                            cplx v2 = __ldg(&Vss[((int64_t)x[a][d] * P + x[c][b]) * MSD_WT]);
+                            cplx v1 = __ldg(&Vss[((unsigned)x(a, b) * P + (unsigned)x(c, d)) * MSD_WT]);
+                            cplx v2 = __ldg(&Vss[((unsigned)x(a, d) * P + (unsigned)x(c, b)) * MSD_WT]);
                             Ess = cfma(t, csub(v1, v2), Ess);
                         }
         }
     }
 };
 
+template <int NWORD> struct RowData { uint32_t w[NWORD]; double cf; };
+
 template <int KA, int KB, int MODE>
 __device__ __forceinline__ void run_bucket(const DetsParams& p, const WorkItem& it, int tile, int slot, int nslots,
-                                           int j, cplx& Wl, cplx& El)
+                                           int j, const cplx* gsm, cplx& Wl, cplx& El)
 {
     constexpr int NB = 2 * KA + 2 * KB;
     constexpr int NWORD = (NB + 3) / 4 > 0 ? (NB + 3) / 4 : 1;
-    const cplx* gA = p.g[0] + (int64_t)tile * p.P[0] * MSD_WT + j;
-    const cplx* gB = p.g[1] + (int64_t)tile * p.P[1] * MSD_WT + j;
-    cplx* CA = p.C[0] + (int64_t)tile * p.P[0] * MSD_WT + j;
-    cplx* CB = p.C[1] + (int64_t)tile * p.P[1] * MSD_WT + j;
+    const cplx* gA = gsm + j;
+    const cplx* gB = gsm + p.P[0] * MSD_WT + j;
+    double* CA = p.C[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j;
+    double* CB = p.C[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j;
     const cplx* VA = (MODE == 2) ? p.Vss[0] + (int64_t)tile * p.P[0] * p.P[0] * MSD_WT + j : nullptr;
     const cplx* VB = (MODE == 2) ? p.Vss[1] + (int64_t)tile * p.P[1] * p.P[1] * MSD_WT + j : nullptr;
     const cplx* VAB = (MODE == 2) ? p.Vab + (int64_t)tile * p.P[0] * p.P[1] * MSD_WT + j : nullptr;
-    for (int i = slot; i < it.det_count; i += nslots) {
-        union { uint32_t w[NWORD]; unsigned char b[NWORD * 4]; } row;
-        const uint32_t* rp = reinterpret_cast<const uint32_t*>(p.tab + it.tab_off + (int64_t)i * it.rs);
+    const unsigned char* tab = p.tab + it.tab_off;
+    const double* coef = p.coef + it.det_begin;
+    auto load_row = [&](int i, RowData<NWORD>& r) {
+        const uint32_t* rp = reinterpret_cast<const uint32_t*>(tab + (int64_t)i * it.rs);
 #pragma unroll
-        for (int t = 0; t < NWORD; t++) row.w[t] = (NB > 0) ? __ldg(rp + t) : 0u;
-        const double cf = __ldg(&p.coef[it.det_begin + i]);
+        for (int t = 0; t < NWORD; t++) r.w[t] = (NB > 0) ? __ldg(rp + t) : 0u;
+        r.cf = __ldg(coef + i);
+    };
+    int i = slot;
+    RowData<NWORD> cur, nxt;
+    if (i < it.det_count) load_row(i, cur);
+    while (i < it.det_count) {
+        const int inext = i + nslots;
+        nxt = cur;
+        if (inext < it.det_count) load_row(inext, nxt);      // software prefetch of the next table row
+        const unsigned char* rb = reinterpret_cast<const unsigned char*>(cur.w);
+        const double cf = cur.cf;
         SpinEval<KA, MODE> ea;
         SpinEval<KB, MODE> eb;
-        ea.run(row.b, gA, p.no[0], VA, p.P[0]);
-        eb.run(row.b + 2 * KA, gB, p.no[1], VB, p.P[1]);
+        ea.run(rb, gA, p.no[0], VA, (unsigned)p.P[0]);
+        eb.run(rb + 2 * KA, gB, p.no[1], VB, (unsigned)p.P[1]);
         const cplx cRa = cscale(cf, ea.R), cRb = cscale(cf, eb.R);
         Wl = cfma(cRa, eb.R, Wl);
-        if (MODE >= 1) {
-#pragma unroll
-            for (int a = 0; a < KA; a++)
-#pragma unroll
-                for (int b = 0; b < KA; b++) red_add(&CA[(int64_t)ea.x[a][b] * MSD_WT], cmul(cRb, ea.A[b][a]));
-#pragma unroll
-            for (int a = 0; a < KB; a++)
-#pragma unroll
-                for (int b = 0; b < KB; b++) red_add(&CB[(int64_t)eb.x[a][b] * MSD_WT], cmul(cRa, eb.A[b][a]));
-        }
         if (MODE == 2) {
             cplx e = cmake(0.0, 0.0);
             if (KA > 0 && KB > 0) {
@@ -212,13 +217,13 @@ __device__ __forceinline__ void run_bucket(const DetsParams& p, const WorkItem& 
                 for (int a = 0; a < KA; a++)
 #pragma unroll
                     for (int b = 0; b < KA; b++) {
-                        const cplx* vrow = VAB + (int64_t)ea.x[a][b] * p.P[1] * MSD_WT;
+                        const cplx* vrow = VAB + (unsigned)ea.x(a, b) * (unsigned)p.P[1] * MSD_WT;
                         cplx z = cmake(0.0, 0.0);
 #pragma unroll
                         for (int a2 = 0; a2 < KB; a2++)
 #pragma unroll
                             for (int b2 = 0; b2 < KB; b2++)
-                                z = cfma(eb.A[b2][a2], __ldg(&vrow[(int64_t)eb.x[a2][b2] * MSD_WT]), z);
+                                z = cfma(eb.A[b2][a2], __ldg(&vrow[eb.x(a2, b2) * MSD_WT]), z);
                         e = cfma(ea.A[b][a], z, e);
                     }
             }
@@ -227,6 +232,18 @@ __device__ __forceinline__ void run_bucket(const DetsParams& p, const WorkItem& 
             El.x = fma(cf, e.x, El.x);
             El.y = fma(cf, e.y, El.y);
         }
+        if (MODE >= 1) {
+#pragma unroll
+            for (int a = 0; a < KA; a++)
+#pragma unroll
+                for (int b = 0; b < KA; b++) red_add_planar(CA, ea.x(a, b), cmul(cRb, ea.A[b][a]));
+#pragma unroll
+            for (int a = 0; a < KB; a++)
+#pragma unroll
+                for (int b = 0; b < KB; b++) red_add_planar(CB, eb.x(a, b), cmul(cRa, eb.A[b][a]));
+        }
+        cur = nxt;
+        i = inext;
     }
 }
 
@@ -259,52 +276,71 @@ __device__ __forceinline__ void flush_walker_sums(const DetsParams& p, int tile,
     }
 }
 
+// stage the walker tile's active slices g^a, g^b ([P][WT] complex each) in shared memory
+__device__ __forceinline__ void stage_g(const DetsParams& p, int tile, cplx* gsm)
+{
+    const int na = p.P[0] * MSD_WT, nb = p.P[1] * MSD_WT;
+    const cplx* ga = p.g[0] + (int64_t)tile * na;
+    const cplx* gb = p.g[1] + (int64_t)tile * nb;
+    for (int e = threadIdx.x; e < na; e += blockDim.x) gsm[e] = __ldg(ga + e);
+    for (int e = threadIdx.x; e < nb; e += blockDim.x) gsm[na + e] = __ldg(gb + e);
+    __syncthreads();
+}
+
 #define CF_CASE(KA_, KB_)                                                                              \
     case KA_ * 5 + KB_:                                                                                \
         if constexpr ((KA_ > KB_ ? KA_ : KB_) > KLO && (KA_ > KB_ ? KA_ : KB_) <= KHI)                  \
-            run_bucket<KA_, KB_, MODE>(p, it, tile, slot, nslots, j, Wl, El);                          \
+            run_bucket<KA_, KB_, MODE>(p, it, tile, slot, nslots, j, gsm, Wl, El);                     \
         break;
 
-// register class (KLO, KHI]: buckets whose larger level lies in that range (KLO = -1 admits (0,0))
-template <int MODE, int KLO, int KHI>
-__global__ void __launch_bounds__(128) k_dets_cf(DetsParams p, const WorkItem* __restrict__ items)
+// register class (KLO, KHI]: buckets whose larger level lies in that range (KLO = -1 admits (0,0)).
+// Persistent per walker tile: CTA (worker, tile) stages g once and strides over the class's work items.
+template <int MODE, int KLO, int KHI, int NTHR, int MINB>
+__global__ void __launch_bounds__(NTHR, MINB) k_dets_cf(DetsParams p, const WorkItem* __restrict__ items, int n_items)
 {
-    const WorkItem it = items[blockIdx.x];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* gsm = reinterpret_cast<cplx*>(smem_raw);
     const int tile = blockIdx.y;
     const int j = threadIdx.x & (MSD_WT - 1);
-    const int slot = threadIdx.x / MSD_WT, nslots = blockDim.x / MSD_WT;
+    const int slot = threadIdx.x / MSD_WT, nslots = NTHR / MSD_WT;
+    stage_g(p, tile, gsm);
     cplx Wl = cmake(0.0, 0.0), El = cmake(0.0, 0.0);
-    switch (it.ka * 5 + it.kb) {
-        CF_CASE(0, 0) CF_CASE(0, 1) CF_CASE(0, 2) CF_CASE(0, 3) CF_CASE(0, 4)
-        CF_CASE(1, 0) CF_CASE(1, 1) CF_CASE(1, 2) CF_CASE(1, 3) CF_CASE(1, 4)
-        CF_CASE(2, 0) CF_CASE(2, 1) CF_CASE(2, 2) CF_CASE(2, 3) CF_CASE(2, 4)
-        CF_CASE(3, 0) CF_CASE(3, 1) CF_CASE(3, 2) CF_CASE(3, 3) CF_CASE(3, 4)
-        CF_CASE(4, 0) CF_CASE(4, 1) CF_CASE(4, 2) CF_CASE(4, 3) CF_CASE(4, 4)
-        default: break;
+    for (int r = 0, ii; (ii = r * (int)gridDim.x + ((r & 1) ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x)),
+                        r * (int)gridDim.x < n_items; r++) {
+        if (ii >= n_items) continue;
+        const WorkItem it = items[ii];
+        switch (it.ka * 5 + it.kb) {
+            CF_CASE(0, 0) CF_CASE(0, 1) CF_CASE(0, 2) CF_CASE(0, 3) CF_CASE(0, 4)
+            CF_CASE(1, 0) CF_CASE(1, 1) CF_CASE(1, 2) CF_CASE(1, 3) CF_CASE(1, 4)
+            CF_CASE(2, 0) CF_CASE(2, 1) CF_CASE(2, 2) CF_CASE(2, 3) CF_CASE(2, 4)
+            CF_CASE(3, 0) CF_CASE(3, 1) CF_CASE(3, 2) CF_CASE(3, 3) CF_CASE(3, 4)
+            CF_CASE(4, 0) CF_CASE(4, 1) CF_CASE(4, 2) CF_CASE(4, 3) CF_CASE(4, 4)
+            default: break;
+        }
     }
     flush_walker_sums(p, tile, Wl, El, MODE);
 }
 
 // ------------------------------------------------------------------------------------------------
 // generic levels (k >= 5 in at least one spin): one matrix per thread in shared memory, element e of
-// thread t at sm[e * T + t]
+// thread t at sm[e * T + t] (consecutive lanes -> consecutive 16-byte words: conflict-free for any per-lane e)
 // ------------------------------------------------------------------------------------------------
 struct SmMat {
     cplx* base; int T;
-    __device__ __forceinline__ cplx& at(int e) { return base[(int64_t)e * T]; }
+    __device__ __forceinline__ cplx& at(int e) { return base[e * T]; }
 };
 
 // in-place Gauss-Jordan inverse with partial pivoting; returns det (0 if an exactly zero pivot appears,
 // in which case the matrix content is zeroed: adj and second cofactors are taken as 0 -- reading A11)
 __device__ cplx gauss_jordan(SmMat m, int k)
 {
-    int ipiv[MSD_MAX_LEVEL];
+    unsigned long long ipiv = 0ull;          // 4 bits per pivot row (k <= 16)
     cplx det = cmake(1.0, 0.0);
     bool sing = false;
     for (int j = 0; j < k; j++) {
         int p = j; double best = cabs2(m.at(j * k + j));
         for (int i = j + 1; i < k; i++) { double v = cabs2(m.at(i * k + j)); if (v > best) { best = v; p = i; } }
-        ipiv[j] = p;
+        ipiv |= (unsigned long long)p << (4 * j);
         if (!(best > 0.0)) { sing = true; break; }
         if (p != j) {
             for (int c = 0; c < k; c++) { cplx t = m.at(j * k + c); m.at(j * k + c) = m.at(p * k + c); m.at(p * k + c) = t; }
@@ -327,15 +363,17 @@ __device__ cplx gauss_jordan(SmMat m, int k)
         return cmake(0.0, 0.0);
     }
     for (int j = k - 1; j >= 0; j--) {
-        int p = ipiv[j];
+        int p = (int)((ipiv >> (4 * j)) & 15ull);
         if (p != j)
             for (int i = 0; i < k; i++) { cplx t = m.at(i * k + j); m.at(i * k + j) = m.at(i * k + p); m.at(i * k + p) = t; }
     }
     return det;
 }
 
+struct HP { int h[MSD_MAX_LEVEL], pn[MSD_MAX_LEVEL]; __device__ __forceinline__ int x(int a, int b) const { return pn[b] + h[a]; } };
+
 template <int K>
-__device__ __forceinline__ cplx closed_to_smem(SmMat m, cplx* Ess, const int* x, const cplx* __restrict__ Vss, int P,
+__device__ __forceinline__ cplx closed_to_smem(SmMat m, cplx* Ess, const HP& q, const cplx* __restrict__ Vss, unsigned P,
                                                int mode)
 {
     cplx M[K][K], A[K][K];
@@ -359,8 +397,8 @@ __device__ __forceinline__ cplx closed_to_smem(SmMat m, cplx* Ess, const int* x,
 #pragma unroll
                     for (int d = b + 1; d < K; d++) {
                         cplx t = second_cofactor<K>(M, a, c, b, d);
-                        cplx v1 = __ldg(&Vss[((int64_t)x[a * K + b] * P + x[c * K + d]) * MSD_WT]);
-                        cplx v2 = __ldg(&Vss[((int64_t)x[a * K + d] * P + x[c * K + b]) * MSD_WT]);
+                        cplx v1 = __ldg(&Vss[((unsigned)q.x(a, b) * P + (unsigned)q.x(c, d)) * MSD_WT]);
+                        cplx v2 = __ldg(&Vss[((unsigned)q.x(a, d) * P + (unsigned)q.x(c, b)) * MSD_WT]);
                         e = cfma(t, csub(v1, v2), e);
                     }
     }
@@ -369,22 +407,19 @@ __device__ __forceinline__ cplx closed_to_smem(SmMat m, cplx* Ess, const int* x,
 }
 
 // one spin, runtime level k; on exit m holds A (A[b][a] at element b*k+a), returns R, *Ess
-__device__ cplx spin_generic(SmMat m, int k, const unsigned char* hp, const cplx* __restrict__ g, int no, int* x,
-                             const cplx* __restrict__ Vss, int P, int mode, cplx* Ess)
+__device__ cplx spin_generic(SmMat m, int k, const unsigned char* hp, const cplx* __restrict__ g, int no, HP& q,
+                             const cplx* __restrict__ Vss, unsigned P, int mode, cplx* Ess)
 {
     *Ess = cmake(0.0, 0.0);
     if (k == 0) return cmake(1.0, 0.0);
+    for (int a = 0; a < k; a++) { q.h[a] = (int)hp[a]; q.pn[a] = (int)hp[k + a] * no; }
     for (int a = 0; a < k; a++)
-        for (int b = 0; b < k; b++) {
-            int xx = (int)hp[k + b] * no + (int)hp[a];
-            x[a * k + b] = xx;
-            m.at(a * k + b) = __ldg(&g[(int64_t)xx * MSD_WT]);
-        }
+        for (int b = 0; b < k; b++) m.at(a * k + b) = __ldg(&g[q.x(a, b) * MSD_WT]);
     switch (k) {
-        case 1: return closed_to_smem<1>(m, Ess, x, Vss, P, mode);
-        case 2: return closed_to_smem<2>(m, Ess, x, Vss, P, mode);
-        case 3: return closed_to_smem<3>(m, Ess, x, Vss, P, mode);
-        case 4: return closed_to_smem<4>(m, Ess, x, Vss, P, mode);
+        case 1: return closed_to_smem<1>(m, Ess, q, Vss, P, mode);
+        case 2: return closed_to_smem<2>(m, Ess, q, Vss, P, mode);
+        case 3: return closed_to_smem<3>(m, Ess, q, Vss, P, mode);
+        case 4: return closed_to_smem<4>(m, Ess, q, Vss, P, mode);
         default: break;
     }
     cplx R = gauss_jordan(m, k);          // m = M^-1 (or zeros)
@@ -394,106 +429,134 @@ __device__ cplx spin_generic(SmMat m, int k, const unsigned char* hp, const cplx
         cplx e = cmake(0.0, 0.0);
         for (int a = 0; a < k; a++)
             for (int c = a + 1; c < k; c++)
-                for (int b = 0; b < k; b++)
+                for (int b = 0; b < k; b++) {
+                    const cplx Aba = m.at(b * k + a), Abc = m.at(b * k + c);
+                    const unsigned xab = (unsigned)q.x(a, b) * P, xcb = (unsigned)q.x(c, b);
                     for (int d = b + 1; d < k; d++) {
-                        cplx t = cmul(m.at(b * k + a), m.at(d * k + c));
-                        t = cfms(m.at(b * k + c), m.at(d * k + a), t);
-                        cplx v1 = __ldg(&Vss[((int64_t)x[a * k + b] * P + x[c * k + d]) * MSD_WT]);
-                        cplx v2 = __ldg(&Vss[((int64_t)x[a * k + d] * P + x[c * k + b]) * MSD_WT]);
+                        cplx t = cmul(Aba, m.at(d * k + c));
+                        t = cfms(Abc, m.at(d * k + a), t);
+                        cplx v1 = __ldg(&Vss[(xab + (unsigned)q.x(c, d)) * MSD_WT]);
+                        cplx v2 = __ldg(&Vss[((unsigned)q.x(a, d) * P + xcb) * MSD_WT]);
                         e = cfma(t, csub(v1, v2), e);
                     }
+                }
         *Ess = cmul(e, cinv(R));
     }
     return R;
 }
 
+// Persistent per walker tile like k_dets_cf; shared memory = g tile + (max ka^2+kb^2 of the launch) per thread.
 template <int MODE>
-__global__ void k_dets_gen(DetsParams p, const WorkItem* __restrict__ items, int smem_elems_per_thread)
+__global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkItem* __restrict__ items, int n_items)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const WorkItem it = items[blockIdx.x];
+    cplx* gsm = reinterpret_cast<cplx*>(smem_raw);
     const int tile = blockIdx.y;
     const int j = threadIdx.x & (MSD_WT - 1);
     const int slot = threadIdx.x / MSD_WT, nslots = blockDim.x / MSD_WT;
     const int T = blockDim.x;
-    cplx* sm = reinterpret_cast<cplx*>(smem_raw) + threadIdx.x;
-    (void)smem_elems_per_thread;
-    const int ka = it.ka, kb = it.kb;
-    SmMat mA{sm, T}, mB{sm + (int64_t)ka * ka * T, T};
-    const cplx* gA = p.g[0] + (int64_t)tile * p.P[0] * MSD_WT + j;
+    cplx* sm = gsm + threadIdx.x;
+    const cplx* gA = p.g[0] + (int64_t)tile * p.P[0] * MSD_WT + j;      // L1/L2 resident (57 KB per tile)
     const cplx* gB = p.g[1] + (int64_t)tile * p.P[1] * MSD_WT + j;
-    cplx* CA = p.C[0] + (int64_t)tile * p.P[0] * MSD_WT + j;
-    cplx* CB = p.C[1] + (int64_t)tile * p.P[1] * MSD_WT + j;
+    double* CA = p.C[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j;
+    double* CB = p.C[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j;
     const cplx* VA = (MODE == 2) ? p.Vss[0] + (int64_t)tile * p.P[0] * p.P[0] * MSD_WT + j : nullptr;
     const cplx* VB = (MODE == 2) ? p.Vss[1] + (int64_t)tile * p.P[1] * p.P[1] * MSD_WT + j : nullptr;
     const cplx* VAB = (MODE == 2) ? p.Vab + (int64_t)tile * p.P[0] * p.P[1] * MSD_WT + j : nullptr;
     cplx Wl = cmake(0.0, 0.0), El = cmake(0.0, 0.0);
-    int xa[MSD_MAX_LEVEL * MSD_MAX_LEVEL], xb[MSD_MAX_LEVEL * MSD_MAX_LEVEL];
-    for (int i = slot; i < it.det_count; i += nslots) {
-        const unsigned char* row = p.tab + it.tab_off + (int64_t)i * it.rs;
-        unsigned char hp[4 * MSD_MAX_LEVEL];
-        for (int t = 0; t < 2 * ka + 2 * kb; t++) hp[t] = __ldg(row + t);
-        const double cf = __ldg(&p.coef[it.det_begin + i]);
-        cplx EssA, EssB;
-        cplx Ra = spin_generic(mA, ka, hp, gA, p.no[0], xa, VA, p.P[0], MODE, &EssA);
-        cplx Rb = spin_generic(mB, kb, hp + 2 * ka, gB, p.no[1], xb, VB, p.P[1], MODE, &EssB);
-        const cplx cRa = cscale(cf, Ra), cRb = cscale(cf, Rb);
-        Wl = cfma(cRa, Rb, Wl);
-        if (MODE >= 1) {
-            for (int a = 0; a < ka; a++)
-                for (int b = 0; b < ka; b++) red_add(&CA[(int64_t)xa[a * ka + b] * MSD_WT], cmul(cRb, mA.at(b * ka + a)));
-            for (int a = 0; a < kb; a++)
-                for (int b = 0; b < kb; b++) red_add(&CB[(int64_t)xb[a * kb + b] * MSD_WT], cmul(cRa, mB.at(b * kb + a)));
-        }
-        if (MODE == 2) {
-            cplx e = cmake(0.0, 0.0);
-            for (int a = 0; a < ka; a++)
-                for (int b = 0; b < ka; b++) {
-                    const cplx* vrow = VAB + (int64_t)xa[a * ka + b] * p.P[1] * MSD_WT;
-                    cplx z = cmake(0.0, 0.0);
-                    for (int a2 = 0; a2 < kb; a2++)
-                        for (int b2 = 0; b2 < kb; b2++)
-                            z = cfma(mB.at(b2 * kb + a2), __ldg(&vrow[(int64_t)xb[a2 * kb + b2] * MSD_WT]), z);
-                    e = cfma(mA.at(b * ka + a), z, e);
-                }
-            e = cfma(Rb, EssA, e);
-            e = cfma(Ra, EssB, e);
-            El.x = fma(cf, e.x, El.x);
-            El.y = fma(cf, e.y, El.y);
+    // snake order over rounds: items are sorted by descending cost, so alternate the direction to even out
+    for (int r = 0, ii; (ii = r * (int)gridDim.x + ((r & 1) ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x)),
+                        r * (int)gridDim.x < n_items; r++) {
+        if (ii >= n_items) continue;
+        const WorkItem it = items[ii];
+        const int ka = it.ka, kb = it.kb;
+        SmMat mA{sm, T}, mB{sm + ka * ka * T, T};
+        for (int i = slot; i < it.det_count; i += nslots) {
+            const uint32_t* rp = reinterpret_cast<const uint32_t*>(p.tab + it.tab_off + (int64_t)i * it.rs);
+            union { uint32_t w[MSD_MAX_LEVEL]; unsigned char b[4 * MSD_MAX_LEVEL]; } row;
+            for (int t = 0; t < it.rs / 4; t++) row.w[t] = __ldg(rp + t);
+            const double cf = __ldg(&p.coef[it.det_begin + i]);
+            HP qa, qb;
+            cplx EssA, EssB;
+            cplx Ra = spin_generic(mA, ka, row.b, gA, p.no[0], qa, VA, (unsigned)p.P[0], MODE, &EssA);
+            cplx Rb = spin_generic(mB, kb, row.b + 2 * ka, gB, p.no[1], qb, VB, (unsigned)p.P[1], MODE, &EssB);
+            const cplx cRa = cscale(cf, Ra), cRb = cscale(cf, Rb);
+            Wl = cfma(cRa, Rb, Wl);
+            if (MODE == 2) {
+                cplx e = cmake(0.0, 0.0);
+                for (int a = 0; a < ka; a++)
+                    for (int b = 0; b < ka; b++) {
+                        const cplx* vrow = VAB + (unsigned)qa.x(a, b) * (unsigned)p.P[1] * MSD_WT;
+                        cplx z = cmake(0.0, 0.0);
+                        for (int a2 = 0; a2 < kb; a2++)
+                            for (int b2 = 0; b2 < kb; b2++)
+                                z = cfma(mB.at(b2 * kb + a2), __ldg(&vrow[qb.x(a2, b2) * MSD_WT]), z);
+                        e = cfma(mA.at(b * ka + a), z, e);
+                    }
+                e = cfma(Rb, EssA, e);
+                e = cfma(Ra, EssB, e);
+                El.x = fma(cf, e.x, El.x);
+                El.y = fma(cf, e.y, El.y);
+            }
+            if (MODE >= 1) {
+                for (int a = 0; a < ka; a++)
+                    for (int b = 0; b < ka; b++) red_add_planar(CA, qa.x(a, b), cmul(cRb, mA.at(b * ka + a)));
+                for (int a = 0; a < kb; a++)
+                    for (int b = 0; b < kb; b++) red_add_planar(CB, qb.x(a, b), cmul(cRa, mB.at(b * kb + a)));
+            }
         }
     }
     flush_walker_sums(p, tile, Wl, El, MODE);
 }
 
 // ------------------------------------------------------------------------------------------------
+template <class K>
+static cudaError_t launch_persistent(K kernel, int nthr, size_t smem, int n_sm, const DetsParams& p, const WorkItem* items,
+                                     int n_items, int ntiles, cudaStream_t st)
+{
+    if (n_items == 0) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int occ = 1;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, nthr, smem);
+    if (e != cudaSuccess) return e;
+    if (occ < 1) return cudaErrorInvalidConfiguration;
+    // about two walker tiles resident at a time (their V slices stay in L2), every SM full
+    int workers = (n_sm * occ + 1) / 2;
+    if (workers > n_items) workers = n_items;
+    if (ntiles == 1) workers = n_items < n_sm * occ ? n_items : n_sm * occ;
+    dim3 grid(workers, ntiles);
+    kernel<<<grid, nthr, smem, st>>>(p, items, n_items);
+    return cudaGetLastError();
+}
+
 template <int MODE>
 static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cudaStream_t st)
 {
-    // three register classes of the closed-form kernel, split on the host by the items' larger level
-    const WorkItem* d = c->d_items_cf;
-    size_t n = c->items_cf.size();
-    size_t i0 = 0;
-    // items_cf is sorted by class (ascending larger level), see build_work_items()
-    auto cls = [&](const WorkItem& w) { int m = w.ka > w.kb ? w.ka : w.kb; return m <= 2 ? 0 : (m == 3 ? 1 : 2); };
-    while (i0 < n) {
-        size_t i1 = i0; int cl = cls(c->items_cf[i0]);
-        while (i1 < n && cls(c->items_cf[i1]) == cl) i1++;
-        dim3 grid((unsigned)(i1 - i0), ntiles);
-        if (cl == 0) k_dets_cf<MODE, -1, 2><<<grid, 128, 0, st>>>(p, d + i0);
-        else if (cl == 1) k_dets_cf<MODE, 2, 3><<<grid, 128, 0, st>>>(p, d + i0);
-        else k_dets_cf<MODE, 3, 4><<<grid, 128, 0, st>>>(p, d + i0);
-        c->launches++;
-        i0 = i1;
-    }
-    if (!c->items_gen.empty()) {
-        size_t smem = (size_t)c->gen_smem_per_thread * c->gen_threads;
-        cudaError_t e = cudaFuncSetAttribute(k_dets_gen<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const size_t gbytes = (size_t)(p.P[0] + p.P[1]) * MSD_WT * sizeof(cplx);
+    // closed-form kernel: three register classes, items sorted by class on the host (msd_api.cu)
+    for (int cl = 0; cl < 3; cl++) {
+        const int i0 = c->cf_class_begin[cl], i1 = c->cf_class_begin[cl + 1];
+        if (i1 == i0) continue;
+        cudaError_t e;
+        if (cl == 0) e = launch_persistent(k_dets_cf<MODE, -1, 2, 256, 3>, 256, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, st);
+        else if (cl == 1) e = launch_persistent(k_dets_cf<MODE, 2, 3, 256, 2>, 256, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, st);
+        else e = launch_persistent(k_dets_cf<MODE, 3, 4, 128, 2>, 128, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, st);
         if (e != cudaSuccess) return e;
-        dim3 grid((unsigned)c->items_gen.size(), ntiles);
-        k_dets_gen<MODE><<<grid, c->gen_threads, smem, st>>>(p, c->d_items_gen, c->gen_smem_per_thread / 16);
         c->launches++;
     }
-    return cudaGetLastError();
+    // generic kernel: one launch per shared-memory group
+    for (size_t gi = 0; gi + 1 < c->gen_group_begin.size(); gi++) {
+        const int i0 = c->gen_group_begin[gi], i1 = c->gen_group_begin[gi + 1];
+        if (i1 == i0) continue;
+        int nthr = 128;
+        while (nthr > 32 && (size_t)c->gen_group_elems[gi] * sizeof(cplx) * nthr > 200 * 1024) nthr -= 32;
+        size_t smem = (size_t)c->gen_group_elems[gi] * sizeof(cplx) * nthr;
+        cudaError_t e = launch_persistent(k_dets_gen<MODE>, nthr, smem, c->n_sm, p, c->d_items_gen + i0, i1 - i0, ntiles, st);
+        if (e != cudaSuccess) return e;
+        c->launches++;
+    }
+    return cudaSuccess;
 }
 
 cudaError_t launch_dets(msd_ctx* c, int mode, int64_t nw, Workspace& ws, cudaStream_t st)

@@ -208,25 +208,25 @@ static int do_setup(msd_ctx* c, std::string* errp, int N, int na, int nb, int n_
     for (const Bucket& b : c->buckets)
         for (int64_t i = 0; i < b.count; i++) { c->h_ka[b.start + i] = b.ka; c->h_kb[b.start + i] = b.kb; }
     // --- work items ---
-    int gen_elems = 0;
     for (const Bucket& b : c->buckets)
-        if (std::max(b.ka, b.kb) > MSD_CF_MAX) gen_elems = std::max(gen_elems, b.ka * b.ka + b.kb * b.kb);
-    if (gen_elems > 400) return fail(errp, MSD_EUNSUPPORTED, "k_alpha^2 + k_beta^2 <= 400 required");
-    c->gen_smem_per_thread = std::max(gen_elems, 1) * 16;
-    {
-        int t = (200 * 1024) / c->gen_smem_per_thread;
-        t = std::min(128, t / 32 * 32);
-        c->gen_threads = std::max(32, t);
-    }
-    auto cost = [](const Bucket& b) {
-        double a = b.ka, bb = b.kb;
-        return 1.0 + a * a * a + bb * bb * bb + a * a * bb * bb;
+        if (b.ka * b.ka + b.kb * b.kb > 400) return fail(errp, MSD_EUNSUPPORTED, "k_alpha^2 + k_beta^2 <= 400 required");
+    auto cost = [](int ka, int kb) {
+        double a = ka, b = kb;
+        return 1.0 + a * a * a + b * b * b + a * a * b * b;
+    };
+    auto cls = [](const WorkItem& w) { int m = std::max(w.ka, w.kb); return m <= 2 ? 0 : (m == 3 ? 1 : 2); };
+    static const int gen_thresholds[] = {26, 34, 41, 50, 72, 100, 128, 162, 200, 400};
+    auto grp = [](const WorkItem& w) {
+        int e = w.ka * w.ka + w.kb * w.kb, g = 0;
+        while (gen_thresholds[g] < e) g++;
+        return g;
     };
     for (int bi = 0; bi < nbk; bi++) {
         const Bucket& b = c->buckets[bi];
         const bool gen = std::max(b.ka, b.kb) > MSD_CF_MAX;
-        int slots = gen ? c->gen_threads / MSD_WT : 128 / MSD_WT;
-        int iters = (int)std::max(2.0, std::min(32.0, 512.0 / cost(b)));
+        const int m = std::max(b.ka, b.kb);
+        int slots = gen ? 128 / MSD_WT : (m <= 3 ? 256 : 128) / MSD_WT;
+        int iters = (int)std::max(4.0, std::min(32.0, 1024.0 / cost(b.ka, b.kb)));
         int dpc = slots * iters;
         for (int64_t i0 = 0; i0 < b.count; i0 += dpc) {
             WorkItem it;
@@ -237,17 +237,27 @@ static int do_setup(msd_ctx* c, std::string* errp, int N, int na, int nb, int n_
             (gen ? c->items_gen : c->items_cf).push_back(it);
         }
     }
-    auto cls = [](const WorkItem& w) { int m = std::max(w.ka, w.kb); return m <= 2 ? 0 : (m == 3 ? 1 : 2); };
-    auto icost = [](const WorkItem& w) {
-        double a = w.ka, b = w.kb;
-        return (1.0 + a * a * a + b * b * b + a * a * b * b) * w.det_count;
-    };
+    auto icost = [&](const WorkItem& w) { return cost(w.ka, w.kb) * w.det_count; };
     std::stable_sort(c->items_cf.begin(), c->items_cf.end(), [&](const WorkItem& x, const WorkItem& y) {
         if (cls(x) != cls(y)) return cls(x) < cls(y);
         return icost(x) > icost(y);
     });
-    std::stable_sort(c->items_gen.begin(), c->items_gen.end(),
-                     [&](const WorkItem& x, const WorkItem& y) { return icost(x) > icost(y); });
+    std::stable_sort(c->items_gen.begin(), c->items_gen.end(), [&](const WorkItem& x, const WorkItem& y) {
+        if (grp(x) != grp(y)) return grp(x) < grp(y);
+        return icost(x) > icost(y);
+    });
+    for (int cl = 0; cl <= 3; cl++) {
+        int i = 0;
+        while (i < (int)c->items_cf.size() && cls(c->items_cf[i]) < cl) i++;
+        c->cf_class_begin[cl] = i;
+    }
+    c->gen_group_begin.clear(); c->gen_group_elems.clear();
+    for (int g = 0; g <= 10; g++) {
+        int i = 0;
+        while (i < (int)c->items_gen.size() && grp(c->items_gen[i]) < g) i++;
+        c->gen_group_begin.push_back(i);
+        if (g < 10) c->gen_group_elems.push_back(gen_thresholds[g]);
+    }
     CK(upload(&c->d_items_cf, c->items_cf.data(), c->items_cf.size(), st));
     CK(upload(&c->d_items_gen, c->items_gen.data(), c->items_gen.size(), st));
     CK(cudaStreamSynchronize(st));
@@ -411,7 +421,7 @@ static size_t carve(const msd_ctx* c, Workspace& ws, char* base, int64_t wc, int
     const int64_t nt = wc / MSD_WT;
     // zero region first
     char* z0 = base ? base : nullptr;
-    for (int s = 0; s < 2; s++) ws.C[s] = k.take<cplx>((size_t)nt * c->sp[s].P * MSD_WT);
+    for (int s = 0; s < 2; s++) ws.C[s] = k.take<double>((size_t)nt * c->sp[s].P * 2 * MSD_WT);
     ws.Wacc = k.take<cplx>(wc);
     ws.E2nd = k.take<cplx>(wc);
     ws.wflags = k.take<int>(wc);

@@ -44,6 +44,16 @@ __device__ __forceinline__ void red_add(cplx* p, cplx v) {
     atomicAdd(&p->x, v.x);
     atomicAdd(&p->y, v.y);
 }
+// CI-matrix accumulators are PLANAR per pair index x: C[x][0][WT] real parts, C[x][1][WT] imaginary parts, so that the
+// 8 walkers of a determinant hit 64 contiguous bytes per reduction (measured 2x the L2 reduction rate of interleaved
+// complex: profiles/r01_probes.md).  p points at the lane's walker inside the tile.
+__device__ __forceinline__ void red_add_planar(double* p, int x, cplx v) {
+    atomicAdd(p + x * (2 * MSD_WT), v.x);
+    atomicAdd(p + x * (2 * MSD_WT) + MSD_WT, v.y);
+}
+__device__ __forceinline__ cplx load_planar(const double* p, int x) {
+    return make_double2(p[x * (2 * MSD_WT)], p[x * (2 * MSD_WT) + MSD_WT]);
+}
 
 // ---------------------------------------------------------------------------------------------
 // packed trial (device pointers live in the context; this POD is passed to kernels by value)
@@ -85,7 +95,7 @@ struct Workspace {
     double* thetaT[2] = {nullptr, nullptr};   // [wc][n][2][N]  rows (w,i,c), K = N contiguous
     cplx* det0 = nullptr;                     // [wc][2]
     cplx* g[2] = {nullptr, nullptr};          // [nt][P][WT]
-    cplx* C[2] = {nullptr, nullptr};          // [nt][P][WT]      (zeroed every call)
+    double* C[2] = {nullptr, nullptr};        // [nt][P][2][WT] planar re/im (zeroed every call)
     cplx* Wacc = nullptr;                     // [wc]             (zeroed)
     cplx* E2nd = nullptr;                     // [wc]             (zeroed)
     int* wflags = nullptr;                    // [wc]
@@ -121,8 +131,9 @@ struct msd_ctx {
     std::vector<Bucket> buckets;
     std::vector<WorkItem> items_cf, items_gen;
     WorkItem* d_items_cf = nullptr; WorkItem* d_items_gen = nullptr;
-    int gen_smem_per_thread = 0;              // bytes of shared memory per thread of the generic kernel
-    int gen_threads = 0;
+    int cf_class_begin[4] = {0, 0, 0, 0};      // items_cf is sorted by register class (larger level <=2, 3, 4)
+    std::vector<int> gen_group_begin;         // items_gen is sorted by shared-memory group
+    std::vector<int> gen_group_elems;         // ka^2+kb^2 bound of each group (complex elements per thread)
     // host copies for introspection
     std::vector<int64_t> h_perm; std::vector<double> h_coef; std::vector<int> h_ka, h_kb;
     Workspace ws;
