@@ -224,13 +224,10 @@ def main():
     total_ms = reduce_max_time(sum(step_ms), world, dev)
     value = total_units(inp.n_w, inp.n_det, args.steps, world) / (total_ms * 1e-3)
 
-    # ---- end to end: host buffers, H2D + both calls + D2H inside the timed region ----
+    # ---- end to end: the C-ABI *_host calls (pinned HOST buffers; H2D + kernels + D2H inside each call) ----
     def e2e_step():
-        d_a.copy_(h_a, non_blocking=True)
-        d_b.copy_(h_b, non_blocking=True)
-        step()
-        h_fb.copy_(fb, non_blocking=True)
-        h_en.copy_(en, non_blocking=True)
+        trial.force_bias_host(h_a, h_b, out=h_fb)
+        trial.local_energy_host(h_a, h_b, out=h_en)
 
     e2e_step()
     barrier()
@@ -243,7 +240,7 @@ def main():
     barrier()
     e2e_ms = reduce_max_time(ea.elapsed_time(eb), world, dev)
     e2e_val = total_units(inp.n_w, inp.n_det, n_e2e, world) / (e2e_ms * 1e-3)
-    h2d = h_a.numel() * 16 + h_b.numel() * 16
+    h2d = 2 * (h_a.numel() * 16 + h_b.numel() * 16)      # each of the two host calls copies the walkers in
     d2h = h_fb.numel() * 16 + h_en.numel() * 16
 
     # ---- roofline of the dominant kernel (phase timings from CUDA events inside the library, same stream) ----

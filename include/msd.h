@@ -104,6 +104,18 @@ int msd_local_energy(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* p
 int msd_greens(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
                void* G, int32_t* flags, void* stream);
 
+/* HOST-buffer variants of the three hot calls (the end-to-end path: bench.py's "e2e").  phi_a / phi_b / the result /
+ * flags are HOST pointers with the same layouts as above (pinned memory makes the copies asynchronous, pageable
+ * memory works too).  Each call enqueues on `stream`: host->device copy of the walkers into staging buffers owned by
+ * the context, the same kernels as the device variant, device->host copy of the result (and flags); it then
+ * synchronises `stream`, so the result is valid on return.  Same return codes. */
+int msd_overlap_host(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
+                     void* ovlp, int32_t* flags, void* stream);
+int msd_force_bias_host(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
+                        void* fb, int32_t* flags, void* stream);
+int msd_local_energy_host(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
+                          void* e, int32_t* flags, void* stream);
+
 /* Introspection of the packed trial (host-side copies made at setup; for tests of the packer).
  * msd_get_info fills: info[0]=n_o_alpha, [1]=n_v_alpha, [2]=n_o_beta, [3]=n_v_beta, [4]=number of level
  * buckets, [5]=max level alpha, [6]=max level beta, [7]=walker tile width.

@@ -4,8 +4,10 @@ The product is the C-ABI library ``libmsd_b200.so`` (include/msd.h); this packag
 binding.  Import is lazy so that tools which only need the package path do not require the built
 library; any call goes through the CUDA kernels and fails loudly if the library is missing.
 """
-from .binding import (MSDError, MSDTrial, load_library, msd_force_bias, msd_greens, msd_local_energy,  # noqa: F401
-                      msd_overlap, msd_probe_fp64_tflops, msd_setup, msd_setup_from_occ, setup_from_inputs)
+from .binding import (MSDError, MSDTrial, load_library, msd_force_bias, msd_force_bias_host, msd_greens,  # noqa: F401
+                      msd_local_energy, msd_local_energy_host, msd_overlap, msd_overlap_host,
+                      msd_probe_fp64_tflops, msd_setup, msd_setup_from_occ, setup_from_inputs)
 
 __all__ = ["MSDError", "MSDTrial", "load_library", "msd_setup", "msd_setup_from_occ", "msd_overlap",
-           "msd_force_bias", "msd_local_energy", "msd_greens", "msd_probe_fp64_tflops", "setup_from_inputs"]
+           "msd_force_bias", "msd_local_energy", "msd_greens", "msd_overlap_host", "msd_force_bias_host",
+           "msd_local_energy_host", "msd_probe_fp64_tflops", "setup_from_inputs"]

@@ -20,6 +20,7 @@ _CODES = {MSD_EINVAL: "MSD_EINVAL", MSD_ENOMEM: "MSD_ENOMEM", MSD_ECUDA: "MSD_EC
           MSD_EUNSUPPORTED: "MSD_EUNSUPPORTED"}
 
 EXPORTS = ["msd_setup", "msd_setup_from_occ", "msd_overlap", "msd_force_bias", "msd_local_energy", "msd_greens",
+           "msd_overlap_host", "msd_force_bias_host", "msd_local_energy_host",
            "msd_get_info", "msd_get_packed", "msd_set_workspace_limit", "msd_launch_count", "msd_set_profiling",
            "msd_get_phase_ms", "msd_probe_fp64_tflops", "msd_destroy", "msd_last_error"]
 
@@ -47,7 +48,8 @@ def load_library() -> C.CDLL:
     lib.msd_setup.argtypes = [C.POINTER(vp), i32, i32, i32, i32, i64, vp, vp, dbl, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.msd_setup_from_occ.restype = i32
     lib.msd_setup_from_occ.argtypes = [C.POINTER(vp), i32, i32, i32, i32, i64, vp, vp, dbl, vp, vp, vp, vp]
-    for name in ("msd_overlap", "msd_force_bias", "msd_local_energy", "msd_greens"):
+    for name in ("msd_overlap", "msd_force_bias", "msd_local_energy", "msd_greens",
+                 "msd_overlap_host", "msd_force_bias_host", "msd_local_energy_host"):
         f = getattr(lib, name)
         f.restype = i32
         f.argtypes = [vp, i64, vp, vp, vp, vp, vp]
@@ -159,6 +161,37 @@ class MSDTrial:
         out = torch.empty((nw, 2, self.N, self.N), dtype=torch.complex128, device=phi_a.device) if out is None else out
         return self._call(load_library().msd_greens, phi_a, phi_b, out, flags, stream)
 
+    # -- HOST-buffer variants (numpy or CPU torch arrays in and out; copies happen inside the C call) ----
+    def _call_host(self, fn, phi_a, phi_b, out, flags, stream):
+        def host_ptr(a, dtype, shape_tail=None):
+            if hasattr(a, "data_ptr"):                 # CPU torch tensor (e.g. pinned)
+                if a.is_cuda or not a.is_contiguous():
+                    raise ValueError("host variants take contiguous CPU buffers")
+                return a.data_ptr()
+            if not (isinstance(a, np.ndarray) and a.dtype == dtype and a.flags.c_contiguous):
+                raise ValueError("host variants take contiguous %s arrays" % np.dtype(dtype).name)
+            return a.ctypes.data
+        nw = int(phi_a.shape[0])
+        if tuple(phi_a.shape) != (nw, self.N, self.n_alpha) or tuple(phi_b.shape) != (nw, self.N, self.n_beta):
+            raise ValueError("walkers must be [n_w][N][n_sigma]")
+        rc = fn(self._h, nw, host_ptr(phi_a, np.complex128), host_ptr(phi_b, np.complex128),
+                host_ptr(out, np.complex128), host_ptr(flags, np.int32) if flags is not None else None,
+                _stream_ptr(stream))
+        self._check(rc)
+        return out
+
+    def overlap_host(self, phi_a, phi_b, out=None, flags=None, stream=None):
+        out = np.empty(phi_a.shape[0], dtype=np.complex128) if out is None else out
+        return self._call_host(load_library().msd_overlap_host, phi_a, phi_b, out, flags, stream)
+
+    def force_bias_host(self, phi_a, phi_b, out=None, flags=None, stream=None):
+        out = np.empty((phi_a.shape[0], self.n_chol), dtype=np.complex128) if out is None else out
+        return self._call_host(load_library().msd_force_bias_host, phi_a, phi_b, out, flags, stream)
+
+    def local_energy_host(self, phi_a, phi_b, out=None, flags=None, stream=None):
+        out = np.empty((phi_a.shape[0], 3), dtype=np.complex128) if out is None else out
+        return self._call_host(load_library().msd_local_energy_host, phi_a, phi_b, out, flags, stream)
+
     # -- introspection -------------------------------------------------------------------------
     def info(self) -> dict:
         a = np.zeros(8, dtype=np.int64)
@@ -246,6 +279,18 @@ def msd_local_energy(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, stream
 
 def msd_greens(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, stream=None):
     return trial.greens(phi_a, phi_b, out, flags, stream)
+
+
+def msd_overlap_host(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, stream=None):
+    return trial.overlap_host(phi_a, phi_b, out, flags, stream)
+
+
+def msd_force_bias_host(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, stream=None):
+    return trial.force_bias_host(phi_a, phi_b, out, flags, stream)
+
+
+def msd_local_energy_host(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, stream=None):
+    return trial.local_energy_host(phi_a, phi_b, out, flags, stream)
 
 
 def msd_probe_fp64_tflops(use_dmma: bool = True, ms: float = 50.0, stream=None) -> float:

@@ -349,6 +349,7 @@ extern "C" void msd_destroy(msd_ctx* c)
     }
     cudaFree(c->d_tab); cudaFree(c->d_coef); cudaFree(c->d_items_cf); cudaFree(c->d_items_gen);
     cudaFree(c->ws.base);
+    cudaFree(c->stg_a); cudaFree(c->stg_b); cudaFree(c->stg_out); cudaFree(c->stg_flags);
     for (auto& e : c->ev) if (e) cudaEventDestroy(e);
     delete c;
 }
@@ -644,3 +645,69 @@ extern "C" int msd_local_energy(msd_ctx* c, int64_t n_w, const void* phi_a, cons
 extern "C" int msd_greens(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* G, int32_t* flags,
                           void* stream)
 { return hot_call(c, CALL_GREENS, n_w, phi_a, phi_b, G, flags, stream); }
+
+// ---------------------------------------------------------------------------------------------
+// HOST-buffer variants: H2D of the walkers, the hot call, D2H of the result, all on `stream`, synchronised before
+// returning.  The staging buffers belong to the context (grown on demand).
+// ---------------------------------------------------------------------------------------------
+static int ensure_staging(msd_ctx* c, int64_t n_w, size_t out_elems_per_walker, std::string* errp)
+{
+    const size_t need_a = sizeof(cplx) * (size_t)n_w * c->N * c->sp[0].n;
+    const size_t need_b = sizeof(cplx) * (size_t)n_w * c->N * c->sp[1].n;
+    const size_t need_o = sizeof(cplx) * (size_t)n_w * out_elems_per_walker;
+    const size_t need_f = sizeof(int32_t) * (size_t)n_w;
+    auto grow = [&](void** p, size_t* have, size_t need) -> cudaError_t {
+        if (*have >= need && *p) return cudaSuccess;
+        if (*p) { cudaError_t e = cudaDeviceSynchronize(); if (e != cudaSuccess) return e; cudaFree(*p); *p = nullptr; *have = 0; }
+        cudaError_t e = cudaMalloc(p, std::max<size_t>(need, 16));
+        if (e == cudaSuccess) *have = std::max<size_t>(need, 16);
+        return e;
+    };
+    CK(grow(&c->stg_a, &c->stg_a_bytes, need_a));
+    CK(grow(&c->stg_b, &c->stg_b_bytes, need_b));
+    CK(grow(&c->stg_out, &c->stg_out_bytes, need_o));
+    CK(grow(&c->stg_flags, &c->stg_flags_bytes, need_f));
+    return MSD_OK;
+}
+
+static int hot_call_host(msd_ctx* c, int call, size_t per_walker, int64_t n_w, const void* phi_a, const void* phi_b,
+                         void* out, int32_t* flags, void* stream)
+{
+    if (!c) return MSD_EINVAL;
+    if (n_w < 0 || (n_w > 0 && (!out || (c->sp[0].n > 0 && !phi_a) || (c->sp[1].n > 0 && !phi_b)))) {
+        c->err = "bad argument";
+        return MSD_EINVAL;
+    }
+    if (n_w == 0) return MSD_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    std::string err;
+    std::string* errp = &err;
+    int rc = ensure_staging(c, n_w, per_walker, errp);
+    if (rc != MSD_OK) { c->err = err; cudaGetLastError(); return rc; }
+    auto body = [&]() -> int {
+        const size_t ba = sizeof(cplx) * (size_t)n_w * c->N * c->sp[0].n, bb = sizeof(cplx) * (size_t)n_w * c->N * c->sp[1].n;
+        if (ba) CK(cudaMemcpyAsync(c->stg_a, phi_a, ba, cudaMemcpyHostToDevice, st));
+        if (bb) CK(cudaMemcpyAsync(c->stg_b, phi_b, bb, cudaMemcpyHostToDevice, st));
+        int r = hot_call(c, call, n_w, c->stg_a, c->stg_b, c->stg_out, flags ? (int32_t*)c->stg_flags : nullptr, stream);
+        if (r != MSD_OK) { err = c->err; return r; }
+        CK(cudaMemcpyAsync(out, c->stg_out, sizeof(cplx) * (size_t)n_w * per_walker, cudaMemcpyDeviceToHost, st));
+        if (flags) CK(cudaMemcpyAsync(flags, c->stg_flags, sizeof(int32_t) * (size_t)n_w, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        return MSD_OK;
+    };
+    rc = body();
+    if (rc != MSD_OK) { c->err = err; cudaGetLastError(); }
+    return rc;
+}
+
+extern "C" int msd_overlap_host(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* ovlp, int32_t* flags,
+                                void* stream)
+{ return hot_call_host(c, CALL_OVERLAP, 1, n_w, phi_a, phi_b, ovlp, flags, stream); }
+
+extern "C" int msd_force_bias_host(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* fb, int32_t* flags,
+                                   void* stream)
+{ return hot_call_host(c, CALL_FB, c ? (size_t)c->n_chol : 0, n_w, phi_a, phi_b, fb, flags, stream); }
+
+extern "C" int msd_local_energy_host(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* e, int32_t* flags,
+                                     void* stream)
+{ return hot_call_host(c, CALL_ENERGY, 3, n_w, phi_a, phi_b, e, flags, stream); }

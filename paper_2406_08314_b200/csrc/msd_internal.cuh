@@ -137,6 +137,9 @@ struct msd_ctx {
     // host copies for introspection
     std::vector<int64_t> h_perm; std::vector<double> h_coef; std::vector<int> h_ka, h_kb;
     Workspace ws;
+    // device staging of the *_host entry points
+    void* stg_a = nullptr; void* stg_b = nullptr; void* stg_out = nullptr; void* stg_flags = nullptr;
+    size_t stg_a_bytes = 0, stg_b_bytes = 0, stg_out_bytes = 0, stg_flags_bytes = 0;
     int64_t ws_limit = 0;
     int64_t ws_limit_auto = 0;
     int64_t launches = 0;

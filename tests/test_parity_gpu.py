@@ -172,6 +172,26 @@ def test_empty_and_ragged_batches(torch_cuda):
     trial.close()
 
 
+def test_host_buffer_entry_points(torch_cuda):
+    """msd_*_host (the e2e path of bench.py): numpy in, numpy out, copies inside the C call; pinned torch buffers too."""
+    torch = torch_cuda
+    msd = _msd()
+    x = mi.generate("small", n_w=13)
+    ref = o2.run(x, return_G=False)
+    trial = msd.setup_from_inputs(x)
+    fl = np.full(x.n_w, -1, dtype=np.int32)
+    got = dict(ovlp=trial.overlap_host(x.phi_a, x.phi_b, flags=fl), fb=trial.force_bias_host(x.phi_a, x.phi_b),
+               E=trial.local_energy_host(x.phi_a, x.phi_b))
+    assert (fl == 0).all()
+    assert_parity(got, ref, what=("ovlp", "fb", "E"))
+    ha, hb = torch.from_numpy(x.phi_a).pin_memory(), torch.from_numpy(x.phi_b).pin_memory()
+    he = torch.empty((x.n_w, 3), dtype=torch.complex128).pin_memory()
+    trial.local_energy_host(ha, hb, out=he)
+    assert np.abs(he.numpy() - ref["E"]).max() <= TOL_E
+    assert trial.overlap_host(x.phi_a[:0], x.phi_b[:0]).shape == (0,)
+    trial.close()
+
+
 def test_single_determinant_trial(torch_cuda):
     """P1/P2: the MSD path with one determinant is SD-AFQMC (Eq. 13-14)."""
     x = mi.generate("small", n_w=9).subset_dets([0])
