@@ -534,29 +534,36 @@ template <int MODE>
 static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cudaStream_t st)
 {
     const size_t gbytes = (size_t)(p.P[0] + p.P[1]) * MSD_WT * sizeof(cplx);
-    // closed-form kernel: three register classes, items sorted by class on the host (msd_api.cu)
-    for (int cl = 0; cl < 3; cl++) {
-        const int i0 = c->cf_class_begin[cl], i1 = c->cf_class_begin[cl + 1];
-        if (i1 == i0) continue;
-        cudaError_t e;
-        if (cl == 0) e = launch_persistent(k_dets_cf<MODE, -1, 2, 256, 3>, 256, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, st);
-        else if (cl == 1) e = launch_persistent(k_dets_cf<MODE, 2, 3, 256, 2>, 256, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, st);
-        else e = launch_persistent(k_dets_cf<MODE, 3, 4, 128, 2>, 128, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, st);
-        if (e != cudaSuccess) return e;
-        c->launches++;
-    }
-    // generic kernel: one launch per shared-memory group
-    for (size_t gi = 0; gi + 1 < c->gen_group_begin.size(); gi++) {
+    // The launches below are independent (they only meet in the RED accumulators), so they are forked over the
+    // context's side streams: the small high-level groups no longer serialise their tails behind one another.
+    Fork f(c, st);
+    int li = 0;
+    // generic kernel first (longest per-item latency): one launch per shared-memory group, highest levels first
+    for (size_t gi = c->gen_group_begin.size() - 1; gi-- > 0;) {
         const int i0 = c->gen_group_begin[gi], i1 = c->gen_group_begin[gi + 1];
         if (i1 == i0) continue;
         int nthr = 128;
         while (nthr > 32 && (size_t)c->gen_group_elems[gi] * sizeof(cplx) * nthr > 200 * 1024) nthr -= 32;
         size_t smem = (size_t)c->gen_group_elems[gi] * sizeof(cplx) * nthr;
-        cudaError_t e = launch_persistent(k_dets_gen<MODE>, nthr, smem, c->n_sm, p, c->d_items_gen + i0, i1 - i0, ntiles, st);
-        if (e != cudaSuccess) return e;
+        cudaError_t e = launch_persistent(k_dets_gen<MODE>, nthr, smem, c->n_sm, p, c->d_items_gen + i0, i1 - i0, ntiles,
+                                          f.stream(li++));
+        if (e != cudaSuccess) { f.join(); return e; }
         c->launches++;
     }
-    return cudaSuccess;
+    // closed-form kernel: three register classes, items sorted by class on the host (msd_api.cu)
+    for (int cl = 2; cl >= 0; cl--) {
+        const int i0 = c->cf_class_begin[cl], i1 = c->cf_class_begin[cl + 1];
+        if (i1 == i0) continue;
+        cudaError_t e;
+        cudaStream_t s = f.stream(li++);
+        if (cl == 0) e = launch_persistent(k_dets_cf<MODE, -1, 2, 256, 3>, 256, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+        else if (cl == 1) e = launch_persistent(k_dets_cf<MODE, 2, 3, 256, 2>, 256, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+        else e = launch_persistent(k_dets_cf<MODE, 3, 4, 128, 2>, 128, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+        if (e != cudaSuccess) { f.join(); return e; }
+        c->launches++;
+    }
+    cudaError_t e = f.join();
+    return e != cudaSuccess ? e : f.err;
 }
 
 cudaError_t launch_dets(msd_ctx* c, int mode, int64_t nw, Workspace& ws, cudaStream_t st)

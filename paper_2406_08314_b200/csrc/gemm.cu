@@ -39,17 +39,22 @@ k_gemm_tn(GemmArgs g)
     extern __shared__ __align__(16) double smem_gemm[];
     double* As = smem_gemm;                                    // [STAGES][BM][LDS_]
     double* Bs = smem_gemm + STAGES * BM * LDS_;               // [STAGES][BN][LDS_]
-    const int z = blockIdx.z;
+    const int z = blockIdx.z / g.ksplit, ks = blockIdx.z - z * g.ksplit;
+    if (g.symmetric && (int)(blockIdx.x * BN + BN) / 2 - 1 < (int)(blockIdx.y * BM)) return;   // strictly lower tile
     const double* A = g.A + (int64_t)z * g.strideA;
     const double* B = g.B + (int64_t)z * g.strideB;
     const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int wm = (wid % WARPS_M) * WM, wn = (wid / WARPS_M) * WN;
     const int gq = lane >> 2, tq = lane & 3;
-    const int KT = (g.K + BK - 1) / BK;
+    const int KT_all = (g.K + BK - 1) / BK;
+    const int kt_per = (KT_all + g.ksplit - 1) / g.ksplit;
+    const int kt_begin = ks * kt_per;
+    const int KT = min(kt_per, KT_all - kt_begin);             // k-tiles of this split (may be <= 0 for the last)
+    if (KT <= 0) return;
 
     auto load_tile = [&](int stage, int kt) {
-        const int k0 = kt * BK;
+        const int k0 = (kt_begin + kt) * BK;
         double* as = As + stage * BM * LDS_;
         double* bs = Bs + stage * BN * LDS_;
         for (int c = tid; c < BM * (BK / 2); c += NT) {
@@ -115,6 +120,15 @@ k_gemm_tn(GemmArgs g)
             if (n >= g.N) continue;
             double2* dst = reinterpret_cast<double2*>(Cz + 2 * ((int64_t)m * g.cs_m + (int64_t)(n >> 1) * g.cs_j));
             double2 v = make_double2(acc[i][j][0], acc[i][j][1]);
+            if (g.symmetric) {
+                const int jc = n >> 1;
+                if (jc < m) continue;
+                *dst = v;
+                if (jc > m)
+                    *reinterpret_cast<double2*>(Cz + 2 * ((int64_t)jc * g.cs_m + (int64_t)m * g.cs_j)) = v;
+                continue;
+            }
+            if (g.accumulate == 2) { atomicAdd(&dst->x, v.x); atomicAdd(&dst->y, v.y); continue; }
             if (g.accumulate) { double2 o = *dst; v.x += o.x; v.y += o.y; }
             *dst = v;
         }
@@ -132,7 +146,7 @@ static cudaError_t launch_cfg(const GemmArgs& a, cudaStream_t st)
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    dim3 grid((a.N + BN - 1) / BN, (a.M + BM - 1) / BM, a.batch);
+    dim3 grid((a.N + BN - 1) / BN, (a.M + BM - 1) / BM, a.batch * a.ksplit);
     k_gemm_tn<BM, BN, WARPS_M, WARPS_N><<<grid, WARPS_M * WARPS_N * 32, smem, st>>>(a);
     return cudaGetLastError();
 }
@@ -142,8 +156,11 @@ cudaError_t launch_gemm_tn(const GemmArgs& a, int n_sm, cudaStream_t st)
     if (a.M <= 0 || a.N <= 0 || a.batch <= 0) return cudaSuccess;
     if ((a.N & 1) || (a.K & 1) || (a.lda & 1) || (a.ldb & 1) || (a.strideA & 1) || (a.strideB & 1))
         return cudaErrorInvalidValue;     // callers pad to even sizes (16-byte cp.async chunks)
-    int64_t big = (int64_t)((a.M + 127) / 128) * ((a.N + 63) / 64) * a.batch;
-    if (big >= 2 * (int64_t)n_sm) return launch_cfg<128, 64, 4, 2>(a, st);
+    if (a.ksplit < 1 || (a.ksplit > 1 && a.accumulate != 2) || (a.symmetric && (a.N != 2 * a.M || a.accumulate)))
+        return cudaErrorInvalidValue;
+    int64_t big = (int64_t)((a.M + 127) / 128) * ((a.N + 63) / 64) * a.batch * a.ksplit;
+    // symmetric outputs use the square 64 x 32-complex tile: finer skipping of the lower triangle
+    if (big >= 2 * (int64_t)n_sm && !a.symmetric) return launch_cfg<128, 64, 4, 2>(a, st);
     return launch_cfg<64, 64, 2, 2>(a, st);
 }
 

@@ -351,6 +351,9 @@ extern "C" void msd_destroy(msd_ctx* c)
     cudaFree(c->ws.base);
     cudaFree(c->stg_a); cudaFree(c->stg_b); cudaFree(c->stg_out); cudaFree(c->stg_flags);
     for (auto& e : c->ev) if (e) cudaEventDestroy(e);
+    for (auto& a : c->aux) if (a) cudaStreamDestroy(a);
+    for (auto& e : c->ev_join) if (e) cudaEventDestroy(e);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     delete c;
 }
 
@@ -398,6 +401,43 @@ extern "C" int msd_get_phase_ms(msd_ctx* c, float* ms, int n)
 extern "C" double msd_probe_fp64_tflops(int use_dmma, double ms, void* stream)
 {
     return probe_fp64(use_dmma, ms, (cudaStream_t)stream);
+}
+
+// ---------------------------------------------------------------------------------------------
+// fork/join over the context's side streams
+// ---------------------------------------------------------------------------------------------
+cudaStream_t Fork::stream(int i)
+{
+    if (err != cudaSuccess) return st;
+    const int a = (i - 1) % msd_ctx::NAUX;
+    if (!c->ev_fork) {
+        if ((err = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming)) != cudaSuccess) return st;
+        for (int k = 0; k < msd_ctx::NAUX; k++) {
+            if ((err = cudaStreamCreateWithFlags(&c->aux[k], cudaStreamNonBlocking)) != cudaSuccess) return st;
+            if ((err = cudaEventCreateWithFlags(&c->ev_join[k], cudaEventDisableTiming)) != cudaSuccess) return st;
+        }
+    }
+    if (!forked) {
+        if ((err = cudaEventRecord(c->ev_fork, st)) != cudaSuccess) return st;
+        forked = true;       // the fork point precedes every launch of the group, also those on st itself
+    }
+    if (i <= 0) return st;
+    if (!(used & (1 << a))) {
+        if ((err = cudaStreamWaitEvent(c->aux[a], c->ev_fork, 0)) != cudaSuccess) return st;
+        used |= 1 << a;
+    }
+    return c->aux[a];
+}
+
+cudaError_t Fork::join()
+{
+    for (int a = 0; a < msd_ctx::NAUX && err == cudaSuccess; a++) {
+        if (!(used & (1 << a))) continue;
+        if ((err = cudaEventRecord(c->ev_join[a], c->aux[a])) != cudaSuccess) break;
+        err = cudaStreamWaitEvent(st, c->ev_join[a], 0);
+    }
+    used = 0; forked = false;
+    return err;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -552,7 +592,13 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
                     a.lda = (int64_t)sp.n_r * ldN; a.ldb = (int64_t)sp.n_r * ldN;
                     a.strideA = 0; a.strideB = 0; a.batch = 1;
                     a.zdiv = 1; a.strideC_hi = 0; a.strideC_lo = 0; a.cs_m = 1; a.cs_j = ng;
-                    a.accumulate = 1;
+                    // skinny output (n_chol x 2 n_w): split K over the SMs, partial sums meet in RED.ADD.F64
+                    a.accumulate = 2;
+                    {
+                        int64_t tiles = (int64_t)((a.M + 63) / 64) * ((a.N + 63) / 64);
+                        int ks = (int)std::max<int64_t>(1, (2 * c->n_sm + tiles - 1) / tiles);
+                        a.ksplit = std::min(ks, std::max(1, a.K / 64));
+                    }
                     CK(launch_gemm_tn(a, c->n_sm, st));
                     c->launches++;
                 }
@@ -592,6 +638,7 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
                 a.zdiv = MSD_WT; a.strideC_hi = (int64_t)A_.P * B_.P * MSD_WT; a.strideC_lo = 1;
                 a.cs_m = (int64_t)B_.P * MSD_WT; a.cs_j = MSD_WT;
                 a.accumulate = 0;
+                a.symmetric = (pr > 0) ? 1 : 0;     // V^{ss}[x][y] = V^{ss}[y][x]
                 CK(launch_gemm_tn(a, c->n_sm, st));
                 c->launches++;
             }

@@ -146,6 +146,11 @@ struct msd_ctx {
     bool profiling = false;
     cudaEvent_t ev[8] = {};
     float phase_ms[6] = {};
+    // fork/join side streams: independent launches of one call (the dets kernels of different register / shared-memory
+    // classes, the per-spin GEMMs) run concurrently and rejoin the caller's stream before the call returns
+    static constexpr int NAUX = 4;
+    cudaStream_t aux[NAUX] = {};
+    cudaEvent_t ev_fork = nullptr, ev_join[NAUX] = {};
     std::string err;
     SpinDev dev(int s) const {
         SpinDev d; d.n = sp[s].n; d.n_o = sp[s].n_o; d.n_v = sp[s].n_v; d.n_r = sp[s].n_r; d.P = sp[s].P;
@@ -191,6 +196,14 @@ cudaError_t launch_finish_energy(msd_ctx* c, int64_t nw, Workspace& ws, cplx* e,
 cudaError_t launch_finish_flags(msd_ctx* c, int64_t nw, Workspace& ws, cplx* out, int64_t per_walker, int* flags,
                                 cudaStream_t st);
 
+// msd_api.cu : fork/join helper.  Fork f(c, st): launch i of a group goes to stream(i); join() makes st wait for all.
+struct Fork {
+    msd_ctx* c; cudaStream_t st; int used = 0; bool forked = false; cudaError_t err = cudaSuccess;
+    Fork(msd_ctx* c_, cudaStream_t st_) : c(c_), st(st_) {}
+    cudaStream_t stream(int i);     // i == 0: the caller's stream; i > 0: a side stream that waits for the fork point
+    cudaError_t join();
+};
+
 // gemm.cu : C[m][n] (+)= sum_k A[m][k] * B[n][k]   (both K-contiguous, FP64 DMMA m8n8k4)
 struct GemmArgs {
     const double* A; const double* B; double* C;
@@ -201,7 +214,10 @@ struct GemmArgs {
     // output addressing: column pair (2j, 2j+1) of row m is one complex at
     //   C + 2*( (z / zdiv)*strideC_hi + (z % zdiv)*strideC_lo + m*cs_m + j*cs_j )   [complex units inside]
     int zdiv; int64_t strideC_hi, strideC_lo, cs_m, cs_j;
-    int accumulate;             // 1: C += result
+    int accumulate;             // 0: C = result; 1: C += result (plain read-modify-write); 2: RED.ADD (split-K)
+    int ksplit = 1;             // grid.z = batch * ksplit; slice z % ksplit covers a BK-aligned K range (accumulate == 2)
+    int symmetric = 0;          // 1: C is complex symmetric (M == N/2, A and B describe the same rows): only tiles that
+                                //    touch the upper triangle are computed, element (m, j >= m) is also written to (j, m)
 };
 cudaError_t launch_gemm_tn(const GemmArgs& a, int n_sm, cudaStream_t st);
 double probe_fp64(int use_dmma, double ms, cudaStream_t st);
