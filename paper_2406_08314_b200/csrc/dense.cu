@@ -225,6 +225,236 @@ k_energy_dense(int n_chol, int64_t nw, SpinDev sa, SpinDev sb, const cplx* __res
     if (tid == 0) red_add(&Eacc[w * 2 + 1], cscale(-0.5, ex));
 }
 
+// ------------------------------------------------------------------------------------------------
+// S7 on the FP64 tensor cores: the same quantities as k_energy_dense (which stays as the fallback for active windows
+// wider than 16 x 16), with the two small complex products of every (walker, spin, slice) written as real DMMA
+// m8n8k4 tiles.  One WARP owns one Cholesky slice g at a time; a CTA = (chunk of slices, walker, spin).
+//   step 2   Bfull = Lam_v - Theta_v T        [Re; Im](2 n_v x n)  =  Lam_v + A'(2 n_v x 2n) B'(2n x n)
+//            A'[r][2l+c]       = -(Theta_r, -Theta_i)[c]   (Re rows)     B'[2l+c][i] = (T_r, T_i)[c]
+//            A'[half + r][2l+c] = -(Theta_i,  Theta_r)[c]   (Im rows)
+//   step 4   FK += Bfull T[:, pos]              A''[r][2l+c] = (B_r, -B_i)[c] / (B_i, B_r)[c] read straight from the
+//                                               complex Bfull tile with a per-lane component swap and sign
+// Shared-memory strides are chosen so that every fragment load is a minimal 2-wavefront access.
+// ------------------------------------------------------------------------------------------------
+struct DenseMmaLayout {
+    int half;      // n_v rounded up to 8: Im rows of the stacked outputs start here
+    int Kp;        // 2n rounded up to 4
+    int lda;       // row stride of A'     (doubles), = 4 mod 8
+    int ldt;       // row stride of T      (doubles), = 8 mod 16
+    int ldb;       // row stride of Lam_v  (doubles), = 4 mod 8
+    int trows;     // rows of the T buffer (n, +1 zero row if n is odd)
+    int warp_doubles;   // per-warp buffer: T then Lam_v/Bfull (+ slack for padded-tile over-reads)
+    __host__ __device__ static int up(int v, int m, int r) { while (v % m != r) v++; return v; }
+    __host__ __device__ DenseMmaLayout(int n, int nv) {
+        half = (nv + 7) / 8 * 8;
+        Kp = (2 * n + 3) / 4 * 4;
+        lda = up(Kp, 8, 4);
+        ldt = up(2 * n, 16, 8);
+        ldb = up(Kp, 8, 4);
+        trows = Kp / 2;
+        warp_doubles = trows * ldt + half * ldb + 64;
+        if (warp_doubles < 2 * half * 16) warp_doubles = 2 * half * 16;     // the FK partials alias this buffer
+    }
+};
+
+template <int NWARP>
+__global__ void __launch_bounds__(NWARP * 32, NWARP == 8 ? 2 : 3)
+k_energy_dense_mma(int n_chol, int64_t nw, int gchunk, SpinDev sa, SpinDev sb, const cplx* __restrict__ theta_a,
+                   const cplx* __restrict__ theta_b, const cplx* __restrict__ Lam_a, const cplx* __restrict__ Lam_b,
+                   cplx* Bp_a, cplx* Bp_b, double* Bq_a, double* Bq_b, cplx* X0 /*[2][nw][n_chol]*/, cplx* F_a, cplx* F_b,
+                   cplx* Hrot_a, cplx* Hrot_b, cplx* Eacc, int N)
+{
+    extern __shared__ __align__(16) double smd[];
+    const int s = blockIdx.z;
+    const int64_t w = blockIdx.y;
+    const SpinDev sp = s ? sb : sa;
+    const int n = sp.n, no = sp.n_o, nv = sp.n_v, nr = sp.n_r, P = sp.P;
+    if (n == 0) return;
+    const DenseMmaLayout L(n, nv);
+    const cplx* theta = (s ? theta_b : theta_a) + w * (int64_t)N * n;
+    const cplx* Lam = s ? Lam_b : Lam_a;
+    cplx* Bp = (s ? Bp_b : Bp_a) + w * (int64_t)P * n_chol;
+    double* Bq = (s ? Bq_b : Bq_a) + w * (int64_t)2 * P * 2 * n_chol;
+    cplx* F = (s ? F_b : F_a) + w * (int64_t)P;
+    cplx* Hrot = (s ? Hrot_b : Hrot_a) + w * (int64_t)P;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int gq = lane >> 2, tq = lane & 3;
+
+    double* Ap = smd;                                         // [2 half][lda]
+    double* wbuf = Ap + 2 * L.half * L.lda + wid * L.warp_doubles;
+    double* Tb = wbuf;                                        // [trows][ldt]   (i, c) interleaved
+    double* Lb = wbuf + L.trows * L.ldt;                      // [half][ldb]    Lam_v, then Bfull in place
+    int* pos = reinterpret_cast<int*>(Ap + 2 * L.half * L.lda + NWARP * L.warp_doubles);   // [16]
+
+    // zero everything once (padding must stay finite: padded K columns multiply zero rows)
+    {
+        const int tot = 2 * L.half * L.lda + NWARP * L.warp_doubles;
+        for (int e = tid; e < tot; e += NWARP * 32) smd[e] = 0.0;
+        if (tid < 16) pos[tid] = tid < no ? sp.pos_o[tid] : 0;
+    }
+    __syncthreads();
+    for (int e = tid; e < nv * n; e += NWARP * 32) {
+        const int r = e / n, l = e - r * n;
+        const cplx t = theta[(int64_t)sp.act_v[r] * n + l];
+        Ap[r * L.lda + 2 * l] = -t.x;            Ap[r * L.lda + 2 * l + 1] = t.y;
+        Ap[(L.half + r) * L.lda + 2 * l] = -t.y; Ap[(L.half + r) * L.lda + 2 * l + 1] = -t.x;
+    }
+    __syncthreads();
+
+    const int MT = 2 * L.half / 8;            // <= 4
+    const int NT = (n + 7) / 8;
+    const int KS = L.Kp / 4;
+    // per-lane constants of the step-4 fragments
+    const int posh[2] = {pos[gq], pos[8 + gq]};
+    const int kc = tq & 1, kl = tq >> 1;      // k = 4 kk + tq  ->  l = 2 kk + kl, component kc
+    double fk[4][2][2];
+#pragma unroll
+    for (int a = 0; a < 4; a++)
+#pragma unroll
+        for (int b = 0; b < 2; b++) { fk[a][b][0] = 0.0; fk[a][b][1] = 0.0; }
+    cplx ex_part = cmake(0.0, 0.0);
+
+    const int g_begin = blockIdx.x * gchunk;
+    const int g_end = min(g_begin + gchunk, n_chol + 1);
+    for (int g0 = g_begin; g0 < g_end; g0 += NWARP) {
+        const int g = g0 + wid;
+        const bool live = g < g_end;
+        if (live) {
+            // stage T^g (rows l < n) and Lam_v^g (rows n + r) of this walker: n complex = 2n doubles per row
+            const cplx* lam = Lam + ((int64_t)g * nr * nw + w) * n;
+            for (int e = lane; e < nr * n; e += 32) {
+                const int r = e / n, i = e - r * n;
+                double* dst = (r < n) ? Tb + r * L.ldt + 2 * i : Lb + (r - n) * L.ldb + 2 * i;
+                cp_async16(dst, lam + (int64_t)r * nw * n + i, 16);
+            }
+            cp_async_commit();
+            cp_async_wait<0>();
+        }
+        __syncwarp();
+        if (live) {
+            // X0 = tr T, Ex0 += sum T[l][i] T[i][l]
+            cplx tr = cmake(0.0, 0.0);
+            for (int l = lane; l < n; l += 32) tr = cadd(tr, cmake(Tb[l * L.ldt + 2 * l], Tb[l * L.ldt + 2 * l + 1]));
+            if (g < n_chol)
+                for (int e = lane; e < n * n; e += 32) {
+                    const int l = e / n, i = e - l * n;
+                    ex_part = cfma(cmake(Tb[l * L.ldt + 2 * i], Tb[l * L.ldt + 2 * i + 1]),
+                                   cmake(Tb[i * L.ldt + 2 * l], Tb[i * L.ldt + 2 * l + 1]), ex_part);
+                }
+            for (int o = 16; o > 0; o >>= 1) {
+                tr.x += __shfl_down_sync(0xffffffffu, tr.x, o);
+                tr.y += __shfl_down_sync(0xffffffffu, tr.y, o);
+            }
+            if (lane == 0) {
+                if (g < n_chol) X0[((int64_t)s * nw + w) * n_chol + g] = tr;
+                else red_add(&Eacc[w * 2 + 0], tr);
+            }
+            // step 2: Bfull = Lam_v + A' B', n-tiles in chunks of 3
+            for (int nt0 = 0; nt0 < NT; nt0 += 3) {
+                double acc[4][3][2];
+#pragma unroll
+                for (int mt = 0; mt < 4; mt++) {
+                    const int m = 8 * mt + gq, im = m >= L.half, r = m - im * L.half;
+#pragma unroll
+                    for (int j = 0; j < 3; j++) {
+                        const int i = 8 * (nt0 + j) + 2 * tq;
+                        const bool ok = mt < MT && r < nv;
+                        acc[mt][j][0] = (ok && i < n) ? Lb[r * L.ldb + 2 * i + im] : 0.0;
+                        acc[mt][j][1] = (ok && i + 1 < n) ? Lb[r * L.ldb + 2 * i + 2 + im] : 0.0;
+                    }
+                }
+                for (int kk = 0; kk < KS; kk++) {
+                    double a[4], b[3];
+#pragma unroll
+                    for (int mt = 0; mt < 4; mt++) a[mt] = mt < MT ? Ap[(8 * mt + gq) * L.lda + 4 * kk + tq] : 0.0;
+#pragma unroll
+                    for (int j = 0; j < 3; j++)
+                        b[j] = (nt0 + j < NT) ? Tb[(2 * kk + kl) * L.ldt + 2 * (8 * (nt0 + j) + gq) + kc] : 0.0;
+#pragma unroll
+                    for (int mt = 0; mt < 4; mt++)
+#pragma unroll
+                        for (int j = 0; j < 3; j++) dmma884(acc[mt][j][0], acc[mt][j][1], a[mt], b[j]);
+                }
+#pragma unroll
+                for (int mt = 0; mt < 4; mt++) {
+                    const int m = 8 * mt + gq, im = m >= L.half, r = m - im * L.half;
+#pragma unroll
+                    for (int j = 0; j < 3; j++) {
+                        const int i = 8 * (nt0 + j) + 2 * tq;
+                        const bool ok = mt < MT && r < nv;
+                        if (ok && i < n) Lb[r * L.ldb + 2 * i + im] = acc[mt][j][0];
+                        if (ok && i + 1 < n) Lb[r * L.ldb + 2 * i + 2 + im] = acc[mt][j][1];
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if (live && g < n_chol) {
+            // step 4: FK += A''(Bfull) B''(T[:, pos])
+            for (int kk = 0; kk < KS; kk++) {
+                double a[4], b[2];
+#pragma unroll
+                for (int mt = 0; mt < 4; mt++) {
+                    const int m = 8 * mt + gq, im = m >= L.half, r = m - im * L.half;
+                    double v = mt < MT ? Lb[r * L.ldb + 2 * (2 * kk + kl) + (kc ^ im)] : 0.0;
+                    a[mt] = (!im && kc) ? -v : v;
+                }
+#pragma unroll
+                for (int j = 0; j < 2; j++) b[j] = Tb[(2 * kk + kl) * L.ldt + 2 * posh[j] + kc];
+#pragma unroll
+                for (int mt = 0; mt < 4; mt++)
+#pragma unroll
+                    for (int j = 0; j < 2; j++) dmma884(fk[mt][j][0], fk[mt][j][1], a[mt], b[j]);
+            }
+        }
+        __syncthreads();
+        // cooperative output of the round's slices: thread (x, gi) -> NWARP consecutive slices of one pair index
+        {
+            const int gcount = min(NWARP, g_end - g0);
+            for (int e = tid; e < P * NWARP; e += NWARP * 32) {
+                const int x = e / NWARP, gi = e - x * NWARP;
+                if (gi >= gcount) continue;
+                const int g = g0 + gi;
+                const int r = x / no, h = x - r * no;
+                const double* lb = Ap + 2 * L.half * L.lda + gi * L.warp_doubles + L.trows * L.ldt;
+                const cplx b = cmake(lb[r * L.ldb + 2 * pos[h]], lb[r * L.ldb + 2 * pos[h] + 1]);
+                if (g < n_chol) {
+                    Bp[(int64_t)x * n_chol + g] = b;
+                    double* q0 = Bq + ((int64_t)(2 * x) * 2 * n_chol) + 2 * g;
+                    *reinterpret_cast<double2*>(q0) = make_double2(b.x, -b.y);
+                    *reinterpret_cast<double2*>(q0 + 2 * n_chol) = make_double2(b.y, b.x);
+                } else {
+                    Hrot[x] = b;
+                }
+            }
+        }
+        __syncthreads();
+    }
+
+    // FK: sum the warps' partial tiles, then F -= FK (exchange-like part of F, W9); Ex0
+    double* red = Ap + 2 * L.half * L.lda;                   // aliases the warp buffers (all reads are done)
+#pragma unroll
+    for (int mt = 0; mt < 4; mt++)
+#pragma unroll
+        for (int j = 0; j < 2; j++) {
+            if (mt >= MT) continue;
+            double* dst = red + ((wid * 2 * L.half) + 8 * mt + gq) * 16 + 8 * j + 2 * tq;
+            dst[0] = fk[mt][j][0]; dst[1] = fk[mt][j][1];
+        }
+    __syncthreads();
+    for (int x = tid; x < P; x += NWARP * 32) {
+        const int r = x / no, h = x - r * no;
+        double re = 0.0, im = 0.0;
+        for (int ww = 0; ww < NWARP; ww++) {
+            re += red[((ww * 2 * L.half) + r) * 16 + h];
+            im += red[((ww * 2 * L.half) + L.half + r) * 16 + h];
+        }
+        red_add(&F[x], cmake(-re, -im));
+    }
+    cplx ex = block_sum(ex_part);
+    if (tid == 0) red_add(&Eacc[w * 2 + 1], cscale(-0.5, ex));
+}
+
 // F[x] += sum_g Xt_g B^g[x]  (Coulomb-like part of F, W9);   one warp per x
 __global__ void __launch_bounds__(256)
 k_fx(int n_chol, int64_t nw, int Pa, int Pb, const cplx* __restrict__ X0, const cplx* __restrict__ Bp_a,
@@ -248,29 +478,61 @@ k_fx(int n_chol, int64_t nw, int Pa, int Pb, const cplx* __restrict__ X0, const 
     if (lane == 0) { cplx* F = (s ? F_b : F_a) + w * (int64_t)P + x; *F = cadd(*F, acc); }
 }
 
+template <int NWARP>
+static cudaError_t launch_dense_mma(msd_ctx* c, int64_t nw, Workspace& ws, size_t smem, cudaStream_t st)
+{
+    cudaError_t e = cudaFuncSetAttribute(k_energy_dense_mma<NWARP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const int gchunk = 4 * NWARP;
+    dim3 grid((c->n_chol + 1 + gchunk - 1) / gchunk, (unsigned)nw, 2);
+    k_energy_dense_mma<NWARP><<<grid, NWARP * 32, smem, st>>>(c->n_chol, nw, gchunk, c->dev(0), c->dev(1), ws.theta[0],
+                                                             ws.theta[1], ws.Lam[0], ws.Lam[1], ws.Bp[0], ws.Bp[1], ws.Bq[0],
+                                                             ws.Bq[1], ws.X0, ws.F[0], ws.F[1], ws.Hrot[0], ws.Hrot[1],
+                                                             ws.Eacc, c->N);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_energy_dense(msd_ctx* c, int64_t nw, Workspace& ws, cudaStream_t st)
 {
     if (nw == 0) return cudaSuccess;
-    constexpr int GC = 8;
-    size_t smem = 0;
+    // tensor-core kernel when both active windows fit its register tiles (n_o, n_v <= 16), scalar kernel otherwise
+    bool mma_ok = true;
+    size_t need[2] = {0, 0};     // shared memory with 8 / 4 warps
     for (int s = 0; s < 2; s++) {
         const auto& sp = c->sp[s];
-        size_t v = ((size_t)sp.n * sp.n + 2 * (size_t)sp.n_v * sp.n + (size_t)sp.P * (1 + GC) + 1) * sizeof(cplx) +
-                   (size_t)(sp.n_o + 4) * sizeof(int);
-        if (v > smem) smem = v;
+        if (sp.n == 0) continue;
+        if (sp.n_o > 16 || sp.n_v > 16) mma_ok = false;
+        DenseMmaLayout L(sp.n, sp.n_v);
+        for (int k = 0; k < 2; k++) {
+            size_t v = ((size_t)2 * L.half * L.lda + (size_t)(k ? 4 : 8) * L.warp_doubles) * sizeof(double) + 64;
+            if (v > need[k]) need[k] = v;
+        }
     }
-    if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
-    cudaError_t e = cudaFuncSetAttribute(k_energy_dense<GC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    // X0 of a spin with no electrons must read as zero: ws.X0 lies in the region zeroed per call
-    dim3 grid((c->n_chol + 1 + GC - 1) / GC, (unsigned)nw, 2);
-    cplx* X0 = ws.X0;
-    k_energy_dense<GC><<<grid, 256, smem, st>>>(c->n_chol, nw, c->dev(0), c->dev(1), ws.theta[0], ws.theta[1],
-                                                ws.Lam[0], ws.Lam[1], ws.Bp[0], ws.Bp[1], ws.Bq[0], ws.Bq[1], X0,
-                                                ws.F[0], ws.F[1], ws.Hrot[0], ws.Hrot[1], ws.Eacc, c->N);
+    cudaError_t e = cudaSuccess;
+    if (mma_ok && need[0] <= 113 * 1024) e = launch_dense_mma<8>(c, nw, ws, need[0], st);
+    else if (mma_ok && need[1] <= 227 * 1024) e = launch_dense_mma<4>(c, nw, ws, need[1], st);
+    else {
+        constexpr int GC = 8;
+        size_t smem = 0;
+        for (int s = 0; s < 2; s++) {
+            const auto& sp = c->sp[s];
+            size_t v = ((size_t)sp.n * sp.n + 2 * (size_t)sp.n_v * sp.n + (size_t)sp.P * (1 + GC) + 1) * sizeof(cplx) +
+                       (size_t)(sp.n_o + 4) * sizeof(int);
+            if (v > smem) smem = v;
+        }
+        if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
+        e = cudaFuncSetAttribute(k_energy_dense<GC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        // X0 of a spin with no electrons must read as zero: ws.X0 lies in the region zeroed per call
+        dim3 grid((c->n_chol + 1 + GC - 1) / GC, (unsigned)nw, 2);
+        k_energy_dense<GC><<<grid, 256, smem, st>>>(c->n_chol, nw, c->dev(0), c->dev(1), ws.theta[0], ws.theta[1],
+                                                    ws.Lam[0], ws.Lam[1], ws.Bp[0], ws.Bp[1], ws.Bq[0], ws.Bq[1], ws.X0,
+                                                    ws.F[0], ws.F[1], ws.Hrot[0], ws.Hrot[1], ws.Eacc, c->N);
+        e = cudaGetLastError();
+    }
     c->launches++;
-    e = cudaGetLastError();
     if (e != cudaSuccess) return e;
+    cplx* X0 = ws.X0;
     int Pmax = c->sp[0].P > c->sp[1].P ? c->sp[0].P : c->sp[1].P;
     if (Pmax > 0) {
         dim3 g2((Pmax + 7) / 8, (unsigned)nw, 2);

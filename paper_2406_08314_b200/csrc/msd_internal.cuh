@@ -55,6 +55,21 @@ __device__ __forceinline__ cplx load_planar(const double* p, int x) {
     return make_double2(p[x * (2 * MSD_WT)], p[x * (2 * MSD_WT) + MSD_WT]);
 }
 
+// cp.async (16-byte, L2-only) and the FP64 tensor-core tile D(8x8) += A(8x4) B(4x8)
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, int src_bytes)
+{
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
 // ---------------------------------------------------------------------------------------------
 // packed trial (device pointers live in the context; this POD is passed to kernels by value)
 // ---------------------------------------------------------------------------------------------
