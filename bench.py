@@ -53,6 +53,20 @@ def reduce_max_time(ms: float, world: int, device=None) -> float:
     return float(t.item())
 
 
+def ncu_traffic(kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, averaged over its launches of one step,
+    from the committed ncu --set full summary (profiles/r01c_traffic.csv); None if the file is absent."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "r01c_traffic.csv")
+    try:
+        rows = [r for r in csv.DictReader(open(path)) if r["kernel"] == kernel]
+    except OSError:
+        return None
+    if not rows:
+        return None
+    return sum(float(r["dram_read_bytes"]) + float(r["dram_write_bytes"]) for r in rows) / len(rows)
+
+
 def total_units(n_w: int, n_det: int, steps: int, world: int) -> float:
     return float(n_w) * float(n_det) * steps * world
 
@@ -282,7 +296,8 @@ def main():
                     "peak_source": "measured live: register-resident DMMA m8n8k4 loop (msd_probe_fp64_tflops); "
                                    "MEASURED_PEAKS.json has no FP64 entry; derived 148 SM x 64 FMA/clk x 1.965 GHz = %.1f"
                                    % FP64_PEAK_DERIVED,
-                    "traffic": None,
+                    "traffic": ncu_traffic("k_gemm_tn"),
+                    "traffic_note": "DRAM bytes per launch (mean of the 5 launches), ncu --set full, profiles/r01c_traffic.csv",
                     "share_of_step": gemm_ms / (sum(step_ms) / len(step_ms)),
                     "algorithmic_flops_per_step": flops_v + flops_lam}
 
