@@ -9,10 +9,12 @@
 //   R = det M,  A = adj M (A[b][a] = cofactor of M[a][b]),  T[b,d;a,c] = signed complementary (k-2) minor
 //   W      += c~ R^a R^b
 //   C^s[x] += c~ R^sbar A^s[b][a]               x = (p_b, h_a)
-//   E2nd   += c~ [ sum A^a[b][a] A^b[b'][a'] Vab[x][x'] + sum_s R^sbar sum_{a<c,b<d} T^s (Vss[x_ab][x_cd] - Vss[x_ad][x_cb]) ]
+//   E2nd   += c~ [ sum A^a[b][a] A^b[b'][a'] Vab[x][x'] + sum_s R^sbar sum_{a<c,b<d} T^s Vbar^s[x_ab][x_cd] ]
+//   Vbar^s[x_ab][x_cd] = V^ss[x_ab][x_cd] - V^ss[x_ad][x_cb]  (k_vbar, in place on the h_a<h_c, p_b<p_d entries of Vss)
 // Levels <= 4 use division-free closed forms in registers (exact for singular minors: pin P7);
 // higher levels use in-place Gauss-Jordan with partial pivoting in shared memory (one matrix per thread).
 #include "msd_internal.cuh"
+#include <algorithm>
 
 struct DetsParams {
     const unsigned char* tab;
@@ -20,7 +22,7 @@ struct DetsParams {
     const cplx* g[2];      // [nt][P][WT]
     double* C[2];          // [nt][P][2][WT] planar
     const cplx* Vab;       // [nt][Pa][Pb][WT]
-    const cplx* Vss[2];    // [nt][P][P][WT]
+    const cplx* Vss[2];    // [nt][P][P][WT]; entries (h_a<h_c, p_b<p_d) hold the antisymmetrised Vbar (k_vbar)
     cplx* Wacc;            // [nt*WT]
     cplx* E2nd;            // [nt*WT]
     int no[2], P[2];
@@ -164,9 +166,7 @@ struct SpinEval {
 #pragma unroll
                         for (int d = b + 1; d < K; d++) {
                             cplx t = second_cofactor<K>(M, a, c, b, d);
-                            cplx v1 = __ldg(&Vss[((unsigned)x(a, b) * P + (unsigned)x(c, d)) * MSD_WT]);
-                            cplx v2 = __ldg(&Vss[((unsigned)x(a, d) * P + (unsigned)x(c, b)) * MSD_WT]);
-                            Ess = cfma(t, csub(v1, v2), Ess);
+                            Ess = cfma(t, __ldg(&Vss[((unsigned)x(a, b) * P + (unsigned)x(c, d)) * MSD_WT]), Ess);
                         }
         }
     }
@@ -323,11 +323,18 @@ __global__ void __launch_bounds__(NTHR, MINB) k_dets_cf(DetsParams p, const Work
 
 // ------------------------------------------------------------------------------------------------
 // generic levels (k >= 5 in at least one spin): one matrix per thread in shared memory, element e of
-// thread t at sm[e * T + t] (consecutive lanes -> consecutive 16-byte words: conflict-free for any per-lane e)
+// thread t at sm[e * T + t] (consecutive lanes -> consecutive 16-byte words: conflict-free for any per-lane e).
+// After a spin is evaluated its region holds A (entry e = b*k+a is A[b][a]) and the int region holds the pair
+// index x(a,b) of the same entry.  Levels 5..8 run with compile-time K (unrolled gathers: K^2 / C(K,2) independent
+// L2 loads in flight per thread); anything above 8 takes the runtime-k path.
 // ------------------------------------------------------------------------------------------------
 struct SmMat {
     cplx* base; int T;
     __device__ __forceinline__ cplx& at(int e) { return base[e * T]; }
+};
+struct SmIdx {
+    int* base; int T;
+    __device__ __forceinline__ int& at(int e) { return base[e * T]; }
 };
 
 // in-place Gauss-Jordan inverse with partial pivoting; returns det (0 if an exactly zero pivot appears,
@@ -370,22 +377,85 @@ __device__ cplx gauss_jordan(SmMat m, int k)
     return det;
 }
 
-struct HP { int h[MSD_MAX_LEVEL], pn[MSD_MAX_LEVEL]; __device__ __forceinline__ int x(int a, int b) const { return pn[b] + h[a]; } };
-
+// the same elimination with compile-time K: the scaled pivot row lives in registers, so every update is one
+// shared-memory load and one store
 template <int K>
-__device__ __forceinline__ cplx closed_to_smem(SmMat m, cplx* Ess, const HP& q, const cplx* __restrict__ Vss, unsigned P,
-                                               int mode)
+__device__ __forceinline__ cplx gauss_jordan_t(SmMat m)
 {
+    unsigned ipiv = 0u;                       // 4 bits per pivot row (K <= 8)
+    cplx det = cmake(1.0, 0.0);
+    bool sing = false;
+#pragma unroll 1
+    for (int j = 0; j < K; j++) {
+        int p = j; double best = cabs2(m.at(j * K + j));
+#pragma unroll
+        for (int i = 1; i < K; i++) {
+            if (i > j) { double v = cabs2(m.at(i * K + j)); if (v > best) { best = v; p = i; } }
+        }
+        ipiv |= (unsigned)p << (4 * j);
+        if (!(best > 0.0)) { sing = true; break; }
+        cplx prow[K];
+#pragma unroll
+        for (int c = 0; c < K; c++) prow[c] = m.at(p * K + c);
+        if (p != j) {
+#pragma unroll
+            for (int c = 0; c < K; c++) m.at(p * K + c) = m.at(j * K + c);
+            det = cneg(det);
+        }
+        cplx pv = cmake(0.0, 0.0);
+#pragma unroll
+        for (int c = 0; c < K; c++) if (c == j) { pv = prow[c]; prow[c] = cmake(1.0, 0.0); }
+        det = cmul(det, pv);
+        const cplx r = cinv(pv);
+#pragma unroll
+        for (int c = 0; c < K; c++) { prow[c] = cmul(prow[c], r); m.at(j * K + c) = prow[c]; }
+#pragma unroll
+        for (int i = 0; i < K; i++) {
+            if (i == j) continue;
+            const cplx f = m.at(i * K + j);
+#pragma unroll
+            for (int c = 0; c < K; c++) {
+                cplx v = m.at(i * K + c);
+                if (c == j) v = cmake(0.0, 0.0);
+                m.at(i * K + c) = cfms(f, prow[c], v);
+            }
+        }
+    }
+    if (sing) {
+#pragma unroll
+        for (int e = 0; e < K * K; e++) m.at(e) = cmake(0.0, 0.0);
+        return cmake(0.0, 0.0);
+    }
+#pragma unroll 1
+    for (int j = K - 1; j >= 0; j--) {
+        const int p = (int)((ipiv >> (4 * j)) & 15u);
+        if (p != j) {
+#pragma unroll
+            for (int i = 0; i < K; i++) { cplx t = m.at(i * K + j); m.at(i * K + j) = m.at(i * K + p); m.at(i * K + p) = t; }
+        }
+    }
+    return det;
+}
+
+// levels 1..4 inside the generic kernel (the other spin of a high-level bucket): closed forms in registers,
+// A and x written to the thread's shared-memory regions
+template <int K>
+__device__ __forceinline__ cplx closed_to_smem(SmMat m, SmIdx xs, const unsigned char* hp, const cplx* __restrict__ g, int no,
+                                               cplx* Ess, const cplx* __restrict__ Vss, unsigned P, int mode)
+{
+    int h[K], pn[K];
+#pragma unroll
+    for (int a = 0; a < K; a++) { h[a] = (int)hp[a]; pn[a] = (int)hp[K + a] * no; }
     cplx M[K][K], A[K][K];
 #pragma unroll
     for (int a = 0; a < K; a++)
 #pragma unroll
-        for (int b = 0; b < K; b++) M[a][b] = m.at(a * K + b);
+        for (int b = 0; b < K; b++) M[a][b] = __ldg(&g[(pn[b] + h[a]) * MSD_WT]);
     cplx R = Closed<K>::det_adj(M, A);
 #pragma unroll
     for (int a = 0; a < K; a++)
 #pragma unroll
-        for (int b = 0; b < K; b++) m.at(b * K + a) = A[b][a];
+        for (int b = 0; b < K; b++) { m.at(b * K + a) = A[b][a]; xs.at(b * K + a) = pn[b] + h[a]; }
     cplx e = cmake(0.0, 0.0);
     if (mode == 2 && K >= 2) {
 #pragma unroll
@@ -397,47 +467,99 @@ __device__ __forceinline__ cplx closed_to_smem(SmMat m, cplx* Ess, const HP& q, 
 #pragma unroll
                     for (int d = b + 1; d < K; d++) {
                         cplx t = second_cofactor<K>(M, a, c, b, d);
-                        cplx v1 = __ldg(&Vss[((unsigned)q.x(a, b) * P + (unsigned)q.x(c, d)) * MSD_WT]);
-                        cplx v2 = __ldg(&Vss[((unsigned)q.x(a, d) * P + (unsigned)q.x(c, b)) * MSD_WT]);
-                        e = cfma(t, csub(v1, v2), e);
+                        e = cfma(t, __ldg(&Vss[((unsigned)(pn[b] + h[a]) * P + (unsigned)(pn[d] + h[c])) * MSD_WT]), e);
                     }
     }
     *Ess = e;
     return R;
 }
 
-// one spin, runtime level k; on exit m holds A (A[b][a] at element b*k+a), returns R, *Ess
-__device__ cplx spin_generic(SmMat m, int k, const unsigned char* hp, const cplx* __restrict__ g, int no, HP& q,
-                             const cplx* __restrict__ Vss, unsigned P, int mode, cplx* Ess)
+// levels 5..8 with compile-time K: gather, Gauss-Jordan, A = R M^-1, and the same-spin second-order sum
+//   Ess = (1/R) sum_{a<c} sum_{b<d} (A[b][a] A[d][c] - A[b][c] A[d][a]) Vbar[x_ab][x_cd]        (Jacobi)
+// with columns a and c of A in registers and the C(K,2) loads of one (a,c) pair independent of one another.
+template <int K, int MODE>
+__device__ __noinline__ cplx spin_big(cplx* mbase, int* xbase, int T, const unsigned char* hp, const cplx* __restrict__ g, int no,
+                                      const cplx* __restrict__ Vss, unsigned P, cplx* Ess)
 {
-    *Ess = cmake(0.0, 0.0);
-    if (k == 0) return cmake(1.0, 0.0);
-    for (int a = 0; a < k; a++) { q.h[a] = (int)hp[a]; q.pn[a] = (int)hp[k + a] * no; }
-    for (int a = 0; a < k; a++)
-        for (int b = 0; b < k; b++) m.at(a * k + b) = __ldg(&g[q.x(a, b) * MSD_WT]);
-    switch (k) {
-        case 1: return closed_to_smem<1>(m, Ess, q, Vss, P, mode);
-        case 2: return closed_to_smem<2>(m, Ess, q, Vss, P, mode);
-        case 3: return closed_to_smem<3>(m, Ess, q, Vss, P, mode);
-        case 4: return closed_to_smem<4>(m, Ess, q, Vss, P, mode);
-        default: break;
+    SmMat m{mbase, T};
+    SmIdx xs{xbase, T};
+    int pn[K];
+    unsigned long long hpack = 0ull;
+#pragma unroll
+    for (int a = 0; a < K; a++) { hpack |= (unsigned long long)hp[a] << (8 * a); pn[a] = (int)hp[K + a] * no; }
+#pragma unroll
+    for (int a = 0; a < K; a++) {
+        const int ha = (int)((hpack >> (8 * a)) & 255ull);
+        cplx row[K];
+#pragma unroll
+        for (int b = 0; b < K; b++) row[b] = __ldg(&g[(pn[b] + ha) * MSD_WT]);
+#pragma unroll
+        for (int b = 0; b < K; b++) { m.at(a * K + b) = row[b]; xs.at(b * K + a) = pn[b] + ha; }
     }
-    cplx R = gauss_jordan(m, k);          // m = M^-1 (or zeros)
-    for (int e = 0; e < k * k; e++) m.at(e) = cmul(R, m.at(e));   // A = R M^-1
+    const cplx R = gauss_jordan_t<K>(m);          // m = M^-1 (or zeros)
+#pragma unroll
+    for (int e = 0; e < K * K; e++) m.at(e) = cmul(R, m.at(e));   // A = R M^-1, entry b*K+a = A[b][a]
+    *Ess = cmake(0.0, 0.0);
+    if (MODE == 2 && (R.x != 0.0 || R.y != 0.0)) {
+        cplx e2[2] = {cmake(0.0, 0.0), cmake(0.0, 0.0)};      // two chains: the FMA latency is not on the critical path
+#pragma unroll 1
+        for (int a = 0; a < K - 1; a++) {
+            const unsigned ha = (unsigned)((hpack >> (8 * a)) & 255ull);
+            cplx ca[K];
+#pragma unroll
+            for (int b = 0; b < K; b++) ca[b] = m.at(b * K + a);
+#pragma unroll 1
+            for (int c = a + 1; c < K; c++) {
+                const unsigned hc = (unsigned)((hpack >> (8 * c)) & 255ull);
+                const cplx* vac = Vss + (ha * P + hc) * MSD_WT;       // x_ab P + x_cd = (pn_b P + pn_d) + (h_a P + h_c)
+                cplx cc[K];
+#pragma unroll
+                for (int b = 0; b < K; b++) cc[b] = m.at(b * K + c);
+#pragma unroll
+                for (int b = 0; b < K; b++)
+#pragma unroll
+                    for (int d = b + 1; d < K; d++) {
+                        const cplx v = __ldg(vac + ((unsigned)pn[b] * P + (unsigned)pn[d]) * MSD_WT);
+                        cplx t = cmul(ca[b], cc[d]);
+                        t = cfms(cc[b], ca[d], t);
+                        e2[(b + d) & 1] = cfma(t, v, e2[(b + d) & 1]);
+                    }
+            }
+        }
+        *Ess = cmul(cadd(e2[0], e2[1]), cinv(R));
+    }
+    return R;
+}
+
+// any level, runtime k (levels above 8)
+__device__ __noinline__ cplx spin_runtime(cplx* mbase, int* xbase, int T, int k, const unsigned char* hp,
+                                          const cplx* __restrict__ g, int no, const cplx* __restrict__ Vss, unsigned P, int mode,
+                                          cplx* Ess)
+{
+    SmMat m{mbase, T};
+    SmIdx xs{xbase, T};
+    for (int a = 0; a < k; a++)
+        for (int b = 0; b < k; b++) {
+            const int x = (int)hp[k + b] * no + (int)hp[a];
+            m.at(a * k + b) = __ldg(&g[x * MSD_WT]);
+            xs.at(b * k + a) = x;
+        }
+    cplx R = gauss_jordan(m, k);
+    for (int e = 0; e < k * k; e++) m.at(e) = cmul(R, m.at(e));
+    *Ess = cmake(0.0, 0.0);
     if (mode == 2 && (R.x != 0.0 || R.y != 0.0)) {
-        // T[b,d;a,c] = R (Minv[b][a] Minv[d][c] - Minv[b][c] Minv[d][a]) = (A[b][a] A[d][c] - A[b][c] A[d][a]) / R
         cplx e = cmake(0.0, 0.0);
         for (int a = 0; a < k; a++)
             for (int c = a + 1; c < k; c++)
                 for (int b = 0; b < k; b++) {
                     const cplx Aba = m.at(b * k + a), Abc = m.at(b * k + c);
-                    const unsigned xab = (unsigned)q.x(a, b) * P, xcb = (unsigned)q.x(c, b);
+                    const unsigned xab = (unsigned)xs.at(b * k + a) * P;
+#pragma unroll 4
                     for (int d = b + 1; d < k; d++) {
+                        const cplx v = __ldg(&Vss[(xab + (unsigned)xs.at(d * k + c)) * MSD_WT]);
                         cplx t = cmul(Aba, m.at(d * k + c));
                         t = cfms(Abc, m.at(d * k + a), t);
-                        cplx v1 = __ldg(&Vss[(xab + (unsigned)q.x(c, d)) * MSD_WT]);
-                        cplx v2 = __ldg(&Vss[((unsigned)q.x(a, d) * P + xcb) * MSD_WT]);
-                        e = cfma(t, csub(v1, v2), e);
+                        e = cfma(t, v, e);
                     }
                 }
         *Ess = cmul(e, cinv(R));
@@ -445,7 +567,65 @@ __device__ cplx spin_generic(SmMat m, int k, const unsigned char* hp, const cplx
     return R;
 }
 
-// Persistent per walker tile like k_dets_cf; shared memory = g tile + (max ka^2+kb^2 of the launch) per thread.
+template <int MODE>
+__device__ __forceinline__ cplx spin_any(cplx* mbase, int* xbase, int T, int k, const unsigned char* hp, const cplx* __restrict__ g,
+                                         int no, const cplx* __restrict__ Vss, unsigned P, cplx* Ess)
+{
+    SmMat m{mbase, T};
+    SmIdx xs{xbase, T};
+    switch (k) {
+        case 0: *Ess = cmake(0.0, 0.0); return cmake(1.0, 0.0);
+        case 1: return closed_to_smem<1>(m, xs, hp, g, no, Ess, Vss, P, MODE);
+        case 2: return closed_to_smem<2>(m, xs, hp, g, no, Ess, Vss, P, MODE);
+        case 3: return closed_to_smem<3>(m, xs, hp, g, no, Ess, Vss, P, MODE);
+        case 4: return closed_to_smem<4>(m, xs, hp, g, no, Ess, Vss, P, MODE);
+        case 5: return spin_big<5, MODE>(mbase, xbase, T, hp, g, no, Vss, P, Ess);
+        case 6: return spin_big<6, MODE>(mbase, xbase, T, hp, g, no, Vss, P, Ess);
+        case 7: return spin_big<7, MODE>(mbase, xbase, T, hp, g, no, Vss, P, Ess);
+        case 8: return spin_big<8, MODE>(mbase, xbase, T, hp, g, no, Vss, P, Ess);
+        default: return spin_runtime(mbase, xbase, T, k, hp, g, no, Vss, P, MODE, Ess);
+    }
+}
+
+// opposite-spin second-order sum  sum_v As[v] sum_u Ab[u] Vab[x_u, x_v]:  the K^2 loads of the higher-level spin
+// are unrolled (independent, four accumulators), the other spin's entries are a runtime loop
+template <int K>
+__device__ __noinline__ cplx opp_big(const cplx* mbig, const int* xbig, const cplx* msm, const int* xsm, int T, int ns,
+                                     const cplx* __restrict__ V, unsigned sbig, unsigned ssm)
+{
+    cplx e = cmake(0.0, 0.0);
+#pragma unroll 1
+    for (int v = 0; v < ns; v++) {
+        const cplx As = msm[v * T];
+        const cplx* vp = V + (unsigned)xsm[v * T] * ssm * MSD_WT;
+        cplx z[4];
+#pragma unroll
+        for (int t = 0; t < 4; t++) z[t] = cmake(0.0, 0.0);
+#pragma unroll
+        for (int u = 0; u < K * K; u++)
+            z[u & 3] = cfma(mbig[u * T], __ldg(vp + (unsigned)xbig[u * T] * sbig * MSD_WT), z[u & 3]);
+        e = cfma(As, cadd(cadd(z[0], z[1]), cadd(z[2], z[3])), e);
+    }
+    return e;
+}
+
+__device__ __noinline__ cplx opp_runtime(const cplx* mbig, const int* xbig, int nb, const cplx* msm, const int* xsm, int T, int ns,
+                                         const cplx* __restrict__ V, unsigned sbig, unsigned ssm)
+{
+    cplx e = cmake(0.0, 0.0);
+    for (int v = 0; v < ns; v++) {
+        const cplx As = msm[v * T];
+        const cplx* vp = V + (unsigned)xsm[v * T] * ssm * MSD_WT;
+        cplx z = cmake(0.0, 0.0);
+#pragma unroll 4
+        for (int u = 0; u < nb; u++) z = cfma(mbig[u * T], __ldg(vp + (unsigned)xbig[u * T] * sbig * MSD_WT), z);
+        e = cfma(As, z, e);
+    }
+    return e;
+}
+
+// Persistent per walker tile like k_dets_cf; shared memory per thread = (ka^2+kb^2) x (complex + int), bounded by the
+// launch group's element count.
 template <int MODE>
 __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkItem* __restrict__ items, int n_items)
 {
@@ -455,7 +635,6 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
     const int j = threadIdx.x & (MSD_WT - 1);
     const int slot = threadIdx.x / MSD_WT, nslots = blockDim.x / MSD_WT;
     const int T = blockDim.x;
-    cplx* sm = gsm + threadIdx.x;
     const cplx* gA = p.g[0] + (int64_t)tile * p.P[0] * MSD_WT + j;      // L1/L2 resident (57 KB per tile)
     const cplx* gB = p.g[1] + (int64_t)tile * p.P[1] * MSD_WT + j;
     double* CA = p.C[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j;
@@ -470,43 +649,79 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
         if (ii >= n_items) continue;
         const WorkItem it = items[ii];
         const int ka = it.ka, kb = it.kb;
-        SmMat mA{sm, T}, mB{sm + ka * ka * T, T};
+        const int na = ka * ka, nb = kb * kb;
+        cplx* mA = gsm + threadIdx.x;
+        cplx* mB = mA + na * T;
+        int* xA = reinterpret_cast<int*>(gsm + (na + nb) * T) + threadIdx.x;
+        int* xB = xA + na * T;
         for (int i = slot; i < it.det_count; i += nslots) {
             const uint32_t* rp = reinterpret_cast<const uint32_t*>(p.tab + it.tab_off + (int64_t)i * it.rs);
             union { uint32_t w[MSD_MAX_LEVEL]; unsigned char b[4 * MSD_MAX_LEVEL]; } row;
             for (int t = 0; t < it.rs / 4; t++) row.w[t] = __ldg(rp + t);
             const double cf = __ldg(&p.coef[it.det_begin + i]);
-            HP qa, qb;
             cplx EssA, EssB;
-            cplx Ra = spin_generic(mA, ka, row.b, gA, p.no[0], qa, VA, (unsigned)p.P[0], MODE, &EssA);
-            cplx Rb = spin_generic(mB, kb, row.b + 2 * ka, gB, p.no[1], qb, VB, (unsigned)p.P[1], MODE, &EssB);
+            const cplx Ra = spin_any<MODE>(mA, xA, T, ka, row.b, gA, p.no[0], VA, (unsigned)p.P[0], &EssA);
+            const cplx Rb = spin_any<MODE>(mB, xB, T, kb, row.b + 2 * ka, gB, p.no[1], VB, (unsigned)p.P[1], &EssB);
             const cplx cRa = cscale(cf, Ra), cRb = cscale(cf, Rb);
             Wl = cfma(cRa, Rb, Wl);
             if (MODE == 2) {
                 cplx e = cmake(0.0, 0.0);
-                for (int a = 0; a < ka; a++)
-                    for (int b = 0; b < ka; b++) {
-                        const cplx* vrow = VAB + (unsigned)qa.x(a, b) * (unsigned)p.P[1] * MSD_WT;
-                        cplx z = cmake(0.0, 0.0);
-                        for (int a2 = 0; a2 < kb; a2++)
-                            for (int b2 = 0; b2 < kb; b2++)
-                                z = cfma(mB.at(b2 * kb + a2), __ldg(&vrow[qb.x(a2, b2) * MSD_WT]), z);
-                        e = cfma(mA.at(b * ka + a), z, e);
+                if (na > 0 && nb > 0) {
+                    const bool abig = ka >= kb;
+                    const cplx* mb_ = abig ? mA : mB; const int* xb_ = abig ? xA : xB;
+                    const cplx* ms_ = abig ? mB : mA; const int* xs_ = abig ? xB : xA;
+                    const unsigned sbig = abig ? (unsigned)p.P[1] : 1u, ssm = abig ? 1u : (unsigned)p.P[1];
+                    const int ns = abig ? nb : na;
+                    switch (abig ? ka : kb) {
+                        case 5: e = opp_big<5>(mb_, xb_, ms_, xs_, T, ns, VAB, sbig, ssm); break;
+                        case 6: e = opp_big<6>(mb_, xb_, ms_, xs_, T, ns, VAB, sbig, ssm); break;
+                        case 7: e = opp_big<7>(mb_, xb_, ms_, xs_, T, ns, VAB, sbig, ssm); break;
+                        case 8: e = opp_big<8>(mb_, xb_, ms_, xs_, T, ns, VAB, sbig, ssm); break;
+                        default: e = opp_runtime(mb_, xb_, abig ? na : nb, ms_, xs_, T, ns, VAB, sbig, ssm); break;
                     }
+                }
                 e = cfma(Rb, EssA, e);
                 e = cfma(Ra, EssB, e);
                 El.x = fma(cf, e.x, El.x);
                 El.y = fma(cf, e.y, El.y);
             }
             if (MODE >= 1) {
-                for (int a = 0; a < ka; a++)
-                    for (int b = 0; b < ka; b++) red_add_planar(CA, qa.x(a, b), cmul(cRb, mA.at(b * ka + a)));
-                for (int a = 0; a < kb; a++)
-                    for (int b = 0; b < kb; b++) red_add_planar(CB, qb.x(a, b), cmul(cRa, mB.at(b * kb + a)));
+#pragma unroll 4
+                for (int e = 0; e < na; e++) red_add_planar(CA, xA[e * T], cmul(cRb, mA[e * T]));
+#pragma unroll 4
+                for (int e = 0; e < nb; e++) red_add_planar(CB, xB[e * T], cmul(cRa, mB[e * T]));
             }
         }
     }
     flush_walker_sums(p, tile, Wl, El, MODE);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Antisymmetrised same-spin tensor, in place: Vbar[x_ab][x_cd] = V[x_ab][x_cd] - V[x_ad][x_cb] on the entries
+// (h_a < h_c, p_b < p_d) -- the only ones the same-spin sum reads (holes and particles of a determinant ascend).
+// V[x_ad][x_cb] is read through the symmetry V[x][y] = V[y][x] as V[(p_b,h_c)][(p_d,h_a)], an entry no thread writes.
+// ------------------------------------------------------------------------------------------------
+__global__ void k_vbar(cplx* __restrict__ V, int no, int nv, int64_t nt)
+{
+    const int nhh = no * (no - 1) / 2, npp = nv * (nv - 1) / 2;
+    const int64_t P = (int64_t)no * nv;
+    const int64_t total = nt * npp * nhh * MSD_WT;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int j = (int)(idx % MSD_WT);
+        int64_t t = idx / MSD_WT;
+        int hh = (int)(t % nhh); t /= nhh;
+        int pp = (int)(t % npp);
+        const int64_t tile = t / npp;
+        int ha = 0; while (hh >= no - 1 - ha) { hh -= no - 1 - ha; ha++; }
+        const int hc = ha + 1 + hh;
+        int pb = 0; while (pp >= nv - 1 - pb) { pp -= nv - 1 - pb; pb++; }
+        const int pd = pb + 1 + pp;
+        cplx* Vt = V + tile * P * P * MSD_WT + j;
+        const int64_t x1 = (int64_t)pb * no + ha, y1 = (int64_t)pd * no + hc;
+        const int64_t x2 = (int64_t)pb * no + hc, y2 = (int64_t)pd * no + ha;
+        const cplx u1 = Vt[(x1 * P + y1) * MSD_WT], u2 = Vt[(x2 * P + y2) * MSD_WT];
+        Vt[(x1 * P + y1) * MSD_WT] = csub(u1, u2);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -543,8 +758,9 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
         const int i0 = c->gen_group_begin[gi], i1 = c->gen_group_begin[gi + 1];
         if (i1 == i0) continue;
         int nthr = 128;
-        while (nthr > 32 && (size_t)c->gen_group_elems[gi] * sizeof(cplx) * nthr > 200 * 1024) nthr -= 32;
-        size_t smem = (size_t)c->gen_group_elems[gi] * sizeof(cplx) * nthr;
+        const size_t per_thread = (size_t)c->gen_group_elems[gi] * (sizeof(cplx) + sizeof(int));
+        while (nthr > 32 && per_thread * nthr > 200 * 1024) nthr -= 32;
+        size_t smem = per_thread * nthr;
         cudaError_t e = launch_persistent(k_dets_gen<MODE>, nthr, smem, c->n_sm, p, c->d_items_gen + i0, i1 - i0, ntiles,
                                           f.stream(li++));
         if (e != cudaSuccess) { f.join(); return e; }
@@ -576,6 +792,18 @@ cudaError_t launch_dets(msd_ctx* c, int mode, int64_t nw, Workspace& ws, cudaStr
     }
     p.Vab = ws.Vab; p.Wacc = ws.Wacc; p.E2nd = ws.E2nd;
     int ntiles = (int)((nw + MSD_WT - 1) / MSD_WT);
+    if (mode == 2) {
+        for (int s = 0; s < 2; s++) {
+            const auto& sp = c->sp[s];
+            if (sp.kmax < 2 || sp.n_o < 2 || sp.n_v < 2) continue;
+            const int64_t total = (int64_t)ntiles * (sp.n_o * (sp.n_o - 1) / 2) * (sp.n_v * (sp.n_v - 1) / 2) * MSD_WT;
+            const int blocks = (int)std::min<int64_t>((total + 255) / 256, (int64_t)c->n_sm * 16);
+            k_vbar<<<blocks, 256, 0, st>>>(ws.Vss[s], sp.n_o, sp.n_v, ntiles);
+            cudaError_t e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
+            c->launches++;
+        }
+    }
     if (mode == 0) return launch_mode<0>(c, p, ntiles, st);
     if (mode == 1) return launch_mode<1>(c, p, ntiles, st);
     return launch_mode<2>(c, p, ntiles, st);

@@ -227,6 +227,7 @@ static int do_setup(msd_ctx* c, std::string* errp, int N, int na, int nb, int n_
         const int m = std::max(b.ka, b.kb);
         int slots = gen ? 128 / MSD_WT : (m <= 3 ? 256 : 128) / MSD_WT;
         int iters = (int)std::max(4.0, std::min(32.0, 1024.0 / cost(b.ka, b.kb)));
+        if (gen) iters = (int)std::max(1.0, std::min(4.0, 1024.0 / cost(b.ka, b.kb)));   // few, heavy determinants: more CTAs
         int dpc = slots * iters;
         for (int64_t i0 = 0; i0 < b.count; i0 += dpc) {
             WorkItem it;
