@@ -572,35 +572,21 @@ __global__ void k_finish_flags(int64_t nw, const cplx* __restrict__ Wacc, const 
         for (int64_t e = threadIdx.x; e < per_walker; e += blockDim.x) out[w * per_walker + e] = cmake(nan_d(), nan_d());
 }
 
-//   E1 = E1_0 + (1/W) sum_s sum_x C^s[x] Hrot^s[x]                                            (W8)
-//   E2 = 1/2 sum_g Xt_g^2 - 1/2 sum_g (Ex0^a_g + Ex0^b_g) + (1/W) [ sum_s sum_x C^s[x] F^s[x] + E2nd ]   (W9)
+//   E1 = E1_0 + (1/W) E1nd,   E1nd = sum_s sum_x C^s[x] Hrot^s[x]  (accumulated per determinant in the dets kernels)   (W8)
+//   E2 = 1/2 sum_g Xt_g^2 - 1/2 sum_g (Ex0^a_g + Ex0^b_g) + (1/W) E2nd,
+//   E2nd = sum_s sum_x C^s[x] F^s[x] + second-order sums                                                          (W9)
 __global__ void __launch_bounds__(256)
-k_finish_energy(int n_chol, int64_t nw, double e0, int Pa, int Pb, const double* __restrict__ C_a,
-                const double* __restrict__ C_b, const cplx* __restrict__ F_a, const cplx* __restrict__ F_b,
-                const cplx* __restrict__ H_a, const cplx* __restrict__ H_b, const cplx* __restrict__ X0,
-                const cplx* __restrict__ Eacc, const cplx* __restrict__ Wacc, const cplx* __restrict__ E2nd,
+k_finish_energy(int n_chol, int64_t nw, double e0, const cplx* __restrict__ X0, const cplx* __restrict__ Eacc,
+                const cplx* __restrict__ Wacc, const cplx* __restrict__ E1nd, const cplx* __restrict__ E2nd,
                 const int* __restrict__ wflags, cplx* eout, int* flags)
 {
     const int64_t w = blockIdx.x;
     const int tid = threadIdx.x, nt = blockDim.x;
-    cplx ch = cmake(0.0, 0.0), cf = cmake(0.0, 0.0), xx = cmake(0.0, 0.0);
-    for (int s = 0; s < 2; s++) {
-        const int P = s ? Pb : Pa;
-        const double* C = (s ? C_b : C_a) + (w / MSD_WT) * (int64_t)P * 2 * MSD_WT + (w % MSD_WT);
-        const cplx* F = (s ? F_b : F_a) + w * (int64_t)P;
-        const cplx* H = (s ? H_b : H_a) + w * (int64_t)P;
-        for (int x = tid; x < P; x += nt) {
-            cplx c = load_planar(C, x);
-            ch = cfma(c, H[x], ch);
-            cf = cfma(c, F[x], cf);
-        }
-    }
+    cplx xx = cmake(0.0, 0.0);
     for (int g = tid; g < n_chol; g += nt) {
         cplx xt = cadd(X0[w * (int64_t)n_chol + g], X0[(nw + w) * (int64_t)n_chol + g]);
         xx = cfma(xt, xt, xx);
     }
-    ch = block_sum(ch);
-    cf = block_sum(cf);
     xx = block_sum(xx);
     if (tid == 0) {
         cplx W = Wacc[w];
@@ -610,8 +596,8 @@ k_finish_energy(int n_chol, int64_t nw, double e0, int Pa, int Pb, const double*
         if (f) { E1 = cmake(nan_d(), nan_d()); E2 = E1; }
         else {
             cplx Winv = cinv(W);
-            E1 = cadd(Eacc[w * 2 + 0], cmul(ch, Winv));
-            E2 = cadd(cadd(cscale(0.5, xx), Eacc[w * 2 + 1]), cmul(cadd(cf, E2nd[w]), Winv));
+            E1 = cadd(Eacc[w * 2 + 0], cmul(E1nd[w], Winv));
+            E2 = cadd(cadd(cscale(0.5, xx), Eacc[w * 2 + 1]), cmul(E2nd[w], Winv));
         }
         eout[w * 3 + 0] = cmake(e0 + E1.x + E2.x, E1.y + E2.y);
         eout[w * 3 + 1] = E1;
@@ -641,9 +627,8 @@ cudaError_t launch_finish_energy(msd_ctx* c, int64_t nw, Workspace& ws, cplx* e,
 {
     if (nw == 0) return cudaSuccess;
     cplx* X0 = ws.X0;
-    k_finish_energy<<<(unsigned)nw, 256, 0, st>>>(c->n_chol, nw, c->e0, c->sp[0].P, c->sp[1].P, ws.C[0], ws.C[1],
-                                                  ws.F[0], ws.F[1], ws.Hrot[0], ws.Hrot[1], X0, ws.Eacc, ws.Wacc,
-                                                  ws.E2nd, ws.wflags, e, flags);
+    k_finish_energy<<<(unsigned)nw, 256, 0, st>>>(c->n_chol, nw, c->e0, X0, ws.Eacc, ws.Wacc, ws.E1nd, ws.E2nd, ws.wflags,
+                                                  e, flags);
     c->launches++;
     return cudaGetLastError();
 }

@@ -8,7 +8,9 @@
 //   M[a][b] = g[h_a, p_b]                       k x k minor of the reference Green's function
 //   R = det M,  A = adj M (A[b][a] = cofactor of M[a][b]),  T[b,d;a,c] = signed complementary (k-2) minor
 //   W      += c~ R^a R^b
-//   C^s[x] += c~ R^sbar A^s[b][a]               x = (p_b, h_a)
+//   C^s[x] += c~ R^sbar A^s[b][a]               x = (p_b, h_a)      (overlap / force-bias modes: RED.ADD.F64 scatter)
+//   energy mode needs C only inside sum_x C[x] Hrot[x] and sum_x C[x] F[x], so those two scalars are accumulated
+//   per determinant from gathers of Hrot / F (two 128-byte lines per entry) and C is never formed: no atomics.
 //   E2nd   += c~ [ sum A^a[b][a] A^b[b'][a'] Vab[x][x'] + sum_s R^sbar sum_{a<c,b<d} T^s Vbar^s[x_ab][x_cd] ]
 //   Vbar^s[x_ab][x_cd] = V^ss[x_ab][x_cd] - V^ss[x_ad][x_cb]  (k_vbar, in place on the h_a<h_c, p_b<p_d entries of Vss)
 // Levels <= 4 use division-free closed forms in registers (exact for singular minors: pin P7);
@@ -23,8 +25,10 @@ struct DetsParams {
     double* C[2];          // [nt][P][2][WT] planar
     const cplx* Vab;       // [nt][Pa][Pb][WT]
     const cplx* Vss[2];    // [nt][P][P][WT]; entries (h_a<h_c, p_b<p_d) hold the antisymmetrised Vbar (k_vbar)
+    const cplx* FH[2];     // [nt][P][2][WT]: Hrot (slot 0) and F (slot 1), walker fastest (k_fh_tile); energy mode only
     cplx* Wacc;            // [nt*WT]
-    cplx* E2nd;            // [nt*WT]
+    cplx* E2nd;            // [nt*WT]  second-order two-body sums + sum_x C[x] F[x]
+    cplx* E1nd;            // [nt*WT]  sum_x C[x] Hrot[x]
     int no[2], P[2];
 };
 
@@ -176,7 +180,7 @@ template <int NWORD> struct RowData { uint32_t w[NWORD]; double cf; };
 
 template <int KA, int KB, int MODE>
 __device__ __forceinline__ void run_bucket(const DetsParams& p, const WorkItem& it, int tile, int slot, int nslots,
-                                           int j, const cplx* gsm, cplx& Wl, cplx& El)
+                                           int j, const cplx* gsm, cplx& Wl, cplx& El, cplx& Hl)
 {
     constexpr int NB = 2 * KA + 2 * KB;
     constexpr int NWORD = (NB + 3) / 4 > 0 ? (NB + 3) / 4 : 1;
@@ -187,6 +191,8 @@ __device__ __forceinline__ void run_bucket(const DetsParams& p, const WorkItem& 
     const cplx* VA = (MODE == 2) ? p.Vss[0] + (int64_t)tile * p.P[0] * p.P[0] * MSD_WT + j : nullptr;
     const cplx* VB = (MODE == 2) ? p.Vss[1] + (int64_t)tile * p.P[1] * p.P[1] * MSD_WT + j : nullptr;
     const cplx* VAB = (MODE == 2) ? p.Vab + (int64_t)tile * p.P[0] * p.P[1] * MSD_WT + j : nullptr;
+    const cplx* FHA = (MODE == 2) ? p.FH[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j : nullptr;
+    const cplx* FHB = (MODE == 2) ? p.FH[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j : nullptr;
     const unsigned char* tab = p.tab + it.tab_off;
     const double* coef = p.coef + it.det_begin;
     auto load_row = [&](int i, RowData<NWORD>& r) {
@@ -227,12 +233,34 @@ __device__ __forceinline__ void run_bucket(const DetsParams& p, const WorkItem& 
                         e = cfma(ea.A[b][a], z, e);
                     }
             }
-            e = cfma(eb.R, ea.Ess, e);
-            e = cfma(ea.R, eb.Ess, e);
+            // sum_x C[x] Hrot[x] and sum_x C[x] F[x] without forming C:  s = sum_ab A[b][a] (Hrot, F)[x_ab]
+            cplx shA = cmake(0.0, 0.0), sfA = shA, shB = shA, sfB = shA;
+#pragma unroll
+            for (int a = 0; a < KA; a++)
+#pragma unroll
+                for (int b = 0; b < KA; b++) {
+                    const cplx* q = FHA + ea.x(a, b) * (2 * MSD_WT);
+                    shA = cfma(ea.A[b][a], __ldg(q), shA);
+                    sfA = cfma(ea.A[b][a], __ldg(q + MSD_WT), sfA);
+                }
+#pragma unroll
+            for (int a = 0; a < KB; a++)
+#pragma unroll
+                for (int b = 0; b < KB; b++) {
+                    const cplx* q = FHB + eb.x(a, b) * (2 * MSD_WT);
+                    shB = cfma(eb.A[b][a], __ldg(q), shB);
+                    sfB = cfma(eb.A[b][a], __ldg(q + MSD_WT), sfB);
+                }
+            e = cfma(eb.R, cadd(ea.Ess, sfA), e);
+            e = cfma(ea.R, cadd(eb.Ess, sfB), e);
             El.x = fma(cf, e.x, El.x);
             El.y = fma(cf, e.y, El.y);
+            cplx hsum = cmul(eb.R, shA);
+            hsum = cfma(ea.R, shB, hsum);
+            Hl.x = fma(cf, hsum.x, Hl.x);
+            Hl.y = fma(cf, hsum.y, Hl.y);
         }
-        if (MODE >= 1) {
+        if (MODE == 1) {
 #pragma unroll
             for (int a = 0; a < KA; a++)
 #pragma unroll
@@ -248,21 +276,21 @@ __device__ __forceinline__ void run_bucket(const DetsParams& p, const WorkItem& 
 }
 
 // reduce per-lane partial sums over the CTA's determinant slots and add to the walker accumulators
-__device__ __forceinline__ void flush_walker_sums(const DetsParams& p, int tile, cplx Wl, cplx El, int mode)
+__device__ __forceinline__ void flush_walker_sums(const DetsParams& p, int tile, cplx Wl, cplx El, cplx Hl, int mode)
 {
-    __shared__ double acc[MSD_WT][4];
-    double v[4] = {Wl.x, Wl.y, El.x, El.y};
+    __shared__ double acc[MSD_WT][6];
+    double v[6] = {Wl.x, Wl.y, El.x, El.y, Hl.x, Hl.y};
 #pragma unroll
-    for (int t = 0; t < 4; t++) {      // the 4 determinant slots of a warp share each walker lane j
+    for (int t = 0; t < 6; t++) {      // the 4 determinant slots of a warp share each walker lane j
         v[t] += __shfl_xor_sync(0xffffffffu, v[t], 8);
         v[t] += __shfl_xor_sync(0xffffffffu, v[t], 16);
     }
-    if (threadIdx.x < MSD_WT * 4) acc[threadIdx.x >> 2][threadIdx.x & 3] = 0.0;
+    for (int t = threadIdx.x; t < MSD_WT * 6; t += blockDim.x) acc[t / 6][t % 6] = 0.0;     // blockDim.x may be 32
     __syncthreads();
     const int lane = threadIdx.x & 31;
     if (lane < MSD_WT) {
 #pragma unroll
-        for (int t = 0; t < 4; t++) atomicAdd(&acc[lane][t], v[t]);
+        for (int t = 0; t < 6; t++) if (t < 2 || mode == 2) atomicAdd(&acc[lane][t], v[t]);
     }
     __syncthreads();
     if (threadIdx.x < MSD_WT) {
@@ -272,6 +300,8 @@ __device__ __forceinline__ void flush_walker_sums(const DetsParams& p, int tile,
         if (mode == 2) {
             atomicAdd(&p.E2nd[tile * MSD_WT + jj].x, acc[jj][2]);
             atomicAdd(&p.E2nd[tile * MSD_WT + jj].y, acc[jj][3]);
+            atomicAdd(&p.E1nd[tile * MSD_WT + jj].x, acc[jj][4]);
+            atomicAdd(&p.E1nd[tile * MSD_WT + jj].y, acc[jj][5]);
         }
     }
 }
@@ -290,7 +320,7 @@ __device__ __forceinline__ void stage_g(const DetsParams& p, int tile, cplx* gsm
 #define CF_CASE(KA_, KB_)                                                                              \
     case KA_ * 5 + KB_:                                                                                \
         if constexpr ((KA_ > KB_ ? KA_ : KB_) > KLO && (KA_ > KB_ ? KA_ : KB_) <= KHI)                  \
-            run_bucket<KA_, KB_, MODE>(p, it, tile, slot, nslots, j, gsm, Wl, El);                     \
+            run_bucket<KA_, KB_, MODE>(p, it, tile, slot, nslots, j, gsm, Wl, El, Hl);                     \
         break;
 
 // register class (KLO, KHI]: buckets whose larger level lies in that range (KLO = -1 admits (0,0)).
@@ -304,7 +334,7 @@ __global__ void __launch_bounds__(NTHR, MINB) k_dets_cf(DetsParams p, const Work
     const int j = threadIdx.x & (MSD_WT - 1);
     const int slot = threadIdx.x / MSD_WT, nslots = NTHR / MSD_WT;
     stage_g(p, tile, gsm);
-    cplx Wl = cmake(0.0, 0.0), El = cmake(0.0, 0.0);
+    cplx Wl = cmake(0.0, 0.0), El = cmake(0.0, 0.0), Hl = cmake(0.0, 0.0);
     for (int r = 0, ii; (ii = r * (int)gridDim.x + ((r & 1) ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x)),
                         r * (int)gridDim.x < n_items; r++) {
         if (ii >= n_items) continue;
@@ -318,7 +348,7 @@ __global__ void __launch_bounds__(NTHR, MINB) k_dets_cf(DetsParams p, const Work
             default: break;
         }
     }
-    flush_walker_sums(p, tile, Wl, El, MODE);
+    flush_walker_sums(p, tile, Wl, El, Hl, MODE);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -642,7 +672,9 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
     const cplx* VA = (MODE == 2) ? p.Vss[0] + (int64_t)tile * p.P[0] * p.P[0] * MSD_WT + j : nullptr;
     const cplx* VB = (MODE == 2) ? p.Vss[1] + (int64_t)tile * p.P[1] * p.P[1] * MSD_WT + j : nullptr;
     const cplx* VAB = (MODE == 2) ? p.Vab + (int64_t)tile * p.P[0] * p.P[1] * MSD_WT + j : nullptr;
-    cplx Wl = cmake(0.0, 0.0), El = cmake(0.0, 0.0);
+    const cplx* FHA = (MODE == 2) ? p.FH[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j : nullptr;
+    const cplx* FHB = (MODE == 2) ? p.FH[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j : nullptr;
+    cplx Wl = cmake(0.0, 0.0), El = cmake(0.0, 0.0), Hl = cmake(0.0, 0.0);
     // snake order over rounds: items are sorted by descending cost, so alternate the direction to even out
     for (int r = 0, ii; (ii = r * (int)gridDim.x + ((r & 1) ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x)),
                         r * (int)gridDim.x < n_items; r++) {
@@ -680,12 +712,31 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
                         default: e = opp_runtime(mb_, xb_, abig ? na : nb, ms_, xs_, T, ns, VAB, sbig, ssm); break;
                     }
                 }
-                e = cfma(Rb, EssA, e);
-                e = cfma(Ra, EssB, e);
+                cplx shA = cmake(0.0, 0.0), sfA = shA, shB = shA, sfB = shA;
+#pragma unroll 4
+                for (int u = 0; u < na; u++) {
+                    const cplx* q = FHA + xA[u * T] * (2 * MSD_WT);
+                    const cplx a_ = mA[u * T];
+                    shA = cfma(a_, __ldg(q), shA);
+                    sfA = cfma(a_, __ldg(q + MSD_WT), sfA);
+                }
+#pragma unroll 4
+                for (int u = 0; u < nb; u++) {
+                    const cplx* q = FHB + xB[u * T] * (2 * MSD_WT);
+                    const cplx b_ = mB[u * T];
+                    shB = cfma(b_, __ldg(q), shB);
+                    sfB = cfma(b_, __ldg(q + MSD_WT), sfB);
+                }
+                e = cfma(Rb, cadd(EssA, sfA), e);
+                e = cfma(Ra, cadd(EssB, sfB), e);
                 El.x = fma(cf, e.x, El.x);
                 El.y = fma(cf, e.y, El.y);
+                cplx hsum = cmul(Rb, shA);
+                hsum = cfma(Ra, shB, hsum);
+                Hl.x = fma(cf, hsum.x, Hl.x);
+                Hl.y = fma(cf, hsum.y, Hl.y);
             }
-            if (MODE >= 1) {
+            if (MODE == 1) {
 #pragma unroll 4
                 for (int e = 0; e < na; e++) red_add_planar(CA, xA[e * T], cmul(cRb, mA[e * T]));
 #pragma unroll 4
@@ -693,7 +744,7 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
             }
         }
     }
-    flush_walker_sums(p, tile, Wl, El, MODE);
+    flush_walker_sums(p, tile, Wl, El, Hl, MODE);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -721,6 +772,23 @@ __global__ void k_vbar(cplx* __restrict__ V, int no, int nv, int64_t nt)
         const int64_t x2 = (int64_t)pb * no + hc, y2 = (int64_t)pd * no + ha;
         const cplx u1 = Vt[(x1 * P + y1) * MSD_WT], u2 = Vt[(x2 * P + y2) * MSD_WT];
         Vt[(x1 * P + y1) * MSD_WT] = csub(u1, u2);
+    }
+}
+
+// Hrot and F ([n_w][P] each) interleaved per pair index with the walker fastest: FH[tile][x][0][j] = Hrot, [1][j] = F
+__global__ void k_fh_tile(const cplx* __restrict__ Hrot, const cplx* __restrict__ F, cplx* __restrict__ FH, int P, int64_t nw,
+                          int64_t nt)
+{
+    const int64_t total = nt * P * MSD_WT;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int j = (int)(idx % MSD_WT);
+        const int64_t t = idx / MSD_WT;
+        const int x = (int)(t % P);
+        const int64_t tile = t / P, w = tile * MSD_WT + j;
+        const cplx zero = cmake(0.0, 0.0);
+        cplx* dst = FH + ((tile * P + x) * 2) * MSD_WT + j;
+        dst[0] = (w < nw) ? Hrot[w * P + x] : zero;
+        dst[MSD_WT] = (w < nw) ? F[w * P + x] : zero;
     }
 }
 
@@ -790,7 +858,8 @@ cudaError_t launch_dets(msd_ctx* c, int mode, int64_t nw, Workspace& ws, cudaStr
         p.g[s] = ws.g[s]; p.C[s] = ws.C[s]; p.Vss[s] = ws.Vss[s];
         p.no[s] = c->sp[s].n_o; p.P[s] = c->sp[s].P;
     }
-    p.Vab = ws.Vab; p.Wacc = ws.Wacc; p.E2nd = ws.E2nd;
+    p.Vab = ws.Vab; p.Wacc = ws.Wacc; p.E2nd = ws.E2nd; p.E1nd = ws.E1nd;
+    p.FH[0] = ws.FH[0]; p.FH[1] = ws.FH[1];
     int ntiles = (int)((nw + MSD_WT - 1) / MSD_WT);
     if (mode == 2) {
         for (int s = 0; s < 2; s++) {
@@ -799,6 +868,16 @@ cudaError_t launch_dets(msd_ctx* c, int mode, int64_t nw, Workspace& ws, cudaStr
             const int64_t total = (int64_t)ntiles * (sp.n_o * (sp.n_o - 1) / 2) * (sp.n_v * (sp.n_v - 1) / 2) * MSD_WT;
             const int blocks = (int)std::min<int64_t>((total + 255) / 256, (int64_t)c->n_sm * 16);
             k_vbar<<<blocks, 256, 0, st>>>(ws.Vss[s], sp.n_o, sp.n_v, ntiles);
+            cudaError_t e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
+            c->launches++;
+        }
+        for (int s = 0; s < 2; s++) {
+            const auto& sp = c->sp[s];
+            if (sp.P == 0) continue;
+            const int64_t total = (int64_t)ntiles * sp.P * MSD_WT;
+            k_fh_tile<<<(int)std::min<int64_t>((total + 255) / 256, (int64_t)c->n_sm * 8), 256, 0, st>>>(
+                ws.Hrot[s], ws.F[s], ws.FH[s], sp.P, nw, ntiles);
             cudaError_t e = cudaGetLastError();
             if (e != cudaSuccess) return e;
             c->launches++;

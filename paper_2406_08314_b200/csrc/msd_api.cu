@@ -466,6 +466,7 @@ static size_t carve(const msd_ctx* c, Workspace& ws, char* base, int64_t wc, int
     for (int s = 0; s < 2; s++) ws.C[s] = k.take<double>((size_t)nt * c->sp[s].P * 2 * MSD_WT);
     ws.Wacc = k.take<cplx>(wc);
     ws.E2nd = k.take<cplx>(wc);
+    ws.E1nd = k.take<cplx>(wc);
     ws.wflags = k.take<int>(wc);
     if (level >= 3) {
         for (int s = 0; s < 2; s++) ws.F[s] = k.take<cplx>((size_t)wc * c->sp[s].P);
@@ -492,6 +493,7 @@ static size_t carve(const msd_ctx* c, Workspace& ws, char* base, int64_t wc, int
             ws.Bq[s] = k.take<double>((size_t)wc * 2 * sp.P * 2 * ng);
             ws.Vss[s] = k.take<cplx>((size_t)nt * sp.P * sp.P * MSD_WT);
             ws.Hrot[s] = k.take<cplx>((size_t)wc * sp.P);
+            ws.FH[s] = k.take<cplx>((size_t)nt * sp.P * 2 * MSD_WT);
         }
         ws.Vab = k.take<cplx>((size_t)nt * c->sp[0].P * c->sp[1].P * MSD_WT);
     }

@@ -113,6 +113,8 @@ struct Workspace {
     double* C[2] = {nullptr, nullptr};        // [nt][P][2][WT] planar re/im (zeroed every call)
     cplx* Wacc = nullptr;                     // [wc]             (zeroed)
     cplx* E2nd = nullptr;                     // [wc]             (zeroed)
+    cplx* E1nd = nullptr;                     // [wc]             (zeroed)
+    cplx* FH[2] = {nullptr, nullptr};         // [nt][P][2][WT]   Hrot / F with the walker fastest (energy)
     int* wflags = nullptr;                    // [wc]
     double* Gp[2] = {nullptr, nullptr};       // [wc][2][n_r*N]   planar rows (w,c)
     cplx* Lam[2] = {nullptr, nullptr};        // [(n_chol+1)*n_r][wc][n]
