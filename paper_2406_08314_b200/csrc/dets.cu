@@ -178,7 +178,7 @@ struct SpinEval {
 
 template <int NWORD> struct RowData { uint32_t w[NWORD]; double cf; };
 
-template <int KA, int KB, int MODE>
+template <int KA, int KB, int MODE, bool FHS>
 __device__ __forceinline__ void run_bucket(const DetsParams& p, const WorkItem& it, int tile, int slot, int nslots,
                                            int j, const cplx* gsm, cplx& Wl, cplx& El, cplx& Hl)
 {
@@ -191,8 +191,11 @@ __device__ __forceinline__ void run_bucket(const DetsParams& p, const WorkItem& 
     const cplx* VA = (MODE == 2) ? p.Vss[0] + (int64_t)tile * p.P[0] * p.P[0] * MSD_WT + j : nullptr;
     const cplx* VB = (MODE == 2) ? p.Vss[1] + (int64_t)tile * p.P[1] * p.P[1] * MSD_WT + j : nullptr;
     const cplx* VAB = (MODE == 2) ? p.Vab + (int64_t)tile * p.P[0] * p.P[1] * MSD_WT + j : nullptr;
-    const cplx* FHA = (MODE == 2) ? p.FH[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j : nullptr;
-    const cplx* FHB = (MODE == 2) ? p.FH[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j : nullptr;
+    // Hrot / F of the tile: the shared-memory copy behind g (FHS) or global memory through L1
+    const cplx* FHA = (MODE != 2) ? nullptr : FHS ? gsm + (p.P[0] + p.P[1]) * MSD_WT + j
+                                                  : p.FH[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j;
+    const cplx* FHB = (MODE != 2) ? nullptr : FHS ? FHA + p.P[0] * 2 * MSD_WT
+                                                  : p.FH[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j;
     const unsigned char* tab = p.tab + it.tab_off;
     const double* coef = p.coef + it.det_begin;
     auto load_row = [&](int i, RowData<NWORD>& r) {
@@ -240,16 +243,16 @@ __device__ __forceinline__ void run_bucket(const DetsParams& p, const WorkItem& 
 #pragma unroll
                 for (int b = 0; b < KA; b++) {
                     const cplx* q = FHA + ea.x(a, b) * (2 * MSD_WT);
-                    shA = cfma(ea.A[b][a], __ldg(q), shA);
-                    sfA = cfma(ea.A[b][a], __ldg(q + MSD_WT), sfA);
+                    shA = cfma(ea.A[b][a], FHS ? q[0] : __ldg(q), shA);
+                    sfA = cfma(ea.A[b][a], FHS ? q[MSD_WT] : __ldg(q + MSD_WT), sfA);
                 }
 #pragma unroll
             for (int a = 0; a < KB; a++)
 #pragma unroll
                 for (int b = 0; b < KB; b++) {
                     const cplx* q = FHB + eb.x(a, b) * (2 * MSD_WT);
-                    shB = cfma(eb.A[b][a], __ldg(q), shB);
-                    sfB = cfma(eb.A[b][a], __ldg(q + MSD_WT), sfB);
+                    shB = cfma(eb.A[b][a], FHS ? q[0] : __ldg(q), shB);
+                    sfB = cfma(eb.A[b][a], FHS ? q[MSD_WT] : __ldg(q + MSD_WT), sfB);
                 }
             e = cfma(eb.R, cadd(ea.Ess, sfA), e);
             e = cfma(ea.R, cadd(eb.Ess, sfB), e);
@@ -307,25 +310,32 @@ __device__ __forceinline__ void flush_walker_sums(const DetsParams& p, int tile,
 }
 
 // stage the walker tile's active slices g^a, g^b ([P][WT] complex each) in shared memory
-__device__ __forceinline__ void stage_g(const DetsParams& p, int tile, cplx* gsm)
+__device__ __forceinline__ void stage_g(const DetsParams& p, int tile, cplx* gsm, bool fh)
 {
     const int na = p.P[0] * MSD_WT, nb = p.P[1] * MSD_WT;
     const cplx* ga = p.g[0] + (int64_t)tile * na;
     const cplx* gb = p.g[1] + (int64_t)tile * nb;
     for (int e = threadIdx.x; e < na; e += blockDim.x) gsm[e] = __ldg(ga + e);
     for (int e = threadIdx.x; e < nb; e += blockDim.x) gsm[na + e] = __ldg(gb + e);
+    if (fh) {      // [P_a][2][WT] then [P_b][2][WT] behind the two g slices
+        const cplx* fa = p.FH[0] + (int64_t)tile * 2 * na;
+        const cplx* fb = p.FH[1] + (int64_t)tile * 2 * nb;
+        cplx* dst = gsm + na + nb;
+        for (int e = threadIdx.x; e < 2 * na; e += blockDim.x) dst[e] = __ldg(fa + e);
+        for (int e = threadIdx.x; e < 2 * nb; e += blockDim.x) dst[2 * na + e] = __ldg(fb + e);
+    }
     __syncthreads();
 }
 
 #define CF_CASE(KA_, KB_)                                                                              \
     case KA_ * 5 + KB_:                                                                                \
         if constexpr ((KA_ > KB_ ? KA_ : KB_) > KLO && (KA_ > KB_ ? KA_ : KB_) <= KHI)                  \
-            run_bucket<KA_, KB_, MODE>(p, it, tile, slot, nslots, j, gsm, Wl, El, Hl);                     \
+            run_bucket<KA_, KB_, MODE, FHS>(p, it, tile, slot, nslots, j, gsm, Wl, El, Hl);                     \
         break;
 
 // register class (KLO, KHI]: buckets whose larger level lies in that range (KLO = -1 admits (0,0)).
 // Persistent per walker tile: CTA (worker, tile) stages g once and strides over the class's work items.
-template <int MODE, int KLO, int KHI, int NTHR, int MINB>
+template <int MODE, int KLO, int KHI, int NTHR, int MINB, bool FHS>
 __global__ void __launch_bounds__(NTHR, MINB) k_dets_cf(DetsParams p, const WorkItem* __restrict__ items, int n_items)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -333,7 +343,7 @@ __global__ void __launch_bounds__(NTHR, MINB) k_dets_cf(DetsParams p, const Work
     const int tile = blockIdx.y;
     const int j = threadIdx.x & (MSD_WT - 1);
     const int slot = threadIdx.x / MSD_WT, nslots = NTHR / MSD_WT;
-    stage_g(p, tile, gsm);
+    stage_g(p, tile, gsm, FHS);
     cplx Wl = cmake(0.0, 0.0), El = cmake(0.0, 0.0), Hl = cmake(0.0, 0.0);
     for (int r = 0, ii; (ii = r * (int)gridDim.x + ((r & 1) ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x)),
                         r * (int)gridDim.x < n_items; r++) {
@@ -840,9 +850,21 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
         if (i1 == i0) continue;
         cudaError_t e;
         cudaStream_t s = f.stream(li++);
-        if (cl == 0) e = launch_persistent(k_dets_cf<MODE, -1, 2, 256, 3>, 256, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
-        else if (cl == 1) e = launch_persistent(k_dets_cf<MODE, 2, 3, 256, 2>, 256, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
-        else e = launch_persistent(k_dets_cf<MODE, 3, 4, 128, 2>, 128, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+        // energy mode: one large CTA per SM that also holds Hrot / F of the tile in shared memory (same warps per SM as
+        // the 2-3 smaller CTAs of the other modes); falls back to global Hrot / F when the tile does not fit
+        bool fhs = false;
+        if constexpr (MODE == 2) {
+            fhs = 3 * gbytes <= 200 * 1024;
+            if (!fhs) {}
+            else if (cl == 0) e = launch_persistent(k_dets_cf<MODE, -1, 2, 768, 1, true>, 768, 3 * gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+            else if (cl == 1) e = launch_persistent(k_dets_cf<MODE, 2, 3, 512, 1, true>, 512, 3 * gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+            else e = launch_persistent(k_dets_cf<MODE, 3, 4, 256, 1, true>, 256, 3 * gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+        }
+        if (!fhs) {
+            if (cl == 0) e = launch_persistent(k_dets_cf<MODE, -1, 2, 256, 3, false>, 256, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+            else if (cl == 1) e = launch_persistent(k_dets_cf<MODE, 2, 3, 256, 2, false>, 256, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+            else e = launch_persistent(k_dets_cf<MODE, 3, 4, 128, 2, false>, 128, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+        }
         if (e != cudaSuccess) { f.join(); return e; }
         c->launches++;
     }
