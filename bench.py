@@ -282,7 +282,8 @@ def main():
         nr_a = inp.n_alpha + info["n_v_alpha"]
         nr_b = inp.n_beta + info["n_v_beta"]
         ng, nw, N = inp.n_chol, inp.n_w, inp.N
-        flops_v = 8.0 * ng * nw * (Pa * Pb + Pa * Pa + Pb * Pb)               # complex MAC = 8 flops
+        # complex MAC = 8 flops; the same-spin products are symmetric: only x <= y is algorithmic work
+        flops_v = 8.0 * ng * nw * (Pa * Pb + Pa * (Pa + 1) / 2 + Pb * (Pb + 1) / 2)
         flops_lam = 4.0 * (ng + 1) * N * nw * (nr_a * inp.n_alpha + nr_b * inp.n_beta)   # real x complex MAC = 4
         phases = {"energy_ms": {"reference": acc["reference"], "lambda_gemm": acc["p1"], "energy_dense": acc["p2"],
                                 "v_gemm": acc["p3"], "dets": acc["p4"], "assemble": acc["p5"]},
@@ -300,6 +301,23 @@ def main():
                     "traffic_note": "DRAM bytes per launch (mean of the 5 launches), ncu --set full, profiles/r01c_traffic.csv",
                     "share_of_step": gemm_ms / (sum(step_ms) / len(step_ms)),
                     "algorithmic_flops_per_step": flops_v + flops_lam}
+
+        # energy-mode dets kernels: bound by the L2 -> SM gathers of V / Vbar; algorithmic bytes =
+        # 16 B x (ka^2 kb^2 + C(ka,2)^2 + C(kb,2)^2) per walker x determinant, from the level histogram of the inputs
+        ka = np.diff(inp.exc_off_a).astype(np.float64)
+        kb = np.diff(inp.exc_off_b).astype(np.float64)
+        gathers = float(np.sum(ka * ka * kb * kb + (ka * (ka - 1) / 2) ** 2 + (kb * (kb - 1) / 2) ** 2))
+        l2_bytes = 16.0 * gathers * nw
+        l2_peak = 6300.0 * (clocks.get("sm_mhz") or 1965.0) * 1e6 / 1e9      # B300_MICROARCH.md: ~6300 B/clk LTS cap
+        roofline_dets = {"kernel": "k_dets_cf<2> + k_dets_gen<2> (energy mode, forked over side streams)",
+                         "bound": "l2", "achieved": l2_bytes / (acc["p4"] * 1e-3) / 1e9, "peak": l2_peak, "unit": "GB/s",
+                         "frac": l2_bytes / (acc["p4"] * 1e-3) / 1e9 / l2_peak,
+                         "peak_source": "guide fallback: LTS throughput cap ~6300 B/clk x SM clock (no measured L2 peak "
+                                        "in MEASURED_PEAKS.json)",
+                         "algorithmic_l2_bytes_per_step": l2_bytes, "share_of_step": acc["p4"] / (sum(step_ms) / len(step_ms)),
+                         "fp64_flops_floor_ms": None}
+    else:
+        roofline_dets = None
 
     if rank != 0:
         if world > 1:
@@ -325,7 +343,7 @@ def main():
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": n_e2e},
             "gpu_launches": int(launches),
-            "roofline": roofline, "cpu_baseline": cpu_baseline, "phases": phases,
+            "roofline": roofline, "roofline_dets": roofline_dets, "cpu_baseline": cpu_baseline, "phases": phases,
             "step_ms": {"min": min(step_ms), "median": statistics.median(step_ms), "max": max(step_ms)}}
     print(json.dumps(line), flush=True)
     if world > 1:

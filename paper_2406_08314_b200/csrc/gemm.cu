@@ -144,10 +144,27 @@ cudaError_t launch_gemm_tn(const GemmArgs& a, int n_sm, cudaStream_t st)
         return cudaErrorInvalidValue;     // callers pad to even sizes (16-byte cp.async chunks)
     if (a.ksplit < 1 || (a.ksplit > 1 && a.accumulate != 2) || (a.symmetric && (a.N != 2 * a.M || a.accumulate)))
         return cudaErrorInvalidValue;
-    int64_t big = (int64_t)((a.M + 127) / 128) * ((a.N + 63) / 64) * a.batch * a.ksplit;
-    // symmetric outputs use the square 64 x 32-complex tile: finer skipping of the lower triangle
-    if (big >= 2 * (int64_t)n_sm && !a.symmetric) return launch_cfg<128, 64, 4, 2>(a, st);
-    return launch_cfg<64, 64, 2, 2>(a, st);
+    // Tile shape by a wave model: time ~ waves x (CTAs per SM) x BM x BN, waves = ceil(computed tiles / (SMs x CTAs per SM)).
+    // Padding (e.g. P = 225 rows against 64- or 128-row tiles) and the partly filled last wave are what it minimises.
+    struct Cand { int bm, bn, occ; };
+    static const Cand cands[3] = {{128, 64, 2}, {64, 64, 3}, {48, 96, 3}};
+    int best = 0; double best_cost = 0.0;
+    for (int i = 0; i < 3; i++) {
+        const int tm = (a.M + cands[i].bm - 1) / cands[i].bm, tn = (a.N + cands[i].bn - 1) / cands[i].bn;
+        int64_t tiles = 0;
+        if (a.symmetric) {
+            for (int y = 0; y < tm; y++)
+                for (int x = 0; x < tn; x++)
+                    if (!((x * cands[i].bn + cands[i].bn) / 2 - 1 < y * cands[i].bm)) tiles++;
+        } else tiles = (int64_t)tm * tn;
+        tiles *= (int64_t)a.batch * a.ksplit;
+        const int64_t slots = (int64_t)n_sm * cands[i].occ;
+        const double cost = (double)((tiles + slots - 1) / slots) * cands[i].occ * cands[i].bm * cands[i].bn;
+        if (i == 0 || cost < best_cost * 0.97) { best = i; best_cost = cost; }     // ties go to the larger tile
+    }
+    if (best == 0) return launch_cfg<128, 64, 4, 2>(a, st);
+    if (best == 1) return launch_cfg<64, 64, 2, 2>(a, st);
+    return launch_cfg<48, 96, 2, 2>(a, st);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -611,6 +611,9 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
             mark(c, 4, st); mark(c, 5, st);
         } else {   // energy
             // Lambda = L_sub Theta for every slice (incl. h1), both spins
+            // (independent launches of one phase are forked over the side streams: the last, partly filled wave of one
+            // GEMM overlaps the first wave of the next)
+            Fork fl_(c, st);
             for (int s = 0; s < 2; s++) {
                 const auto& sp = c->sp[s];
                 if (sp.n == 0 || sp.n_r == 0) continue;
@@ -620,13 +623,16 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
                 a.lda = ldN; a.ldb = ldN; a.strideA = 0; a.strideB = 0; a.batch = 1;
                 a.zdiv = 1; a.strideC_hi = 0; a.strideC_lo = 0; a.cs_m = (int64_t)nw * sp.n; a.cs_j = 1;
                 a.accumulate = 0;
-                CK(launch_gemm_tn(a, c->n_sm, st));
+                cudaError_t ge = launch_gemm_tn(a, c->n_sm, fl_.stream(s));
+                if (ge != cudaSuccess) { fl_.join(); CK(ge); }
                 c->launches++;
             }
+            CK(fl_.join());
             mark(c, 2, st);
             CK(launch_energy_dense(c, nw, ws, st));
             mark(c, 3, st);
             // V GEMMs: ab, aa, bb
+            Fork fv_(c, st);
             for (int pr = 0; pr < 3; pr++) {
                 const int s1 = (pr == 2) ? 1 : 0, s2 = (pr == 0) ? 1 : s1;
                 const auto& A_ = c->sp[s1]; const auto& B_ = c->sp[s2];
@@ -642,9 +648,11 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
                 a.cs_m = (int64_t)B_.P * MSD_WT; a.cs_j = MSD_WT;
                 a.accumulate = 0;
                 a.symmetric = (pr > 0) ? 1 : 0;     // V^{ss}[x][y] = V^{ss}[y][x]
-                CK(launch_gemm_tn(a, c->n_sm, st));
+                cudaError_t ge = launch_gemm_tn(a, c->n_sm, fv_.stream(pr));
+                if (ge != cudaSuccess) { fv_.join(); CK(ge); }
                 c->launches++;
             }
+            CK(fv_.join());
             mark(c, 4, st);
             CK(launch_dets(c, 2, nw, ws, st));
             mark(c, 5, st);
