@@ -362,6 +362,115 @@ __global__ void __launch_bounds__(NTHR, MINB) k_dets_cf(DetsParams p, const Work
 }
 
 // ------------------------------------------------------------------------------------------------
+// Force-bias mode of the closed-form levels with the CI reduction done by owner slots in shared memory
+// (msd_internal.cuh C1_*): no RED.ADD.F64 per entry, one flush of the CTA's C tile at the end.
+// g is read through L1 (57 KB per tile, nothing else competes for L1 in this mode); shared memory holds the
+// CTA's C tile [(P_a + P_b)][WT] complex and the round's products val[e][slot][WT].
+// ------------------------------------------------------------------------------------------------
+template <int KA, int KB>
+__device__ __forceinline__ void c1_round(const DetsParams& p, const WorkItem& it, int i, int slot, int S, int j,
+                                         const cplx* gA, const cplx* gB, cplx* val, cplx& Wl)
+{
+    constexpr int NB = 2 * KA + 2 * KB;
+    constexpr int NWORD = (NB + 3) / 4 > 0 ? (NB + 3) / 4 : 1;
+    uint32_t w[NWORD];
+    const uint32_t* rp = reinterpret_cast<const uint32_t*>(p.tab + it.tab_off + (int64_t)i * it.rs);
+#pragma unroll
+    for (int t = 0; t < NWORD; t++) w[t] = (NB > 0) ? __ldg(rp + t) : 0u;
+    const double cf = __ldg(p.coef + it.det_begin + i);
+    const unsigned char* rb = reinterpret_cast<const unsigned char*>(w);
+    SpinEval<KA, 1> ea;
+    SpinEval<KB, 1> eb;
+    ea.run(rb, gA, p.no[0], nullptr, 0u);
+    eb.run(rb + 2 * KA, gB, p.no[1], nullptr, 0u);
+    const cplx cRa = cscale(cf, ea.R), cRb = cscale(cf, eb.R);
+    Wl = cfma(cRa, eb.R, Wl);
+    cplx* v = val + slot * MSD_WT + j;
+#pragma unroll
+    for (int a = 0; a < KA; a++)
+#pragma unroll
+        for (int b = 0; b < KA; b++) v[(a * KA + b) * S * MSD_WT] = cmul(cRb, ea.A[b][a]);
+#pragma unroll
+    for (int a = 0; a < KB; a++)
+#pragma unroll
+        for (int b = 0; b < KB; b++) v[(KA * KA + a * KB + b) * S * MSD_WT] = cmul(cRa, eb.A[b][a]);
+}
+
+#define C1_CASE(KA_, KB_)                                                                              \
+    case KA_ * 5 + KB_:                                                                                \
+        if constexpr ((KA_ > KB_ ? KA_ : KB_) > KLO && (KA_ > KB_ ? KA_ : KB_) <= KHI)                  \
+            c1_round<KA_, KB_>(p, it, i, slot, S, j, gA, gB, val, Wl);                                  \
+        break;
+
+template <int KLO, int KHI, int NTHR>
+__global__ void __launch_bounds__(NTHR, 1) k_dets_c1(DetsParams p, const WorkItem* __restrict__ items, int n_items,
+                                                     const uint32_t* __restrict__ sched)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int S = NTHR / MSD_WT;
+    const int HW = c1_hdr_words(S);
+    cplx* Csm = reinterpret_cast<cplx*>(smem_raw);                  // [(P_a + P_b)][WT]
+    const int PT = p.P[0] + p.P[1];
+    cplx* val = Csm + PT * MSD_WT;                                  // [E][S][WT]
+    const int tile = blockIdx.y;
+    const int j = threadIdx.x & (MSD_WT - 1);
+    const int slot = threadIdx.x / MSD_WT;
+    const cplx* gA = p.g[0] + (int64_t)tile * p.P[0] * MSD_WT + j;
+    const cplx* gB = p.g[1] + (int64_t)tile * p.P[1] * MSD_WT + j;
+    for (int e = threadIdx.x; e < PT * MSD_WT; e += NTHR) Csm[e] = cmake(0.0, 0.0);
+    __syncthreads();
+    cplx Wl = cmake(0.0, 0.0);
+    for (int r0 = 0, ii; (ii = r0 * (int)gridDim.x + ((r0 & 1) ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x)),
+                         r0 * (int)gridDim.x < n_items; r0++) {
+        if (ii >= n_items) continue;
+        const WorkItem it = items[ii];
+        const int E = it.ka * it.ka + it.kb * it.kb;
+        const int nr = (it.det_count + S - 1) / S;
+        for (int r = 0; r < nr; r++) {
+            const int i = r * S + slot;
+            if (i < it.det_count) {
+                switch (it.ka * 5 + it.kb) {
+                    C1_CASE(0, 0) C1_CASE(0, 1) C1_CASE(0, 2) C1_CASE(0, 3) C1_CASE(0, 4)
+                    C1_CASE(1, 0) C1_CASE(1, 1) C1_CASE(1, 2) C1_CASE(1, 3) C1_CASE(1, 4)
+                    C1_CASE(2, 0) C1_CASE(2, 1) C1_CASE(2, 2) C1_CASE(2, 3) C1_CASE(2, 4)
+                    C1_CASE(3, 0) C1_CASE(3, 1) C1_CASE(3, 2) C1_CASE(3, 3) C1_CASE(3, 4)
+                    C1_CASE(4, 0) C1_CASE(4, 1) C1_CASE(4, 2) C1_CASE(4, 3) C1_CASE(4, 4)
+                    default: break;
+                }
+            }
+            if (E == 0) continue;                                   // uniform over the CTA
+            __syncthreads();
+            // owner phase: slot q adds the entries with x % S == q, in list order
+            const uint32_t* hdr = sched + it.sched_off + (int64_t)r * (HW + (int64_t)S * E);
+            const uint32_t* ent = hdr + HW;
+            const int lo = (int)((__ldg(hdr + (slot >> 1)) >> (16 * (slot & 1))) & 0xffffu);
+            const int hi = (int)((__ldg(hdr + ((slot + 1) >> 1)) >> (16 * ((slot + 1) & 1))) & 0xffffu);
+            for (int t = lo; t < hi; t++) {
+                const uint32_t en = __ldg(ent + t);
+                const int x = (int)(en >> 12), sl = (int)((en >> 5) & 127u), e = (int)(en & 31u);
+                const cplx v = val[(e * S + sl) * MSD_WT + j];
+                cplx cacc = Csm[x * MSD_WT + j];
+                cacc.x += v.x; cacc.y += v.y;
+                Csm[x * MSD_WT + j] = cacc;
+            }
+            __syncthreads();
+        }
+    }
+    // flush the CTA's C tile into the planar global accumulators
+    __syncthreads();
+    for (int e = threadIdx.x; e < PT * MSD_WT; e += NTHR) {
+        const cplx v = Csm[e];
+        if (v.x == 0.0 && v.y == 0.0) continue;
+        const int x = e / MSD_WT, jj = e - x * MSD_WT;
+        const int sp = x >= p.P[0];
+        const int xl = sp ? x - p.P[0] : x;
+        double* C = p.C[sp] + (int64_t)tile * p.P[sp] * 2 * MSD_WT + jj;
+        red_add_planar(C, xl, v);
+    }
+    flush_walker_sums(p, tile, Wl, cmake(0.0, 0.0), cmake(0.0, 0.0), 1);
+}
+
+// ------------------------------------------------------------------------------------------------
 // generic levels (k >= 5 in at least one spin): one matrix per thread in shared memory, element e of
 // thread t at sm[e * T + t] (consecutive lanes -> consecutive 16-byte words: conflict-free for any per-lane e).
 // After a spin is evaluated its region holds A (entry e = b*k+a is A[b][a]) and the int region holds the pair
@@ -823,6 +932,21 @@ static cudaError_t launch_persistent(K kernel, int nthr, size_t smem, int n_sm, 
     return cudaGetLastError();
 }
 
+template <class K>
+static cudaError_t launch_c1(K kernel, int nthr, size_t smem, int n_sm, const DetsParams& p, const WorkItem* items, int n_items,
+                             int ntiles, const uint32_t* sched, cudaStream_t st)
+{
+    if (n_items == 0) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int workers = (n_sm + 1) / 2;                  // one CTA per SM, about two walker tiles resident at a time
+    if (workers > n_items) workers = n_items;
+    if (ntiles == 1) workers = n_items < n_sm ? n_items : n_sm;
+    dim3 grid(workers, ntiles);
+    kernel<<<grid, nthr, smem, st>>>(p, items, n_items, sched);
+    return cudaGetLastError();
+}
+
 template <int MODE>
 static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cudaStream_t st)
 {
@@ -853,6 +977,16 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
         // energy mode: one large CTA per SM that also holds Hrot / F of the tile in shared memory (same warps per SM as
         // the 2-3 smaller CTAs of the other modes); falls back to global Hrot / F when the tile does not fit
         bool fhs = false;
+        if constexpr (MODE == 1) {
+            const size_t csm = (size_t)(p.P[0] + p.P[1]) * MSD_WT * sizeof(cplx);
+            const size_t sm1 = csm + (size_t)C1_EMAX[cl] * C1_SLOTS[cl] * MSD_WT * sizeof(cplx);
+            if (sm1 <= 227 * 1024 && c->d_sched && p.P[0] + p.P[1] < 8192) {
+                fhs = true;     // handled here
+                if (cl == 0) e = launch_c1(k_dets_c1<-1, 2, 768>, 768, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
+                else if (cl == 1) e = launch_c1(k_dets_c1<2, 3, 512>, 512, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
+                else e = launch_c1(k_dets_c1<3, 4, 256>, 256, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
+            }
+        }
         if constexpr (MODE == 2) {
             fhs = 3 * gbytes <= 200 * 1024;
             if (!fhs) {}

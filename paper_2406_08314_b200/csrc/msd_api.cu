@@ -259,6 +259,54 @@ static int do_setup(msd_ctx* c, std::string* errp, int N, int na, int nb, int n_
         c->gen_group_begin.push_back(i);
         if (g < 10) c->gen_group_elems.push_back(gen_thresholds[g]);
     }
+    // CI-reduction schedules (msd_internal.cuh C1_*): entries of every round grouped by owner slot x % S
+    {
+        int64_t tab_bytes_all = 0;
+        for (const Bucket& b : c->buckets) tab_bytes_all = std::max<int64_t>(tab_bytes_all, b.tab_off + (b.count * b.rs + 15) / 16 * 16);
+        std::vector<unsigned char> htab((size_t)std::max<int64_t>(tab_bytes_all, 16));
+        CK(cudaMemcpyAsync(htab.data(), c->d_tab, (size_t)tab_bytes_all, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        int64_t words = 0;
+        for (WorkItem& w : c->items_cf) {
+            const int S = C1_SLOTS[cls(w)], E = w.ka * w.ka + w.kb * w.kb;
+            w.sched_off = words;
+            words += (int64_t)((w.det_count + S - 1) / S) * (c1_hdr_words(S) + (int64_t)S * E);
+        }
+        std::vector<uint32_t> sched((size_t)std::max<int64_t>(words, 1), 0u);
+        const int noa = c->sp[0].n_o, nob = c->sp[1].n_o, Pa = c->sp[0].P;
+        std::vector<uint32_t> ent; std::vector<int> cnt;
+        for (const WorkItem& w : c->items_cf) {
+            const int S = C1_SLOTS[cls(w)], ka = w.ka, kb = w.kb, E = ka * ka + kb * kb, HW = c1_hdr_words(S);
+            if (E == 0) { continue; }
+            const int nr = (w.det_count + S - 1) / S;
+            for (int r = 0; r < nr; r++) {
+                uint32_t* hdr = sched.data() + w.sched_off + (int64_t)r * (HW + (int64_t)S * E);
+                uint32_t* out = hdr + HW;
+                const int nd = std::min(S, w.det_count - r * S);
+                ent.clear(); cnt.assign(S + 1, 0);
+                for (int sl = 0; sl < nd; sl++) {
+                    const unsigned char* row = htab.data() + w.tab_off + (int64_t)(r * S + sl) * w.rs;
+                    for (int a = 0; a < ka; a++)
+                        for (int b = 0; b < ka; b++) {
+                            const uint32_t x = (uint32_t)row[ka + b] * noa + row[a];
+                            ent.push_back(x << 12 | (uint32_t)sl << 5 | (uint32_t)(a * ka + b));
+                        }
+                    for (int a = 0; a < kb; a++)
+                        for (int b = 0; b < kb; b++) {
+                            const uint32_t x = (uint32_t)Pa + (uint32_t)row[2 * ka + kb + b] * nob + row[2 * ka + a];
+                            ent.push_back(x << 12 | (uint32_t)sl << 5 | (uint32_t)(ka * ka + a * kb + b));
+                        }
+                }
+                for (uint32_t e : ent) cnt[(e >> 12) % S + 1]++;
+                for (int q = 0; q < S; q++) cnt[q + 1] += cnt[q];
+                for (int q = 0; q <= S; q++) hdr[q >> 1] |= (uint32_t)cnt[q] << (16 * (q & 1));
+                std::vector<int> fill(cnt.begin(), cnt.end() - 1);
+                for (uint32_t e : ent) out[fill[(e >> 12) % S]++] = e;
+            }
+        }
+        CK(upload(&c->d_sched, sched.data(), sched.size(), st));
+        CK(cudaStreamSynchronize(st));
+    }
     CK(upload(&c->d_items_cf, c->items_cf.data(), c->items_cf.size(), st));
     CK(upload(&c->d_items_gen, c->items_gen.data(), c->items_gen.size(), st));
     CK(cudaStreamSynchronize(st));
@@ -348,7 +396,7 @@ extern "C" void msd_destroy(msd_ctx* c)
     for (int s = 0; s < 2; s++) {
         cudaFree(c->sp[s].d_occ_ref); cudaFree(c->sp[s].d_act_v); cudaFree(c->sp[s].d_pos_o); cudaFree(c->sp[s].d_Lsub);
     }
-    cudaFree(c->d_tab); cudaFree(c->d_coef); cudaFree(c->d_items_cf); cudaFree(c->d_items_gen);
+    cudaFree(c->d_tab); cudaFree(c->d_coef); cudaFree(c->d_items_cf); cudaFree(c->d_items_gen); cudaFree(c->d_sched);
     cudaFree(c->ws.base);
     cudaFree(c->stg_a); cudaFree(c->stg_b); cudaFree(c->stg_out); cudaFree(c->stg_flags);
     for (auto& e : c->ev) if (e) cudaEventDestroy(e);

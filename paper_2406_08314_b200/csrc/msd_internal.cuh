@@ -97,7 +97,19 @@ struct WorkItem {          // a chunk of one bucket, processed by one CTA per wa
     int64_t det_begin;     // in the sorted list
     int det_count;
     int64_t tab_off;       // byte offset of the chunk's first row
+    int64_t sched_off;     // closed-form items: first word of the item's CI-reduction schedule (see C1_* below)
 };
+
+// Force-bias CI reduction without atomics (k_dets_c1, dets.cu).  A CTA of C1_SLOTS[cls] determinant slots x 8 walkers
+// works in rounds of C1_SLOTS determinants: every thread first leaves its c~ R^sbar A[b][a] products in shared memory,
+// then the 8 lanes of slot q add up, in order, exactly the entries whose pair index x satisfies x % C1_SLOTS == q
+// ("owner computes": plain shared-memory read-modify-write, no two threads ever touch the same accumulator).
+// Which entries those are depends only on the excitation table, so the lists are built once at setup:
+//   round r of an item = C1_HDR(S) header words (S+1 uint16 offsets) + S*E entry words, E = ka^2 + kb^2,
+//   entry = x_unified << 12 | slot << 5 | e      (x_unified = x for alpha, P_alpha + x for beta; e = a*k+b, beta after alpha)
+static const int C1_SLOTS[3] = {96, 64, 32};     // register classes: larger level <= 2, == 3, == 4
+static const int C1_EMAX[3] = {8, 18, 32};
+__host__ __device__ inline int c1_hdr_words(int S) { return (S + 2) / 2; }
 
 struct Workspace {
     int64_t wc = 0;        // walker capacity of one chunk (multiple of MSD_WT)
@@ -148,6 +160,7 @@ struct msd_ctx {
     std::vector<Bucket> buckets;
     std::vector<WorkItem> items_cf, items_gen;
     WorkItem* d_items_cf = nullptr; WorkItem* d_items_gen = nullptr;
+    uint32_t* d_sched = nullptr;              // CI-reduction schedules of the closed-form items
     int cf_class_begin[4] = {0, 0, 0, 0};      // items_cf is sorted by register class (larger level <=2, 3, 4)
     std::vector<int> gen_group_begin;         // items_gen is sorted by shared-memory group
     std::vector<int> gen_group_elems;         // ka^2+kb^2 bound of each group (complex elements per thread)
