@@ -55,9 +55,9 @@ def reduce_max_time(ms: float, world: int, device=None) -> float:
 
 def ncu_traffic(kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, averaged over its launches of one step,
-    from the committed ncu --set full summary (profiles/r01c_traffic.csv); None if the file is absent."""
+    from the committed ncu --set full summary (profiles/r01d_traffic.csv); None if the file is absent."""
     import csv
-    path = os.path.join(ROOT, "profiles", "r01c_traffic.csv")
+    path = os.path.join(ROOT, "profiles", "r01d_traffic.csv")
     try:
         rows = [r for r in csv.DictReader(open(path)) if r["kernel"] == kernel]
     except OSError:
@@ -137,6 +137,18 @@ def cpu_oracle_sample(inp, n_det_sample: int, steps: int = 1, warmup: int = 0):
         ts.append(time.perf_counter() - t)
     sec = sum(ts) / len(ts)
     return sub.n_det / sec, sec, o2.threads()
+
+
+def cpu_wick_sample(inp, n_walkers: int):
+    """the same Wick's-theorem algorithm restated for the CPU (oracle/wick_cpu.c, OpenMP), force bias
+    and local energy of the first n_walkers walkers against ALL determinants.  Returns (walker*det/s, seconds, threads)."""
+    from oracle import wick
+    ws = list(range(min(n_walkers, inp.n_w)))
+    wick.run(inp, walkers=ws[:1])              # warm-up (page in L, build the library)
+    t = time.perf_counter()
+    wick.run(inp, walkers=ws, want=("fb", "energy"))
+    sec = time.perf_counter() - t
+    return len(ws) * inp.n_det / sec, sec, wick.threads()
 
 
 def run_reference(args, rank):
@@ -298,7 +310,7 @@ def main():
                                    "MEASURED_PEAKS.json has no FP64 entry; derived 148 SM x 64 FMA/clk x 1.965 GHz = %.1f"
                                    % FP64_PEAK_DERIVED,
                     "traffic": ncu_traffic("k_gemm_tn"),
-                    "traffic_note": "DRAM bytes per launch (mean of the 5 launches), ncu --set full, profiles/r01c_traffic.csv",
+                    "traffic_note": "DRAM bytes per launch (mean of the 5 launches), ncu --set full, profiles/r01d_traffic.csv",
                     "share_of_step": gemm_ms / (sum(step_ms) / len(step_ms)),
                     "algorithmic_flops_per_step": flops_v + flops_lam}
 
@@ -332,6 +344,12 @@ def main():
         cpu_baseline = {"value": thr, "unit": UNIT, "cores": cores, "kind": "oracle",
                         "sample": "walker 0 x first %d of %d determinants (force bias + local energy, tier O2), %.1f s"
                                   % (min(args.oracle_dets, inp.n_det), inp.n_det, sec)}
+    cpu_wick = None
+    if not args.no_cpu_baseline:
+        thr, sec, cores = cpu_wick_sample(inp, 8)
+        cpu_wick = {"value": thr, "unit": UNIT, "cores": cores, "kind": "wick (same algorithm on the CPU, oracle/wick_cpu.c)",
+                    "sample": "walkers 0..7 x all %d determinants (force bias + local energy in one pass), %.1f s"
+                              % (inp.n_det, sec)}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64 (complex128)", "data": "synthetic",
@@ -343,7 +361,7 @@ def main():
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": n_e2e},
             "gpu_launches": int(launches),
-            "roofline": roofline, "roofline_dets": roofline_dets, "cpu_baseline": cpu_baseline, "phases": phases,
+            "roofline": roofline, "roofline_dets": roofline_dets, "cpu_baseline": cpu_baseline, "cpu_wick_baseline": cpu_wick, "phases": phases,
             "step_ms": {"min": min(step_ms), "median": statistics.median(step_ms), "max": max(step_ms)}}
     print(json.dumps(line), flush=True)
     if world > 1:

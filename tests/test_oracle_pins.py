@@ -221,3 +221,38 @@ def test_generator_roundtrip_and_shapes():
         assert np.abs(np.einsum("wpi,wpj->wij", x.phi_a.conj(), x.phi_a) - np.eye(x.n_alpha)).max() < 1e-12
         assert np.abs(x.L - x.L.transpose(0, 2, 1)).max() == 0.0
     assert mi.generate("tiny").n_det == 36 and mi.generate("tiny-full").n_det == 199
+
+
+# ----------------------------------------------------------------------------------------------
+# the CPU restatement of the Wick's-theorem algorithm (oracle/wick_cpu.c) against the oracle
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,kw", [("tiny", {}), ("open-shell", {}), ("small", {}),
+                                     ("sweep", dict(n_det=400, max_level=7, n_w=8))])
+def test_cpu_wick_baseline_matches_o2(name, kw):
+    """W1-W10 on the CPU (division-based cofactors, V-route) equals the explicit-determinant oracle O2: overlap and
+    force bias to 1e-10 relative, energies to 1e-8 Ha -- the tolerances of the CUDA path."""
+    from oracle import o2, wick
+    x = mi.generate(name, **kw)
+    ws = list(range(min(x.n_w, 4)))
+    r = o2.run(x, walkers=ws, return_G=False)
+    q = wick.run(x, walkers=ws)
+    assert (np.abs(q["ovlp"] - r["ovlp"]) / np.abs(r["ovlp"])).max() < 1e-10
+    assert (np.abs(q["fb"] - r["fb"]).max(axis=1) / np.abs(r["fb"]).max(axis=1)).max() < 1e-10
+    assert np.abs(q["E"] - r["E"]).max() < 1e-8
+
+
+def test_cpu_wick_baseline_at_bench_size_against_stored_oracle_values():
+    """fe2s2 (the bench workload), walker 0: the stored O2 values (tests/golden/make_golden.py) are reproduced."""
+    import json
+    import os
+    from oracle import wick
+    path = os.path.join(os.path.dirname(__file__), "golden", "fe2s2_seed0.json")
+    gold = json.load(open(path))
+    x = mi.generate("fe2s2")
+    w = gold["walkers"][0]
+    q = wick.run(x, walkers=[w])
+    c = lambda a: np.array(a)[..., 0] + 1j * np.array(a)[..., 1]
+    assert abs(q["ovlp"][0] - c(gold["ovlp"])[0]) / abs(c(gold["ovlp"])[0]) < 1e-10
+    assert np.abs(q["E"][0] - c(gold["E"])[0]).max() < 1e-8
+    gs = gold["fb_gamma_sample"]
+    assert np.abs(q["fb"][0][gs] - c(gold["fb"])[0]).max() / gold["fb_max_abs"][0] < 1e-10
