@@ -534,7 +534,8 @@ __device__ __forceinline__ cplx gauss_jordan_t(SmMat m)
     unsigned ipiv = 0u;                       // 4 bits per pivot row (K <= 8)
     cplx det = cmake(1.0, 0.0);
     bool sing = false;
-#pragma unroll 1
+    // K <= 6: pivot steps unrolled too (the c == j / i > j tests resolve at compile time: no selects in the update)
+#pragma unroll (K <= 6 ? K : 1)
     for (int j = 0; j < K; j++) {
         int p = j; double best = cabs2(m.at(j * K + j));
 #pragma unroll
