@@ -257,7 +257,9 @@ struct DenseMmaLayout {
     }
 };
 
-template <int NWARP>
+// MTC / NTC > 0 fix the row-tile and column-tile counts at compile time (the common shapes: every guard and tile loop of the
+// DMMA steps folds away); 0 keeps them as run-time values.
+template <int NWARP, int MTC, int NTC>
 __global__ void __launch_bounds__(NWARP * 32, NWARP == 8 ? 2 : 3)
 k_energy_dense_mma(int n_chol, int64_t nw, int gchunk, SpinDev sa, SpinDev sb, const cplx* __restrict__ theta_a,
                    const cplx* __restrict__ theta_b, const cplx* __restrict__ Lam_a, const cplx* __restrict__ Lam_b,
@@ -301,8 +303,8 @@ k_energy_dense_mma(int n_chol, int64_t nw, int gchunk, SpinDev sa, SpinDev sb, c
     }
     __syncthreads();
 
-    const int MT = 2 * L.half / 8;            // <= 4
-    const int NT = (n + 7) / 8;
+    const int MT = MTC > 0 ? MTC : 2 * L.half / 8;            // <= 4
+    const int NT = NTC > 0 ? NTC : (n + 7) / 8;
     const int KS = L.Kp / 4;
     // per-lane constants of the step-4 fragments
     const int posh[2] = {pos[gq], pos[8 + gq]};
@@ -478,18 +480,39 @@ k_fx(int n_chol, int64_t nw, int Pa, int Pb, const cplx* __restrict__ X0, const 
     if (lane == 0) { cplx* F = (s ? F_b : F_a) + w * (int64_t)P + x; *F = cadd(*F, acc); }
 }
 
-template <int NWARP>
-static cudaError_t launch_dense_mma(msd_ctx* c, int64_t nw, Workspace& ws, size_t smem, cudaStream_t st)
+template <int NWARP, int MTC, int NTC>
+static cudaError_t launch_dense_mma_t(msd_ctx* c, int64_t nw, Workspace& ws, size_t smem, cudaStream_t st)
 {
-    cudaError_t e = cudaFuncSetAttribute(k_energy_dense_mma<NWARP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(k_energy_dense_mma<NWARP, MTC, NTC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)smem);
     if (e != cudaSuccess) return e;
     const int gchunk = 4 * NWARP;
     dim3 grid((c->n_chol + 1 + gchunk - 1) / gchunk, (unsigned)nw, 2);
-    k_energy_dense_mma<NWARP><<<grid, NWARP * 32, smem, st>>>(c->n_chol, nw, gchunk, c->dev(0), c->dev(1), ws.theta[0],
-                                                             ws.theta[1], ws.Lam[0], ws.Lam[1], ws.Bp[0], ws.Bp[1], ws.Bq[0],
-                                                             ws.Bq[1], ws.X0, ws.F[0], ws.F[1], ws.Hrot[0], ws.Hrot[1],
-                                                             ws.Eacc, c->N);
+    k_energy_dense_mma<NWARP, MTC, NTC><<<grid, NWARP * 32, smem, st>>>(
+        c->n_chol, nw, gchunk, c->dev(0), c->dev(1), ws.theta[0], ws.theta[1], ws.Lam[0], ws.Lam[1], ws.Bp[0], ws.Bp[1],
+        ws.Bq[0], ws.Bq[1], ws.X0, ws.F[0], ws.F[1], ws.Hrot[0], ws.Hrot[1], ws.Eacc, c->N);
     return cudaGetLastError();
+}
+
+template <int NWARP>
+static cudaError_t launch_dense_mma(msd_ctx* c, int64_t nw, Workspace& ws, size_t smem, cudaStream_t st)
+{
+    // compile-time tile counts when both spins (those with electrons) have the same ones
+    int mt = -1, nt = -1;
+    for (int s = 0; s < 2; s++) {
+        const auto& sp = c->sp[s];
+        if (sp.n == 0) continue;
+        const int m = 2 * ((sp.n_v + 7) / 8 * 8) / 8, t = (sp.n + 7) / 8;
+        if (mt == -1) { mt = m; nt = t; }
+        else if (mt != m || nt != t) { mt = 0; nt = 0; }
+    }
+    if (mt == 4 && nt == 3) return launch_dense_mma_t<NWARP, 4, 3>(c, nw, ws, smem, st);
+    if (mt == 4 && nt == 2) return launch_dense_mma_t<NWARP, 4, 2>(c, nw, ws, smem, st);
+    if (mt == 4 && nt == 1) return launch_dense_mma_t<NWARP, 4, 1>(c, nw, ws, smem, st);
+    if (mt == 2 && nt == 3) return launch_dense_mma_t<NWARP, 2, 3>(c, nw, ws, smem, st);
+    if (mt == 2 && nt == 2) return launch_dense_mma_t<NWARP, 2, 2>(c, nw, ws, smem, st);
+    if (mt == 2 && nt == 1) return launch_dense_mma_t<NWARP, 2, 1>(c, nw, ws, smem, st);
+    return launch_dense_mma_t<NWARP, 0, 0>(c, nw, ws, smem, st);
 }
 
 cudaError_t launch_energy_dense(msd_ctx* c, int64_t nw, Workspace& ws, cudaStream_t st)
