@@ -113,7 +113,7 @@ cudaError_t launch_green_rows(msd_ctx* c, int64_t nw, Workspace& ws, cplx* Gfull
 // S7: from Lam = L_sub Theta (rows (g, r), r < n: T^g = occupied block; r >= n: active-virtual block)   (W7)
 //   X0_g = tr T^g,  Ex0_g = tr(T^g T^g)
 //   Bfull^g[r'][i] = Lam_v^g[r'][i] - sum_l Theta_v[r'][l] T^g[l][i]
-//   B^g[x=(r',h)]  = Bfull^g[r'][pos(h)]             -> Bp (complex rows) and Bq (rows (br,-bi), (bi,br))
+//   B^g[x=(r',h)]  = Bfull^g[r'][pos(h)]             -> Bp (complex rows; the V GEMM expands them to the real (br,-bi | bi,br) form itself)
 //   FK[x]         += sum_l Bfull^g[r'][l] T^g[l][pos(h)]      (exchange-like part of F, W9)
 //   slice g = n_chol holds h1: Hrot[x] = B^{h1}[x], E1_0 += tr T^{h1}                              (W8)
 // CTA = (chunk of GC slices, walker, spin).
@@ -122,7 +122,7 @@ template <int GC>
 __global__ void __launch_bounds__(256)
 k_energy_dense(int n_chol, int64_t nw, SpinDev sa, SpinDev sb, const cplx* __restrict__ theta_a,
                const cplx* __restrict__ theta_b, const cplx* __restrict__ Lam_a, const cplx* __restrict__ Lam_b,
-               cplx* Bp_a, cplx* Bp_b, double* Bq_a, double* Bq_b, cplx* X0 /*[2][nw][n_chol]*/, cplx* F_a, cplx* F_b,
+               cplx* Bp_a, cplx* Bp_b, cplx* X0 /*[2][nw][n_chol]*/, cplx* F_a, cplx* F_b,
                cplx* Hrot_a, cplx* Hrot_b, cplx* Eacc, int N)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -135,7 +135,6 @@ k_energy_dense(int n_chol, int64_t nw, SpinDev sa, SpinDev sb, const cplx* __res
     const cplx* theta = (s ? theta_b : theta_a) + w * (int64_t)N * n;
     const cplx* Lam = s ? Lam_b : Lam_a;
     cplx* Bp = (s ? Bp_b : Bp_a) + w * (int64_t)P * n_chol;
-    double* Bq = (s ? Bq_b : Bq_a) + w * (int64_t)2 * P * 2 * n_chol;
     cplx* F = (s ? F_b : F_a) + w * (int64_t)P;
     cplx* Hrot = (s ? Hrot_b : Hrot_a) + w * (int64_t)P;
     const int tid = threadIdx.x, nt = blockDim.x;
@@ -215,10 +214,6 @@ k_energy_dense(int n_chol, int64_t nw, SpinDev sa, SpinDev sb, const cplx* __res
         cplx b = Bout[e];
         const int g = g0 + gi;
         Bp[(int64_t)x * n_chol + g] = b;
-        double* q0 = Bq + ((int64_t)(2 * x) * 2 * n_chol) + 2 * g;
-        q0[0] = b.x; q0[1] = -b.y;
-        double* q1 = q0 + 2 * n_chol;
-        q1[0] = b.y; q1[1] = b.x;
     }
     for (int x = tid; x < P; x += nt) red_add(&F[x], cneg(Fk[x]));
     cplx ex = block_sum(ex_part);
@@ -263,7 +258,7 @@ template <int NWARP, int MTC, int NTC>
 __global__ void __launch_bounds__(NWARP * 32, NWARP == 8 ? 2 : 3)
 k_energy_dense_mma(int n_chol, int64_t nw, int gchunk, SpinDev sa, SpinDev sb, const cplx* __restrict__ theta_a,
                    const cplx* __restrict__ theta_b, const cplx* __restrict__ Lam_a, const cplx* __restrict__ Lam_b,
-                   cplx* Bp_a, cplx* Bp_b, double* Bq_a, double* Bq_b, cplx* X0 /*[2][nw][n_chol]*/, cplx* F_a, cplx* F_b,
+                   cplx* Bp_a, cplx* Bp_b, cplx* X0 /*[2][nw][n_chol]*/, cplx* F_a, cplx* F_b,
                    cplx* Hrot_a, cplx* Hrot_b, cplx* Eacc, int N)
 {
     extern __shared__ __align__(16) double smd[];
@@ -276,7 +271,6 @@ k_energy_dense_mma(int n_chol, int64_t nw, int gchunk, SpinDev sa, SpinDev sb, c
     const cplx* theta = (s ? theta_b : theta_a) + w * (int64_t)N * n;
     const cplx* Lam = s ? Lam_b : Lam_a;
     cplx* Bp = (s ? Bp_b : Bp_a) + w * (int64_t)P * n_chol;
-    double* Bq = (s ? Bq_b : Bq_a) + w * (int64_t)2 * P * 2 * n_chol;
     cplx* F = (s ? F_b : F_a) + w * (int64_t)P;
     cplx* Hrot = (s ? Hrot_b : Hrot_a) + w * (int64_t)P;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -422,9 +416,6 @@ k_energy_dense_mma(int n_chol, int64_t nw, int gchunk, SpinDev sa, SpinDev sb, c
                 const cplx b = cmake(lb[r * L.ldb + 2 * pos[h]], lb[r * L.ldb + 2 * pos[h] + 1]);
                 if (g < n_chol) {
                     Bp[(int64_t)x * n_chol + g] = b;
-                    double* q0 = Bq + ((int64_t)(2 * x) * 2 * n_chol) + 2 * g;
-                    *reinterpret_cast<double2*>(q0) = make_double2(b.x, -b.y);
-                    *reinterpret_cast<double2*>(q0 + 2 * n_chol) = make_double2(b.y, b.x);
                 } else {
                     Hrot[x] = b;
                 }
@@ -490,7 +481,7 @@ static cudaError_t launch_dense_mma_t(msd_ctx* c, int64_t nw, Workspace& ws, siz
     dim3 grid((c->n_chol + 1 + gchunk - 1) / gchunk, (unsigned)nw, 2);
     k_energy_dense_mma<NWARP, MTC, NTC><<<grid, NWARP * 32, smem, st>>>(
         c->n_chol, nw, gchunk, c->dev(0), c->dev(1), ws.theta[0], ws.theta[1], ws.Lam[0], ws.Lam[1], ws.Bp[0], ws.Bp[1],
-        ws.Bq[0], ws.Bq[1], ws.X0, ws.F[0], ws.F[1], ws.Hrot[0], ws.Hrot[1], ws.Eacc, c->N);
+        ws.X0, ws.F[0], ws.F[1], ws.Hrot[0], ws.Hrot[1], ws.Eacc, c->N);
     return cudaGetLastError();
 }
 
@@ -549,7 +540,7 @@ cudaError_t launch_energy_dense(msd_ctx* c, int64_t nw, Workspace& ws, cudaStrea
         // X0 of a spin with no electrons must read as zero: ws.X0 lies in the region zeroed per call
         dim3 grid((c->n_chol + 1 + GC - 1) / GC, (unsigned)nw, 2);
         k_energy_dense<GC><<<grid, 256, smem, st>>>(c->n_chol, nw, c->dev(0), c->dev(1), ws.theta[0], ws.theta[1],
-                                                    ws.Lam[0], ws.Lam[1], ws.Bp[0], ws.Bp[1], ws.Bq[0], ws.Bq[1], ws.X0,
+                                                    ws.Lam[0], ws.Lam[1], ws.Bp[0], ws.Bp[1], ws.X0,
                                                     ws.F[0], ws.F[1], ws.Hrot[0], ws.Hrot[1], ws.Eacc, c->N);
         e = cudaGetLastError();
     }

@@ -15,7 +15,7 @@
 #define LDS_ 20       // BK + 4
 #define STAGES 3
 
-template <int BM, int BN, int WARPS_M, int WARPS_N>
+template <int BM, int BN, int WARPS_M, int WARPS_N, bool BX>
 __global__ void __launch_bounds__(WARPS_M * WARPS_N * 32)
 k_gemm_tn(GemmArgs g)
 {
@@ -50,6 +50,15 @@ k_gemm_tn(GemmArgs g)
             const double* src = ok ? (A + (int64_t)m * g.lda + k) : A;
             cp_async16(as + r * LDS_ + kc, src, ok ? 16 : 0);
         }
+        if (BX) {              // BN/2 complex rows: real column n = 2y + c is read from row y at fragment time
+            for (int c = tid; c < (BN / 2) * (BK / 2); c += NT) {
+                int r = c / (BK / 2), kc = (c % (BK / 2)) * 2;
+                int y = n0 / 2 + r, k = k0 + kc;
+                bool ok = (2 * y < g.N) && (k < g.K);
+                const double* src = ok ? (B + (int64_t)y * g.ldb + k) : B;
+                cp_async16(bs + r * LDS_ + kc, src, ok ? 16 : 0);
+            }
+        } else
         for (int c = tid; c < BN * (BK / 2); c += NT) {
             int r = c / (BK / 2), kc = (c % (BK / 2)) * 2;
             int n = n0 + r, k = k0 + kc;
@@ -78,14 +87,20 @@ k_gemm_tn(GemmArgs g)
             cp_async_commit();
         }
         const double* as = As + (kt % STAGES) * BM * LDS_ + (wm + gq) * LDS_ + tq;
-        const double* bs = Bs + (kt % STAGES) * BN * LDS_ + (wn + gq) * LDS_ + tq;
+        // bexpand: B[2y + c][2 gam + c'] = component (c ^ c') of the complex B[y][gam], negated for (c, c') = (0, 1);
+        // c = gq & 1 and c' = tq & 1 are per-lane constants (warp and tile offsets are even)
+        const double* bs = BX ? Bs + (kt % STAGES) * BN * LDS_ + ((wn + gq) >> 1) * LDS_ + ((tq & 2) | ((tq ^ gq) & 1))
+                                     : Bs + (kt % STAGES) * BN * LDS_ + (wn + gq) * LDS_ + tq;
+        constexpr int brow = BX ? 4 * LDS_ : 8 * LDS_;
+        const long long bsign = (BX && !(gq & 1) && (tq & 1)) ? (long long)0x8000000000000000ull : 0ll;   // sign flip as an
+        // integer XOR: a DADD/DMUL would take issue slots of the FP64 pipe that the DMMAs need
 #pragma unroll
         for (int kk = 0; kk < BK / 4; kk++) {
             double a[TM], b[TN];
 #pragma unroll
             for (int i = 0; i < TM; i++) a[i] = as[i * 8 * LDS_ + kk * 4];
 #pragma unroll
-            for (int j = 0; j < TN; j++) b[j] = bs[j * 8 * LDS_ + kk * 4];
+            for (int j = 0; j < TN; j++) { b[j] = bs[j * brow + kk * 4]; if (BX) b[j] = __longlong_as_double(__double_as_longlong(b[j]) ^ bsign); }
 #pragma unroll
             for (int i = 0; i < TM; i++)
 #pragma unroll
@@ -121,20 +136,26 @@ k_gemm_tn(GemmArgs g)
     }
 }
 
-template <int BM, int BN, int WARPS_M, int WARPS_N>
-static cudaError_t launch_cfg(const GemmArgs& a, cudaStream_t st)
+template <int BM, int BN, int WARPS_M, int WARPS_N, bool BX>
+static cudaError_t launch_cfg_x(const GemmArgs& a, cudaStream_t st)
 {
     size_t smem = (size_t)STAGES * (BM + BN) * LDS_ * sizeof(double);
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_gemm_tn<BM, BN, WARPS_M, WARPS_N>,
+        cudaError_t e = cudaFuncSetAttribute(k_gemm_tn<BM, BN, WARPS_M, WARPS_N, BX>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured = true;
     }
     dim3 grid((a.N + BN - 1) / BN, (a.M + BM - 1) / BM, a.batch * a.ksplit);
-    k_gemm_tn<BM, BN, WARPS_M, WARPS_N><<<grid, WARPS_M * WARPS_N * 32, smem, st>>>(a);
+    k_gemm_tn<BM, BN, WARPS_M, WARPS_N, BX><<<grid, WARPS_M * WARPS_N * 32, smem, st>>>(a);
     return cudaGetLastError();
+}
+
+template <int BM, int BN, int WARPS_M, int WARPS_N>
+static cudaError_t launch_cfg(const GemmArgs& a, cudaStream_t st)
+{
+    return a.bexpand ? launch_cfg_x<BM, BN, WARPS_M, WARPS_N, true>(a, st) : launch_cfg_x<BM, BN, WARPS_M, WARPS_N, false>(a, st);
 }
 
 cudaError_t launch_gemm_tn(const GemmArgs& a, int n_sm, cudaStream_t st)
@@ -142,6 +163,7 @@ cudaError_t launch_gemm_tn(const GemmArgs& a, int n_sm, cudaStream_t st)
     if (a.M <= 0 || a.N <= 0 || a.batch <= 0) return cudaSuccess;
     if ((a.N & 1) || (a.K & 1) || (a.lda & 1) || (a.ldb & 1) || (a.strideA & 1) || (a.strideB & 1))
         return cudaErrorInvalidValue;     // callers pad to even sizes (16-byte cp.async chunks)
+    if (a.bexpand && ((a.N & 1) || (a.strideB & 1))) return cudaErrorInvalidValue;
     if (a.ksplit < 1 || (a.ksplit > 1 && a.accumulate != 2) || (a.symmetric && (a.N != 2 * a.M || a.accumulate)))
         return cudaErrorInvalidValue;
     // Tile shape by a wave model: time ~ waves x (CTAs per SM) x BM x BN, waves = ceil(computed tiles / (SMs x CTAs per SM)).

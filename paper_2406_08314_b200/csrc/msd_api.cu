@@ -538,7 +538,6 @@ static size_t carve(const msd_ctx* c, Workspace& ws, char* base, int64_t wc, int
             ws.thetaT[s] = k.take<double>((size_t)wc * sp.n * 2 * ldN);
             ws.Lam[s] = k.take<cplx>((size_t)(ng + 1) * sp.n_r * wc * sp.n);
             ws.Bp[s] = k.take<cplx>((size_t)wc * sp.P * ng);
-            ws.Bq[s] = k.take<double>((size_t)wc * 2 * sp.P * 2 * ng);
             ws.Vss[s] = k.take<cplx>((size_t)nt * sp.P * sp.P * MSD_WT);
             ws.Hrot[s] = k.take<cplx>((size_t)wc * sp.P);
             ws.FH[s] = k.take<cplx>((size_t)nt * sp.P * 2 * MSD_WT);
@@ -687,11 +686,12 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
                 if (A_.P == 0 || B_.P == 0) continue;
                 if (pr > 0 && A_.kmax < 2) continue;          // same-spin V only feeds levels >= 2
                 GemmArgs a;
-                a.A = reinterpret_cast<const double*>(ws.Bp[s1]); a.B = ws.Bq[s2];
+                a.A = reinterpret_cast<const double*>(ws.Bp[s1]); a.B = reinterpret_cast<const double*>(ws.Bp[s2]);
+                a.bexpand = 1;
                 a.C = reinterpret_cast<double*>(pr == 0 ? ws.Vab : ws.Vss[s1]);
                 a.M = A_.P; a.N = 2 * B_.P; a.K = 2 * ng;
                 a.lda = 2 * ng; a.ldb = 2 * ng;
-                a.strideA = (int64_t)A_.P * 2 * ng; a.strideB = (int64_t)2 * B_.P * 2 * ng; a.batch = (int)nw;
+                a.strideA = (int64_t)A_.P * 2 * ng; a.strideB = (int64_t)B_.P * 2 * ng; a.batch = (int)nw;
                 a.zdiv = MSD_WT; a.strideC_hi = (int64_t)A_.P * B_.P * MSD_WT; a.strideC_lo = 1;
                 a.cs_m = (int64_t)B_.P * MSD_WT; a.cs_j = MSD_WT;
                 a.accumulate = 0;

@@ -131,7 +131,6 @@ struct Workspace {
     double* Gp[2] = {nullptr, nullptr};       // [wc][2][n_r*N]   planar rows (w,c)
     cplx* Lam[2] = {nullptr, nullptr};        // [(n_chol+1)*n_r][wc][n]
     cplx* Bp[2] = {nullptr, nullptr};         // [wc][P][n_chol]
-    double* Bq[2] = {nullptr, nullptr};       // [wc][2P][2 n_chol]
     cplx* Vab = nullptr;                      // [nt][Pa][Pb][WT]
     cplx* Vss[2] = {nullptr, nullptr};        // [nt][P][P][WT]
     cplx* F[2] = {nullptr, nullptr};          // [wc][P]          (zeroed)
@@ -246,6 +245,8 @@ struct GemmArgs {
     int zdiv; int64_t strideC_hi, strideC_lo, cs_m, cs_j;
     int accumulate;             // 0: C = result; 1: C += result (plain read-modify-write); 2: RED.ADD (split-K)
     int ksplit = 1;             // grid.z = batch * ksplit; slice z % ksplit covers a BK-aligned K range (accumulate == 2)
+    int bexpand = 0;            // 1: B holds N/2 COMPLEX rows (re,im interleaved along K); the kernel reads them as the real
+                                //    rows (b_r, -b_i), (b_i, b_r) of a complex product, so that form is never written out
     int symmetric = 0;          // 1: C is complex symmetric (M == N/2, A and B describe the same rows): only tiles that
                                 //    touch the upper triangle are computed, element (m, j >= m) is also written to (j, m)
 };
