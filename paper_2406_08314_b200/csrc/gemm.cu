@@ -94,8 +94,7 @@ k_gemm_tn(GemmArgs g)
         constexpr int brow = BX ? 4 * LDS_ : 8 * LDS_;
         const long long bsign = (BX && !(gq & 1) && (tq & 1)) ? (long long)0x8000000000000000ull : 0ll;   // sign flip as an
         // integer XOR: a DADD/DMUL would take issue slots of the FP64 pipe that the DMMAs need
-#pragma unroll
-        for (int kk = 0; kk < BK / 4; kk++) {
+        auto kstep = [&](int kk) {
             double a[TM], b[TN];
 #pragma unroll
             for (int i = 0; i < TM; i++) a[i] = as[i * 8 * LDS_ + kk * 4];
@@ -105,6 +104,14 @@ k_gemm_tn(GemmArgs g)
             for (int i = 0; i < TM; i++)
 #pragma unroll
                 for (int j = 0; j < TN; j++) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        };
+        const int kleft = g.K - (kt_begin + kt) * BK;
+        if (kleft >= BK) {
+#pragma unroll
+            for (int kk = 0; kk < BK / 4; kk++) kstep(kk);
+        } else {               // short last k-tile (K = 100: 6 x 16 + 4): the zero-padded k-steps are skipped
+#pragma unroll 1
+            for (int kk = 0; kk < (kleft + 3) / 4; kk++) kstep(kk);
         }
     }
     cp_async_wait<0>();
