@@ -24,7 +24,8 @@ k_gemm_tn(GemmArgs g)
     constexpr int TM = WM / 8, TN = WN / 8;
     extern __shared__ __align__(16) double smem_gemm[];
     double* As = smem_gemm;                                    // [STAGES][BM][LDS_]
-    double* Bs = smem_gemm + STAGES * BM * LDS_;               // [STAGES][BN][LDS_]
+    constexpr int BROWS = BX ? BN / 2 : BN;                    // expand mode stages BN/2 complex rows
+    double* Bs = smem_gemm + STAGES * BM * LDS_;               // [STAGES][BROWS][LDS_]
     const int z = blockIdx.z / g.ksplit, ks = blockIdx.z - z * g.ksplit;
     if (g.symmetric && (int)(blockIdx.x * BN + BN) / 2 - 1 < (int)(blockIdx.y * BM)) return;   // strictly lower tile
     const double* A = g.A + (int64_t)z * g.strideA;
@@ -42,7 +43,7 @@ k_gemm_tn(GemmArgs g)
     auto load_tile = [&](int stage, int kt) {
         const int k0 = (kt_begin + kt) * BK;
         double* as = As + stage * BM * LDS_;
-        double* bs = Bs + stage * BN * LDS_;
+        double* bs = Bs + stage * BROWS * LDS_;
         for (int c = tid; c < BM * (BK / 2); c += NT) {
             int r = c / (BK / 2), kc = (c % (BK / 2)) * 2;
             int m = m0 + r, k = k0 + kc;
@@ -89,8 +90,8 @@ k_gemm_tn(GemmArgs g)
         const double* as = As + (kt % STAGES) * BM * LDS_ + (wm + gq) * LDS_ + tq;
         // bexpand: B[2y + c][2 gam + c'] = component (c ^ c') of the complex B[y][gam], negated for (c, c') = (0, 1);
         // c = gq & 1 and c' = tq & 1 are per-lane constants (warp and tile offsets are even)
-        const double* bs = BX ? Bs + (kt % STAGES) * BN * LDS_ + ((wn + gq) >> 1) * LDS_ + ((tq & 2) | ((tq ^ gq) & 1))
-                                     : Bs + (kt % STAGES) * BN * LDS_ + (wn + gq) * LDS_ + tq;
+        const double* bs = BX ? Bs + (kt % STAGES) * BROWS * LDS_ + ((wn + gq) >> 1) * LDS_ + ((tq & 2) | ((tq ^ gq) & 1))
+                                     : Bs + (kt % STAGES) * BROWS * LDS_ + (wn + gq) * LDS_ + tq;
         constexpr int brow = BX ? 4 * LDS_ : 8 * LDS_;
         const long long bsign = (BX && !(gq & 1) && (tq & 1)) ? (long long)0x8000000000000000ull : 0ll;   // sign flip as an
         // integer XOR: a DADD/DMUL would take issue slots of the FP64 pipe that the DMMAs need
@@ -146,7 +147,7 @@ k_gemm_tn(GemmArgs g)
 template <int BM, int BN, int WARPS_M, int WARPS_N, bool BX>
 static cudaError_t launch_cfg_x(const GemmArgs& a, cudaStream_t st)
 {
-    size_t smem = (size_t)STAGES * (BM + BN) * LDS_ * sizeof(double);
+    size_t smem = (size_t)STAGES * (BM + (BX ? BN / 2 : BN)) * LDS_ * sizeof(double);
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(k_gemm_tn<BM, BN, WARPS_M, WARPS_N, BX>,
@@ -176,7 +177,8 @@ cudaError_t launch_gemm_tn(const GemmArgs& a, int n_sm, cudaStream_t st)
     // Tile shape by a wave model: time ~ waves x (CTAs per SM) x BM x BN, waves = ceil(computed tiles / (SMs x CTAs per SM)).
     // Padding (e.g. P = 225 rows against 64- or 128-row tiles) and the partly filled last wave are what it minimises.
     struct Cand { int bm, bn, occ; };
-    static const Cand cands[3] = {{128, 64, 2}, {64, 64, 3}, {48, 96, 3}};
+    // CTAs per SM from shared memory and registers; the expand mode stages half the B rows
+    const Cand cands[3] = {{128, 64, 2}, {64, 64, a.bexpand ? 4 : 3}, {48, 96, a.bexpand ? 4 : 3}};
     int best = 0; double best_cost = 0.0;
     for (int i = 0; i < 3; i++) {
         const int tm = (a.M + cands[i].bm - 1) / cands[i].bm, tn = (a.N + cands[i].bn - 1) / cands[i].bn;
