@@ -55,9 +55,9 @@ def reduce_max_time(ms: float, world: int, device=None) -> float:
 
 def ncu_traffic(kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, averaged over its launches of one step,
-    from the committed ncu --set full summary (profiles/r01d_traffic.csv); None if the file is absent."""
+    from the committed ncu --set full summary (profiles/r01e_traffic.csv); None if the file is absent."""
     import csv
-    path = os.path.join(ROOT, "profiles", "r01d_traffic.csv")
+    path = os.path.join(ROOT, "profiles", "r01e_traffic.csv")
     try:
         rows = [r for r in csv.DictReader(open(path)) if r["kernel"] == kernel]
     except OSError:
@@ -310,7 +310,7 @@ def main():
                                    "MEASURED_PEAKS.json has no FP64 entry; derived 148 SM x 64 FMA/clk x 1.965 GHz = %.1f"
                                    % FP64_PEAK_DERIVED,
                     "traffic": ncu_traffic("k_gemm_tn"),
-                    "traffic_note": "DRAM bytes per launch (mean of the 5 launches), ncu --set full, profiles/r01d_traffic.csv",
+                    "traffic_note": "DRAM bytes per launch (mean of the 5 launches), ncu --set full, profiles/r01e_traffic.csv",
                     "share_of_step": gemm_ms / (sum(step_ms) / len(step_ms)),
                     "algorithmic_flops_per_step": flops_v + flops_lam}
 
@@ -346,10 +346,10 @@ def main():
                                   % (min(args.oracle_dets, inp.n_det), inp.n_det, sec)}
     cpu_wick = None
     if not args.no_cpu_baseline:
-        thr, sec, cores = cpu_wick_sample(inp, 8)
+        thr, sec, cores = cpu_wick_sample(inp, inp.n_w)
         cpu_wick = {"value": thr, "unit": UNIT, "cores": cores, "kind": "wick (same algorithm on the CPU, oracle/wick_cpu.c)",
-                    "sample": "walkers 0..7 x all %d determinants (force bias + local energy in one pass), %.1f s"
-                              % (inp.n_det, sec)}
+                    "sample": "all %d walkers x all %d determinants (force bias + local energy in one pass), %.1f s"
+                              % (inp.n_w, inp.n_det, sec)}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64 (complex128)", "data": "synthetic",
