@@ -310,6 +310,14 @@ k_energy_dense_mma(int n_chol, int64_t nw, int gchunk, SpinDev sa, SpinDev sb, c
         for (int b = 0; b < 2; b++) { fk[a][b][0] = 0.0; fk[a][b][1] = 0.0; }
     cplx ex_part = cmake(0.0, 0.0);
 
+    // output phase: element offset of pair index x = tid / NWARP + 32 t inside a warp's Bfull tile (P <= 256: 8 values)
+    int ooff[8];
+#pragma unroll
+    for (int t = 0; t < 8; t++) {
+        const int x = tid / NWARP + 32 * t;
+        const int r = x / no, h = x - r * no;
+        ooff[t] = (x < P) ? r * L.ldb + 2 * pos[h] : 0;
+    }
     const int g_begin = blockIdx.x * gchunk;
     const int g_end = min(g_begin + gchunk, n_chol + 1);
     for (int g0 = g_begin; g0 < g_end; g0 += NWARP) {
@@ -318,10 +326,9 @@ k_energy_dense_mma(int n_chol, int64_t nw, int gchunk, SpinDev sa, SpinDev sb, c
         if (live) {
             // stage T^g (rows l < n) and Lam_v^g (rows n + r) of this walker: n complex = 2n doubles per row
             const cplx* lam = Lam + ((int64_t)g * nr * nw + w) * n;
-            for (int e = lane; e < nr * n; e += 32) {
-                const int r = e / n, i = e - r * n;
-                double* dst = (r < n) ? Tb + r * L.ldt + 2 * i : Lb + (r - n) * L.ldb + 2 * i;
-                cp_async16(dst, lam + (int64_t)r * nw * n + i, 16);
+            for (int i = lane; i < n; i += 32) {               // (no integer division in the per-slice loops)
+                for (int r = 0; r < n; r++) cp_async16(Tb + r * L.ldt + 2 * i, lam + (int64_t)r * nw * n + i, 16);
+                for (int r = n; r < nr; r++) cp_async16(Lb + (r - n) * L.ldb + 2 * i, lam + (int64_t)r * nw * n + i, 16);
             }
             cp_async_commit();
             cp_async_wait<0>();
@@ -332,10 +339,15 @@ k_energy_dense_mma(int n_chol, int64_t nw, int gchunk, SpinDev sa, SpinDev sb, c
             cplx tr = cmake(0.0, 0.0);
             for (int l = lane; l < n; l += 32) tr = cadd(tr, cmake(Tb[l * L.ldt + 2 * l], Tb[l * L.ldt + 2 * l + 1]));
             if (g < n_chol)
-                for (int e = lane; e < n * n; e += 32) {
-                    const int l = e / n, i = e - l * n;
-                    ex_part = cfma(cmake(Tb[l * L.ldt + 2 * i], Tb[l * L.ldt + 2 * i + 1]),
-                                   cmake(Tb[i * L.ldt + 2 * l], Tb[i * L.ldt + 2 * l + 1]), ex_part);
+                // sum_{l,i} T[l][i] T[i][l], lane = i; the column read T[i][.] is skewed by i so that the lanes of a
+                // warp do not all hit the two banks that the row stride (= 8 mod 16 doubles) maps a column to
+                for (int i = lane; i < n; i += 32) {
+                    int l = i;
+                    for (int t = 0; t < n; t++) {
+                        ex_part = cfma(cmake(Tb[l * L.ldt + 2 * i], Tb[l * L.ldt + 2 * i + 1]),
+                                       cmake(Tb[i * L.ldt + 2 * l], Tb[i * L.ldt + 2 * l + 1]), ex_part);
+                        l = (l + 1 == n) ? 0 : l + 1;
+                    }
                 }
             for (int o = 16; o > 0; o >>= 1) {
                 tr.x += __shfl_down_sync(0xffffffffu, tr.x, o);
@@ -407,13 +419,14 @@ k_energy_dense_mma(int n_chol, int64_t nw, int gchunk, SpinDev sa, SpinDev sb, c
         // cooperative output of the round's slices: thread (x, gi) -> NWARP consecutive slices of one pair index
         {
             const int gcount = min(NWARP, g_end - g0);
-            for (int e = tid; e < P * NWARP; e += NWARP * 32) {
-                const int x = e / NWARP, gi = e - x * NWARP;
-                if (gi >= gcount) continue;
+            const int gi = tid % NWARP;                        // thread (x, gi): x = tid / NWARP + 32 t
+#pragma unroll
+            for (int t = 0; t < 8; t++) {
+                const int x = tid / NWARP + 32 * t;
+                if (x >= P || gi >= gcount) continue;
                 const int g = g0 + gi;
-                const int r = x / no, h = x - r * no;
                 const double* lb = Ap + 2 * L.half * L.lda + gi * L.warp_doubles + L.trows * L.ldt;
-                const cplx b = cmake(lb[r * L.ldb + 2 * pos[h]], lb[r * L.ldb + 2 * pos[h] + 1]);
+                const cplx b = cmake(lb[ooff[t]], lb[ooff[t] + 1]);
                 if (g < n_chol) {
                     Bp[(int64_t)x * n_chol + g] = b;
                 } else {
