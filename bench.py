@@ -181,6 +181,8 @@ def main():
     ap.add_argument("--config", default="fe2s2")
     ap.add_argument("--oracle-dets", type=int, default=4000, help="determinants in the CPU-oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--n-det", type=int, default=None, help="override the determinant count (kernel sweep, configs[4])")
+    ap.add_argument("--max-level", type=int, default=None, help="override the maximum excitation level (kernel sweep)")
     args = ap.parse_args()
     rank, world, local = shard_info(args.gpus)
     if args.impl == "reference":
@@ -201,7 +203,12 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
 
-    inp = mi.generate(args.config)
+    over = {}
+    if args.n_det is not None:
+        over["n_det"] = args.n_det
+    if args.max_level is not None:
+        over["max_level"] = args.max_level
+    inp = mi.generate(args.config, **over)
     if rank > 0:   # replicas: same trial, a different walker batch per rank
         rng = np.random.default_rng(inp.params["seed"] + 7919 * rank)
         inp = inp.with_walkers(mi.walkers_from_rng(rng, inp.n_w, inp.N, inp.n_alpha),

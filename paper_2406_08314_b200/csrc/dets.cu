@@ -785,6 +785,9 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
     const int j = threadIdx.x & (MSD_WT - 1);
     const int slot = threadIdx.x / MSD_WT, nslots = blockDim.x / MSD_WT;
     const int T = blockDim.x;
+    unsigned dyn_smem;
+    asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn_smem));
+    const int elems_group = (int)(dyn_smem / ((sizeof(cplx) + sizeof(int)) * T));     // (complex + int) per element per thread
     const cplx* gA = p.g[0] + (int64_t)tile * p.P[0] * MSD_WT + j;      // L1/L2 resident (57 KB per tile)
     const cplx* gB = p.g[1] + (int64_t)tile * p.P[1] * MSD_WT + j;
     double* CA = p.C[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j;
@@ -804,7 +807,9 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
         const int na = ka * ka, nb = kb * kb;
         cplx* mA = gsm + threadIdx.x;
         cplx* mB = mA + na * T;
-        int* xA = reinterpret_cast<int*>(gsm + (na + nb) * T) + threadIdx.x;
+        // the int region starts at the LAUNCH GROUP's element bound, not at this item's na + nb: warps of a CTA are not
+        // synchronised at item boundaries, so an item-dependent split would let one warp's indices alias another's matrix
+        int* xA = reinterpret_cast<int*>(gsm + elems_group * T) + threadIdx.x;
         int* xB = xA + na * T;
         for (int i = slot; i < it.det_count; i += nslots) {
             const uint32_t* rp = reinterpret_cast<const uint32_t*>(p.tab + it.tab_off + (int64_t)i * it.rs);

@@ -412,3 +412,14 @@ def test_native_library_is_the_path(torch_cuda):
     trial.close()
     maps = open("/proc/self/maps").read()
     assert "libmsd_b200.so" in maps
+
+
+def test_many_generic_items_per_cta(torch_cuda):
+    """Kernel-sweep shape with enough high-level determinants that every CTA of the generic-level kernel walks through
+    several work items of different level pairs (regression: the shared-memory split between a thread's matrices and
+    its pair indices must not depend on the item).  Overlap against O2 on every walker, force bias and energy on one."""
+    x = mi.generate("sweep", n_det=40000, max_level=6, n_w=8)
+    got = gpu_all(torch_cuda, x, want_G=False)
+    assert (got["flags"] == 0).all()
+    assert_parity(got, o2.run(x, want=("ovlp",)), what=("ovlp",))
+    assert_parity(got, o2.run(x, walkers=[5], return_G=False), walkers=[5])
