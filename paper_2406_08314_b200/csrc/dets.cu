@@ -873,6 +873,216 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
 }
 
 // ------------------------------------------------------------------------------------------------
+// very high levels (ka^2 + kb^2 > 100), cooperative form: a warp = ONE determinant x 8 walkers x 4 helper lanes
+// (lane = helper * 8 + walker).  The four helpers of a (determinant, walker) share its matrices in shared memory
+// (element e of walker j at mw[e * 8 + j]) and split every loop -- pivot search, row updates, the V gathers -- four ways.
+// One matrix per THREAD (k_dets_gen) needs 2-4 KB of shared memory per thread at these levels, i.e. one or two warps per
+// SM; here it is a quarter of that.  (At levels 5..8 the per-thread form with compile-time K is faster: measured.)
+// Partial sums of the helpers meet in flush_walker_sums (which already adds lanes j, j+8, j+16, j+24).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ cplx shfl_c(cplx v, int src) {
+    return make_double2(__shfl_sync(0xffffffffu, v.x, src), __shfl_sync(0xffffffffu, v.y, src));
+}
+
+// in-place inverse of the k x k matrix of every walker of the warp (partial pivoting); returns det, 0 for an exactly
+// singular matrix (content zeroed: reading A11).  All four helpers of a walker return the same value.
+__device__ __noinline__ cplx co_gauss_jordan(cplx* mw, int k, int hq)
+{
+    unsigned long long ipiv = 0ull;
+    cplx det = cmake(1.0, 0.0);
+    bool sing = false;
+    for (int j0 = 0; j0 < k; j0++) {
+        int p = j0; double best = -1.0;
+        for (int i = j0 + hq; i < k; i += 4) { const double v = cabs2(mw[(i * k + j0) * 8]); if (v > best) { best = v; p = i; } }
+#pragma unroll
+        for (int o = 8; o <= 16; o <<= 1) {
+            const double ob = __shfl_xor_sync(0xffffffffu, best, o);
+            const int op = __shfl_xor_sync(0xffffffffu, p, o);
+            if (ob > best || (ob == best && op < p)) { best = ob; p = op; }
+        }
+        ipiv |= (unsigned long long)p << (4 * j0);
+        if (!(best > 0.0)) sing = true;
+        if (p != j0) {
+            for (int c = hq; c < k; c += 4) { const cplx t = mw[(j0 * k + c) * 8]; mw[(j0 * k + c) * 8] = mw[(p * k + c) * 8]; mw[(p * k + c) * 8] = t; }
+            det = cneg(det);
+        }
+        __syncwarp();
+        const cplx pv = mw[(j0 * k + j0) * 8];
+        det = cmul(det, pv);
+        const cplx r = sing ? cmake(0.0, 0.0) : cinv(pv);
+        __syncwarp();
+        for (int c = hq; c < k; c += 4) {
+            const cplx v = (c == j0) ? cmake(1.0, 0.0) : mw[(j0 * k + c) * 8];
+            mw[(j0 * k + c) * 8] = cmul(v, r);
+        }
+        __syncwarp();
+        for (int i = hq; i < k; i += 4) {
+            if (i == j0) continue;
+            const cplx f = mw[(i * k + j0) * 8];
+            for (int c = 0; c < k; c++) {
+                const cplx v = (c == j0) ? cmake(0.0, 0.0) : mw[(i * k + c) * 8];
+                mw[(i * k + c) * 8] = cfms(f, mw[(j0 * k + c) * 8], v);
+            }
+        }
+        __syncwarp();
+    }
+    for (int j0 = k - 1; j0 >= 0; j0--) {
+        const int p = (int)((ipiv >> (4 * j0)) & 15ull);
+        if (p != j0)
+            for (int i = hq; i < k; i += 4) { const cplx t = mw[(i * k + j0) * 8]; mw[(i * k + j0) * 8] = mw[(i * k + p) * 8]; mw[(i * k + p) * 8] = t; }
+        __syncwarp();
+    }
+    if (sing) {
+        for (int e = hq; e < k * k; e += 4) mw[e * 8] = cmake(0.0, 0.0);
+        det = cmake(0.0, 0.0);
+    }
+    __syncwarp();
+    return det;
+}
+
+// one spin of the warp's determinant.  mw: this lane's walker column of the spin's matrix region; xw: the spin's pair
+// indices (one copy per warp).  On exit mw holds A (entry b*k+a = A[b][a]), xw[b*k+a] = x(a,b); returns R (all helpers);
+// *ess = this helper's share of the same-spin second-order sum.
+template <int MODE>
+__device__ __forceinline__ cplx co_spin(cplx* mw, int* xw, int k, const unsigned char* hp, const cplx* __restrict__ g, int no,
+                                        const cplx* __restrict__ Vss, unsigned P, int hq, int j, cplx* ess)
+{
+    *ess = cmake(0.0, 0.0);
+    if (k == 0) return cmake(1.0, 0.0);
+    if (k <= MSD_CF_MAX) {          // closed forms by helper 0, result shared through shared memory
+        cplx R = cmake(0.0, 0.0);
+        if (hq == 0) {
+            SmMat m{mw, 8};
+            SmIdx xs{xw, 1};
+            switch (k) {
+                case 1: R = closed_to_smem<1>(m, xs, hp, g, no, ess, Vss, P, MODE); break;
+                case 2: R = closed_to_smem<2>(m, xs, hp, g, no, ess, Vss, P, MODE); break;
+                case 3: R = closed_to_smem<3>(m, xs, hp, g, no, ess, Vss, P, MODE); break;
+                default: R = closed_to_smem<4>(m, xs, hp, g, no, ess, Vss, P, MODE); break;
+            }
+        }
+        __syncwarp();
+        return shfl_c(R, j);
+    }
+    const int lane = hq * 8 + j;
+    for (int e = lane; e < k * k; e += 32) {      // pair indices, once per warp
+        const int b = e / k, a = e - b * k;
+        xw[e] = (int)hp[k + b] * no + (int)hp[a];
+    }
+    __syncwarp();
+    for (int e = hq; e < k * k; e += 4) {         // M[a][b] = g[x(a,b)]; x(a,b) sits at xw[b*k+a]
+        const int a = e / k, b = e - a * k;
+        mw[e * 8] = __ldg(&g[xw[b * k + a] * MSD_WT]);
+    }
+    __syncwarp();
+    const cplx R = co_gauss_jordan(mw, k, hq);
+    for (int e = hq; e < k * k; e += 4) mw[e * 8] = cmul(R, mw[e * 8]);      // A = R M^-1
+    __syncwarp();
+    if (MODE == 2 && (R.x != 0.0 || R.y != 0.0)) {
+        // T[b,d;a,c] = (A[b][a] A[d][c] - A[b][c] A[d][a]) / R; (a,c) pairs dealt round-robin to the helpers
+        cplx e = cmake(0.0, 0.0);
+        int t = 0;
+        for (int a = 0; a < k; a++)
+            for (int c = a + 1; c < k; c++, t++) {
+                if ((t & 3) != hq) continue;
+                for (int b = 0; b < k; b++) {
+                    const cplx Aba = mw[(b * k + a) * 8], Abc = mw[(b * k + c) * 8];
+                    const unsigned xab = (unsigned)xw[b * k + a] * P;
+#pragma unroll 4
+                    for (int d = b + 1; d < k; d++) {
+                        const cplx v = __ldg(&Vss[(xab + (unsigned)xw[d * k + c]) * MSD_WT]);
+                        cplx tt = cmul(Aba, mw[(d * k + c) * 8]);
+                        tt = cfms(Abc, mw[(d * k + a) * 8], tt);
+                        e = cfma(tt, v, e);
+                    }
+                }
+            }
+        *ess = cmul(e, cinv(R));
+    }
+    return R;
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(128, 4) k_dets_coop(DetsParams p, const WorkItem* __restrict__ items, int n_items, int elems)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tile = blockIdx.y;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int j = lane & 7, hq = lane >> 3;
+    cplx* mwarp = reinterpret_cast<cplx*>(smem_raw) + (size_t)wid * elems * 8;            // [elems][8 walkers]
+    int* xwarp = reinterpret_cast<int*>(reinterpret_cast<cplx*>(smem_raw) + (size_t)nwarps * elems * 8) + wid * elems;
+    const cplx* gA = p.g[0] + (int64_t)tile * p.P[0] * MSD_WT + j;
+    const cplx* gB = p.g[1] + (int64_t)tile * p.P[1] * MSD_WT + j;
+    double* CA = p.C[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j;
+    double* CB = p.C[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j;
+    const cplx* VA = (MODE == 2) ? p.Vss[0] + (int64_t)tile * p.P[0] * p.P[0] * MSD_WT + j : nullptr;
+    const cplx* VB = (MODE == 2) ? p.Vss[1] + (int64_t)tile * p.P[1] * p.P[1] * MSD_WT + j : nullptr;
+    const cplx* VAB = (MODE == 2) ? p.Vab + (int64_t)tile * p.P[0] * p.P[1] * MSD_WT + j : nullptr;
+    const cplx* FHA = (MODE == 2) ? p.FH[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j : nullptr;
+    const cplx* FHB = (MODE == 2) ? p.FH[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j : nullptr;
+    cplx Wl = cmake(0.0, 0.0), El = cmake(0.0, 0.0), Hl = cmake(0.0, 0.0);
+    for (int r = 0, ii; (ii = r * (int)gridDim.x + ((r & 1) ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x)),
+                        r * (int)gridDim.x < n_items; r++) {
+        if (ii >= n_items) continue;
+        const WorkItem it = items[ii];
+        const int ka = it.ka, kb = it.kb;
+        const int na = ka * ka, nb = kb * kb;
+        cplx* mA = mwarp + j;
+        cplx* mB = mA + na * 8;
+        int* xA = xwarp;
+        int* xB = xwarp + na;
+        for (int i = wid; i < it.det_count; i += nwarps) {
+            const uint32_t* rp = reinterpret_cast<const uint32_t*>(p.tab + it.tab_off + (int64_t)i * it.rs);
+            union { uint32_t w[MSD_MAX_LEVEL]; unsigned char b[4 * MSD_MAX_LEVEL]; } row;
+            for (int t = 0; t < it.rs / 4; t++) row.w[t] = __ldg(rp + t);
+            const double cf = __ldg(&p.coef[it.det_begin + i]);
+            cplx EssA, EssB;
+            const cplx Ra = co_spin<MODE>(mA, xA, ka, row.b, gA, p.no[0], VA, (unsigned)p.P[0], hq, j, &EssA);
+            const cplx Rb = co_spin<MODE>(mB, xB, kb, row.b + 2 * ka, gB, p.no[1], VB, (unsigned)p.P[1], hq, j, &EssB);
+            __syncwarp();
+            const cplx cRa = cscale(cf, Ra), cRb = cscale(cf, Rb);
+            if (hq == 0) Wl = cfma(cRa, Rb, Wl);
+            if (MODE == 2) {
+                // this helper's share: opposite-spin entries u = hq, hq+4, ... of alpha; Hrot / F entries likewise
+                cplx e = cmake(0.0, 0.0), shA = e, sfA = e, shB = e, sfB = e;
+                for (int u = hq; u < na; u += 4) {
+                    const cplx Au = mA[u * 8];
+                    const int xu = xA[u];
+                    const cplx* vrow = VAB + (unsigned)xu * (unsigned)p.P[1] * MSD_WT;
+                    cplx z = cmake(0.0, 0.0);
+#pragma unroll 4
+                    for (int v = 0; v < nb; v++) z = cfma(mB[v * 8], __ldg(&vrow[xB[v] * MSD_WT]), z);
+                    e = cfma(Au, z, e);
+                    const cplx* q = FHA + xu * (2 * MSD_WT);
+                    shA = cfma(Au, __ldg(q), shA);
+                    sfA = cfma(Au, __ldg(q + MSD_WT), sfA);
+                }
+                for (int v = hq; v < nb; v += 4) {
+                    const cplx Bv = mB[v * 8];
+                    const cplx* q = FHB + xB[v] * (2 * MSD_WT);
+                    shB = cfma(Bv, __ldg(q), shB);
+                    sfB = cfma(Bv, __ldg(q + MSD_WT), sfB);
+                }
+                e = cfma(Rb, cadd(EssA, sfA), e);
+                e = cfma(Ra, cadd(EssB, sfB), e);
+                El.x = fma(cf, e.x, El.x);
+                El.y = fma(cf, e.y, El.y);
+                cplx hsum = cmul(Rb, shA);
+                hsum = cfma(Ra, shB, hsum);
+                Hl.x = fma(cf, hsum.x, Hl.x);
+                Hl.y = fma(cf, hsum.y, Hl.y);
+            }
+            if (MODE == 1) {
+                for (int u = hq; u < na; u += 4) red_add_planar(CA, xA[u], cmul(cRb, mA[u * 8]));
+                for (int v = hq; v < nb; v += 4) red_add_planar(CB, xB[v], cmul(cRa, mB[v * 8]));
+            }
+            __syncwarp();       // the next determinant overwrites the warp's matrices
+        }
+    }
+    flush_walker_sums(p, tile, Wl, El, Hl, MODE);
+}
+
+// ------------------------------------------------------------------------------------------------
 // Antisymmetrised same-spin tensor, in place: Vbar[x_ab][x_cd] = V[x_ab][x_cd] - V[x_ad][x_cb] on the entries
 // (h_a < h_c, p_b < p_d) -- the only ones the same-spin sum reads (holes and particles of a determinant ascend).
 // V[x_ad][x_cb] is read through the symmetry V[x][y] = V[y][x] as V[(p_b,h_c)][(p_d,h_a)], an entry no thread writes.
@@ -965,6 +1175,23 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
     for (size_t gi = c->gen_group_begin.size() - 1; gi-- > 0;) {
         const int i0 = c->gen_group_begin[gi], i1 = c->gen_group_begin[gi + 1];
         if (i1 == i0) continue;
+        if (c->gen_group_elems[gi] > 72) {        // the per-thread form would run with at most 3 warps per SM (measured crossover)
+            const int elems = c->gen_group_elems[gi];
+            const size_t smem = (size_t)4 * elems * (8 * sizeof(cplx) + sizeof(int));
+            auto kern = k_dets_coop<MODE>;
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            int occ = 1;
+            if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 128, smem);
+            if (e == cudaSuccess && occ < 1) e = cudaErrorInvalidConfiguration;
+            if (e != cudaSuccess) { f.join(); return e; }
+            int workers = std::min(i1 - i0, (c->n_sm * occ + 1) / 2);
+            if (ntiles == 1) workers = std::min(i1 - i0, c->n_sm * occ);
+            kern<<<dim3(workers, ntiles), 128, smem, f.stream(li++)>>>(p, c->d_items_gen + i0, i1 - i0, elems);
+            e = cudaGetLastError();
+            if (e != cudaSuccess) { f.join(); return e; }
+            c->launches++;
+            continue;
+        }
         int nthr = 128;
         const size_t per_thread = (size_t)c->gen_group_elems[gi] * (sizeof(cplx) + sizeof(int));
         while (nthr > 32 && per_thread * nthr > 200 * 1024) nthr -= 32;
