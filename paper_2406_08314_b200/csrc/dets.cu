@@ -1049,10 +1049,17 @@ __global__ void __launch_bounds__(128, 4) k_dets_coop(DetsParams p, const WorkIt
                     const cplx Au = mA[u * 8];
                     const int xu = xA[u];
                     const cplx* vrow = VAB + (unsigned)xu * (unsigned)p.P[1] * MSD_WT;
-                    cplx z = cmake(0.0, 0.0);
-#pragma unroll 4
-                    for (int v = 0; v < nb; v++) z = cfma(mB[v * 8], __ldg(&vrow[xB[v] * MSD_WT]), z);
-                    e = cfma(Au, z, e);
+                    cplx z0 = cmake(0.0, 0.0), z1 = z0;       // eight independent loads in flight, two FMA chains
+                    int v = 0;
+                    for (; v + 8 <= nb; v += 8) {
+                        cplx w[8];
+#pragma unroll
+                        for (int t = 0; t < 8; t++) w[t] = __ldg(&vrow[xB[v + t] * MSD_WT]);
+#pragma unroll
+                        for (int t = 0; t < 8; t += 2) { z0 = cfma(mB[(v + t) * 8], w[t], z0); z1 = cfma(mB[(v + t + 1) * 8], w[t + 1], z1); }
+                    }
+                    for (; v < nb; v++) z0 = cfma(mB[v * 8], __ldg(&vrow[xB[v] * MSD_WT]), z0);
+                    e = cfma(Au, cadd(z0, z1), e);
                     const cplx* q = FHA + xu * (2 * MSD_WT);
                     shA = cfma(Au, __ldg(q), shA);
                     sfA = cfma(Au, __ldg(q + MSD_WT), sfA);
