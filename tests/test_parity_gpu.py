@@ -423,3 +423,19 @@ def test_many_generic_items_per_cta(torch_cuda):
     assert (got["flags"] == 0).all()
     assert_parity(got, o2.run(x, want=("ovlp",)), what=("ovlp",))
     assert_parity(got, o2.run(x, walkers=[5], return_G=False), walkers=[5])
+
+
+def test_many_high_level_items_per_cta(torch_cuda):
+    """The same at levels up to 10 (cooperative kernel, one determinant per warp): 20000 determinants so that a CTA
+    processes many items; overlap on every walker, force bias on two (the oracle needs no L loop per determinant for
+    either), energy against the CPU restatement of the Wick algorithm (itself pinned to O2 in test_oracle_pins.py),
+    because the brute-force oracle needs minutes per walker here."""
+    from oracle import wick
+    x = mi.generate("sweep", n_det=20000, max_level=10, n_w=8)
+    got = gpu_all(torch_cuda, x, want_G=False)
+    assert (got["flags"] == 0).all()
+    assert_parity(got, o2.run(x, want=("ovlp",)), what=("ovlp",))
+    ws = [0, 7]
+    assert_parity(got, o2.run(x, walkers=ws, want=("ovlp", "greens"), return_G=False), walkers=ws, what=("ovlp", "fb"))
+    q = wick.run(x, walkers=[3], want=("energy",))
+    assert np.abs(got["E"][3] - q["E"][0]).max() <= TOL_E
