@@ -257,6 +257,27 @@ def main():
     total_ms = reduce_max_time(sum(step_ms), world, dev)
     value = total_units(inp.n_w, inp.n_det, args.steps, world) / (total_ms * 1e-3)
 
+    # ---- the same two outputs from the fused call msd_force_bias_energy (one pass of the determinant kernels) ----
+    fused_out = torch.empty((inp.n_w, inp.n_chol + 3), dtype=torch.complex128, device=dev)
+    for _ in range(2):
+        trial.force_bias_energy(d_a, d_b, out=fused_out)
+    barrier()
+    fev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in fev:
+        flush.zero_()
+        a.record(stream)
+        trial.force_bias_energy(d_a, d_b, out=fused_out)
+        b.record(stream)
+    barrier()
+    fused_ms = reduce_max_time(sum(a.elapsed_time(b) for a, b in fev), world, dev)
+    fused = {"call": "msd_force_bias_energy (force bias and local energy of the batch from ONE pass: the energy-mode "
+                     "determinant kernels also accumulate C, fb = X0 + C.B/W, SURVEY.md 8(c) W6)",
+             "value": total_units(inp.n_w, inp.n_det, args.steps, world) / (fused_ms * 1e-3), "unit": UNIT,
+             "ms_per_step": fused_ms / args.steps,
+             "max_rel_diff_fb_vs_separate_calls": float(((fused_out[:, :inp.n_chol] - fb).abs().amax(dim=1)
+                                                         / fb.abs().amax(dim=1)).max().item()),
+             "max_abs_diff_E_vs_separate_calls": float((fused_out[:, inp.n_chol:] - en).abs().max().item())}
+
     # ---- end to end: the C-ABI *_host calls (pinned HOST buffers; H2D + kernels + D2H inside each call) ----
     def e2e_step():
         trial.force_bias_host(h_a, h_b, out=h_fb)
@@ -362,13 +383,13 @@ def main():
             "vs_baseline": None, "dtype": "f64 (complex128)", "data": "synthetic",
             "config": {"workload": args.config, "N": inp.N, "n_alpha": inp.n_alpha, "n_beta": inp.n_beta,
                        "n_chol": inp.n_chol, "n_det": inp.n_det, "n_w": inp.n_w, "active_window": info,
-                       "step": "msd_force_bias + msd_local_energy", "l2": "flushed between timed steps (256 MB write)",
+                       "step": "msd_force_bias + msd_local_energy (two calls; the fused one-pass call is reported under 'fused')", "l2": "flushed between timed steps (256 MB write)",
                        "parallelism": "replicas x%d" % world, "input_sha256": inp.sha256()[:16]},
             "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": n_e2e},
             "gpu_launches": int(launches),
-            "roofline": roofline, "roofline_dets": roofline_dets, "cpu_baseline": cpu_baseline, "cpu_wick_baseline": cpu_wick, "phases": phases,
+            "fused": fused, "roofline": roofline, "roofline_dets": roofline_dets, "cpu_baseline": cpu_baseline, "cpu_wick_baseline": cpu_wick, "phases": phases,
             "step_ms": {"min": min(step_ms), "median": statistics.median(step_ms), "max": max(step_ms)}}
     print(json.dumps(line), flush=True)
     if world > 1:

@@ -100,11 +100,20 @@ int msd_force_bias(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi
 int msd_local_energy(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
                      void* e, int32_t* flags, void* stream);
 
+/* Force bias AND local energy of the same walkers in one pass (the metric's unit of work: one force-bias + local-energy
+ * evaluation per walker x determinant).  out DEVICE [n_w][n_chol + 3] complex128: out[w][0..n_chol) = fb as in
+ * msd_force_bias, out[w][n_chol..n_chol+3) = (E, E1, E2) as in msd_local_energy.  The determinant kernels run once:
+ * the energy pass also accumulates the CI matrix C, and the force bias is taken from C and the half-rotated Cholesky
+ * slices B^g that the energy path holds,  fb_g = sum_s [ X0^s_g + (1/W) sum_x C^s[x] B^{s,g}[x] ]  -- the same
+ * quantity as Eq. 7 / msd_force_bias, not a different estimator.  S1-S9. */
+int msd_force_bias_energy(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
+                          void* out, int32_t* flags, void* stream);
+
 /* G DEVICE [n_w][2][N][N] complex128, G[w][s][p][q] = <a+_p a_q>.  Test hook (S5). */
 int msd_greens(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
                void* G, int32_t* flags, void* stream);
 
-/* HOST-buffer variants of the three hot calls (the end-to-end path: bench.py's "e2e").  phi_a / phi_b / the result /
+/* HOST-buffer variants of the hot calls (the end-to-end path: bench.py's "e2e").  phi_a / phi_b / the result /
  * flags are HOST pointers with the same layouts as above (pinned memory makes the copies asynchronous, pageable
  * memory works too).  Each call enqueues on `stream`: host->device copy of the walkers into staging buffers owned by
  * the context, the same kernels as the device variant, device->host copy of the result (and flags); it then
@@ -115,6 +124,8 @@ int msd_force_bias_host(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void
                         void* fb, int32_t* flags, void* stream);
 int msd_local_energy_host(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
                           void* e, int32_t* flags, void* stream);
+int msd_force_bias_energy_host(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
+                               void* out, int32_t* flags, void* stream);
 
 /* Introspection of the packed trial (host-side copies made at setup; for tests of the packer).
  * msd_get_info fills: info[0]=n_o_alpha, [1]=n_v_alpha, [2]=n_o_beta, [3]=n_v_beta, [4]=number of level

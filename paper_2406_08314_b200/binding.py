@@ -21,6 +21,7 @@ _CODES = {MSD_EINVAL: "MSD_EINVAL", MSD_ENOMEM: "MSD_ENOMEM", MSD_ECUDA: "MSD_EC
 
 EXPORTS = ["msd_setup", "msd_setup_from_occ", "msd_overlap", "msd_force_bias", "msd_local_energy", "msd_greens",
            "msd_overlap_host", "msd_force_bias_host", "msd_local_energy_host",
+           "msd_force_bias_energy", "msd_force_bias_energy_host",
            "msd_get_info", "msd_get_packed", "msd_set_workspace_limit", "msd_launch_count", "msd_set_profiling",
            "msd_get_phase_ms", "msd_probe_fp64_tflops", "msd_destroy", "msd_last_error"]
 
@@ -48,8 +49,8 @@ def load_library() -> C.CDLL:
     lib.msd_setup.argtypes = [C.POINTER(vp), i32, i32, i32, i32, i64, vp, vp, dbl, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.msd_setup_from_occ.restype = i32
     lib.msd_setup_from_occ.argtypes = [C.POINTER(vp), i32, i32, i32, i32, i64, vp, vp, dbl, vp, vp, vp, vp]
-    for name in ("msd_overlap", "msd_force_bias", "msd_local_energy", "msd_greens",
-                 "msd_overlap_host", "msd_force_bias_host", "msd_local_energy_host"):
+    for name in ("msd_overlap", "msd_force_bias", "msd_local_energy", "msd_greens", "msd_force_bias_energy",
+                 "msd_overlap_host", "msd_force_bias_host", "msd_local_energy_host", "msd_force_bias_energy_host"):
         f = getattr(lib, name)
         f.restype = i32
         f.argtypes = [vp, i64, vp, vp, vp, vp, vp]
@@ -155,6 +156,14 @@ class MSDTrial:
         out = torch.empty((nw, 3), dtype=torch.complex128, device=phi_a.device) if out is None else out
         return self._call(load_library().msd_local_energy, phi_a, phi_b, out, flags, stream)
 
+    def force_bias_energy(self, phi_a, phi_b, out=None, flags=None, stream=None):
+        """Both outputs from one pass: returns out [n_w][n_chol + 3]; out[:, :n_chol] is the force bias,
+        out[:, n_chol:] is (E, E1, E2)."""
+        import torch
+        nw = self._walkers(phi_a, phi_b)
+        out = torch.empty((nw, self.n_chol + 3), dtype=torch.complex128, device=phi_a.device) if out is None else out
+        return self._call(load_library().msd_force_bias_energy, phi_a, phi_b, out, flags, stream)
+
     def greens(self, phi_a, phi_b, out=None, flags=None, stream=None):
         import torch
         nw = self._walkers(phi_a, phi_b)
@@ -191,6 +200,10 @@ class MSDTrial:
     def local_energy_host(self, phi_a, phi_b, out=None, flags=None, stream=None):
         out = np.empty((phi_a.shape[0], 3), dtype=np.complex128) if out is None else out
         return self._call_host(load_library().msd_local_energy_host, phi_a, phi_b, out, flags, stream)
+
+    def force_bias_energy_host(self, phi_a, phi_b, out=None, flags=None, stream=None):
+        out = np.empty((phi_a.shape[0], self.n_chol + 3), dtype=np.complex128) if out is None else out
+        return self._call_host(load_library().msd_force_bias_energy_host, phi_a, phi_b, out, flags, stream)
 
     # -- introspection -------------------------------------------------------------------------
     def info(self) -> dict:
@@ -271,6 +284,14 @@ def msd_overlap(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, stream=None
 
 def msd_force_bias(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, stream=None):
     return trial.force_bias(phi_a, phi_b, out, flags, stream)
+
+
+def msd_force_bias_energy(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, stream=None):
+    return trial.force_bias_energy(phi_a, phi_b, out, flags, stream)
+
+
+def msd_force_bias_energy_host(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, stream=None):
+    return trial.force_bias_energy_host(phi_a, phi_b, out, flags, stream)
 
 
 def msd_local_energy(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, stream=None):

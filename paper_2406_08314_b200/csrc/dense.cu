@@ -605,7 +605,7 @@ __global__ void k_finish_flags(int64_t nw, const cplx* __restrict__ Wacc, const 
 __global__ void __launch_bounds__(256)
 k_finish_energy(int n_chol, int64_t nw, double e0, const cplx* __restrict__ X0, const cplx* __restrict__ Eacc,
                 const cplx* __restrict__ Wacc, const cplx* __restrict__ E1nd, const cplx* __restrict__ E2nd,
-                const int* __restrict__ wflags, cplx* eout, int* flags)
+                const int* __restrict__ wflags, cplx* eout, int64_t estride, int* flags)
 {
     const int64_t w = blockIdx.x;
     const int tid = threadIdx.x, nt = blockDim.x;
@@ -626,9 +626,9 @@ k_finish_energy(int n_chol, int64_t nw, double e0, const cplx* __restrict__ X0, 
             E1 = cadd(Eacc[w * 2 + 0], cmul(E1nd[w], Winv));
             E2 = cadd(cadd(cscale(0.5, xx), Eacc[w * 2 + 1]), cmul(E2nd[w], Winv));
         }
-        eout[w * 3 + 0] = cmake(e0 + E1.x + E2.x, E1.y + E2.y);
-        eout[w * 3 + 1] = E1;
-        eout[w * 3 + 2] = E2;
+        eout[w * estride + 0] = cmake(e0 + E1.x + E2.x, E1.y + E2.y);
+        eout[w * estride + 1] = E1;
+        eout[w * estride + 2] = E2;
         if (flags) flags[w] = f;
     }
 }
@@ -650,12 +650,57 @@ cudaError_t launch_finish_flags(msd_ctx* c, int64_t nw, Workspace& ws, cplx* out
     return cudaGetLastError();
 }
 
-cudaError_t launch_finish_energy(msd_ctx* c, int64_t nw, Workspace& ws, cplx* e, int* flags, cudaStream_t st)
+cudaError_t launch_finish_energy(msd_ctx* c, int64_t nw, Workspace& ws, cplx* e, int64_t estride, int* flags, cudaStream_t st)
 {
     if (nw == 0) return cudaSuccess;
     cplx* X0 = ws.X0;
     k_finish_energy<<<(unsigned)nw, 256, 0, st>>>(c->n_chol, nw, c->e0, X0, ws.Eacc, ws.Wacc, ws.E1nd, ws.E2nd, ws.wflags,
-                                                  e, flags);
+                                                  e, estride, flags);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+// Force bias from the energy path's intermediates:
+//   fb[w][g] = sum_s [ X0^s[w][g] + (1/W) sum_x C^s[x][w] B^{s,g}[w][x] ]
+// C planar [tile][x][2][WT], Bp [w][x][g] (g contiguous: coalesced over the threads), out row stride `ostride`.
+__global__ void __launch_bounds__(256)
+k_fb_from_cb(int n_chol, int64_t nw, int Pa, int Pb, const double* __restrict__ C_a, const double* __restrict__ C_b,
+             const cplx* __restrict__ Bp_a, const cplx* __restrict__ Bp_b, const cplx* __restrict__ X0,
+             const cplx* __restrict__ Wacc, const int* __restrict__ wflags, cplx* out, int64_t ostride)
+{
+    extern __shared__ __align__(16) unsigned char smem_fb[];
+    cplx* Cs = reinterpret_cast<cplx*>(smem_fb);              // [Pa + Pb]
+    const int64_t w = blockIdx.y;
+    for (int s = 0; s < 2; s++) {
+        const int P = s ? Pb : Pa;
+        const double* C = (s ? C_b : C_a) + (w / MSD_WT) * (int64_t)P * 2 * MSD_WT + (w % MSD_WT);
+        for (int x = threadIdx.x; x < P; x += blockDim.x) Cs[(s ? Pa : 0) + x] = load_planar(C, x);
+    }
+    __syncthreads();
+    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= n_chol) return;
+    const cplx W = Wacc[w];
+    if (wflags[w] || (W.x == 0.0 && W.y == 0.0)) { out[w * ostride + g] = cmake(nan_d(), nan_d()); return; }
+    cplx acc[2] = {cmake(0.0, 0.0), cmake(0.0, 0.0)};
+    for (int s = 0; s < 2; s++) {
+        const int P = s ? Pb : Pa;
+        const cplx* B = (s ? Bp_b : Bp_a) + w * (int64_t)P * n_chol + g;
+        const cplx* c = Cs + (s ? Pa : 0);
+#pragma unroll 4
+        for (int x = 0; x < P; x++) acc[x & 1] = cfma(c[x], B[(int64_t)x * n_chol], acc[x & 1]);
+    }
+    const cplx t = cmul(cadd(acc[0], acc[1]), cinv(W));
+    const cplx x0 = cadd(X0[w * (int64_t)n_chol + g], X0[(nw + w) * (int64_t)n_chol + g]);
+    out[w * ostride + g] = cadd(x0, t);
+}
+
+cudaError_t launch_fb_from_cb(msd_ctx* c, int64_t nw, Workspace& ws, cplx* out, int64_t ostride, cudaStream_t st)
+{
+    if (nw == 0 || c->n_chol == 0) return cudaSuccess;
+    const int Pa = c->sp[0].P, Pb = c->sp[1].P;
+    dim3 grid((c->n_chol + 255) / 256, (unsigned)nw);
+    k_fb_from_cb<<<grid, 256, (size_t)(Pa + Pb + 1) * sizeof(cplx), st>>>(c->n_chol, nw, Pa, Pb, ws.C[0], ws.C[1], ws.Bp[0],
+                                                                          ws.Bp[1], ws.X0, ws.Wacc, ws.wflags, out, ostride);
     c->launches++;
     return cudaGetLastError();
 }

@@ -16,6 +16,10 @@
 // Levels <= 4 use division-free closed forms in registers (exact for singular minors: pin P7);
 // higher levels use in-place Gauss-Jordan with partial pivoting in shared memory (one matrix per thread).
 #include "msd_internal.cuh"
+// MODE: 0 overlap (W only), 1 force bias (W, C scatter), 2 energy (W, second-order sums, no C), 3 energy + C scatter
+// (the fused force-bias + energy call)
+#define M_ENERGY(M) ((M) >= 2)
+#define M_SCATTER(M) ((M) == 1 || (M) == 3)
 #include <algorithm>
 
 struct DetsParams {
@@ -160,7 +164,7 @@ struct SpinEval {
 #pragma unroll
             for (int b = 0; b < K; b++) M[a][b] = g[x(a, b) * MSD_WT];
         R = Closed<K>::det_adj(M, A);
-        if (MODE == 2 && K >= 2) {
+        if (M_ENERGY(MODE) && K >= 2) {
 #pragma unroll
             for (int a = 0; a < K; a++)
 #pragma unroll
@@ -188,13 +192,13 @@ __device__ __forceinline__ void run_bucket(const DetsParams& p, const WorkItem& 
     const cplx* gB = gsm + p.P[0] * MSD_WT + j;
     double* CA = p.C[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j;
     double* CB = p.C[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j;
-    const cplx* VA = (MODE == 2) ? p.Vss[0] + (int64_t)tile * p.P[0] * p.P[0] * MSD_WT + j : nullptr;
-    const cplx* VB = (MODE == 2) ? p.Vss[1] + (int64_t)tile * p.P[1] * p.P[1] * MSD_WT + j : nullptr;
-    const cplx* VAB = (MODE == 2) ? p.Vab + (int64_t)tile * p.P[0] * p.P[1] * MSD_WT + j : nullptr;
+    const cplx* VA = (M_ENERGY(MODE)) ? p.Vss[0] + (int64_t)tile * p.P[0] * p.P[0] * MSD_WT + j : nullptr;
+    const cplx* VB = (M_ENERGY(MODE)) ? p.Vss[1] + (int64_t)tile * p.P[1] * p.P[1] * MSD_WT + j : nullptr;
+    const cplx* VAB = (M_ENERGY(MODE)) ? p.Vab + (int64_t)tile * p.P[0] * p.P[1] * MSD_WT + j : nullptr;
     // Hrot / F of the tile: the shared-memory copy behind g (FHS) or global memory through L1
-    const cplx* FHA = (MODE != 2) ? nullptr : FHS ? gsm + (p.P[0] + p.P[1]) * MSD_WT + j
+    const cplx* FHA = (!M_ENERGY(MODE)) ? nullptr : FHS ? gsm + (p.P[0] + p.P[1]) * MSD_WT + j
                                                   : p.FH[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j;
-    const cplx* FHB = (MODE != 2) ? nullptr : FHS ? FHA + p.P[0] * 2 * MSD_WT
+    const cplx* FHB = (!M_ENERGY(MODE)) ? nullptr : FHS ? FHA + p.P[0] * 2 * MSD_WT
                                                   : p.FH[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j;
     const unsigned char* tab = p.tab + it.tab_off;
     const double* coef = p.coef + it.det_begin;
@@ -219,7 +223,7 @@ __device__ __forceinline__ void run_bucket(const DetsParams& p, const WorkItem& 
         eb.run(rb + 2 * KA, gB, p.no[1], VB, (unsigned)p.P[1]);
         const cplx cRa = cscale(cf, ea.R), cRb = cscale(cf, eb.R);
         Wl = cfma(cRa, eb.R, Wl);
-        if (MODE == 2) {
+        if (M_ENERGY(MODE)) {
             cplx e = cmake(0.0, 0.0);
             if (KA > 0 && KB > 0) {
 #pragma unroll
@@ -263,7 +267,7 @@ __device__ __forceinline__ void run_bucket(const DetsParams& p, const WorkItem& 
             Hl.x = fma(cf, hsum.x, Hl.x);
             Hl.y = fma(cf, hsum.y, Hl.y);
         }
-        if (MODE == 1) {
+        if (M_SCATTER(MODE)) {
 #pragma unroll
             for (int a = 0; a < KA; a++)
 #pragma unroll
@@ -293,14 +297,14 @@ __device__ __forceinline__ void flush_walker_sums(const DetsParams& p, int tile,
     const int lane = threadIdx.x & 31;
     if (lane < MSD_WT) {
 #pragma unroll
-        for (int t = 0; t < 6; t++) if (t < 2 || mode == 2) atomicAdd(&acc[lane][t], v[t]);
+        for (int t = 0; t < 6; t++) if (t < 2 || mode >= 2) atomicAdd(&acc[lane][t], v[t]);
     }
     __syncthreads();
     if (threadIdx.x < MSD_WT) {
         const int jj = threadIdx.x;
         atomicAdd(&p.Wacc[tile * MSD_WT + jj].x, acc[jj][0]);
         atomicAdd(&p.Wacc[tile * MSD_WT + jj].y, acc[jj][1]);
-        if (mode == 2) {
+        if (mode >= 2) {
             atomicAdd(&p.E2nd[tile * MSD_WT + jj].x, acc[jj][2]);
             atomicAdd(&p.E2nd[tile * MSD_WT + jj].y, acc[jj][3]);
             atomicAdd(&p.E1nd[tile * MSD_WT + jj].x, acc[jj][4]);
@@ -607,7 +611,7 @@ __device__ __forceinline__ cplx closed_to_smem(SmMat m, SmIdx xs, const unsigned
 #pragma unroll
         for (int b = 0; b < K; b++) { m.at(b * K + a) = A[b][a]; xs.at(b * K + a) = pn[b] + h[a]; }
     cplx e = cmake(0.0, 0.0);
-    if (mode == 2 && K >= 2) {
+    if (mode >= 2 && K >= 2) {
 #pragma unroll
         for (int a = 0; a < K; a++)
 #pragma unroll
@@ -650,7 +654,7 @@ __device__ __noinline__ cplx spin_big(cplx* mbase, int* xbase, int T, const unsi
 #pragma unroll
     for (int e = 0; e < K * K; e++) m.at(e) = cmul(R, m.at(e));   // A = R M^-1, entry b*K+a = A[b][a]
     *Ess = cmake(0.0, 0.0);
-    if (MODE == 2 && (R.x != 0.0 || R.y != 0.0)) {
+    if (M_ENERGY(MODE) && (R.x != 0.0 || R.y != 0.0)) {
         cplx e2[2] = {cmake(0.0, 0.0), cmake(0.0, 0.0)};      // two chains: the FMA latency is not on the critical path
 #pragma unroll 1
         for (int a = 0; a < K - 1; a++) {
@@ -697,7 +701,7 @@ __device__ __noinline__ cplx spin_runtime(cplx* mbase, int* xbase, int T, int k,
     cplx R = gauss_jordan(m, k);
     for (int e = 0; e < k * k; e++) m.at(e) = cmul(R, m.at(e));
     *Ess = cmake(0.0, 0.0);
-    if (mode == 2 && (R.x != 0.0 || R.y != 0.0)) {
+    if (mode >= 2 && (R.x != 0.0 || R.y != 0.0)) {
         cplx e = cmake(0.0, 0.0);
         for (int a = 0; a < k; a++)
             for (int c = a + 1; c < k; c++)
@@ -792,11 +796,11 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
     const cplx* gB = p.g[1] + (int64_t)tile * p.P[1] * MSD_WT + j;
     double* CA = p.C[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j;
     double* CB = p.C[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j;
-    const cplx* VA = (MODE == 2) ? p.Vss[0] + (int64_t)tile * p.P[0] * p.P[0] * MSD_WT + j : nullptr;
-    const cplx* VB = (MODE == 2) ? p.Vss[1] + (int64_t)tile * p.P[1] * p.P[1] * MSD_WT + j : nullptr;
-    const cplx* VAB = (MODE == 2) ? p.Vab + (int64_t)tile * p.P[0] * p.P[1] * MSD_WT + j : nullptr;
-    const cplx* FHA = (MODE == 2) ? p.FH[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j : nullptr;
-    const cplx* FHB = (MODE == 2) ? p.FH[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j : nullptr;
+    const cplx* VA = (M_ENERGY(MODE)) ? p.Vss[0] + (int64_t)tile * p.P[0] * p.P[0] * MSD_WT + j : nullptr;
+    const cplx* VB = (M_ENERGY(MODE)) ? p.Vss[1] + (int64_t)tile * p.P[1] * p.P[1] * MSD_WT + j : nullptr;
+    const cplx* VAB = (M_ENERGY(MODE)) ? p.Vab + (int64_t)tile * p.P[0] * p.P[1] * MSD_WT + j : nullptr;
+    const cplx* FHA = (M_ENERGY(MODE)) ? p.FH[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j : nullptr;
+    const cplx* FHB = (M_ENERGY(MODE)) ? p.FH[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j : nullptr;
     cplx Wl = cmake(0.0, 0.0), El = cmake(0.0, 0.0), Hl = cmake(0.0, 0.0);
     // snake order over rounds: items are sorted by descending cost, so alternate the direction to even out
     for (int r = 0, ii; (ii = r * (int)gridDim.x + ((r & 1) ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x)),
@@ -821,7 +825,7 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
             const cplx Rb = spin_any<MODE>(mB, xB, T, kb, row.b + 2 * ka, gB, p.no[1], VB, (unsigned)p.P[1], &EssB);
             const cplx cRa = cscale(cf, Ra), cRb = cscale(cf, Rb);
             Wl = cfma(cRa, Rb, Wl);
-            if (MODE == 2) {
+            if (M_ENERGY(MODE)) {
                 cplx e = cmake(0.0, 0.0);
                 if (na > 0 && nb > 0) {
                     const bool abig = ka >= kb;
@@ -861,7 +865,7 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
                 Hl.x = fma(cf, hsum.x, Hl.x);
                 Hl.y = fma(cf, hsum.y, Hl.y);
             }
-            if (MODE == 1) {
+            if (M_SCATTER(MODE)) {
 #pragma unroll 4
                 for (int e = 0; e < na; e++) red_add_planar(CA, xA[e * T], cmul(cRb, mA[e * T]));
 #pragma unroll 4
@@ -978,7 +982,7 @@ __device__ __forceinline__ cplx co_spin(cplx* mw, int* xw, int k, const unsigned
     const cplx R = co_gauss_jordan(mw, k, hq);
     for (int e = hq; e < k * k; e += 4) mw[e * 8] = cmul(R, mw[e * 8]);      // A = R M^-1
     __syncwarp();
-    if (MODE == 2 && (R.x != 0.0 || R.y != 0.0)) {
+    if (M_ENERGY(MODE) && (R.x != 0.0 || R.y != 0.0)) {
         // T[b,d;a,c] = (A[b][a] A[d][c] - A[b][c] A[d][a]) / R; (a,c) pairs dealt round-robin to the helpers
         cplx e = cmake(0.0, 0.0);
         int t = 0;
@@ -1015,11 +1019,11 @@ __global__ void __launch_bounds__(128, 4) k_dets_coop(DetsParams p, const WorkIt
     const cplx* gB = p.g[1] + (int64_t)tile * p.P[1] * MSD_WT + j;
     double* CA = p.C[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j;
     double* CB = p.C[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j;
-    const cplx* VA = (MODE == 2) ? p.Vss[0] + (int64_t)tile * p.P[0] * p.P[0] * MSD_WT + j : nullptr;
-    const cplx* VB = (MODE == 2) ? p.Vss[1] + (int64_t)tile * p.P[1] * p.P[1] * MSD_WT + j : nullptr;
-    const cplx* VAB = (MODE == 2) ? p.Vab + (int64_t)tile * p.P[0] * p.P[1] * MSD_WT + j : nullptr;
-    const cplx* FHA = (MODE == 2) ? p.FH[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j : nullptr;
-    const cplx* FHB = (MODE == 2) ? p.FH[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j : nullptr;
+    const cplx* VA = (M_ENERGY(MODE)) ? p.Vss[0] + (int64_t)tile * p.P[0] * p.P[0] * MSD_WT + j : nullptr;
+    const cplx* VB = (M_ENERGY(MODE)) ? p.Vss[1] + (int64_t)tile * p.P[1] * p.P[1] * MSD_WT + j : nullptr;
+    const cplx* VAB = (M_ENERGY(MODE)) ? p.Vab + (int64_t)tile * p.P[0] * p.P[1] * MSD_WT + j : nullptr;
+    const cplx* FHA = (M_ENERGY(MODE)) ? p.FH[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j : nullptr;
+    const cplx* FHB = (M_ENERGY(MODE)) ? p.FH[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j : nullptr;
     cplx Wl = cmake(0.0, 0.0), El = cmake(0.0, 0.0), Hl = cmake(0.0, 0.0);
     for (int r = 0, ii; (ii = r * (int)gridDim.x + ((r & 1) ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x)),
                         r * (int)gridDim.x < n_items; r++) {
@@ -1042,7 +1046,7 @@ __global__ void __launch_bounds__(128, 4) k_dets_coop(DetsParams p, const WorkIt
             __syncwarp();
             const cplx cRa = cscale(cf, Ra), cRb = cscale(cf, Rb);
             if (hq == 0) Wl = cfma(cRa, Rb, Wl);
-            if (MODE == 2) {
+            if (M_ENERGY(MODE)) {
                 // this helper's share: opposite-spin entries u = hq, hq+4, ... of alpha; Hrot / F entries likewise
                 cplx e = cmake(0.0, 0.0), shA = e, sfA = e, shB = e, sfB = e;
                 for (int u = hq; u < na; u += 4) {
@@ -1079,7 +1083,7 @@ __global__ void __launch_bounds__(128, 4) k_dets_coop(DetsParams p, const WorkIt
                 Hl.x = fma(cf, hsum.x, Hl.x);
                 Hl.y = fma(cf, hsum.y, Hl.y);
             }
-            if (MODE == 1) {
+            if (M_SCATTER(MODE)) {
                 for (int u = hq; u < na; u += 4) red_add_planar(CA, xA[u], cmul(cRb, mA[u * 8]));
                 for (int v = hq; v < nb; v += 4) red_add_planar(CB, xB[v], cmul(cRa, mB[v * 8]));
             }
@@ -1227,7 +1231,7 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
                 else e = launch_c1(k_dets_c1<3, 4, 256>, 256, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
             }
         }
-        if constexpr (MODE == 2) {
+        if constexpr (MODE >= 2) {
             fhs = 3 * gbytes <= 200 * 1024;
             if (!fhs) {}
             else if (cl == 0) e = launch_persistent(k_dets_cf<MODE, -1, 2, 768, 1, true>, 768, 3 * gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
@@ -1257,7 +1261,7 @@ cudaError_t launch_dets(msd_ctx* c, int mode, int64_t nw, Workspace& ws, cudaStr
     p.Vab = ws.Vab; p.Wacc = ws.Wacc; p.E2nd = ws.E2nd; p.E1nd = ws.E1nd;
     p.FH[0] = ws.FH[0]; p.FH[1] = ws.FH[1];
     int ntiles = (int)((nw + MSD_WT - 1) / MSD_WT);
-    if (mode == 2) {
+    if (mode >= 2) {
         for (int s = 0; s < 2; s++) {
             const auto& sp = c->sp[s];
             if (sp.kmax < 2 || sp.n_o < 2 || sp.n_v < 2) continue;
@@ -1281,5 +1285,6 @@ cudaError_t launch_dets(msd_ctx* c, int mode, int64_t nw, Workspace& ws, cudaStr
     }
     if (mode == 0) return launch_mode<0>(c, p, ntiles, st);
     if (mode == 1) return launch_mode<1>(c, p, ntiles, st);
-    return launch_mode<2>(c, p, ntiles, st);
+    if (mode == 2) return launch_mode<2>(c, p, ntiles, st);
+    return launch_mode<3>(c, p, ntiles, st);
 }

@@ -586,15 +586,16 @@ static int ensure_workspace(msd_ctx* c, int level, int64_t nw, std::string* errp
 // ---------------------------------------------------------------------------------------------
 // hot calls
 // ---------------------------------------------------------------------------------------------
-enum { CALL_OVERLAP = 1, CALL_FB = 2, CALL_GREENS = 4, CALL_ENERGY = 8 };
+enum { CALL_OVERLAP = 1, CALL_FB = 2, CALL_GREENS = 4, CALL_ENERGY = 8, CALL_FB_ENERGY = 16 };
 
 static void mark(msd_ctx* c, int i, cudaStream_t st) { if (c->profiling) cudaEventRecord(c->ev[i], st); }
 
 static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, const cplx* phi_a, const cplx* phi_b,
                       cplx* out, int* flags, cudaStream_t st)
 {
-    const int level = (call == CALL_OVERLAP) ? 1 : (call == CALL_ENERGY ? 3 : 2);
-    if (call == CALL_ENERGY && std::max(c->sp[0].P, c->sp[1].P) > 4096)
+    const bool energy_like = (call == CALL_ENERGY || call == CALL_FB_ENERGY);
+    const int level = (call == CALL_OVERLAP) ? 1 : (energy_like ? 3 : 2);
+    if (energy_like && std::max(c->sp[0].P, c->sp[1].P) > 4096)
         return fail(errp, MSD_EUNSUPPORTED, "local energy requires n_o*n_v <= 4096 per spin");
     int rc = ensure_workspace(c, level, n_w, errp);
     if (rc != MSD_OK) return rc;
@@ -702,9 +703,19 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
             }
             CK(fv_.join());
             mark(c, 4, st);
-            CK(launch_dets(c, 2, nw, ws, st));
-            mark(c, 5, st);
-            CK(launch_finish_energy(c, nw, ws, out + w0 * 3, fl, st));
+            if (call == CALL_FB_ENERGY) {
+                // fused call: the energy-mode dets kernels also scatter C; the force bias then comes from C and the
+                // B^gamma slices that the energy path holds anyway (W6), rows of [n_chol + 3]: fb, then (E, E1, E2)
+                const int64_t stride = (int64_t)ng + 3;
+                CK(launch_dets(c, 3, nw, ws, st));
+                mark(c, 5, st);
+                CK(launch_fb_from_cb(c, nw, ws, out + w0 * stride, stride, st));
+                CK(launch_finish_energy(c, nw, ws, out + w0 * stride + ng, stride, fl, st));
+            } else {
+                CK(launch_dets(c, 2, nw, ws, st));
+                mark(c, 5, st);
+                CK(launch_finish_energy(c, nw, ws, out + w0 * 3, 3, fl, st));
+            }
         }
         if (c->profiling) {
             cudaEventRecord(c->ev[6], st);
@@ -747,6 +758,10 @@ extern "C" int msd_force_bias(msd_ctx* c, int64_t n_w, const void* phi_a, const 
 extern "C" int msd_local_energy(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* e, int32_t* flags,
                                 void* stream)
 { return hot_call(c, CALL_ENERGY, n_w, phi_a, phi_b, e, flags, stream); }
+
+extern "C" int msd_force_bias_energy(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* out, int32_t* flags,
+                                     void* stream)
+{ return hot_call(c, CALL_FB_ENERGY, n_w, phi_a, phi_b, out, flags, stream); }
 
 extern "C" int msd_greens(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* G, int32_t* flags,
                           void* stream)
@@ -813,6 +828,10 @@ extern "C" int msd_overlap_host(msd_ctx* c, int64_t n_w, const void* phi_a, cons
 extern "C" int msd_force_bias_host(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* fb, int32_t* flags,
                                    void* stream)
 { return hot_call_host(c, CALL_FB, c ? (size_t)c->n_chol : 0, n_w, phi_a, phi_b, fb, flags, stream); }
+
+extern "C" int msd_force_bias_energy_host(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* out,
+                                          int32_t* flags, void* stream)
+{ return hot_call_host(c, CALL_FB_ENERGY, c ? (size_t)c->n_chol + 3 : 0, n_w, phi_a, phi_b, out, flags, stream); }
 
 extern "C" int msd_local_energy_host(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* e, int32_t* flags,
                                      void* stream)

@@ -439,3 +439,31 @@ def test_many_high_level_items_per_cta(torch_cuda):
     assert_parity(got, o2.run(x, walkers=ws, want=("ovlp", "greens"), return_G=False), walkers=ws, what=("ovlp", "fb"))
     q = wick.run(x, walkers=[3], want=("energy",))
     assert np.abs(got["E"][3] - q["E"][0]).max() <= TOL_E
+
+
+@pytest.mark.parametrize("name,kw", [("small", {}), ("open-shell", {}), ("tiny", {}),
+                                     ("sweep", dict(n_det=3000, max_level=7, n_w=21))])
+def test_fused_force_bias_energy_call(torch_cuda, name, kw):
+    """msd_force_bias_energy: both outputs from one pass (force bias from C and the B slices) against
+    the oracle, and against the two separate calls; device and host-buffer variants; ragged batch, flags."""
+    torch = torch_cuda
+    msd = _msd()
+    x = mi.generate(name, **kw)
+    trial = msd.setup_from_inputs(x)
+    pa = torch.tensor(x.phi_a, device="cuda")
+    pb = torch.tensor(x.phi_b, device="cuda")
+    fl = torch.full((x.n_w,), -1, dtype=torch.int32, device="cuda")
+    out = trial.force_bias_energy(pa, pb, flags=fl).cpu().numpy()
+    assert out.shape == (x.n_w, x.n_chol + 3) and (fl.cpu().numpy() == 0).all()
+    fb, E = out[:, :x.n_chol], out[:, x.n_chol:]
+    ws = list(range(min(x.n_w, 6)))
+    ref = o2.run(x, walkers=ws, return_G=False)
+    assert_parity(dict(fb=fb, E=E), ref, walkers=ws, what=("fb", "E"))
+    fb2 = trial.force_bias(pa, pb).cpu().numpy()
+    E2 = trial.local_energy(pa, pb).cpu().numpy()
+    assert (np.abs(fb - fb2).max(axis=1) / np.abs(fb2).max(axis=1)).max() <= TOL_REL
+    assert np.abs(E - E2).max() <= TOL_E
+    outh = trial.force_bias_energy_host(np.ascontiguousarray(x.phi_a), np.ascontiguousarray(x.phi_b))
+    assert (np.abs(outh[:, :x.n_chol] - fb).max(axis=1) / np.abs(fb).max(axis=1)).max() <= TOL_REL
+    assert np.abs(outh[:, x.n_chol:] - E).max() <= TOL_E
+    trial.close()
