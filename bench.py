@@ -193,6 +193,8 @@ def main():
 
     import torch
     import msd_inputs as mi
+    from paper_2406_08314_b200 import build as _build
+    _build.build()                  # no-op when libmsd_b200.so is up to date (nvcc, sm_100a, in-tree)
     import paper_2406_08314_b200 as msd
 
     if not torch.cuda.is_available():
