@@ -8,7 +8,7 @@
 __global__ void __launch_bounds__(128)
 k_reference(int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw, const cplx* __restrict__ phi_a,
             const cplx* __restrict__ phi_b, cplx* theta_a, cplx* theta_b, double* thetaT_a, double* thetaT_b,
-            cplx* det0, cplx* g_a, cplx* g_b, int* wflags)
+            cplx* det0, cplx* g_a, cplx* g_b, int* wflags, int stage_psi)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int s = blockIdx.y;
@@ -30,6 +30,10 @@ k_reference(int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw, const cplx* __re
     int* piv = reinterpret_cast<int*>(inv + n * n);         // [n]
     int* vmap = piv + n;                                    // [N]  orbital -> active-virtual index or -1
     int* omap = vmap + N;                                   // [n]  position in occ_ref -> active-occupied index or -1
+    // the walker block itself, rows padded to n + 1 complex (conflict-free column walks in the Theta product);
+    // read once, coalesced -- the strided global reads psi[q*n + m] were the whole cost of this kernel
+    const int lps = n + 1;
+    cplx* psis = reinterpret_cast<cplx*>(smem_raw + ((((size_t)2 * n * n * sizeof(cplx) + (size_t)(2 * n + N) * sizeof(int)) + 15) / 16) * 16);
     __shared__ int s_p;
     __shared__ int s_sing;
     __shared__ double s_sign;
@@ -40,9 +44,16 @@ k_reference(int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw, const cplx* __re
     __syncthreads();
     for (int r = tid; r < sp.n_v; r += nt) vmap[sp.act_v[r]] = r;
     for (int h = tid; h < sp.n_o; h += nt) omap[sp.pos_o[h]] = h;
+    if (stage_psi) {
+        for (int e = tid; e < N * n; e += nt) {
+            int q = e / n, i = e - q * n;
+            psis[q * lps + i] = psi[e];
+        }
+        __syncthreads();
+    }
     for (int e = tid; e < n * n; e += nt) {
         int l = e / n, i = e - l * n;
-        lu[e] = psi[(int64_t)sp.occ_ref[l] * n + i];
+        lu[e] = stage_psi ? psis[sp.occ_ref[l] * lps + i] : psi[(int64_t)sp.occ_ref[l] * n + i];
     }
     __syncthreads();
 
@@ -106,6 +117,7 @@ k_reference(int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw, const cplx* __re
         int l = e / N, q = e - l * N;            // consecutive threads -> consecutive q
         cplx acc = cmake(0.0, 0.0);
         if (sing) acc = cmake(nanv, nanv);
+        else if (stage_psi) for (int m = 0; m < n; m++) acc = cfma(psis[q * lps + m], inv[m * n + l], acc);
         else for (int m = 0; m < n; m++) acc = cfma(psi[(int64_t)q * n + m], inv[m * n + l], acc);
         theta[(int64_t)q * n + l] = acc;
         if (thetaT) {
@@ -122,7 +134,10 @@ cudaError_t launch_reference(int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw,
                              const cplx* phi_b, Workspace& ws, bool want_thetaT, cudaStream_t st)
 {
     int nmax = sa.n > sb.n ? sa.n : sb.n;
-    size_t smem = (size_t)2 * nmax * nmax * sizeof(cplx) + (size_t)(2 * nmax + N) * sizeof(int) + 16;
+    size_t smem = (size_t)2 * nmax * nmax * sizeof(cplx) + (size_t)(2 * nmax + N) * sizeof(int) + 32;
+    const size_t psi_bytes = (size_t)N * (nmax + 1) * sizeof(cplx);
+    const int stage_psi = smem + psi_bytes <= 100 * 1024;       // two CTAs per SM at least; larger walkers are read from global
+    if (stage_psi) smem += psi_bytes;
     static size_t configured = 0;
     if (smem > 48 * 1024 && smem > configured) {
         cudaError_t e = cudaFuncSetAttribute(k_reference, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -133,6 +148,6 @@ cudaError_t launch_reference(int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw,
     dim3 grid((unsigned)wpad, 2);
     k_reference<<<grid, 128, smem, st>>>(N, ldN, sa, sb, nw, phi_a, phi_b, ws.theta[0], ws.theta[1],
                                          want_thetaT ? ws.thetaT[0] : nullptr, want_thetaT ? ws.thetaT[1] : nullptr,
-                                         ws.det0, ws.g[0], ws.g[1], ws.wflags);
+                                         ws.det0, ws.g[0], ws.g[1], ws.wflags, stage_psi);
     return cudaGetLastError();
 }
