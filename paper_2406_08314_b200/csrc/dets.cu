@@ -406,7 +406,7 @@ __device__ __forceinline__ void c1_round(const DetsParams& p, const WorkItem& it
             c1_round<KA_, KB_>(p, it, i, slot, S, j, gA, gB, val, Wl);                                  \
         break;
 
-template <int KLO, int KHI, int NTHR>
+template <int KLO, int KHI, int NTHR, bool GS>
 __global__ void __launch_bounds__(NTHR, 1) k_dets_c1(DetsParams p, const WorkItem* __restrict__ items, int n_items,
                                                      const uint32_t* __restrict__ sched)
 {
@@ -419,8 +419,16 @@ __global__ void __launch_bounds__(NTHR, 1) k_dets_c1(DetsParams p, const WorkIte
     const int tile = blockIdx.y;
     const int j = threadIdx.x & (MSD_WT - 1);
     const int slot = threadIdx.x / MSD_WT;
-    const cplx* gA = p.g[0] + (int64_t)tile * p.P[0] * MSD_WT + j;
-    const cplx* gB = p.g[1] + (int64_t)tile * p.P[1] * MSD_WT + j;
+    // GS: the tile's g slices sit behind val in shared memory (when they fit); otherwise they are read through L1
+    cplx* gsm = val + (size_t)c1_emax(KHI - 2) * S * MSD_WT;
+    const cplx* gA = GS ? gsm + j : p.g[0] + (int64_t)tile * p.P[0] * MSD_WT + j;
+    const cplx* gB = GS ? gsm + p.P[0] * MSD_WT + j : p.g[1] + (int64_t)tile * p.P[1] * MSD_WT + j;
+    if (GS) {
+        const cplx* ga = p.g[0] + (int64_t)tile * p.P[0] * MSD_WT;
+        const cplx* gb = p.g[1] + (int64_t)tile * p.P[1] * MSD_WT;
+        for (int e = threadIdx.x; e < p.P[0] * MSD_WT; e += NTHR) gsm[e] = __ldg(ga + e);
+        for (int e = threadIdx.x; e < p.P[1] * MSD_WT; e += NTHR) gsm[p.P[0] * MSD_WT + e] = __ldg(gb + e);
+    }
     for (int e = threadIdx.x; e < PT * MSD_WT; e += NTHR) Csm[e] = cmake(0.0, 0.0);
     __syncthreads();
     cplx Wl = cmake(0.0, 0.0);
@@ -1226,9 +1234,13 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
             const size_t sm1 = csm + (size_t)C1_EMAX[cl] * C1_SLOTS[cl] * MSD_WT * sizeof(cplx);
             if (sm1 <= 227 * 1024 && c->d_sched && p.P[0] + p.P[1] < 8192) {
                 fhs = true;     // handled here
-                if (cl == 0) e = launch_c1(k_dets_c1<-1, 2, 768>, 768, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
-                else if (cl == 1) e = launch_c1(k_dets_c1<2, 3, 512>, 512, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
-                else e = launch_c1(k_dets_c1<3, 4, 256>, 256, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
+                const bool gs = sm1 + csm <= 227 * 1024;        // room for the g slices as well
+                if (cl == 0 && gs) e = launch_c1(k_dets_c1<-1, 2, 768, true>, 768, sm1 + csm, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
+                else if (cl == 0) e = launch_c1(k_dets_c1<-1, 2, 768, false>, 768, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
+                else if (cl == 1 && gs) e = launch_c1(k_dets_c1<2, 3, 512, true>, 512, sm1 + csm, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
+                else if (cl == 1) e = launch_c1(k_dets_c1<2, 3, 512, false>, 512, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
+                else if (gs) e = launch_c1(k_dets_c1<3, 4, 256, true>, 256, sm1 + csm, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
+                else e = launch_c1(k_dets_c1<3, 4, 256, false>, 256, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
             }
         }
         if constexpr (MODE >= 2) {

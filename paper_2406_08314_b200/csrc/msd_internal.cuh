@@ -109,6 +109,7 @@ struct WorkItem {          // a chunk of one bucket, processed by one CTA per wa
 //   entry = x_unified << 12 | slot << 5 | e      (x_unified = x for alpha, P_alpha + x for beta; e = a*k+b, beta after alpha)
 static const int C1_SLOTS[3] = {96, 64, 32};     // register classes: larger level <= 2, == 3, == 4
 static const int C1_EMAX[3] = {8, 18, 32};
+__host__ __device__ constexpr int c1_emax(int cls) { return cls == 0 ? 8 : (cls == 1 ? 18 : 32); }
 __host__ __device__ inline int c1_hdr_words(int S) { return (S + 2) / 2; }
 
 struct Workspace {
