@@ -310,6 +310,16 @@ k_energy_dense_mma(int n_chol, int64_t nw, int gchunk, SpinDev sa, SpinDev sb, c
         for (int b = 0; b < 2; b++) { fk[a][b][0] = 0.0; fk[a][b][1] = 0.0; }
     cplx ex_part = cmake(0.0, 0.0);
 
+    // step-4 A'' fragments: row m = 8 mt + gq of the stacked (Re; Im) operand reads component (kc ^ im) of Bfull[r][2kk+kl],
+    // negated for Re rows with kc = 1
+    int a4off[4];
+    long long a4sgn[4];
+#pragma unroll
+    for (int mt = 0; mt < 4; mt++) {
+        const int m = 8 * mt + gq, im = m >= L.half, r = m - im * L.half;
+        a4off[mt] = r * L.ldb + 2 * kl + (kc ^ im);
+        a4sgn[mt] = (!im && kc) ? (long long)0x8000000000000000ull : 0ll;
+    }
     // output phase: element offset of pair index x = tid / NWARP + 32 t inside a warp's Bfull tile (P <= 256: 8 values)
     int ooff[8];
 #pragma unroll
@@ -403,9 +413,10 @@ k_energy_dense_mma(int n_chol, int64_t nw, int gchunk, SpinDev sa, SpinDev sb, c
                 double a[4], b[2];
 #pragma unroll
                 for (int mt = 0; mt < 4; mt++) {
-                    const int m = 8 * mt + gq, im = m >= L.half, r = m - im * L.half;
-                    double v = mt < MT ? Lb[r * L.ldb + 2 * (2 * kk + kl) + (kc ^ im)] : 0.0;
-                    a[mt] = (!im && kc) ? -v : v;
+                    // offsets and sign masks are per-lane constants (a4off / a4sgn); the sign flip is an integer XOR so
+                    // that no DADD competes with the DMMAs for the FP64 pipe
+                    const double v = mt < MT ? Lb[a4off[mt] + 4 * kk] : 0.0;
+                    a[mt] = __longlong_as_double(__double_as_longlong(v) ^ a4sgn[mt]);
                 }
 #pragma unroll
                 for (int j = 0; j < 2; j++) b[j] = Tb[(2 * kk + kl) * L.ldt + 2 * posh[j] + kc];
