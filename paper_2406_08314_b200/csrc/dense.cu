@@ -569,14 +569,19 @@ cudaError_t launch_energy_dense(msd_ctx* c, int64_t nw, Workspace& ws, cudaStrea
         e = cudaGetLastError();
     }
     c->launches++;
-    if (e != cudaSuccess) return e;
+    return e;
+}
+
+// Coulomb-like part of F (k_fx).  Independent of the V GEMMs that follow the dense kernel (both only read Bp), so the
+// caller puts it on a side stream next to them: it is HBM-bound, they are tensor-bound.
+cudaError_t launch_fx(msd_ctx* c, int64_t nw, Workspace& ws, cudaStream_t st)
+{
     cplx* X0 = ws.X0;
     int Pmax = c->sp[0].P > c->sp[1].P ? c->sp[0].P : c->sp[1].P;
-    if (Pmax > 0) {
-        dim3 g2((Pmax + 7) / 8, (unsigned)nw, 2);
-        k_fx<<<g2, 256, 0, st>>>(c->n_chol, nw, c->sp[0].P, c->sp[1].P, X0, ws.Bp[0], ws.Bp[1], ws.F[0], ws.F[1]);
-        c->launches++;
-    }
+    if (nw == 0 || Pmax == 0) return cudaSuccess;
+    dim3 g2((Pmax + 7) / 8, (unsigned)nw, 2);
+    k_fx<<<g2, 256, 0, st>>>(c->n_chol, nw, c->sp[0].P, c->sp[1].P, X0, ws.Bp[0], ws.Bp[1], ws.F[0], ws.F[1]);
+    c->launches++;
     return cudaGetLastError();
 }
 

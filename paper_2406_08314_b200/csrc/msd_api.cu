@@ -701,6 +701,10 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
                 if (ge != cudaSuccess) { fv_.join(); CK(ge); }
                 c->launches++;
             }
+            {   // F += sum_g Xt_g B^g next to the GEMMs (side stream 3)
+                cudaError_t fe = launch_fx(c, nw, ws, fv_.stream(3));
+                if (fe != cudaSuccess) { fv_.join(); CK(fe); }
+            }
             CK(fv_.join());
             mark(c, 4, st);
             if (call == CALL_FB_ENERGY) {

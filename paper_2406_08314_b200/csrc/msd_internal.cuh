@@ -221,6 +221,7 @@ cudaError_t launch_dets(msd_ctx* c, int mode, int64_t nw, Workspace& ws, cudaStr
 // dense.cu
 cudaError_t launch_green_rows(msd_ctx* c, int64_t nw, Workspace& ws, cplx* Gfull /*or null*/, cudaStream_t st);
 cudaError_t launch_energy_dense(msd_ctx* c, int64_t nw, Workspace& ws, cudaStream_t st);
+cudaError_t launch_fx(msd_ctx* c, int64_t nw, Workspace& ws, cudaStream_t st);
 cudaError_t launch_finish_overlap(msd_ctx* c, int64_t nw, Workspace& ws, cplx* ovlp, int* flags, cudaStream_t st);
 cudaError_t launch_finish_energy(msd_ctx* c, int64_t nw, Workspace& ws, cplx* e, int64_t estride, int* flags, cudaStream_t st);
 cudaError_t launch_fb_from_cb(msd_ctx* c, int64_t nw, Workspace& ws, cplx* out, int64_t ostride, cudaStream_t st);
