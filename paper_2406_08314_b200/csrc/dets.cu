@@ -21,6 +21,7 @@
 #define M_ENERGY(M) ((M) >= 2)
 #define M_SCATTER(M) ((M) == 1 || (M) == 3)
 #include <algorithm>
+#include <cstdlib>
 
 struct DetsParams {
     const unsigned char* tab;
@@ -1186,6 +1187,9 @@ template <int MODE>
 static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cudaStream_t st)
 {
     const size_t gbytes = (size_t)(p.P[0] + p.P[1]) * MSD_WT * sizeof(cplx);
+    // test hook: MSD_NO_SMEM_TILES=1 takes the paths used when a walker tile's C / Hrot / F do not fit in shared memory
+    // (RED scatter for the force bias, Hrot / F through L1 for the energy), which no BASELINE config needs
+    const bool no_tiles = getenv("MSD_NO_SMEM_TILES") != nullptr;
     // The launches below are independent (they only meet in the RED accumulators), so they are forked over the
     // context's side streams: the small high-level groups no longer serialise their tails behind one another.
     Fork f(c, st);
@@ -1232,7 +1236,7 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
         if constexpr (MODE == 1) {
             const size_t csm = (size_t)(p.P[0] + p.P[1]) * MSD_WT * sizeof(cplx);
             const size_t sm1 = csm + (size_t)C1_EMAX[cl] * C1_SLOTS[cl] * MSD_WT * sizeof(cplx);
-            if (sm1 <= 227 * 1024 && c->d_sched && p.P[0] + p.P[1] < 8192) {
+            if (sm1 <= 227 * 1024 && c->d_sched && p.P[0] + p.P[1] < 8192 && !no_tiles) {
                 fhs = true;     // handled here
                 const bool gs = sm1 + csm <= 227 * 1024;        // room for the g slices as well
                 if (cl == 0 && gs) e = launch_c1(k_dets_c1<-1, 2, 768, true>, 768, sm1 + csm, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
@@ -1244,7 +1248,7 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
             }
         }
         if constexpr (MODE >= 2) {
-            fhs = 3 * gbytes <= 200 * 1024;
+            fhs = 3 * gbytes <= 200 * 1024 && !no_tiles;
             if (!fhs) {}
             else if (cl == 0) e = launch_persistent(k_dets_cf<MODE, -1, 2, 768, 1, true>, 768, 3 * gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
             else if (cl == 1) e = launch_persistent(k_dets_cf<MODE, 2, 3, 512, 1, true>, 512, 3 * gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);

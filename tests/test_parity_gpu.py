@@ -467,3 +467,17 @@ def test_fused_force_bias_energy_call(torch_cuda, name, kw):
     assert (np.abs(outh[:, :x.n_chol] - fb).max(axis=1) / np.abs(fb).max(axis=1)).max() <= TOL_REL
     assert np.abs(outh[:, x.n_chol:] - E).max() <= TOL_E
     trial.close()
+
+
+def test_paths_for_windows_too_wide_for_shared_memory_tiles(torch_cuda, monkeypatch):
+    """The force-bias RED scatter and the energy path with Hrot / F read through L1 are what runs when a walker tile's
+    C / Hrot / F do not fit in shared memory; no BASELINE config is that wide, so the library's test hook
+    MSD_NO_SMEM_TILES forces them (read at every call)."""
+    monkeypatch.setenv("MSD_NO_SMEM_TILES", "1")
+    x = mi.generate("small")
+    got = gpu_all(torch_cuda, x)
+    assert_parity(got, o2.run(x))
+    x = mi.generate("sweep", n_det=3000, max_level=6, n_w=16)
+    got = gpu_all(torch_cuda, x, want_G=False)
+    ws = [0, 9, 15]
+    assert_parity(got, o2.run(x, walkers=ws, return_G=False), walkers=ws)
