@@ -53,18 +53,64 @@ def reduce_max_time(ms: float, world: int, device=None) -> float:
     return float(t.item())
 
 
-def ncu_traffic(kernel: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, averaged over its launches of one step,
-    from the committed ncu --set full summary (profiles/r01e_traffic.csv); None if the file is absent."""
+NCU_RAW = os.path.join(ROOT, "profiles", "r02_ncu_raw.csv")
+
+
+def ncu_traffic(kernel_prefix: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the kernels whose name starts with `kernel_prefix`,
+    averaged over their launches, parsed from the RAW page of one `ncu --set full` capture of this same command
+    (profiles/r02_ncu_raw.csv = `ncu -i ... --page raw --csv`, command in profiles/r02_ncu_full.md).  Returns
+    (bytes per launch, launches) or (None, 0) when the capture is absent."""
     import csv
-    path = os.path.join(ROOT, "profiles", "r01e_traffic.csv")
     try:
-        rows = [r for r in csv.DictReader(open(path)) if r["kernel"] == kernel]
+        rows = list(csv.reader(open(NCU_RAW)))
     except OSError:
-        return None
-    if not rows:
-        return None
-    return sum(float(r["dram_read_bytes"]) + float(r["dram_write_bytes"]) for r in rows) / len(rows)
+        return None, 0
+    hdr = next((r for r in rows if "Kernel Name" in r), None)
+    if hdr is None:
+        return None, 0
+    units = rows[rows.index(hdr) + 1]
+    k, rd, wr = hdr.index("Kernel Name"), hdr.index("dram__bytes_read.sum"), hdr.index("dram__bytes_write.sum")
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    tot, n = 0.0, 0
+    for r in rows[rows.index(hdr) + 2:]:
+        if len(r) > max(k, rd, wr) and r[k].startswith(kernel_prefix):
+            tot += float(r[rd].replace(",", "")) * scale.get(units[rd], 1.0) + \
+                   float(r[wr].replace(",", "")) * scale.get(units[wr], 1.0)
+            n += 1
+    return (tot / n, n) if n else (None, 0)
+
+
+_probes = None
+
+
+def probes():
+    """libmsd_probes.so (paper_2406_08314_b200/csrc/probes.cu): bench-side peak probes, not part of the product ABI."""
+    global _probes
+    if _probes is None:
+        import ctypes as C
+        lib = C.CDLL(os.path.join(ROOT, "paper_2406_08314_b200", "libmsd_probes.so"))
+        lib.msd_probe_fp64_tflops.restype = C.c_double
+        lib.msd_probe_fp64_tflops.argtypes = [C.c_int, C.c_double, C.c_void_p]
+        lib.msd_probe_l2_gather_gbs.restype = C.c_double
+        lib.msd_probe_l2_gather_gbs.argtypes = [C.c_int, C.c_double, C.c_void_p]
+        _probes = lib
+    return _probes
+
+
+def fb_dets_flops(ka: np.ndarray, kb: np.ndarray) -> float:
+    """Real FP64 flops of one (walker, determinant) unit of the force-bias determinant pass (W2-W4: minors, adjugates, the
+    products c~ R^sbar A[b][a] and their accumulation), from the closed forms of csrc/dets.cu: complex mul = 6, complex
+    fma = 8.  k = 1: 0; 2: 14; 3: 9 minors + expansion = 148; 4: 12 two-by-two minors + R + 16 cofactors = 566;
+    k >= 5: Gauss-Jordan with the pivot row in registers, 8 k^3 + 14 k^2.  Per unit also W (12) and (ka^2 + kb^2) x 8."""
+    def spin(k):
+        out = np.zeros_like(k, dtype=np.float64)
+        for lev, f in ((2, 14.0), (3, 148.0), (4, 566.0)):
+            out[k == lev] = f
+        big = k >= 5
+        out[big] = 8.0 * k[big] ** 3 + 14.0 * k[big] ** 2
+        return out
+    return float(np.sum(spin(ka) + spin(kb) + 12.0 + 8.0 * (ka * ka + kb * kb)))
 
 
 def total_units(n_w: int, n_det: int, steps: int, world: int) -> float:
@@ -280,6 +326,32 @@ def main():
                                                          / fb.abs().amax(dim=1)).max().item()),
              "max_abs_diff_E_vs_separate_calls": float((fused_out[:, inp.n_chol:] - en).abs().max().item())}
 
+    # ---- per-call throughputs and the paper's block mix (a block = 25 propagation
+    # steps, each needing one force bias and one overlap, + 1 energy estimate) ----
+    ov = torch.empty(inp.n_w, dtype=torch.complex128, device=dev)
+    calls = {"msd_overlap": lambda: trial.overlap(d_a, d_b, out=ov),
+             "msd_force_bias": lambda: trial.force_bias(d_a, d_b, out=fb),
+             "msd_local_energy": lambda: trial.local_energy(d_a, d_b, out=en)}
+    per_call = {}
+    for cname, fn in calls.items():
+        fn()
+        barrier()
+        cev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for a, b in cev:
+            flush.zero_()
+            a.record(stream)
+            fn()
+            b.record(stream)
+        barrier()
+        cms = reduce_max_time(sum(a.elapsed_time(b) for a, b in cev), world, dev) / args.steps
+        per_call[cname] = {"ms": cms, "value": total_units(inp.n_w, inp.n_det, 1, world) / (cms * 1e-3), "unit": UNIT}
+    t_ov, t_fb, t_e = (per_call[k]["ms"] for k in ("msd_overlap", "msd_force_bias", "msd_local_energy"))
+    block_mix = {"definition": "N_w N_d 25 / (25 (t_fb + t_ovlp) + t_E): walker x determinant propagation-step evaluations "
+                               "per second in the paper's block of 25 steps + 1 energy estimate (PAPER.md:L303-309)",
+                 "value": total_units(inp.n_w, inp.n_det, 25, world) / ((25.0 * (t_fb + t_ov) + t_e) * 1e-3),
+                 "unit": "walker*det*step/s", "block_ms": 25.0 * (t_fb + t_ov) + t_e,
+                 "energy_share_of_block": t_e / (25.0 * (t_fb + t_ov) + t_e)}
+
     # ---- end to end: the C-ABI *_host calls (pinned HOST buffers; H2D + kernels + D2H inside each call) ----
     def e2e_step():
         trial.force_bias_host(h_a, h_b, out=h_fb)
@@ -303,7 +375,8 @@ def main():
     roofline = None
     phases = None
     if rank == 0:
-        peak = msd.msd_probe_fp64_tflops(True, 30.0)
+        peak = float(probes().msd_probe_fp64_tflops(1, 30.0, None))
+        l2_gather = float(probes().msd_probe_l2_gather_gbs(32, 20.0, None))
         trial.set_profiling(True)
         acc = {}
         reps = 3
@@ -336,11 +409,13 @@ def main():
         roofline = {"kernel": "k_gemm_tn (FP64 DMMA: V and Lambda contractions, %d launches per step)" % 5,
                     "bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                     "frac": achieved / peak if peak > 0 else None,
-                    "peak_source": "measured live: register-resident DMMA m8n8k4 loop (msd_probe_fp64_tflops); "
-                                   "MEASURED_PEAKS.json has no FP64 entry; derived 148 SM x 64 FMA/clk x 1.965 GHz = %.1f"
-                                   % FP64_PEAK_DERIVED,
-                    "traffic": ncu_traffic("k_gemm_tn"),
-                    "traffic_note": "DRAM bytes per launch (mean of the 5 launches), ncu --set full, profiles/r01e_traffic.csv",
+                    "peak_source": "measured live by the bench-side probe (csrc/probes.cu, libmsd_probes.so): register-"
+                                   "resident DMMA m8n8k4 loop; MEASURED_PEAKS.json has no FP64 entry; derived 148 SM x "
+                                   "64 FMA/clk x 1.965 GHz = %.1f" % FP64_PEAK_DERIVED,
+                    "traffic": ncu_traffic("k_gemm_tn")[0],
+                    "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum per launch, mean over the %d k_gemm_tn "
+                                    "launches in profiles/r02_ncu_raw.csv (raw page of one ncu --set full capture of this "
+                                    "command; null when absent)" % ncu_traffic("k_gemm_tn")[1],
                     "share_of_step": gemm_ms / (sum(step_ms) / len(step_ms)),
                     "algorithmic_flops_per_step": flops_v + flops_lam}
 
@@ -350,16 +425,23 @@ def main():
         kb = np.diff(inp.exc_off_b).astype(np.float64)
         gathers = float(np.sum(ka * ka * kb * kb + (ka * (ka - 1) / 2) ** 2 + (kb * (kb - 1) / 2) ** 2))
         l2_bytes = 16.0 * gathers * nw
-        l2_peak = 6300.0 * (clocks.get("sm_mhz") or 1965.0) * 1e6 / 1e9      # B300_MICROARCH.md: ~6300 B/clk LTS cap
         roofline_dets = {"kernel": "k_dets_cf<2> + k_dets_gen<2> (energy mode, forked over side streams)",
-                         "bound": "l2", "achieved": l2_bytes / (acc["p4"] * 1e-3) / 1e9, "peak": l2_peak, "unit": "GB/s",
-                         "frac": l2_bytes / (acc["p4"] * 1e-3) / 1e9 / l2_peak,
-                         "peak_source": "guide fallback: LTS throughput cap ~6300 B/clk x SM clock (no measured L2 peak "
-                                        "in MEASURED_PEAKS.json)",
-                         "algorithmic_l2_bytes_per_step": l2_bytes, "share_of_step": acc["p4"] / (sum(step_ms) / len(step_ms)),
-                         "fp64_flops_floor_ms": None}
+                         "bound": "l2", "achieved": l2_bytes / (acc["p4"] * 1e-3) / 1e9, "peak": l2_gather, "unit": "GB/s",
+                         "frac": l2_bytes / (acc["p4"] * 1e-3) / 1e9 / l2_gather if l2_gather > 0 else None,
+                         "peak_source": "measured live by the bench-side probe (csrc/probes.cu): random 128-byte lines of a "
+                                        "32 MB L2-resident buffer, 16 B per lane, 8 independent loads in flight per lane",
+                         "algorithmic_l2_bytes_per_step": l2_bytes, "share_of_step": acc["p4"] / (sum(step_ms) / len(step_ms))}
+        # force-bias determinant pass (k_dets_c1 + k_dets_gen<1>): plain FP64 ALU work against the FP64 peak
+        fl = fb_dets_flops(ka, kb) * nw
+        roofline_fb_dets = {"kernel": "k_dets_c1 + k_dets_gen<1> (force-bias mode: minors, adjugates, CI reduction)",
+                            "bound": "alu", "achieved": fl / (fbacc["p1"] * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
+                            "frac": fl / (fbacc["p1"] * 1e-3) / 1e12 / peak if peak > 0 else None,
+                            "peak_source": "FP64 pipe (DFMA and DMMA share it): the live DMMA probe",
+                            "algorithmic_flops_per_step": fl, "ms": fbacc["p1"],
+                            "share_of_step": fbacc["p1"] / (sum(step_ms) / len(step_ms))}
     else:
         roofline_dets = None
+        roofline_fb_dets = None
 
     if rank != 0:
         if world > 1:
@@ -391,7 +473,9 @@ def main():
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": n_e2e},
             "gpu_launches": int(launches),
-            "fused": fused, "roofline": roofline, "roofline_dets": roofline_dets, "cpu_baseline": cpu_baseline, "cpu_wick_baseline": cpu_wick, "phases": phases,
+            "fused": fused, "per_call": per_call, "block_mix": block_mix,
+            "roofline": roofline, "roofline_dets": roofline_dets, "roofline_fb_dets": roofline_fb_dets,
+            "cpu_baseline": cpu_baseline, "cpu_wick_baseline": cpu_wick, "phases": phases,
             "step_ms": {"min": min(step_ms), "median": statistics.median(step_ms), "max": max(step_ms)}}
     print(json.dumps(line), flush=True)
     if world > 1:

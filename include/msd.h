@@ -28,6 +28,9 @@
  * has completed.  `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
  * The three hot calls enqueue kernels on `stream` and return without synchronising the host (the first
  * call for a larger n_w than seen before allocates workspace with cudaMalloc, which synchronises).
+ * A context owns ONE workspace and one set of side streams: all calls on a context must be issued from one
+ * host thread and are serialised against each other on the device (a call on another stream than the previous
+ * call's first waits for that call's last kernel); use one context per concurrent stream.
  *
  * Errors: every function returning int returns MSD_OK (0) or a negative code; no exceptions cross the
  * ABI.  msd_last_error() gives a human-readable message for the last failure on that context (or the
@@ -58,9 +61,13 @@ typedef struct msd_ctx msd_ctx;   /* opaque; owns every device copy made at setu
 /* msd_setup: build the trial (PAPER.md:L222-254 inputs h1e, chol, e0, (coeff, occa, occb) in
  * hole/particle form; S0 "pack" of SURVEY.md 8(a)).  Runs the excitation-table packer kernels
  * (validate, phases, level sort into contiguous buckets) and packs the rows of L and h1 that the path touches.
- *   N, n_alpha, n_beta, n_chol, n_det : sizes.  Limits: 1 <= N <= 1024, 0 <= n_s <= 64, n_s <= N,
- *       n_chol >= 1, n_det >= 1, per-spin excitation level <= 16, active window (distinct hole
- *       orbitals n_o, distinct particle orbitals n_v per spin) n_o*n_v <= 65535; else MSD_EUNSUPPORTED.
+ *   N, n_alpha, n_beta, n_chol, n_det : sizes.  Limits, ALL checked here (else MSD_EUNSUPPORTED): 1 <= N <= 1024,
+ *       0 <= n_s <= 64, n_s <= N, n_chol >= 1, 1 <= n_det < 2^31, per-spin excitation level <= 16 and
+ *       k_alpha^2 + k_beta^2 <= 400 for every determinant, active window per spin (n_o distinct hole orbitals,
+ *       n_v distinct particle orbitals) n_o, n_v <= 255 and n_o*n_v <= 8192.
+ *       The energy calls (msd_local_energy, msd_force_bias_energy) additionally need n_o*n_v <= 4096 per spin
+ *       (they hold (n_o n_v)^2 two-body tensors per walker): a wider trial still sets up -- overlap, force bias
+ *       and Green's function work -- msd_get_info()[8] is 0 and the energy calls return MSD_EUNSUPPORTED.
  *   h1   HOST [N][N] row-major, real symmetric.
  *   L    HOST [n_chol][N][N], each slice real symmetric.
  *   e0   constant added to every energy.
@@ -70,7 +77,9 @@ typedef struct msd_ctx msd_ctx;   /* opaque; owns every device copy made at setu
  *       determinant; any order (the a-th smallest hole is paired with the a-th smallest particle).
  *   ci   HOST [n_det] real coefficients in the ascending-string convention.
  *   stream: setup work is enqueued there and synchronised before returning.
- * On success *out is a new context (destroy with msd_destroy).  Invalid tables -> MSD_EINVAL. */
+ * On success *out is a new context (destroy with msd_destroy).  Invalid tables -> MSD_EINVAL: an index out of
+ * range, a hole outside / a particle inside the reference, an orbital repeated inside a determinant, a level
+ * above n_s, or the same determinant listed twice (the CI expansion is orthogonal, Eq. 15). */
 int msd_setup(msd_ctx** out, int N, int n_alpha, int n_beta, int n_chol, int64_t n_det,
               const double* h1, const double* L, double e0,
               const int32_t* occ_ref_a, const int32_t* occ_ref_b,
@@ -128,11 +137,11 @@ int msd_force_bias_energy_host(msd_ctx* ctx, int64_t n_w, const void* phi_a, con
                                void* out, int32_t* flags, void* stream);
 
 /* Introspection of the packed trial (host-side copies made at setup; for tests of the packer).
- * msd_get_info fills: info[0]=n_o_alpha, [1]=n_v_alpha, [2]=n_o_beta, [3]=n_v_beta, [4]=number of level
- * buckets, [5]=max level alpha, [6]=max level beta, [7]=walker tile width.
+ * msd_get_info fills info[0..8]: [0]=n_o_alpha, [1]=n_v_alpha, [2]=n_o_beta, [3]=n_v_beta, [4]=number of level
+ * buckets, [5]=max level alpha, [6]=max level beta, [7]=walker tile width, [8]=1 if the energy calls are supported.
  * msd_get_packed copies, in the packer's sorted order, perm[n_det] (original index of each packed
  * determinant), coef[n_det] (c_I * phase_a * phase_b), level_a[n_det], level_b[n_det]; any may be NULL. HOST. */
-int msd_get_info(const msd_ctx* ctx, int64_t* info8);
+int msd_get_info(const msd_ctx* ctx, int64_t* info9);
 int msd_get_packed(const msd_ctx* ctx, int64_t* perm, double* coef, int32_t* level_a, int32_t* level_b);
 
 /* Set an upper bound (bytes) on the workspace the hot calls may allocate (default: 70 % of free device
@@ -148,9 +157,14 @@ int64_t msd_launch_count(const msd_ctx* ctx);
 int msd_set_profiling(msd_ctx* ctx, int on);
 int msd_get_phase_ms(msd_ctx* ctx, float* ms, int n);
 
-/* Measured FP64 peak of this device (TFLOP/s) from a register-resident DMMA loop run for ~`ms` ms;
- * used as the roofline denominator by bench.py (MEASURED_PEAKS.json has no FP64 entry). */
-double msd_probe_fp64_tflops(int use_dmma, double ms, void* stream);
+/* Options (arguments of the context, no environment variables are read).
+ *   MSD_OPT_NO_SMEM_TILES (value 0, 1 or 2; default 0): TEST HOOK.  Forces the kernel variants that are otherwise chosen
+ *       only for active windows too wide for shared memory, so that those paths can be parity-tested on small inputs:
+ *       1 = a walker tile's CI matrix / Hrot / F do not fit (RED.ADD scatter of C, Hrot / F through L1);
+ *       2 = the tile's g slices do not fit either (n_o n_v summed over spins above ~1600: g through L1 as well).
+ *       Results are the same.  Unknown option or value: MSD_EINVAL. */
+#define MSD_OPT_NO_SMEM_TILES 1
+int msd_set_option(msd_ctx* ctx, int option, int64_t value);
 
 void msd_destroy(msd_ctx* ctx);
 const char* msd_last_error(const msd_ctx* ctx);

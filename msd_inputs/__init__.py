@@ -22,7 +22,7 @@ from typing import Dict, Optional
 import numpy as np
 
 __all__ = ["CONFIGS", "MSDInputs", "generate", "occ_to_tables", "tables_to_occ",
-           "near_reference_walkers", "walkers_from_rng"]
+           "near_reference_walkers", "walkers_from_rng", "wide_window"]
 
 
 # name -> parameters.  "A" is the active-window size (orbitals around the Fermi
@@ -120,6 +120,38 @@ class MSDInputs:
 # ----------------------------------------------------------------------------
 # encodings
 # ----------------------------------------------------------------------------
+def wide_window(seed: int = 0, N: int = 116, n: int = 10, n_virt: int = 100, n_det: int = 600, max_level: int = 5,
+                n_chol: int = 40, n_w: int = 9) -> "MSDInputs":
+    """Closed-shell case whose active window is wider than the 16+16 orbitals of the BASELINE configs (the paper's
+    [Cu2O2]2+ has 16 occupied x 92 virtual per spin): all n occupied orbitals and the lowest n_virt
+    virtuals may be touched; total level uniform on 1..max_level, split binomially over the spins; reference first;
+    coefficients |N(0,1)| exp(-level); h1, L and walkers as in generate("small")."""
+    base = generate("small", seed=seed, N=N, n_alpha=n, n_beta=n, n_chol=n_chol, n_w=n_w, n_det=2, A=2 * min(n, 8))
+    rng = np.random.default_rng(seed + 1000003)
+    ref = np.arange(n, dtype=np.int32)
+    rows, seen = [(tuple(ref), tuple(ref))], {(tuple(ref), tuple(ref))}
+    while len(rows) < n_det:
+        lev = int(rng.integers(1, max_level + 1))
+        ka = int(rng.binomial(lev, 0.5))
+        occ = []
+        for k in (ka, lev - ka):
+            k = min(k, n)
+            keep = np.setdiff1d(ref, rng.choice(n, size=k, replace=False))
+            occ.append(tuple(np.sort(np.concatenate([keep, n + rng.choice(n_virt, size=k, replace=False)])).tolist()))
+        if tuple(occ) not in seen:
+            seen.add(tuple(occ)); rows.append(tuple(occ))
+    occa = np.array([r[0] for r in rows], dtype=np.int32)
+    occb = np.array([r[1] for r in rows], dtype=np.int32)
+    ta, tb = occ_to_tables(occa, ref), occ_to_tables(occb, ref)
+    level = np.diff(ta[0]) + np.diff(tb[0])
+    ci = np.abs(rng.standard_normal(n_det)) * np.exp(-1.0 * level)
+    ci[0] = 1.0
+    ci /= np.sqrt((ci * ci).sum())
+    p = dict(base.params); p.update(n_det=n_det, max_level=max_level, wide_window=(n, n_virt))
+    return dataclasses.replace(base, name="wide-window", n_det=n_det, occa=occa, occb=occb, ci=ci, params=p,
+                               exc_off_a=ta[0], holes_a=ta[1], parts_a=ta[2], exc_off_b=tb[0], holes_b=tb[1], parts_b=tb[2])
+
+
 def occ_to_tables(occ: np.ndarray, occ_ref: np.ndarray):
     """Occupation lists [n_det][n] -> CSR (off, holes, parts): holes = occ_ref \\ occ,
     parts = occ \\ occ_ref, both ascending.  Pure set bookkeeping."""

@@ -27,11 +27,19 @@
 #include <math.h>
 #include <stdlib.h>
 #include <string.h>
+#include <tgmath.h>   /* cabs / creal / cimag follow the type of REAL */
 #ifdef _OPENMP
 #include <omp.h>
 #endif
 
-typedef double complex cplx;
+/* REAL is the working precision: double (the oracle), or long double when built with -DREAL="long double" for the
+ * noise-floor pin P12: same statements, wider type.  The interface stays float64 either way. */
+#ifndef REAL
+#define REAL double
+#endif
+typedef REAL real;
+typedef REAL complex cplx;
+typedef double complex dcplx;
 
 /* LU with partial pivoting of the n x n matrix a (row-major, overwritten); returns det, writes the inverse
  * to inv (row-major).  Returns 0 and leaves inv undefined if a pivot is exactly zero. */
@@ -41,9 +49,9 @@ static cplx lu_det_inverse(int n, cplx *a, cplx *inv, int *piv)
     for (int i = 0; i < n; i++) piv[i] = i;
     for (int j = 0; j < n; j++) {
         int p = j;
-        double best = cabs(a[j * n + j]);
+        real best = cabs(a[j * n + j]);
         for (int i = j + 1; i < n; i++) {
-            double v = cabs(a[i * n + j]);
+            real v = cabs(a[i * n + j]);
             if (v > best) { best = v; p = i; }
         }
         if (best == 0.0) return 0.0;
@@ -89,7 +97,7 @@ typedef struct {
 static cplx det_terms(const spin_ctx *s, const int *occ, int want_energy, int want_theta,
                       cplx *O, cplx *Oinv, int *piv, cplx *theta /* [N][n] */,
                       cplx *tr_h, cplx *X /* [ng] += */, cplx *ex /* [ng] += */,
-                      double *Tr, double *Ti, double *Ir, double *Ii)
+                      real *Tr, real *Ti, real *Ir, real *Ii)
 {
     const int n = s->n, N = s->N, ng = s->ng;
     if (n == 0) { *tr_h = 0.0; return 1.0; }
@@ -117,23 +125,23 @@ static cplx det_terms(const spin_ctx *s, const int *occ, int want_energy, int wa
         const cplx *Lp = s->Lpsi + (size_t)g * N * n;
         /* T = (L^g psi)[occ,:] O^-1 */
         for (int l = 0; l < n; l++) {
-            double *tr = Tr + l * n, *ti = Ti + l * n;
+            real *tr = Tr + l * n, *ti = Ti + l * n;
             for (int i = 0; i < n; i++) { tr[i] = 0.0; ti[i] = 0.0; }
             const cplx *row = Lp + (size_t)occ[l] * n;
             for (int m = 0; m < n; m++) {
-                const double ar = creal(row[m]), ai = cimag(row[m]);
-                const double *br = Ir + m * n, *bi = Ii + m * n;
+                const real ar = creal(row[m]), ai = cimag(row[m]);
+                const real *br = Ir + m * n, *bi = Ii + m * n;
                 for (int i = 0; i < n; i++) {
                     tr[i] += ar * br[i] - ai * bi[i];
                     ti[i] += ar * bi[i] + ai * br[i];
                 }
             }
         }
-        double xr = 0.0, xi = 0.0, er = 0.0, ei = 0.0;
+        real xr = 0.0, xi = 0.0, er = 0.0, ei = 0.0;
         for (int l = 0; l < n; l++) { xr += Tr[l * n + l]; xi += Ti[l * n + l]; }
         for (int l = 0; l < n; l++)
             for (int i = 0; i < n; i++) {
-                const double ar = Tr[l * n + i], ai = Ti[l * n + i], br = Tr[i * n + l], bi = Ti[i * n + l];
+                const real ar = Tr[l * n + i], ai = Ti[l * n + i], br = Tr[i * n + l], bi = Ti[i * n + l];
                 er += ar * br - ai * bi;
                 ei += ar * bi + ai * br;
             }
@@ -151,8 +159,8 @@ static cplx det_terms(const spin_ctx *s, const int *occ, int want_energy, int wa
 int msd_oracle_o2(int N, int na, int nb, int ng, long nd, int nw,
                   const double *h1, const double *L, double e0,
                   const int *occa, const int *occb, const double *ci,
-                  const cplx *phi_a, const cplx *phi_b, int want,
-                  cplx *ovlp, cplx *G, cplx *fb, cplx *E, double *kappa, int nthreads)
+                  const dcplx *phi_a, const dcplx *phi_b, int want,
+                  dcplx *ovlp, dcplx *G, dcplx *fb, dcplx *E, double *kappa, int nthreads)
 {
     if (N <= 0 || na < 0 || nb < 0 || na > 64 || nb > 64 || nd <= 0 || nw < 0) return -1;
     const int want_g = (want & 2) != 0, want_e = (want & 4) != 0;
@@ -163,12 +171,13 @@ int msd_oracle_o2(int N, int na, int nb, int ng, long nd, int nw,
     int nt = 1;
 #endif
     const int nmax = na > nb ? na : nb;
-    cplx *hpsi[2], *Lpsi[2];
+    cplx *hpsi[2], *Lpsi[2], *psiw[2];
     const int ns[2] = {na, nb};
     for (int s = 0; s < 2; s++) {
         hpsi[s] = (cplx *)malloc(sizeof(cplx) * (size_t)N * (ns[s] + 1));
         Lpsi[s] = (cplx *)malloc(sizeof(cplx) * (size_t)(want_e ? ng : 1) * N * (ns[s] + 1));
-        if (!hpsi[s] || !Lpsi[s]) return -1;
+        psiw[s] = (cplx *)malloc(sizeof(cplx) * (size_t)N * (ns[s] + 1));   /* the walker in the working precision */
+        if (!hpsi[s] || !Lpsi[s] || !psiw[s]) return -1;
     }
     /* per-determinant numerators, summed sequentially afterwards (thread-count independent) */
     cplx *wI = (cplx *)malloc(sizeof(cplx) * nd);
@@ -178,7 +187,10 @@ int msd_oracle_o2(int N, int na, int nb, int ng, long nd, int nw,
     if (!wI || !e1I || !e2I || (want_g && !Gthr)) return -1;
 
     for (int w = 0; w < nw; w++) {
-        const cplx *psi[2] = {phi_a + (size_t)w * N * na, phi_b + (size_t)w * N * nb};
+        const dcplx *psi_in[2] = {phi_a + (size_t)w * N * na, phi_b + (size_t)w * N * nb};
+        for (int s = 0; s < 2; s++)
+            for (size_t k = 0; k < (size_t)N * ns[s]; k++) psiw[s][k] = psi_in[s][k];
+        const cplx *psi[2] = {psiw[0], psiw[1]};
         for (int s = 0; s < 2; s++) {
             const int n = ns[s];
             if (!want_e) continue;
@@ -211,8 +223,8 @@ int msd_oracle_o2(int N, int na, int nb, int ng, long nd, int nw,
             cplx *theta = (cplx *)malloc(sizeof(cplx) * ((size_t)N * nmax + 1));
             cplx *X = (cplx *)malloc(sizeof(cplx) * (ng + 1));
             cplx *ex = (cplx *)malloc(sizeof(cplx) * (ng + 1));
-            double *Tr = (double *)malloc(sizeof(double) * 4 * (nmax * nmax + 1));
-            double *Ti = Tr + (nmax * nmax + 1), *Ir = Ti + (nmax * nmax + 1), *Ii = Ir + (nmax * nmax + 1);
+            real *Tr = (real *)malloc(sizeof(real) * 4 * (nmax * nmax + 1));
+            real *Ti = Tr + (nmax * nmax + 1), *Ir = Ti + (nmax * nmax + 1), *Ii = Ir + (nmax * nmax + 1);
             int piv[64];
 #pragma omp for schedule(dynamic, 16)
             for (long Id = 0; Id < nd; Id++) {
@@ -253,7 +265,7 @@ int msd_oracle_o2(int N, int na, int nb, int ng, long nd, int nw,
             free(O); free(Oinv); free(theta); free(X); free(ex); free(Tr);
         }
         cplx den = 0.0, n1 = 0.0, n2 = 0.0;
-        double sabs = 0.0;
+        real sabs = 0.0;
         for (long Id = 0; Id < nd; Id++) { den += wI[Id]; n1 += e1I[Id]; n2 += e2I[Id]; sabs += cabs(wI[Id]); }
         ovlp[w] = den;
         if (kappa) kappa[w] = sabs / cabs(den);
@@ -267,7 +279,7 @@ int msd_oracle_o2(int N, int na, int nb, int ng, long nd, int nw,
             for (int t = 1; t < nt; t++)
                 for (size_t k = 0; k < (size_t)2 * N * N; k++) Gw[k] += Gthr[(size_t)t * 2 * N * N + k];
             for (size_t k = 0; k < (size_t)2 * N * N; k++) Gw[k] /= den;
-            if (G) memcpy(G + (size_t)w * 2 * N * N, Gw, sizeof(cplx) * 2 * N * N);
+            if (G) for (size_t k = 0; k < (size_t)2 * N * N; k++) G[(size_t)w * 2 * N * N + k] = Gw[k];
             for (int g = 0; g < ng; g++) {
                 cplx acc = 0.0;
                 const double *Lg = L + (size_t)g * N * N;
@@ -276,7 +288,7 @@ int msd_oracle_o2(int N, int na, int nb, int ng, long nd, int nw,
             }
         }
     }
-    for (int s = 0; s < 2; s++) { free(hpsi[s]); free(Lpsi[s]); }
+    for (int s = 0; s < 2; s++) { free(hpsi[s]); free(Lpsi[s]); free(psiw[s]); }
     free(wI); free(e1I); free(e2I); free(Gthr);
     return 0;
 }

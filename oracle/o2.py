@@ -9,24 +9,27 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "liboracle_o2.so")
-_lib = None
+_SO_LD = os.path.join(_HERE, "liboracle_o2_ld.so")
+_libs = {}
 
 
-def build(force: bool = False) -> str:
-    """gcc -O2 -fopenmp; no fast-math (the oracle keeps IEEE semantics)."""
+def build(force: bool = False, long_double: bool = False) -> str:
+    """gcc -O2 -fopenmp, no -ffast-math.  -fcx-limited-range only drops the C99 Annex G NaN/Inf recovery of complex
+    multiply/divide (plain (ac-bd, ad+bc) formulas); every real operation stays IEEE.  long_double=True builds the same
+    source with -DREAL="long double" (x87 80-bit) for the noise-floor pin P12."""
     src = os.path.join(_HERE, "o2.c")
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(src):
-        cmd = ["gcc", "-O2", "-march=native", "-fopenmp", "-fcx-limited-range", "-std=c99", "-shared", "-fPIC",
-               "-o", _SO, src, "-lm"]
-        subprocess.check_call(cmd)
-    return _SO
+    so = _SO_LD if long_double else _SO
+    if force or not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(src):
+        cmd = ["gcc", "-O2", "-march=native", "-fopenmp", "-fcx-limited-range", "-std=c99", "-shared", "-fPIC"]
+        if long_double:
+            cmd.append('-DREAL=long double')
+        subprocess.check_call(cmd + ["-o", so, src, "-lm"])
+    return so
 
 
-def _load():
-    global _lib
-    if _lib is None:
-        build()
-        lib = ctypes.CDLL(_SO)
+def _load(long_double: bool = False):
+    if long_double not in _libs:
+        lib = ctypes.CDLL(build(long_double=long_double))
         c = ctypes
         lib.msd_oracle_o2.restype = c.c_int
         lib.msd_oracle_o2.argtypes = [c.c_int, c.c_int, c.c_int, c.c_int, c.c_long, c.c_int,
@@ -35,17 +38,19 @@ def _load():
                                       c.c_void_p, c.c_void_p, c.c_int,
                                       c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p, c.c_int]
         lib.msd_oracle_o2_threads.restype = c.c_int
-        _lib = lib
-    return _lib
+        _libs[long_double] = lib
+    return _libs[long_double]
 
 
 def threads() -> int:
     return int(_load().msd_oracle_o2_threads())
 
 
-def o2(h1, L, e0, occa, occb, ci, phi_a, phi_b, want=("ovlp", "greens", "energy"), return_G=True, nthreads=0):
-    """Returns dict(ovlp[nw], G[nw,2,N,N] (if greens and return_G), fb[nw,ng], E[nw,3], kappa[nw])."""
-    lib = _load()
+def o2(h1, L, e0, occa, occb, ci, phi_a, phi_b, want=("ovlp", "greens", "energy"), return_G=True, nthreads=0,
+       long_double=False):
+    """Returns dict(ovlp[nw], G[nw,2,N,N] (if greens and return_G), fb[nw,ng], E[nw,3], kappa[nw]).
+    long_double: run the 80-bit build (results are rounded to float64 on output)."""
+    lib = _load(long_double)
     h1 = np.ascontiguousarray(h1, dtype=np.float64)
     L = np.ascontiguousarray(L, dtype=np.float64)
     occa = np.ascontiguousarray(occa, dtype=np.int32)
@@ -75,9 +80,9 @@ def o2(h1, L, e0, occa, occb, ci, phi_a, phi_b, want=("ovlp", "greens", "energy"
     return out
 
 
-def run(inp, walkers=None, want=("ovlp", "greens", "energy"), return_G=True, nthreads=0):
+def run(inp, walkers=None, want=("ovlp", "greens", "energy"), return_G=True, nthreads=0, long_double=False):
     pa, pb = inp.phi_a, inp.phi_b
     if walkers is not None:
         pa, pb = pa[walkers], pb[walkers]
     return o2(inp.h1, inp.L, inp.e0, inp.occa, inp.occb, inp.ci, pa, pb, want=want, return_G=return_G,
-              nthreads=nthreads)
+              nthreads=nthreads, long_double=long_double)

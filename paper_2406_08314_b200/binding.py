@@ -22,8 +22,9 @@ _CODES = {MSD_EINVAL: "MSD_EINVAL", MSD_ENOMEM: "MSD_ENOMEM", MSD_ECUDA: "MSD_EC
 EXPORTS = ["msd_setup", "msd_setup_from_occ", "msd_overlap", "msd_force_bias", "msd_local_energy", "msd_greens",
            "msd_overlap_host", "msd_force_bias_host", "msd_local_energy_host",
            "msd_force_bias_energy", "msd_force_bias_energy_host",
-           "msd_get_info", "msd_get_packed", "msd_set_workspace_limit", "msd_launch_count", "msd_set_profiling",
-           "msd_get_phase_ms", "msd_probe_fp64_tflops", "msd_destroy", "msd_last_error"]
+           "msd_get_info", "msd_get_packed", "msd_set_workspace_limit", "msd_set_option", "msd_launch_count",
+           "msd_set_profiling", "msd_get_phase_ms", "msd_destroy", "msd_last_error"]
+MSD_OPT_NO_SMEM_TILES = 1
 
 
 class MSDError(RuntimeError):
@@ -66,8 +67,8 @@ def load_library() -> C.CDLL:
     lib.msd_set_profiling.argtypes = [vp, i32]
     lib.msd_get_phase_ms.restype = i32
     lib.msd_get_phase_ms.argtypes = [vp, vp, i32]
-    lib.msd_probe_fp64_tflops.restype = dbl
-    lib.msd_probe_fp64_tflops.argtypes = [i32, dbl, vp]
+    lib.msd_set_option.restype = i32
+    lib.msd_set_option.argtypes = [vp, i32, i64]
     lib.msd_destroy.restype = None
     lib.msd_destroy.argtypes = [vp]
     lib.msd_last_error.restype = C.c_char_p
@@ -130,13 +131,25 @@ class MSDTrial:
 
     def _call(self, fn, phi_a, phi_b, out, flags, stream):
         import torch
-        if flags is not None and not (flags.is_cuda and flags.dtype == torch.int32 and flags.is_contiguous()):
-            raise ValueError("flags must be a contiguous CUDA int32 tensor")
         nw = self._walkers(phi_a, phi_b)
+        if flags is not None and not (isinstance(flags, torch.Tensor) and flags.is_cuda and flags.dtype == torch.int32
+                                      and flags.is_contiguous() and flags.numel() >= nw
+                                      and flags.device == phi_a.device):
+            raise ValueError("flags must be a contiguous CUDA int32 tensor of at least n_w elements on the walkers' device")
+        shape = self._out_shape(fn, nw)
+        if not (isinstance(out, torch.Tensor) and out.is_cuda and out.device == phi_a.device
+                and out.dtype == torch.complex128 and out.is_contiguous() and tuple(out.shape) == shape):
+            raise ValueError("out must be a contiguous CUDA complex128 tensor of shape %s on the walkers' device" % (shape,))
         rc = fn(self._h, nw, phi_a.data_ptr(), phi_b.data_ptr(), out.data_ptr(),
                 flags.data_ptr() if flags is not None else None, _stream_ptr(stream))
         self._check(rc)
         return out
+
+    def _out_shape(self, fn, nw):
+        """Result shape of a hot call (include/msd.h), by entry-point name."""
+        name = fn.__name__.replace("_host", "")
+        return {"msd_overlap": (nw,), "msd_force_bias": (nw, self.n_chol), "msd_local_energy": (nw, 3),
+                "msd_force_bias_energy": (nw, self.n_chol + 3), "msd_greens": (nw, 2, self.N, self.N)}[name]
 
     def overlap(self, phi_a, phi_b, out=None, flags=None, stream=None):
         import torch
@@ -172,17 +185,26 @@ class MSDTrial:
 
     # -- HOST-buffer variants (numpy or CPU torch arrays in and out; copies happen inside the C call) ----
     def _call_host(self, fn, phi_a, phi_b, out, flags, stream):
-        def host_ptr(a, dtype, shape_tail=None):
+        def host_ptr(a, dtype, shape=None):
             if hasattr(a, "data_ptr"):                 # CPU torch tensor (e.g. pinned)
-                if a.is_cuda or not a.is_contiguous():
-                    raise ValueError("host variants take contiguous CPU buffers")
-                return a.data_ptr()
-            if not (isinstance(a, np.ndarray) and a.dtype == dtype and a.flags.c_contiguous):
+                import torch
+                want = {np.complex128: torch.complex128, np.int32: torch.int32}[dtype]
+                if a.is_cuda or not a.is_contiguous() or a.dtype != want:
+                    raise ValueError("host variants take contiguous CPU %s buffers" % np.dtype(dtype).name)
+                ptr = a.data_ptr()
+            elif isinstance(a, np.ndarray) and a.dtype == dtype and a.flags.c_contiguous:
+                ptr = a.ctypes.data
+            else:
                 raise ValueError("host variants take contiguous %s arrays" % np.dtype(dtype).name)
-            return a.ctypes.data
+            if shape is not None and tuple(a.shape) != tuple(shape):
+                raise ValueError("buffer of shape %s expected, got %s" % (tuple(shape), tuple(a.shape)))
+            return ptr
         nw = int(phi_a.shape[0])
         if tuple(phi_a.shape) != (nw, self.N, self.n_alpha) or tuple(phi_b.shape) != (nw, self.N, self.n_beta):
             raise ValueError("walkers must be [n_w][N][n_sigma]")
+        host_ptr(out, np.complex128, self._out_shape(fn, nw))
+        if flags is not None and int(np.prod(flags.shape)) < nw:
+            raise ValueError("flags must hold at least n_w elements")
         rc = fn(self._h, nw, host_ptr(phi_a, np.complex128), host_ptr(phi_b, np.complex128),
                 host_ptr(out, np.complex128), host_ptr(flags, np.int32) if flags is not None else None,
                 _stream_ptr(stream))
@@ -207,9 +229,10 @@ class MSDTrial:
 
     # -- introspection -------------------------------------------------------------------------
     def info(self) -> dict:
-        a = np.zeros(8, dtype=np.int64)
+        a = np.zeros(9, dtype=np.int64)
         self._check(load_library().msd_get_info(self._h, _ptr(a)))
-        keys = ["n_o_alpha", "n_v_alpha", "n_o_beta", "n_v_beta", "n_buckets", "kmax_alpha", "kmax_beta", "walker_tile"]
+        keys = ["n_o_alpha", "n_v_alpha", "n_o_beta", "n_v_beta", "n_buckets", "kmax_alpha", "kmax_beta", "walker_tile",
+                "energy_supported"]
         return dict(zip(keys, (int(v) for v in a)))
 
     def packed(self) -> dict:
@@ -222,6 +245,9 @@ class MSDTrial:
 
     def set_workspace_limit(self, nbytes: int):
         self._check(load_library().msd_set_workspace_limit(self._h, int(nbytes)))
+
+    def set_option(self, option: int, value: int):
+        self._check(load_library().msd_set_option(self._h, int(option), int(value)))
 
     def launch_count(self) -> int:
         return int(load_library().msd_launch_count(self._h))
@@ -312,10 +338,6 @@ def msd_force_bias_host(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, str
 
 def msd_local_energy_host(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, stream=None):
     return trial.local_energy_host(phi_a, phi_b, out, flags, stream)
-
-
-def msd_probe_fp64_tflops(use_dmma: bool = True, ms: float = 50.0, stream=None) -> float:
-    return float(load_library().msd_probe_fp64_tflops(1 if use_dmma else 0, float(ms), _stream_ptr(stream)))
 
 
 def setup_from_inputs(inp, stream=None) -> MSDTrial:

@@ -14,6 +14,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libmsd_b200.so")
 SOURCES = ["msd_api.cu", "pack.cu", "reference.cu", "dets.cu", "dense.cu", "gemm.cu"]
+# bench-side peak probes (FP64 DMMA/DFMA, L2 gather): a separate library that only bench.py loads, not the product ABI
+PROBES_SO = os.path.join(HERE, "libmsd_probes.so")
+PROBES_SRC = "probes.cu"
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-diag-suppress", "128"]
 
@@ -28,7 +31,7 @@ def _nvcc() -> str:
 
 
 def needs_build() -> bool:
-    if not os.path.exists(SO):
+    if not os.path.exists(SO) or not os.path.exists(PROBES_SO):
         return True
     t = os.path.getmtime(SO)
     deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
@@ -42,7 +45,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     procs, objs = [], []
-    for src in SOURCES:
+    for src in SOURCES + [PROBES_SRC]:
         obj = os.path.join(objdir, src.replace(".cu", ".o"))
         cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
               ["-c", os.path.join(CSRC, src), "-o", obj]
@@ -58,7 +61,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
             sys.stderr.write(out)
     if failed:
         raise RuntimeError("nvcc compilation failed")
-    subprocess.check_call([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", SO] + objs + ["-lcudart"])
+    link = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o"]
+    subprocess.check_call(link + [SO] + objs[:-1] + ["-lcudart"])
+    subprocess.check_call(link + [PROBES_SO] + objs[-1:] + ["-lcudart"])
     return SO
 
 

@@ -98,10 +98,8 @@ cudaError_t launch_green_rows(msd_ctx* c, int64_t nw, Workspace& ws, cplx* Gfull
         size_t v = ((size_t)c->sp[s].n_v * c->sp[s].n_o + (size_t)c->sp[s].n * c->sp[s].n_o + 1) * sizeof(cplx);
         if (v > smem) smem = v;
     }
-    if (smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(k_green_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-    }
+    cudaError_t e = func_config(c, (const void*)k_green_rows, 256, smem, nullptr);
+    if (e != cudaSuccess) return e;
     dim3 grid((unsigned)nw, 2);
     k_green_rows<<<grid, 256, smem, st>>>(c->N, ldN, c->dev(0), c->dev(1), nw, ws.theta[0], ws.theta[1], ws.C[0],
                                           ws.C[1], ws.Wacc, ws.Gp[0], ws.Gp[1], Gfull, ws.wflags);
@@ -498,8 +496,7 @@ k_fx(int n_chol, int64_t nw, int Pa, int Pb, const cplx* __restrict__ X0, const 
 template <int NWARP, int MTC, int NTC>
 static cudaError_t launch_dense_mma_t(msd_ctx* c, int64_t nw, Workspace& ws, size_t smem, cudaStream_t st)
 {
-    cudaError_t e = cudaFuncSetAttribute(k_energy_dense_mma<NWARP, MTC, NTC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)smem);
+    cudaError_t e = func_config(c, (const void*)k_energy_dense_mma<NWARP, MTC, NTC>, NWARP * 32, smem, nullptr);
     if (e != cudaSuccess) return e;
     const int gchunk = 4 * NWARP;
     dim3 grid((c->n_chol + 1 + gchunk - 1) / gchunk, (unsigned)nw, 2);
@@ -530,6 +527,19 @@ static cudaError_t launch_dense_mma(msd_ctx* c, int64_t nw, Workspace& ws, size_
     return launch_dense_mma_t<NWARP, 0, 0>(c, nw, ws, smem, st);
 }
 
+// dynamic shared memory of k_energy_dense<GC> (the larger of the two spins)
+size_t energy_dense_smem(const msd_ctx* c, int GC)
+{
+    size_t smem = 0;
+    for (int s = 0; s < 2; s++) {
+        const auto& sp = c->sp[s];
+        size_t v = ((size_t)sp.n * sp.n + 2 * (size_t)sp.n_v * sp.n + (size_t)sp.P * (1 + GC) + 1) * sizeof(cplx) +
+                   (size_t)(sp.n_o + 4) * sizeof(int);
+        if (v > smem) smem = v;
+    }
+    return smem;
+}
+
 cudaError_t launch_energy_dense(msd_ctx* c, int64_t nw, Workspace& ws, cudaStream_t st)
 {
     if (nw == 0) return cudaSuccess;
@@ -550,23 +560,21 @@ cudaError_t launch_energy_dense(msd_ctx* c, int64_t nw, Workspace& ws, cudaStrea
     if (mma_ok && need[0] <= 113 * 1024) e = launch_dense_mma<8>(c, nw, ws, need[0], st);
     else if (mma_ok && need[1] <= 227 * 1024) e = launch_dense_mma<4>(c, nw, ws, need[1], st);
     else {
-        constexpr int GC = 8;
-        size_t smem = 0;
-        for (int s = 0; s < 2; s++) {
-            const auto& sp = c->sp[s];
-            size_t v = ((size_t)sp.n * sp.n + 2 * (size_t)sp.n_v * sp.n + (size_t)sp.P * (1 + GC) + 1) * sizeof(cplx) +
-                       (size_t)(sp.n_o + 4) * sizeof(int);
-            if (v > smem) smem = v;
-        }
-        if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
-        e = cudaFuncSetAttribute(k_energy_dense<GC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
+        // slices per CTA: as many as fit next to the per-walker tiles (the paper's Cu2O2 window, 16 x 92, takes 4)
+        int GC = 8;
+        while (GC > 1 && energy_dense_smem(c, GC) > 227 * 1024) GC >>= 1;
+        const size_t smem = energy_dense_smem(c, GC);
+        if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;     // excluded at setup (energy_ok)
         // X0 of a spin with no electrons must read as zero: ws.X0 lies in the region zeroed per call
         dim3 grid((c->n_chol + 1 + GC - 1) / GC, (unsigned)nw, 2);
-        k_energy_dense<GC><<<grid, 256, smem, st>>>(c->n_chol, nw, c->dev(0), c->dev(1), ws.theta[0], ws.theta[1],
-                                                    ws.Lam[0], ws.Lam[1], ws.Bp[0], ws.Bp[1], ws.X0,
-                                                    ws.F[0], ws.F[1], ws.Hrot[0], ws.Hrot[1], ws.Eacc, c->N);
-        e = cudaGetLastError();
+        auto go = [&](auto kern) {
+            cudaError_t e2 = func_config(c, (const void*)kern, 256, smem, nullptr);
+            if (e2 != cudaSuccess) return e2;
+            kern<<<grid, 256, smem, st>>>(c->n_chol, nw, c->dev(0), c->dev(1), ws.theta[0], ws.theta[1], ws.Lam[0], ws.Lam[1],
+                                          ws.Bp[0], ws.Bp[1], ws.X0, ws.F[0], ws.F[1], ws.Hrot[0], ws.Hrot[1], ws.Eacc, c->N);
+            return cudaGetLastError();
+        };
+        e = GC == 8 ? go(k_energy_dense<8>) : GC == 4 ? go(k_energy_dense<4>) : GC == 2 ? go(k_energy_dense<2>) : go(k_energy_dense<1>);
     }
     c->launches++;
     return e;
@@ -679,32 +687,35 @@ cudaError_t launch_finish_energy(msd_ctx* c, int64_t nw, Workspace& ws, cplx* e,
 // Force bias from the energy path's intermediates:
 //   fb[w][g] = sum_s [ X0^s[w][g] + (1/W) sum_x C^s[x][w] B^{s,g}[w][x] ]
 // C planar [tile][x][2][WT], Bp [w][x][g] (g contiguous: coalesced over the threads), out row stride `ostride`.
+#define FB_XT 1024
 __global__ void __launch_bounds__(256)
 k_fb_from_cb(int n_chol, int64_t nw, int Pa, int Pb, const double* __restrict__ C_a, const double* __restrict__ C_b,
              const cplx* __restrict__ Bp_a, const cplx* __restrict__ Bp_b, const cplx* __restrict__ X0,
              const cplx* __restrict__ Wacc, const int* __restrict__ wflags, cplx* out, int64_t ostride)
 {
-    extern __shared__ __align__(16) unsigned char smem_fb[];
-    cplx* Cs = reinterpret_cast<cplx*>(smem_fb);              // [Pa + Pb]
+    __shared__ cplx Cs[FB_XT];                                  // one chunk of C^s at a time (any window size)
     const int64_t w = blockIdx.y;
-    for (int s = 0; s < 2; s++) {
-        const int P = s ? Pb : Pa;
-        const double* C = (s ? C_b : C_a) + (w / MSD_WT) * (int64_t)P * 2 * MSD_WT + (w % MSD_WT);
-        for (int x = threadIdx.x; x < P; x += blockDim.x) Cs[(s ? Pa : 0) + x] = load_planar(C, x);
-    }
-    __syncthreads();
     const int g = blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= n_chol) return;
     const cplx W = Wacc[w];
-    if (wflags[w] || (W.x == 0.0 && W.y == 0.0)) { out[w * ostride + g] = cmake(nan_d(), nan_d()); return; }
+    const bool bad = wflags[w] || (W.x == 0.0 && W.y == 0.0);
     cplx acc[2] = {cmake(0.0, 0.0), cmake(0.0, 0.0)};
     for (int s = 0; s < 2; s++) {
         const int P = s ? Pb : Pa;
+        const double* C = (s ? C_b : C_a) + (w / MSD_WT) * (int64_t)P * 2 * MSD_WT + (w % MSD_WT);
         const cplx* B = (s ? Bp_b : Bp_a) + w * (int64_t)P * n_chol + g;
-        const cplx* c = Cs + (s ? Pa : 0);
+        for (int x0 = 0; x0 < P; x0 += FB_XT) {
+            const int nx = min(FB_XT, P - x0);
+            __syncthreads();
+            for (int x = threadIdx.x; x < nx; x += blockDim.x) Cs[x] = load_planar(C, x0 + x);
+            __syncthreads();
+            if (g < n_chol && !bad) {
 #pragma unroll 4
-        for (int x = 0; x < P; x++) acc[x & 1] = cfma(c[x], B[(int64_t)x * n_chol], acc[x & 1]);
+                for (int x = 0; x < nx; x++) acc[x & 1] = cfma(Cs[x], B[(int64_t)(x0 + x) * n_chol], acc[x & 1]);
+            }
+        }
     }
+    if (g >= n_chol) return;
+    if (bad) { out[w * ostride + g] = cmake(nan_d(), nan_d()); return; }
     const cplx t = cmul(cadd(acc[0], acc[1]), cinv(W));
     const cplx x0 = cadd(X0[w * (int64_t)n_chol + g], X0[(nw + w) * (int64_t)n_chol + g]);
     out[w * ostride + g] = cadd(x0, t);
@@ -715,7 +726,7 @@ cudaError_t launch_fb_from_cb(msd_ctx* c, int64_t nw, Workspace& ws, cplx* out, 
     if (nw == 0 || c->n_chol == 0) return cudaSuccess;
     const int Pa = c->sp[0].P, Pb = c->sp[1].P;
     dim3 grid((c->n_chol + 255) / 256, (unsigned)nw);
-    k_fb_from_cb<<<grid, 256, (size_t)(Pa + Pb + 1) * sizeof(cplx), st>>>(c->n_chol, nw, Pa, Pb, ws.C[0], ws.C[1], ws.Bp[0],
+    k_fb_from_cb<<<grid, 256, 0, st>>>(c->n_chol, nw, Pa, Pb, ws.C[0], ws.C[1], ws.Bp[0],
                                                                           ws.Bp[1], ws.X0, ws.Wacc, ws.wflags, out, ostride);
     c->launches++;
     return cudaGetLastError();

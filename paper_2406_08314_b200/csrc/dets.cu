@@ -21,7 +21,6 @@
 #define M_ENERGY(M) ((M) >= 2)
 #define M_SCATTER(M) ((M) == 1 || (M) == 3)
 #include <algorithm>
-#include <cstdlib>
 
 struct DetsParams {
     const unsigned char* tab;
@@ -185,12 +184,10 @@ template <int NWORD> struct RowData { uint32_t w[NWORD]; double cf; };
 
 template <int KA, int KB, int MODE, bool FHS>
 __device__ __forceinline__ void run_bucket(const DetsParams& p, const WorkItem& it, int tile, int slot, int nslots,
-                                           int j, const cplx* gsm, cplx& Wl, cplx& El, cplx& Hl)
+                                           int j, const cplx* gsm, const cplx* gA, const cplx* gB, cplx& Wl, cplx& El, cplx& Hl)
 {
     constexpr int NB = 2 * KA + 2 * KB;
     constexpr int NWORD = (NB + 3) / 4 > 0 ? (NB + 3) / 4 : 1;
-    const cplx* gA = gsm + j;
-    const cplx* gB = gsm + p.P[0] * MSD_WT + j;
     double* CA = p.C[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j;
     double* CB = p.C[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j;
     const cplx* VA = (M_ENERGY(MODE)) ? p.Vss[0] + (int64_t)tile * p.P[0] * p.P[0] * MSD_WT + j : nullptr;
@@ -335,12 +332,14 @@ __device__ __forceinline__ void stage_g(const DetsParams& p, int tile, cplx* gsm
 #define CF_CASE(KA_, KB_)                                                                              \
     case KA_ * 5 + KB_:                                                                                \
         if constexpr ((KA_ > KB_ ? KA_ : KB_) > KLO && (KA_ > KB_ ? KA_ : KB_) <= KHI)                  \
-            run_bucket<KA_, KB_, MODE, FHS>(p, it, tile, slot, nslots, j, gsm, Wl, El, Hl);                     \
+            run_bucket<KA_, KB_, MODE, FHS>(p, it, tile, slot, nslots, j, gsm, gpa, gpb, Wl, El, Hl);           \
         break;
 
 // register class (KLO, KHI]: buckets whose larger level lies in that range (KLO = -1 admits (0,0)).
 // Persistent per walker tile: CTA (worker, tile) stages g once and strides over the class's work items.
-template <int MODE, int KLO, int KHI, int NTHR, int MINB, bool FHS>
+// GSM: the tile's g slices are staged in shared memory; false (windows wider than ~1800 pairs: they do not fit) reads them
+// through L1/L2 and needs no dynamic shared memory at all (FHS implies GSM).
+template <int MODE, int KLO, int KHI, int NTHR, int MINB, bool FHS, bool GSM = true>
 __global__ void __launch_bounds__(NTHR, MINB) k_dets_cf(DetsParams p, const WorkItem* __restrict__ items, int n_items)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -348,7 +347,10 @@ __global__ void __launch_bounds__(NTHR, MINB) k_dets_cf(DetsParams p, const Work
     const int tile = blockIdx.y;
     const int j = threadIdx.x & (MSD_WT - 1);
     const int slot = threadIdx.x / MSD_WT, nslots = NTHR / MSD_WT;
-    stage_g(p, tile, gsm, FHS);
+    const cplx* gpa = gsm + j;
+    const cplx* gpb = gsm + p.P[0] * MSD_WT + j;
+    if (GSM) stage_g(p, tile, gsm, FHS);
+    else { gpa = p.g[0] + (int64_t)tile * p.P[0] * MSD_WT + j; gpb = p.g[1] + (int64_t)tile * p.P[1] * MSD_WT + j; }
     cplx Wl = cmake(0.0, 0.0), El = cmake(0.0, 0.0), Hl = cmake(0.0, 0.0);
     for (int r = 0, ii; (ii = r * (int)gridDim.x + ((r & 1) ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x)),
                         r * (int)gridDim.x < n_items; r++) {
@@ -1149,16 +1151,13 @@ __global__ void k_fh_tile(const cplx* __restrict__ Hrot, const cplx* __restrict_
 
 // ------------------------------------------------------------------------------------------------
 template <class K>
-static cudaError_t launch_persistent(K kernel, int nthr, size_t smem, int n_sm, const DetsParams& p, const WorkItem* items,
-                                     int n_items, int ntiles, cudaStream_t st)
+static cudaError_t launch_persistent(msd_ctx* c, K kernel, int nthr, size_t smem, int n_sm, const DetsParams& p,
+                                     const WorkItem* items, int n_items, int ntiles, cudaStream_t st)
 {
     if (n_items == 0) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
     int occ = 1;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, nthr, smem);
+    cudaError_t e = func_config(c, (const void*)kernel, nthr, smem, &occ);
     if (e != cudaSuccess) return e;
-    if (occ < 1) return cudaErrorInvalidConfiguration;
     // about two walker tiles resident at a time (their V slices stay in L2), every SM full
     int workers = (n_sm * occ + 1) / 2;
     if (workers > n_items) workers = n_items;
@@ -1169,11 +1168,11 @@ static cudaError_t launch_persistent(K kernel, int nthr, size_t smem, int n_sm, 
 }
 
 template <class K>
-static cudaError_t launch_c1(K kernel, int nthr, size_t smem, int n_sm, const DetsParams& p, const WorkItem* items, int n_items,
-                             int ntiles, const uint32_t* sched, cudaStream_t st)
+static cudaError_t launch_c1(msd_ctx* c, K kernel, int nthr, size_t smem, int n_sm, const DetsParams& p, const WorkItem* items,
+                             int n_items, int ntiles, const uint32_t* sched, cudaStream_t st)
 {
     if (n_items == 0) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = func_config(c, (const void*)kernel, nthr, smem, nullptr);
     if (e != cudaSuccess) return e;
     int workers = (n_sm + 1) / 2;                  // one CTA per SM, about two walker tiles resident at a time
     if (workers > n_items) workers = n_items;
@@ -1187,9 +1186,10 @@ template <int MODE>
 static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cudaStream_t st)
 {
     const size_t gbytes = (size_t)(p.P[0] + p.P[1]) * MSD_WT * sizeof(cplx);
-    // test hook: MSD_NO_SMEM_TILES=1 takes the paths used when a walker tile's C / Hrot / F do not fit in shared memory
-    // (RED scatter for the force bias, Hrot / F through L1 for the energy), which no BASELINE config needs
-    const bool no_tiles = getenv("MSD_NO_SMEM_TILES") != nullptr;
+    // test hook (msd_set_option MSD_OPT_NO_SMEM_TILES): take the paths used when a walker tile's C / Hrot / F / g do not fit
+    // in shared memory (RED scatter for the force bias, operands through L1), which no BASELINE config needs
+    const bool no_tiles = c->no_smem_tiles >= 1;
+    const bool gsm_ok = gbytes <= 200 * 1024 && c->no_smem_tiles < 2;
     // The launches below are independent (they only meet in the RED accumulators), so they are forked over the
     // context's side streams: the small high-level groups no longer serialise their tails behind one another.
     Fork f(c, st);
@@ -1202,10 +1202,8 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
             const int elems = c->gen_group_elems[gi];
             const size_t smem = (size_t)4 * elems * (8 * sizeof(cplx) + sizeof(int));
             auto kern = k_dets_coop<MODE>;
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             int occ = 1;
-            if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 128, smem);
-            if (e == cudaSuccess && occ < 1) e = cudaErrorInvalidConfiguration;
+            cudaError_t e = func_config(c, (const void*)kern, 128, smem, &occ);
             if (e != cudaSuccess) { f.join(); return e; }
             int workers = std::min(i1 - i0, (c->n_sm * occ + 1) / 2);
             if (ntiles == 1) workers = std::min(i1 - i0, c->n_sm * occ);
@@ -1219,7 +1217,7 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
         const size_t per_thread = (size_t)c->gen_group_elems[gi] * (sizeof(cplx) + sizeof(int));
         while (nthr > 32 && per_thread * nthr > 200 * 1024) nthr -= 32;
         size_t smem = per_thread * nthr;
-        cudaError_t e = launch_persistent(k_dets_gen<MODE>, nthr, smem, c->n_sm, p, c->d_items_gen + i0, i1 - i0, ntiles,
+        cudaError_t e = launch_persistent(c, k_dets_gen<MODE>, nthr, smem, c->n_sm, p, c->d_items_gen + i0, i1 - i0, ntiles,
                                           f.stream(li++));
         if (e != cudaSuccess) { f.join(); return e; }
         c->launches++;
@@ -1239,25 +1237,29 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
             if (sm1 <= 227 * 1024 && c->d_sched && p.P[0] + p.P[1] < 8192 && !no_tiles) {
                 fhs = true;     // handled here
                 const bool gs = sm1 + csm <= 227 * 1024;        // room for the g slices as well
-                if (cl == 0 && gs) e = launch_c1(k_dets_c1<-1, 2, 768, true>, 768, sm1 + csm, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
-                else if (cl == 0) e = launch_c1(k_dets_c1<-1, 2, 768, false>, 768, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
-                else if (cl == 1 && gs) e = launch_c1(k_dets_c1<2, 3, 512, true>, 512, sm1 + csm, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
-                else if (cl == 1) e = launch_c1(k_dets_c1<2, 3, 512, false>, 512, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
-                else if (gs) e = launch_c1(k_dets_c1<3, 4, 256, true>, 256, sm1 + csm, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
-                else e = launch_c1(k_dets_c1<3, 4, 256, false>, 256, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
+                if (cl == 0 && gs) e = launch_c1(c, k_dets_c1<-1, 2, 768, true>, 768, sm1 + csm, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
+                else if (cl == 0) e = launch_c1(c, k_dets_c1<-1, 2, 768, false>, 768, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
+                else if (cl == 1 && gs) e = launch_c1(c, k_dets_c1<2, 3, 512, true>, 512, sm1 + csm, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
+                else if (cl == 1) e = launch_c1(c, k_dets_c1<2, 3, 512, false>, 512, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
+                else if (gs) e = launch_c1(c, k_dets_c1<3, 4, 256, true>, 256, sm1 + csm, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
+                else e = launch_c1(c, k_dets_c1<3, 4, 256, false>, 256, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
             }
         }
         if constexpr (MODE >= 2) {
             fhs = 3 * gbytes <= 200 * 1024 && !no_tiles;
             if (!fhs) {}
-            else if (cl == 0) e = launch_persistent(k_dets_cf<MODE, -1, 2, 768, 1, true>, 768, 3 * gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
-            else if (cl == 1) e = launch_persistent(k_dets_cf<MODE, 2, 3, 512, 1, true>, 512, 3 * gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
-            else e = launch_persistent(k_dets_cf<MODE, 3, 4, 256, 1, true>, 256, 3 * gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+            else if (cl == 0) e = launch_persistent(c, k_dets_cf<MODE, -1, 2, 768, 1, true>, 768, 3 * gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+            else if (cl == 1) e = launch_persistent(c, k_dets_cf<MODE, 2, 3, 512, 1, true>, 512, 3 * gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+            else e = launch_persistent(c, k_dets_cf<MODE, 3, 4, 256, 1, true>, 256, 3 * gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
         }
-        if (!fhs) {
-            if (cl == 0) e = launch_persistent(k_dets_cf<MODE, -1, 2, 256, 3, false>, 256, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
-            else if (cl == 1) e = launch_persistent(k_dets_cf<MODE, 2, 3, 256, 2, false>, 256, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
-            else e = launch_persistent(k_dets_cf<MODE, 3, 4, 128, 2, false>, 128, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+        if (!fhs && gsm_ok) {
+            if (cl == 0) e = launch_persistent(c, k_dets_cf<MODE, -1, 2, 256, 3, false>, 256, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+            else if (cl == 1) e = launch_persistent(c, k_dets_cf<MODE, 2, 3, 256, 2, false>, 256, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+            else e = launch_persistent(c, k_dets_cf<MODE, 3, 4, 128, 2, false>, 128, gbytes, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+        } else if (!fhs) {      // g through L1/L2 as well: no dynamic shared memory
+            if (cl == 0) e = launch_persistent(c, k_dets_cf<MODE, -1, 2, 256, 3, false, false>, 256, 0, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+            else if (cl == 1) e = launch_persistent(c, k_dets_cf<MODE, 2, 3, 256, 2, false, false>, 256, 0, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
+            else e = launch_persistent(c, k_dets_cf<MODE, 3, 4, 128, 2, false, false>, 128, 0, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, s);
         }
         if (e != cudaSuccess) { f.join(); return e; }
         c->launches++;

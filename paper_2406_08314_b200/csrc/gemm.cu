@@ -5,8 +5,8 @@
 // All three are  C[m][n] (+)= sum_k A[m][k] B[n][k]  with both operands K-contiguous ("TN"), real FP64;
 // complex operands are expressed as real ones by the callers (see dense.cu).
 //
-// tcgen05/UMMA has no f64 kind, so FP64 tensor work on sm_100a goes through warp-level mma.sync; the probe in
-// this file measured 37.1 TFLOP/s for DMMA and 36.3 for DFMA on B200 (they share the FP64 units).
+// tcgen05/UMMA has no f64 kind, so FP64 tensor work on sm_100a goes through warp-level mma.sync; the bench-side probe
+// (csrc/probes.cu) measured 37.1 TFLOP/s for DMMA and 36.3 for DFMA on B200 (they share the FP64 units).
 // Tiles: CTA BM x BN x 16, 3-stage cp.async ring, warp tile 32 x 32 (4 x 4 DMMA tiles), fragments read from
 // shared memory with row stride 20 doubles (conflict-free for the 8x4 fragment pattern).
 #include "msd_internal.cuh"
@@ -145,29 +145,25 @@ k_gemm_tn(GemmArgs g)
 }
 
 template <int BM, int BN, int WARPS_M, int WARPS_N, bool BX>
-static cudaError_t launch_cfg_x(const GemmArgs& a, cudaStream_t st)
+static cudaError_t launch_cfg_x(msd_ctx* c, const GemmArgs& a, cudaStream_t st)
 {
     size_t smem = (size_t)STAGES * (BM + (BX ? BN / 2 : BN)) * LDS_ * sizeof(double);
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_gemm_tn<BM, BN, WARPS_M, WARPS_N, BX>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    cudaError_t e = func_config(c, (const void*)k_gemm_tn<BM, BN, WARPS_M, WARPS_N, BX>, WARPS_M * WARPS_N * 32, smem, nullptr);
+    if (e != cudaSuccess) return e;
     dim3 grid((a.N + BN - 1) / BN, (a.M + BM - 1) / BM, a.batch * a.ksplit);
     k_gemm_tn<BM, BN, WARPS_M, WARPS_N, BX><<<grid, WARPS_M * WARPS_N * 32, smem, st>>>(a);
     return cudaGetLastError();
 }
 
 template <int BM, int BN, int WARPS_M, int WARPS_N>
-static cudaError_t launch_cfg(const GemmArgs& a, cudaStream_t st)
+static cudaError_t launch_cfg(msd_ctx* c, const GemmArgs& a, cudaStream_t st)
 {
-    return a.bexpand ? launch_cfg_x<BM, BN, WARPS_M, WARPS_N, true>(a, st) : launch_cfg_x<BM, BN, WARPS_M, WARPS_N, false>(a, st);
+    return a.bexpand ? launch_cfg_x<BM, BN, WARPS_M, WARPS_N, true>(c, a, st) : launch_cfg_x<BM, BN, WARPS_M, WARPS_N, false>(c, a, st);
 }
 
-cudaError_t launch_gemm_tn(const GemmArgs& a, int n_sm, cudaStream_t st)
+cudaError_t launch_gemm_tn(msd_ctx* c, const GemmArgs& a, cudaStream_t st)
 {
+    const int n_sm = c->n_sm;
     if (a.M <= 0 || a.N <= 0 || a.batch <= 0) return cudaSuccess;
     if ((a.N & 1) || (a.K & 1) || (a.lda & 1) || (a.ldb & 1) || (a.strideA & 1) || (a.strideB & 1))
         return cudaErrorInvalidValue;     // callers pad to even sizes (16-byte cp.async chunks)
@@ -193,72 +189,7 @@ cudaError_t launch_gemm_tn(const GemmArgs& a, int n_sm, cudaStream_t st)
         const double cost = (double)((tiles + slots - 1) / slots) * cands[i].occ * cands[i].bm * cands[i].bn;
         if (i == 0 || cost < best_cost * 0.97) { best = i; best_cost = cost; }     // ties go to the larger tile
     }
-    if (best == 0) return launch_cfg<128, 64, 4, 2>(a, st);
-    if (best == 1) return launch_cfg<64, 64, 2, 2>(a, st);
-    return launch_cfg<48, 96, 2, 2>(a, st);
-}
-
-// ------------------------------------------------------------------------------------------------
-// FP64 peak probe (register-resident): roofline denominator for bench.py
-// ------------------------------------------------------------------------------------------------
-__global__ void k_probe_dmma(double* out, int iters)
-{
-    double d[8][2];
-    for (int j = 0; j < 8; j++) { d[j][0] = 0.0; d[j][1] = 0.0; }
-    double a = threadIdx.x * 1e-3, b = 1e-3;
-    for (int i = 0; i < iters; i++) {
-#pragma unroll
-        for (int j = 0; j < 8; j++) dmma884(d[j][0], d[j][1], a, b);
-    }
-    double s = 0.0;
-    for (int j = 0; j < 8; j++) s += d[j][0] + d[j][1];
-    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
-}
-__global__ void k_probe_dfma(double* out, int iters)
-{
-    double a[8];
-    for (int j = 0; j < 8; j++) a[j] = threadIdx.x * 1e-9 + j;
-    const double b = 1.0000001, c = 1e-9;
-    for (int i = 0; i < iters; i++) {
-#pragma unroll
-        for (int j = 0; j < 8; j++) a[j] = fma(a[j], b, c);
-    }
-    double s = 0.0;
-    for (int j = 0; j < 8; j++) s += a[j];
-    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
-}
-
-double probe_fp64(int use_dmma, double ms_target, cudaStream_t st)
-{
-    int dev = 0, nsm = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return -1.0;
-    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    const int thr = 512, blocks = nsm * 2;
-    double* out = nullptr;
-    if (cudaMalloc(&out, sizeof(double) * thr * blocks) != cudaSuccess) return -1.0;
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
-    int iters = 20000;
-    double best = 0.0;
-    for (int rep = 0; rep < 3; rep++) {
-        cudaEventRecord(e0, st);
-        if (use_dmma) k_probe_dmma<<<blocks, thr, 0, st>>>(out, iters);
-        else k_probe_dfma<<<blocks, thr, 0, st>>>(out, iters);
-        cudaEventRecord(e1, st);
-        if (cudaEventSynchronize(e1) != cudaSuccess) { best = -1.0; break; }
-        float ms = 0.f;
-        cudaEventElapsedTime(&ms, e0, e1);
-        double fl = use_dmma ? 2.0 * 8 * 8 * 4 * 8 * (double)iters * blocks * thr / 32.0
-                             : 2.0 * 8 * (double)iters * blocks * thr;
-        double tf = fl / (ms * 1e-3) / 1e12;
-        if (rep > 0 && tf > best) best = tf;
-        if (rep == 0 && ms > 0.f && ms_target > 0.0) {
-            double scale = ms_target / ms;
-            if (scale > 200.0) scale = 200.0;
-            if (scale > 1.0) iters = (int)(iters * scale);
-        }
-    }
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    cudaFree(out);
-    return best;
+    if (best == 0) return launch_cfg<128, 64, 4, 2>(c, a, st);
+    if (best == 1) return launch_cfg<64, 64, 2, 2>(c, a, st);
+    return launch_cfg<48, 96, 2, 2>(c, a, st);
 }

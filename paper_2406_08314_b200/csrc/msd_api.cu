@@ -5,9 +5,38 @@
 #include <algorithm>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 static std::string g_setup_error;
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is state of the (device, function) pair shared by every context of the
+// process: it is only ever raised, under a lock; occupancy is cached per context.
+static std::mutex g_func_mutex;
+static std::map<std::pair<int, const void*>, size_t> g_func_smem;
+
+cudaError_t func_config(msd_ctx* c, const void* func, int nthr, size_t smem, int* occ)
+{
+    const auto key = std::make_pair(func, smem * 2048 + (size_t)nthr);
+    auto it = c->occ_cache.find(key);
+    if (it != c->occ_cache.end()) { if (occ) *occ = it->second; return cudaSuccess; }
+    {
+        std::lock_guard<std::mutex> lock(g_func_mutex);
+        size_t& cur = g_func_smem[std::make_pair(c->device, func)];
+        if (smem > cur && smem > 32 * 1024) {      // (static shared memory counts against the 48 KB default too)
+            cudaError_t e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+            cur = smem;
+        }
+    }
+    int o = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, func, nthr, smem);
+    if (e != cudaSuccess) return e;
+    if (o < 1) return cudaErrorInvalidConfiguration;
+    c->occ_cache[key] = o;
+    if (occ) *occ = o;
+    return cudaSuccess;
+}
 
 #define CK(call)                                                                                        \
     do {                                                                                                \
@@ -43,7 +72,7 @@ static int do_setup(msd_ctx* c, std::string* errp, int N, int na, int nb, int n_
     if (N < 1 || na < 0 || nb < 0 || n_chol < 1 || n_det < 1) return fail(errp, MSD_EINVAL, "non-positive size");
     if (N > 1024 || na > MSD_MAX_NOCC || nb > MSD_MAX_NOCC || na > N || nb > N)
         return fail(errp, MSD_EUNSUPPORTED, "N <= 1024 and n_alpha, n_beta <= 64 required");
-    if (n_det > (int64_t)1 << 31) return fail(errp, MSD_EUNSUPPORTED, "n_det too large");
+    if (n_det >= (int64_t)1 << 31) return fail(errp, MSD_EUNSUPPORTED, "n_det < 2^31 required");
     CK(cudaGetDevice(&c->device));
     CK(cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device));
     c->N = N; c->n_chol = n_chol; c->n_det = n_det; c->e0 = e0;
@@ -111,12 +140,21 @@ static int do_setup(msd_ctx* c, std::string* errp, int N, int na, int nb, int n_
         }
         sp.n_o = (int)sp.act_o.size(); sp.n_v = (int)sp.act_v.size();
         sp.n_r = sp.n + sp.n_v; sp.P = sp.n_o * sp.n_v;
-        if (sp.n_o > 255 || sp.n_v > 255 || sp.P > 65535)
-            return fail(errp, MSD_EUNSUPPORTED, "active window too large (n_o, n_v <= 255, n_o*n_v <= 65535)");
+        if (sp.n_o > 255 || sp.n_v > 255 || sp.P > 8192)
+            return fail(errp, MSD_EUNSUPPORTED, "active window too large (n_o, n_v <= 255, n_o*n_v <= 8192 per spin)");
+        if (sp.P > 4096) { c->energy_ok = false; c->energy_why = "local energy requires n_o*n_v <= 4096 per spin"; }
         CK(upload(&d_map[2 * s], map_h[s].data(), N, st));
         CK(upload(&d_map[2 * s + 1], map_p[s].data(), N, st));
         CK(upload(&sp.d_act_v, sp.act_v.data(), sp.act_v.size(), st));
         CK(upload(&sp.d_pos_o, sp.pos_o.data(), sp.pos_o.size(), st));
+    }
+    {   // the scalar S7 kernel (windows wider than 16 x 16) keeps per-walker tiles in shared memory
+        bool mma = true;
+        for (int s = 0; s < 2; s++) if (c->sp[s].n > 0 && (c->sp[s].n_o > 16 || c->sp[s].n_v > 16)) mma = false;
+        if (!mma && energy_dense_smem(c, 1) > 227 * 1024 && c->energy_ok) {
+            c->energy_ok = false;
+            c->energy_why = "local energy: n^2 + 2 n n_v + 2 n_o n_v complex numbers per spin must fit in 227 KB of shared memory";
+        }
     }
     // --- pass 2: per-determinant rows, phases, level keys ---
     constexpr int NK = (MSD_MAX_LEVEL + 1) * (MSD_MAX_LEVEL + 1);
@@ -136,6 +174,19 @@ static int do_setup(msd_ctx* c, std::string* errp, int N, int na, int nb, int n_
     CK(cudaMemcpyAsync(&err2, d_err, sizeof(int), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     if (err2 != 0) return fail(errp, MSD_EINVAL, "invalid excitation table (repeated index inside a determinant, or level > n)");
+    // --- pass 3: the same determinant listed twice?  (Eq. 15: orthogonal CI expansion) ---
+    {
+        int64_t nslots = 16;
+        while (nslots < 2 * n_det) nslots <<= 1;
+        int* d_slots; CK(cudaMalloc(&d_slots, sizeof(int) * nslots));
+        CK(cudaMemsetAsync(d_slots, 0xff, sizeof(int) * nslots, st));
+        CK(launch_pack_dedup(n_det, d_tmp, d_key, d_slots, nslots, d_err, st));
+        c->launches++;
+        CK(cudaMemcpyAsync(&err2, d_err, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        cudaFree(d_slots);
+        if (err2 != 0) return fail(errp, MSD_EINVAL, "invalid excitation table (the same determinant is listed twice)");
+    }
     // --- buckets ---
     std::vector<int> bucket_keys, bucket_of_key(NK, -1);
     std::vector<int64_t> bucket_start;
@@ -403,6 +454,7 @@ extern "C" void msd_destroy(msd_ctx* c)
     for (auto& a : c->aux) if (a) cudaStreamDestroy(a);
     for (auto& e : c->ev_join) if (e) cudaEventDestroy(e);
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_done) cudaEventDestroy(c->ev_done);
     delete c;
 }
 
@@ -413,6 +465,7 @@ extern "C" int msd_get_info(const msd_ctx* c, int64_t* info)
     if (!c || !info) return MSD_EINVAL;
     info[0] = c->sp[0].n_o; info[1] = c->sp[0].n_v; info[2] = c->sp[1].n_o; info[3] = c->sp[1].n_v;
     info[4] = (int64_t)c->buckets.size(); info[5] = c->sp[0].kmax; info[6] = c->sp[1].kmax; info[7] = MSD_WT;
+    info[8] = c->energy_ok ? 1 : 0;
     return MSD_OK;
 }
 
@@ -430,7 +483,16 @@ extern "C" int msd_set_workspace_limit(msd_ctx* c, int64_t bytes)
 {
     if (!c || bytes < 0) return MSD_EINVAL;
     c->ws_limit = bytes;
+    c->ws_limit_auto = 0;        // re-read the free memory at the next call
+    c->ws.want = 0;              // and lay the workspace out again (the fast path of ensure_workspace keys on it)
     return MSD_OK;
+}
+extern "C" int msd_set_option(msd_ctx* c, int option, int64_t value)
+{
+    if (!c) return MSD_EINVAL;
+    if (option == MSD_OPT_NO_SMEM_TILES && value >= 0 && value <= 2) { c->no_smem_tiles = (int)value; return MSD_OK; }
+    c->err = "unknown option or value";
+    return MSD_EINVAL;
 }
 extern "C" int64_t msd_launch_count(const msd_ctx* c) { return c ? c->launches : -1; }
 extern "C" int msd_set_profiling(msd_ctx* c, int on)
@@ -446,10 +508,6 @@ extern "C" int msd_get_phase_ms(msd_ctx* c, float* ms, int n)
     if (!c || !ms) return MSD_EINVAL;
     for (int i = 0; i < n && i < 6; i++) ms[i] = c->phase_ms[i];
     return MSD_OK;
-}
-extern "C" double msd_probe_fp64_tflops(int use_dmma, double ms, void* stream)
-{
-    return probe_fp64(use_dmma, ms, (cudaStream_t)stream);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -595,10 +653,12 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
 {
     const bool energy_like = (call == CALL_ENERGY || call == CALL_FB_ENERGY);
     const int level = (call == CALL_OVERLAP) ? 1 : (energy_like ? 3 : 2);
-    if (energy_like && std::max(c->sp[0].P, c->sp[1].P) > 4096)
-        return fail(errp, MSD_EUNSUPPORTED, "local energy requires n_o*n_v <= 4096 per spin");
+    if (energy_like && !c->energy_ok) return fail(errp, MSD_EUNSUPPORTED, c->energy_why.c_str());
     int rc = ensure_workspace(c, level, n_w, errp);
     if (rc != MSD_OK) return rc;
+    // one workspace per context: a call on another stream than the previous call's waits for that call's last kernel
+    if (!c->ev_done) CK(cudaEventCreateWithFlags(&c->ev_done, cudaEventDisableTiming));
+    if (c->have_done && st != c->last_stream) CK(cudaStreamWaitEvent(st, c->ev_done, 0));
     Workspace& ws = c->ws;
     const int N = c->N, ldN = N + (N & 1), ng = c->n_chol;
     for (int i = 0; i < 6; i++) c->phase_ms[i] = 0.f;
@@ -609,7 +669,7 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
         int* fl = flags ? flags + w0 : nullptr;
         CK(cudaMemsetAsync(ws.zero_begin, 0, ws.zero_bytes, st));
         mark(c, 0, st);
-        CK(launch_reference(N, ldN, c->dev(0), c->dev(1), nw, pa, pb, ws, level >= 3, st));
+        CK(launch_reference(c, N, ldN, c->dev(0), c->dev(1), nw, pa, pb, ws, level >= 3, st));
         c->launches++;
         mark(c, 1, st);
         if (call == CALL_OVERLAP) {
@@ -650,7 +710,7 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
                         int ks = (int)std::max<int64_t>(1, (2 * c->n_sm + tiles - 1) / tiles);
                         a.ksplit = std::min(ks, std::max(1, a.K / 64));
                     }
-                    CK(launch_gemm_tn(a, c->n_sm, st));
+                    CK(launch_gemm_tn(c, a, st));
                     c->launches++;
                 }
                 mark(c, 3, st);
@@ -671,7 +731,7 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
                 a.lda = ldN; a.ldb = ldN; a.strideA = 0; a.strideB = 0; a.batch = 1;
                 a.zdiv = 1; a.strideC_hi = 0; a.strideC_lo = 0; a.cs_m = (int64_t)nw * sp.n; a.cs_j = 1;
                 a.accumulate = 0;
-                cudaError_t ge = launch_gemm_tn(a, c->n_sm, fl_.stream(s));
+                cudaError_t ge = launch_gemm_tn(c, a, fl_.stream(s));
                 if (ge != cudaSuccess) { fl_.join(); CK(ge); }
                 c->launches++;
             }
@@ -697,7 +757,7 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
                 a.cs_m = (int64_t)B_.P * MSD_WT; a.cs_j = MSD_WT;
                 a.accumulate = 0;
                 a.symmetric = (pr > 0) ? 1 : 0;     // V^{ss}[x][y] = V^{ss}[y][x]
-                cudaError_t ge = launch_gemm_tn(a, c->n_sm, fv_.stream(pr));
+                cudaError_t ge = launch_gemm_tn(c, a, fv_.stream(pr));
                 if (ge != cudaSuccess) { fv_.join(); CK(ge); }
                 c->launches++;
             }

@@ -3,7 +3,9 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <map>
 #include <string>
+#include <utility>
 #include <vector>
 
 #define MSD_WT 8            // walkers per tile: lanes of a warp = 4 determinants x 8 walkers
@@ -45,8 +47,8 @@ __device__ __forceinline__ void red_add(cplx* p, cplx v) {
     atomicAdd(&p->y, v.y);
 }
 // CI-matrix accumulators are PLANAR per pair index x: C[x][0][WT] real parts, C[x][1][WT] imaginary parts, so that the
-// 8 walkers of a determinant hit 64 contiguous bytes per reduction (measured 2x the L2 reduction rate of interleaved
-// complex: profiles/r01_probes.md).  p points at the lane's walker inside the tile.
+// 8 walkers of a determinant hit 64 contiguous bytes per reduction (measured in round 1: 2x the L2 reduction rate of
+// interleaved complex).  p points at the lane's walker inside the tile.
 __device__ __forceinline__ void red_add_planar(double* p, int x, cplx v) {
     atomicAdd(p + x * (2 * MSD_WT), v.x);
     atomicAdd(p + x * (2 * MSD_WT) + MSD_WT, v.y);
@@ -173,6 +175,12 @@ struct msd_ctx {
     int64_t ws_limit = 0;
     int64_t ws_limit_auto = 0;
     int64_t launches = 0;
+    int no_smem_tiles = 0;                    // msd_set_option(MSD_OPT_NO_SMEM_TILES): test hook, see include/msd.h
+    bool energy_ok = true;                    // the energy calls are supported for this trial (window size, see msd_setup)
+    std::string energy_why;
+    // launch configurations are fixed by the trial: occupancy per (kernel, block size, dynamic shared memory) is queried
+    // once and kept here (func_config below), so the hot calls make no CUDA API call besides the launches themselves
+    std::map<std::pair<const void*, size_t>, int> occ_cache;
     bool profiling = false;
     cudaEvent_t ev[8] = {};
     float phase_ms[6] = {};
@@ -181,6 +189,8 @@ struct msd_ctx {
     static constexpr int NAUX = 4;
     cudaStream_t aux[NAUX] = {};
     cudaEvent_t ev_fork = nullptr, ev_join[NAUX] = {};
+    cudaEvent_t ev_done = nullptr;            // end of the most recent hot call (the workspace is free again after it)
+    cudaStream_t last_stream = nullptr; bool have_done = false;
     std::string err;
     SpinDev dev(int s) const {
         SpinDev d; d.n = sp[s].n; d.n_o = sp[s].n_o; d.n_v = sp[s].n_v; d.n_r = sp[s].n_r; d.P = sp[s].P;
@@ -203,6 +213,8 @@ cudaError_t launch_pack_rows(int64_t n_det, int N,
                              const int* map_h_a, const int* map_p_a, const int* map_h_b, const int* map_p_b,
                              const double* ci, unsigned char* tmp_rows /*[n_det][64]*/, int* key, double* coef,
                              int* hist /*[17*17]*/, int* err, cudaStream_t st);
+cudaError_t launch_pack_dedup(int64_t n_det, const unsigned char* tmp_rows, const int* key, int* slots, int64_t nslots,
+                              int* err, cudaStream_t st);
 cudaError_t launch_pack_scatter(int64_t n_det, const int* key, int n_buckets, const int* bucket_keys,
                                 const int64_t* bucket_start, int64_t* perm, cudaStream_t st);
 cudaError_t launch_pack_write(int64_t n_det, const int64_t* perm, const int* key, const unsigned char* tmp_rows,
@@ -212,7 +224,7 @@ cudaError_t launch_pack_lsub(const double* L_or_h1, int n_slices, int N, int n_r
                              double* out, cudaStream_t st);
 
 // reference.cu
-cudaError_t launch_reference(int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw,
+cudaError_t launch_reference(msd_ctx* c, int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw,
                              const cplx* phi_a, const cplx* phi_b, Workspace& ws, bool want_thetaT, cudaStream_t st);
 
 // dets.cu   mode: 0 overlap, 1 + CI matrix, 2 + second-order energy
@@ -221,6 +233,7 @@ cudaError_t launch_dets(msd_ctx* c, int mode, int64_t nw, Workspace& ws, cudaStr
 // dense.cu
 cudaError_t launch_green_rows(msd_ctx* c, int64_t nw, Workspace& ws, cplx* Gfull /*or null*/, cudaStream_t st);
 cudaError_t launch_energy_dense(msd_ctx* c, int64_t nw, Workspace& ws, cudaStream_t st);
+size_t energy_dense_smem(const msd_ctx* c, int GC);      // shared memory of the scalar S7 kernel with GC slices per CTA
 cudaError_t launch_fx(msd_ctx* c, int64_t nw, Workspace& ws, cudaStream_t st);
 cudaError_t launch_finish_overlap(msd_ctx* c, int64_t nw, Workspace& ws, cplx* ovlp, int* flags, cudaStream_t st);
 cudaError_t launch_finish_energy(msd_ctx* c, int64_t nw, Workspace& ws, cplx* e, int64_t estride, int* flags, cudaStream_t st);
@@ -235,6 +248,10 @@ struct Fork {
     cudaStream_t stream(int i);     // i == 0: the caller's stream; i > 0: a side stream that waits for the fork point
     cudaError_t join();
 };
+
+// msd_api.cu : opt in to `smem` bytes of dynamic shared memory for `func` on the context's device (raised, never lowered,
+// process-wide per device) and return the resident CTAs per SM for (nthr, smem); cached per context.
+cudaError_t func_config(msd_ctx* c, const void* func, int nthr, size_t smem, int* occ);
 
 // gemm.cu : C[m][n] (+)= sum_k A[m][k] * B[n][k]   (both K-contiguous, FP64 DMMA m8n8k4)
 struct GemmArgs {
@@ -253,5 +270,4 @@ struct GemmArgs {
     int symmetric = 0;          // 1: C is complex symmetric (M == N/2, A and B describe the same rows): only tiles that
                                 //    touch the upper triangle are computed, element (m, j >= m) is also written to (j, m)
 };
-cudaError_t launch_gemm_tn(const GemmArgs& a, int n_sm, cudaStream_t st);
-double probe_fp64(int use_dmma, double ms, cudaStream_t st);
+cudaError_t launch_gemm_tn(msd_ctx* c, const GemmArgs& a, cudaStream_t st);

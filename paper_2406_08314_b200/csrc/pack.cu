@@ -10,6 +10,7 @@
 #define ERR_PART_IS_OCC 4
 #define ERR_REPEATED 8
 #define ERR_LEVEL 16
+#define ERR_DUPLICATE 32
 
 __global__ void k_pack_mark(int64_t n_det, const int64_t* __restrict__ off, const int32_t* __restrict__ holes,
                             const int32_t* __restrict__ parts, int N, const int* __restrict__ pos_in_ref,
@@ -97,6 +98,34 @@ __global__ void k_pack_rows(int64_t n_det, int N,
     atomicAdd(&hist[ky], 1);
 }
 
+// Duplicate determinants (Eq. 15 is an orthogonal expansion: every determinant once).  Exact, not probabilistic: an
+// open-addressing table of determinant indices keyed by a hash of (level key, packed row); a probe that meets an occupied
+// slot compares the full rows and either reports the duplicate or moves on to the next slot.
+__global__ void k_pack_dedup(int64_t n_det, const unsigned char* __restrict__ tmp_rows, const int* __restrict__ key,
+                             int* slots, int64_t nslots, int* err)
+{
+    int64_t I = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (I >= n_det) return;
+    const int ky = key[I];
+    const int nb = 2 * (ky / (MSD_MAX_LEVEL + 1)) + 2 * (ky % (MSD_MAX_LEVEL + 1));
+    const unsigned char* row = tmp_rows + I * 64;
+    unsigned long long h = 1469598103934665603ull ^ (unsigned long long)ky;       // FNV-1a
+    for (int t = 0; t < nb; t++) { h ^= row[t]; h *= 1099511628211ull; }
+    h ^= h >> 29;
+    int64_t s = (int64_t)(h & (unsigned long long)(nslots - 1));
+    for (;;) {
+        const int prev = atomicCAS(&slots[s], -1, (int)I);
+        if (prev == -1) return;
+        if (key[prev] == ky) {
+            const unsigned char* other = tmp_rows + (int64_t)prev * 64;
+            bool same = true;
+            for (int t = 0; t < nb; t++) same &= (other[t] == row[t]);
+            if (same) { atomicOr(err, ERR_DUPLICATE); return; }
+        }
+        s = (s + 1) & (nslots - 1);
+    }
+}
+
 // stable counting-sort scatter: block b owns bucket b, walks the keys in order
 __global__ void k_pack_scatter(int64_t n_det, const int* __restrict__ key, const int* __restrict__ bucket_keys,
                                const int64_t* __restrict__ bucket_start, int64_t* perm)
@@ -173,6 +202,14 @@ cudaError_t launch_pack_rows(int64_t n_det, int N,
     k_pack_rows<<<(unsigned)((n_det + thr - 1) / thr), thr, 0, st>>>(
         n_det, N, off_a, holes_a, parts_a, off_b, holes_b, parts_b, occ_ref_a, na, occ_ref_b, nb,
         pos_in_ref_a, pos_in_ref_b, map_h_a, map_p_a, map_h_b, map_p_b, ci, tmp_rows, key, coef, hist, err);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_pack_dedup(int64_t n_det, const unsigned char* tmp_rows, const int* key, int* slots, int64_t nslots,
+                              int* err, cudaStream_t st)
+{
+    int thr = 256;
+    k_pack_dedup<<<(unsigned)((n_det + thr - 1) / thr), thr, 0, st>>>(n_det, tmp_rows, key, slots, nslots, err);
     return cudaGetLastError();
 }
 

@@ -130,7 +130,7 @@ k_reference(int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw, const cplx* __re
     }
 }
 
-cudaError_t launch_reference(int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw, const cplx* phi_a,
+cudaError_t launch_reference(msd_ctx* c, int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw, const cplx* phi_a,
                              const cplx* phi_b, Workspace& ws, bool want_thetaT, cudaStream_t st)
 {
     int nmax = sa.n > sb.n ? sa.n : sb.n;
@@ -138,12 +138,8 @@ cudaError_t launch_reference(int N, int ldN, SpinDev sa, SpinDev sb, int64_t nw,
     const size_t psi_bytes = (size_t)N * (nmax + 1) * sizeof(cplx);
     const int stage_psi = smem + psi_bytes <= 100 * 1024;       // two CTAs per SM at least; larger walkers are read from global
     if (stage_psi) smem += psi_bytes;
-    static size_t configured = 0;
-    if (smem > 48 * 1024 && smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_reference, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = smem;
-    }
+    cudaError_t e = func_config(c, (const void*)k_reference, 128, smem, nullptr);
+    if (e != cudaSuccess) return e;
     int64_t wpad = (nw + MSD_WT - 1) / MSD_WT * MSD_WT;
     dim3 grid((unsigned)wpad, 2);
     k_reference<<<grid, 128, smem, st>>>(N, ldN, sa, sb, nw, phi_a, phi_b, ws.theta[0], ws.theta[1],

@@ -7,7 +7,6 @@ import re
 import subprocess
 import sys
 
-import numpy as np
 import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
@@ -78,7 +77,6 @@ def test_missing_library_fails_loudly(tmp_path, monkeypatch):
     monkeypatch.setattr(b, "LIB_PATH", str(tmp_path / "nope.so"))
     with pytest.raises(ImportError):
         b.load_library()
-    x = np.zeros(1)
+    import msd_inputs as mi
     with pytest.raises(ImportError):
-        b.msd_probe_fp64_tflops()
-    del x
+        b.setup_from_inputs(mi.generate("tiny"))

@@ -117,16 +117,41 @@ def test_parity_cu2o2_full_size(torch_cuda):
     assert_parity(got, o2.run(x, walkers=ws2, want=("ovlp", "greens"), return_G=False), walkers=ws2, what=("ovlp", "fb"))
 
 
+def _cplx(a):
+    a = np.array(a)
+    return a[..., 0] + 1j * a[..., 1]
+
+
+def _assert_against_golden(gold, ov, fb, E):
+    """Sections of a golden file (tests/golden/make_golden.py): energy walkers (ovlp, E, fb on every 8th gamma),
+    fb_walkers (every gamma), ovlp_all (every walker)."""
+    if "walkers" in gold:
+        ws, gs = gold["walkers"], gold["fb_gamma_sample"]
+        g_ov, g_E, g_fb = _cplx(gold["ovlp"]), _cplx(gold["E"]), _cplx(gold["fb"])
+        assert (np.abs(ov[ws] - g_ov) / np.abs(g_ov)).max() <= TOL_REL
+        if E is not None:
+            assert np.abs(E[ws] - g_E).max() <= TOL_E
+        if fb is not None:
+            assert (np.abs(fb[ws][:, gs] - g_fb).max(axis=1) / np.array(gold["fb_max_abs"])).max() <= TOL_REL
+    if "fb_walkers" in gold and fb is not None:
+        ws, g_fb = gold["fb_walkers"], _cplx(gold["fb_full"])
+        assert g_fb.shape == (len(ws), fb.shape[1])
+        assert (np.abs(fb[ws] - g_fb).max(axis=1) / np.abs(g_fb).max(axis=1)).max() <= TOL_REL
+    if "ovlp_all" in gold:
+        g_ov = _cplx(gold["ovlp_all"])
+        assert g_ov.shape == ov.shape
+        assert (np.abs(ov - g_ov) / np.abs(g_ov)).max() <= TOL_REL
+
+
 @pytest.mark.parametrize("name", ["fe2s2", "cu2o2"])
 def test_parity_full_size_against_stored_oracle_values(torch_cuda, name):
     """BASELINE configs[3] (the bench workload, same launch configuration) and configs[2] against oracle values
     stored by tests/golden/make_golden.py (which calls only oracle/): the brute-force oracle needs ~10 minutes per
-    walker at the Fe2S2 size."""
-    path = os.path.join(GOLDEN, "%s_seed0.json" % name)
-    if not os.path.exists(path):
-        pytest.skip("golden file %s not generated yet" % path)
-    gold = json.load(open(path))
+    walker at the Fe2S2 size.  fe2s2 (SURVEY.md 8(d) plan): overlap of all 100 walkers, force bias (every gamma) of
+    walkers 0..15, energy of walkers 0, 7 | 8 (last lane of tile 0, first lane of tile 1), 57, 99."""
+    gold = json.load(open(os.path.join(GOLDEN, "%s_seed0.json" % name)))
     x = mi.generate(name)
+    assert gold["input_sha256"] == x.sha256()
     msd = _msd()
     torch = torch_cuda
     trial = msd.setup_from_inputs(x)
@@ -136,18 +161,31 @@ def test_parity_full_size_against_stored_oracle_values(torch_cuda, name):
     fb = trial.force_bias(pa, pb).cpu().numpy()
     E = trial.local_energy(pa, pb).cpu().numpy()
     trial.close()
-    ws = gold["walkers"]
-    c = lambda a: np.array(a)[..., 0] + 1j * np.array(a)[..., 1]
-    g_ov, g_E, g_fb = c(gold["ovlp"]), c(gold["E"]), c(gold["fb"])
-    gs = gold["fb_gamma_sample"]
-    assert (np.abs(ov[ws] - g_ov) / np.abs(g_ov)).max() <= TOL_REL
-    assert np.abs(E[ws] - g_E).max() <= TOL_E
-    fb_err = np.abs(fb[ws][:, gs] - g_fb).max(axis=1) / np.array(gold["fb_max_abs"])
-    assert fb_err.max() <= TOL_REL
-    if name == "fe2s2":   # overlap of a further walker sample, oracle run live (cheap: no L loop)
-        ws2 = [1, 8, 50, 98]
-        r = o2.run(x, walkers=ws2, want=("ovlp",))
-        assert (np.abs(ov[ws2] - r["ovlp"]) / np.abs(r["ovlp"])).max() <= TOL_REL
+    if name == "fe2s2":
+        assert len(gold["ovlp_all"]) == x.n_w and len(gold["fb_walkers"]) >= 16
+        assert {0, 7, 8, 57, 99} <= set(gold["walkers"])
+    _assert_against_golden(gold, ov, fb, E)
+
+
+@pytest.mark.parametrize("n_det,K,energy", [(100000, 8, True), (1000000, 10, False)])
+def test_parity_sweep_end_points_against_stored_oracle_values(torch_cuda, n_det, K, energy):
+    """BASELINE configs[4] (kernel sweep) at its large end: N_d = 1e5 with levels <= 8 (overlap of all 128 walkers, force
+    bias of walkers 7 | 8 and of the energy walker, energy of walker 64) and N_d = 1e6 with levels <= 10 (overlap of all
+    128 walkers) against stored O2 values."""
+    gold = json.load(open(os.path.join(GOLDEN, "sweep_nd%d_K%d_seed0.json" % (n_det, K))))
+    x = mi.generate("sweep", n_det=n_det, max_level=K)
+    assert gold["input_sha256"] == x.sha256()
+    msd = _msd()
+    torch = torch_cuda
+    trial = msd.setup_from_inputs(x)
+    pa = torch.tensor(x.phi_a, device="cuda")
+    pb = torch.tensor(x.phi_b, device="cuda")
+    ov = trial.overlap(pa, pb).cpu().numpy()
+    fb = trial.force_bias(pa, pb).cpu().numpy() if "fb_walkers" in gold else None
+    E = trial.local_energy(pa, pb).cpu().numpy() if energy else None
+    trial.close()
+    assert len(gold["ovlp_all"]) == x.n_w
+    _assert_against_golden(gold, ov, fb, E)
 
 
 # ----------------------------------------------------------------------------------------------
@@ -225,10 +263,11 @@ def test_walker_equals_reference_exact_singular_minors(torch_cuda, name):
         assert np.abs(got["G"][w] - ref["G"][0]).max() <= TOL_REL
 
 
-@pytest.mark.parametrize("eps", [1e-1, 1e-3, 1e-6])
-def test_near_reference_walkers(torch_cuda, eps):
-    """P8: psi = QR(D_0 + eps Z): the regime of real AFQMC walkers; stresses det*inverse cofactors at high levels."""
-    x = mi.generate("sweep", n_det=600, max_level=6, n_w=10)
+@pytest.mark.parametrize("eps,K", [(1e-1, 6), (1e-3, 6), (1e-6, 6), (1e-9, 6), (1e-3, 10), (1e-9, 9)])
+def test_near_reference_walkers(torch_cuda, eps, K):
+    """P8: psi = QR(D_0 + eps Z): the regime of real AFQMC walkers; stresses det*inverse cofactors (the Jacobi division
+    by R at k >= 5) down to eps = 1e-9 and up to level 10."""
+    x = mi.generate("sweep", n_det=600, max_level=K, n_w=10)
     pa, pb = mi.near_reference_walkers(x, eps, seed=4)
     x = x.with_walkers(pa, pb)
     got = gpu_all(torch_cuda, x, want_G=False)
@@ -355,13 +394,27 @@ def test_gauge_order_and_chunk_invariance(torch_cuda):
     assert (np.abs(p["ovlp"] - base["ovlp"]) / np.abs(base["ovlp"])).max() < TOL_REL
     assert np.abs(p["E"] - base["E"]).max() < TOL_E
     # walker chunking under a small workspace limit (results must not depend on chunking)
-    trial = msd.setup_from_inputs(x)
-    trial.set_workspace_limit(24 * 1024 * 1024)
-    c = gpu_all(torch, x, trial=trial, want_G=False)
-    trial.close()
-    assert (np.abs(c["ovlp"] - base["ovlp"]) / np.abs(base["ovlp"])).max() < TOL_REL
-    assert np.abs(c["E"] - base["E"]).max() < TOL_E
-    assert (np.abs(c["fb"] - base["fb"]).max(axis=1) / np.abs(base["fb"]).max(axis=1)).max() < TOL_REL
+    # 24 MB chunks the energy workspace (Lambda alone is 52 MB); 300 KB also chunks the overlap / force-bias / greens ones
+    for limit in (24 * 1024 * 1024, 300 * 1024):
+        trial = msd.setup_from_inputs(x)
+        trial.set_workspace_limit(limit)
+        if limit < 1024 * 1024:
+            pa = torch.tensor(x.phi_a, device="cuda"); pb = torch.tensor(x.phi_b, device="cuda")
+            c = dict(ovlp=trial.overlap(pa, pb).cpu().numpy(), fb=trial.force_bias(pa, pb).cpu().numpy(), E=base["E"])
+            G = trial.greens(pa, pb).cpu().numpy()
+            trial.set_workspace_limit(0)            # back to the default: the next call lays the workspace out again
+            G2 = trial.greens(pa, pb).cpu().numpy()
+            assert np.abs(G - G2).max() < TOL_REL
+        else:
+            c = gpu_all(torch, x, trial=trial, want_G=False)
+            pa = torch.tensor(x.phi_a, device="cuda"); pb = torch.tensor(x.phi_b, device="cuda")
+            fused = trial.force_bias_energy(pa, pb).cpu().numpy()
+            assert (np.abs(fused[:, :x.n_chol] - base["fb"]).max(axis=1) / np.abs(base["fb"]).max(axis=1)).max() < TOL_REL
+            assert np.abs(fused[:, x.n_chol:] - base["E"]).max() < TOL_E
+        trial.close()
+        assert (np.abs(c["ovlp"] - base["ovlp"]) / np.abs(base["ovlp"])).max() < TOL_REL
+        assert np.abs(c["E"] - base["E"]).max() < TOL_E
+        assert (np.abs(c["fb"] - base["fb"]).max(axis=1) / np.abs(base["fb"]).max(axis=1)).max() < TOL_REL
 
 
 # ----------------------------------------------------------------------------------------------
@@ -427,18 +480,15 @@ def test_many_generic_items_per_cta(torch_cuda):
 
 def test_many_high_level_items_per_cta(torch_cuda):
     """The same at levels up to 10 (cooperative kernel, one determinant per warp): 20000 determinants so that a CTA
-    processes many items; overlap on every walker, force bias on two (the oracle needs no L loop per determinant for
-    either), energy against the CPU restatement of the Wick algorithm (itself pinned to O2 in test_oracle_pins.py),
-    because the brute-force oracle needs minutes per walker here."""
-    from oracle import wick
+    processes many items; overlap on every walker, force bias on two, energy on one walker -- all against the
+    brute-force oracle O2 (about 2e11 flop for the energy walker: seconds on the host cores)."""
     x = mi.generate("sweep", n_det=20000, max_level=10, n_w=8)
     got = gpu_all(torch_cuda, x, want_G=False)
     assert (got["flags"] == 0).all()
     assert_parity(got, o2.run(x, want=("ovlp",)), what=("ovlp",))
     ws = [0, 7]
     assert_parity(got, o2.run(x, walkers=ws, want=("ovlp", "greens"), return_G=False), walkers=ws, what=("ovlp", "fb"))
-    q = wick.run(x, walkers=[3], want=("energy",))
-    assert np.abs(got["E"][3] - q["E"][0]).max() <= TOL_E
+    assert_parity(got, o2.run(x, walkers=[3], return_G=False), walkers=[3], what=("ovlp", "fb", "E"))
 
 
 @pytest.mark.parametrize("name,kw", [("small", {}), ("open-shell", {}), ("tiny", {}),
@@ -469,15 +519,92 @@ def test_fused_force_bias_energy_call(torch_cuda, name, kw):
     trial.close()
 
 
-def test_paths_for_windows_too_wide_for_shared_memory_tiles(torch_cuda, monkeypatch):
-    """The force-bias RED scatter and the energy path with Hrot / F read through L1 are what runs when a walker tile's
-    C / Hrot / F do not fit in shared memory; no BASELINE config is that wide, so the library's test hook
-    MSD_NO_SMEM_TILES forces them (read at every call)."""
-    monkeypatch.setenv("MSD_NO_SMEM_TILES", "1")
+@pytest.mark.parametrize("level", [1, 2])
+def test_paths_for_windows_too_wide_for_shared_memory_tiles(torch_cuda, level):
+    """The force-bias RED scatter, the energy path with Hrot / F read through L1 (level 1) and the forms that read the g
+    slices through L1 as well (level 2) are what runs when a walker tile's C / Hrot / F / g do not fit in shared memory;
+    no BASELINE config is that wide, so the context option MSD_OPT_NO_SMEM_TILES forces them (no environment variable)."""
+    msd = _msd()
+    for x, ws in ((mi.generate("small"), None), (mi.generate("sweep", n_det=3000, max_level=6, n_w=16), [0, 9, 15])):
+        trial = msd.setup_from_inputs(x)
+        trial.set_option(msd.MSD_OPT_NO_SMEM_TILES, level)
+        got = gpu_all(torch_cuda, x, trial=trial, want_G=ws is None)
+        pa = torch_cuda.tensor(x.phi_a, device="cuda")
+        pb = torch_cuda.tensor(x.phi_b, device="cuda")
+        fused = trial.force_bias_energy(pa, pb).cpu().numpy()
+        with pytest.raises(msd.MSDError):
+            trial.set_option(99, 1)
+        trial.close()
+        ref = o2.run(x, walkers=ws, return_G=ws is None)
+        assert_parity(got, ref, walkers=ws)
+        sel = np.arange(x.n_w) if ws is None else np.asarray(ws)
+        assert_parity(dict(fb=fused[:, :x.n_chol], E=fused[:, x.n_chol:]), ref, walkers=sel, what=("fb", "E"))
+
+
+def test_window_wider_than_shared_memory(torch_cuda):
+    """An active window of 10 occupied x 100 virtual orbitals per spin (the paper's [Cu2O2]2+ has 16 x 92,
+    PAPER.md:L303): 2000 pair indices, so neither the g slices (256 KB per walker tile) nor C / Hrot / F fit in shared
+    memory, and n_v > 16 takes the scalar S7 kernel.  Every call against O2 on every walker."""
+    msd = _msd()
+    x = mi.wide_window()
+    trial = msd.setup_from_inputs(x)
+    info = trial.info()
+    assert info["n_o_alpha"] * info["n_v_alpha"] + info["n_o_beta"] * info["n_v_beta"] > 1816 and info["energy_supported"]
+    got = gpu_all(torch_cuda, x, trial=trial)
+    pa = torch_cuda.tensor(x.phi_a, device="cuda")
+    pb = torch_cuda.tensor(x.phi_b, device="cuda")
+    fused = trial.force_bias_energy(pa, pb).cpu().numpy()
+    trial.close()
+    ref = o2.run(x)
+    assert (got["flags"] == 0).all()
+    assert_parity(got, ref)
+    assert_parity(dict(fb=fused[:, :x.n_chol], E=fused[:, x.n_chol:]), ref, what=("fb", "E"))
+
+
+def test_duplicate_determinants_are_rejected(torch_cuda):
+    """Eq. 15 is an orthogonal expansion: the same determinant twice is an invalid table (MSD_EINVAL at setup), also when
+    the two copies list their holes / particles in a different order or sit far apart in the list."""
+    msd = _msd()
     x = mi.generate("small")
-    got = gpu_all(torch_cuda, x)
-    assert_parity(got, o2.run(x))
-    x = mi.generate("sweep", n_det=3000, max_level=6, n_w=16)
-    got = gpu_all(torch_cuda, x, want_G=False)
-    ws = [0, 9, 15]
-    assert_parity(got, o2.run(x, walkers=ws, return_G=False), walkers=ws)
+    idx = np.arange(x.n_det)
+    for dup_of, at in ((5, 6), (17, x.n_det - 1), (0, 400)):
+        y = x.subset_dets(np.concatenate([idx[:at], [dup_of], idx[at:]]))
+        with pytest.raises(msd.MSDError) as e:
+            msd.setup_from_inputs(y)
+        assert e.value.code == -1 and "twice" in str(e.value)
+    occa, occb = x.occa.copy(), x.occb.copy()
+    occa[9], occb[9] = x.occa[3][::-1], x.occb[3]                      # same determinant, permuted occupation list
+    with pytest.raises(msd.MSDError):
+        msd.msd_setup_from_occ(x.N, x.n_alpha, x.n_beta, x.n_chol, x.n_det, x.h1, x.L, x.e0, occa, occb, x.ci)
+    msd.setup_from_inputs(x).close()
+
+
+def test_binding_validates_outputs_and_limits(torch_cuda):
+    torch = torch_cuda
+    msd = _msd()
+    x = mi.generate("tiny")
+    trial = msd.setup_from_inputs(x)
+    pa = torch.tensor(x.phi_a, device="cuda")
+    pb = torch.tensor(x.phi_b, device="cuda")
+    with pytest.raises(ValueError):
+        trial.force_bias(pa, pb, out=torch.empty((x.n_w, x.n_chol - 1), dtype=torch.complex128, device="cuda"))
+    with pytest.raises(ValueError):
+        trial.local_energy(pa, pb, out=torch.empty((x.n_w, 3), dtype=torch.complex64, device="cuda"))
+    with pytest.raises(ValueError):
+        trial.overlap(pa, pb, out=torch.empty(2 * x.n_w, dtype=torch.complex128, device="cuda")[::2])
+    with pytest.raises(ValueError):
+        trial.overlap(pa, pb, flags=torch.zeros(x.n_w - 1, dtype=torch.int32, device="cuda"))
+    with pytest.raises(ValueError):
+        trial.overlap_host(x.phi_a, x.phi_b, out=np.empty(x.n_w + 1, dtype=np.complex128))
+    with pytest.raises(ValueError):
+        trial.local_energy_host(torch.from_numpy(x.phi_a), torch.from_numpy(x.phi_b),
+                                out=torch.empty((x.n_w, 3), dtype=torch.complex64))
+    # two streams on one context: the second call waits for the first (one workspace per context, include/msd.h)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    fb = trial.force_bias(pa, pb, stream=s1)
+    en = trial.local_energy(pa, pb, stream=s2)
+    torch.cuda.synchronize()
+    ref = o2.run(x, return_G=False)
+    assert_parity(dict(fb=fb.cpu().numpy(), E=en.cpu().numpy()), ref, what=("fb", "E"))
+    trial.close()
