@@ -369,63 +369,113 @@ __global__ void __launch_bounds__(NTHR, MINB) k_dets_cf(DetsParams p, const Work
 }
 
 // ------------------------------------------------------------------------------------------------
-// Force-bias mode of the closed-form levels with the CI reduction done by owner slots in shared memory
-// (msd_internal.cuh C1_*): no RED.ADD.F64 per entry, one flush of the CTA's C tile at the end.
-// g is read through L1 (57 KB per tile, nothing else competes for L1 in this mode); shared memory holds the
-// CTA's C tile [(P_a + P_b)][WT] complex and the round's products val[e][slot][WT].
+// Force-bias mode of the closed-form levels: CI reduction by OWNER PULL (msd_internal.cuh PULL_*).  Nothing is scattered:
+//   pass A  thread = (determinant, walker): R^a, R^b (levels <= 2: determinant only; levels 3, 4: determinant and adjugate by
+//           the division-free closed forms, adjugate left UNSCALED in shared memory), W += c~ R^a R^b, and the two scale
+//           factors c~ R^b (for alpha entries), c~ R^a (for beta entries) to shared memory;
+//   pass B  lane group q (8 walkers) walks piece q of the chunk's entry list, which the setup sorted by pair index x and cut at
+//           changes of x: the sum of an x-run stays in registers and is added to the CTA's C tile once, by its only owner.
+// Replaces round 1's k_dets_c1 (products staged per round of 32-96 determinants, owner lists by x mod S read entry by entry
+// with a shared-memory read-modify-write each: 2.0 ms at fe2s2, FP64 pipe 10-20 %).
 // ------------------------------------------------------------------------------------------------
+template <int K> __device__ __forceinline__ cplx det_only(const cplx (*M)[K > 0 ? K : 1])
+{
+    if constexpr (K == 0) return cmake(1.0, 0.0);
+    else if constexpr (K == 1) return M[0][0];
+    else return minor2(M[0][0], M[0][1], M[1][0], M[1][1]);
+}
+
+// byte `i` (compile-time after unrolling) of a table row held in registers as 32-bit words
+template <int NWORD> __device__ __forceinline__ int row_byte(const uint32_t (&w)[NWORD], int i)
+{
+    return (int)((w[i >> 2] >> (8 * (i & 3))) & 255u);
+}
+
+// one spin of pass A: gather, determinant; levels >= 3 also leave the adjugate, element a*K+b = A[b][a], at
+// stage[(a*K+b) * stride]  (stride = 8 x determinants of the chunk: consecutive threads -> consecutive 16-byte words)
+template <int K, int OFF, int NWORD>
+__device__ __forceinline__ cplx pull_spin(const uint32_t (&w)[NWORD], const cplx* g, int no, cplx* stage, int stride)
+{
+    constexpr int K1 = K > 0 ? K : 1;
+    cplx M[K1][K1];
+    int h[K1], pn[K1];
+#pragma unroll
+    for (int a = 0; a < K; a++) { h[a] = row_byte(w, OFF + a); pn[a] = row_byte(w, OFF + K + a) * no; }
+#pragma unroll
+    for (int a = 0; a < K; a++)
+#pragma unroll
+        for (int b = 0; b < K; b++) M[a][b] = g[(pn[b] + h[a]) * MSD_WT];
+    if constexpr (K <= 2) return det_only<K>(M);
+    else {
+        cplx A[K1][K1];
+        const cplx R = Closed<K>::det_adj(M, A);
+#pragma unroll
+        for (int a = 0; a < K; a++)
+#pragma unroll
+            for (int b = 0; b < K; b++) stage[(a * K + b) * stride] = A[b][a];
+        return R;
+    }
+}
+
 template <int KA, int KB>
-__device__ __forceinline__ void c1_round(const DetsParams& p, const WorkItem& it, int i, int slot, int S, int j,
-                                         const cplx* gA, const cplx* gB, cplx* val, cplx& Wl)
+__device__ __forceinline__ void pull_pass_a(const DetsParams& p, const WorkItem& it, int slot, int nslots, int j, const cplx* gA,
+                                            const cplx* gB, cplx* sR, cplx* stage, cplx& Wl)
 {
     constexpr int NB = 2 * KA + 2 * KB;
     constexpr int NWORD = (NB + 3) / 4 > 0 ? (NB + 3) / 4 : 1;
-    uint32_t w[NWORD];
-    const uint32_t* rp = reinterpret_cast<const uint32_t*>(p.tab + it.tab_off + (int64_t)i * it.rs);
+    constexpr int EA = KA >= 3 ? KA * KA : 0;
+    const unsigned char* tab = p.tab + it.tab_off;
+    const double* coef = p.coef + it.det_begin;
+    const int stride = it.det_count * MSD_WT;
+    for (int i = slot; i < it.det_count; i += nslots) {
+        uint32_t w[NWORD];
+        const uint32_t* rp = reinterpret_cast<const uint32_t*>(tab + (int64_t)i * it.rs);
 #pragma unroll
-    for (int t = 0; t < NWORD; t++) w[t] = (NB > 0) ? __ldg(rp + t) : 0u;
-    const double cf = __ldg(p.coef + it.det_begin + i);
-    const unsigned char* rb = reinterpret_cast<const unsigned char*>(w);
-    SpinEval<KA, 1> ea;
-    SpinEval<KB, 1> eb;
-    ea.run(rb, gA, p.no[0], nullptr, 0u);
-    eb.run(rb + 2 * KA, gB, p.no[1], nullptr, 0u);
-    const cplx cRa = cscale(cf, ea.R), cRb = cscale(cf, eb.R);
-    Wl = cfma(cRa, eb.R, Wl);
-    cplx* v = val + slot * MSD_WT + j;
-#pragma unroll
-    for (int a = 0; a < KA; a++)
-#pragma unroll
-        for (int b = 0; b < KA; b++) v[(a * KA + b) * S * MSD_WT] = cmul(cRb, ea.A[b][a]);
-#pragma unroll
-    for (int a = 0; a < KB; a++)
-#pragma unroll
-        for (int b = 0; b < KB; b++) v[(KA * KA + a * KB + b) * S * MSD_WT] = cmul(cRa, eb.A[b][a]);
+        for (int t = 0; t < NWORD; t++) w[t] = (NB > 0) ? __ldg(rp + t) : 0u;
+        const double cf = __ldg(coef + i);
+        cplx* st = stage + i * MSD_WT + j;
+        const cplx Ra = pull_spin<KA, 0>(w, gA, p.no[0], st, stride);
+        const cplx Rb = pull_spin<KB, 2 * KA>(w, gB, p.no[1], st + EA * stride, stride);
+        const cplx cRa = cscale(cf, Ra), cRb = cscale(cf, Rb);
+        Wl = cfma(cRa, Rb, Wl);
+        sR[(i * 2 + 0) * MSD_WT + j] = cRb;       // scale of the alpha entries
+        sR[(i * 2 + 1) * MSD_WT + j] = cRa;       // scale of the beta entries
+    }
 }
 
-#define C1_CASE(KA_, KB_)                                                                              \
+__device__ __forceinline__ cplx flip(cplx v, uint32_t neg)       // neg = 0 or 1: integer sign flip, keeps the FP64 pipe free
+{
+    const long long m = (long long)neg << 63;
+    return make_double2(__longlong_as_double(__double_as_longlong(v.x) ^ m), __longlong_as_double(__double_as_longlong(v.y) ^ m));
+}
+
+#define PULL_CASE(KA_, KB_)                                                                            \
     case KA_ * 5 + KB_:                                                                                \
         if constexpr ((KA_ > KB_ ? KA_ : KB_) > KLO && (KA_ > KB_ ? KA_ : KB_) <= KHI)                  \
-            c1_round<KA_, KB_>(p, it, i, slot, S, j, gA, gB, val, Wl);                                  \
+            pull_pass_a<KA_, KB_>(p, it, slot, NTHR / MSD_WT, j, gA, gB, sR, stage, Wl);               \
         break;
 
-template <int KLO, int KHI, int NTHR, bool GS>
-__global__ void __launch_bounds__(NTHR, 1) k_dets_c1(DetsParams p, const WorkItem* __restrict__ items, int n_items,
-                                                     const uint32_t* __restrict__ sched)
+// class (KLO, KHI] of the larger level; GS: the tile's g slices are staged in shared memory (else read through L1)
+template <int NTHR, int KLO, int KHI, bool GS>
+__global__ void __launch_bounds__(NTHR, 1) k_dets_pull(DetsParams p, const WorkItem* __restrict__ items, int n_items,
+                                                       const unsigned short* __restrict__ pull_off,
+                                                       const uint2* __restrict__ pull_ent, int pool_bytes)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int S = NTHR / MSD_WT;
-    const int HW = c1_hdr_words(S);
-    cplx* Csm = reinterpret_cast<cplx*>(smem_raw);                  // [(P_a + P_b)][WT]
+    constexpr int G = NTHR / MSD_WT;
     const int PT = p.P[0] + p.P[1];
-    cplx* val = Csm + PT * MSD_WT;                                  // [E][S][WT]
+    cplx* Csm = reinterpret_cast<cplx*>(smem_raw);                  // [(P_a + P_b)][WT]
+    cplx* one = Csm + PT * MSD_WT;                                  // 16 walkers' worth of the constant 1.0 (level-1 entries)
+    cplx* sR = one + 2 * MSD_WT;                                    // pool: [D][2][WT] scale factors, then the staged adjugates
+    cplx* gsm = reinterpret_cast<cplx*>(reinterpret_cast<unsigned char*>(sR) + pool_bytes);     // [(P_a + P_b)][WT]   (GS)
+    if (threadIdx.x < 2 * MSD_WT) one[threadIdx.x] = cmake(1.0, 0.0);
     const int tile = blockIdx.y;
     const int j = threadIdx.x & (MSD_WT - 1);
     const int slot = threadIdx.x / MSD_WT;
-    // GS: the tile's g slices sit behind val in shared memory (when they fit); otherwise they are read through L1
-    cplx* gsm = val + (size_t)c1_emax(KHI - 2) * S * MSD_WT;
-    const cplx* gA = GS ? gsm + j : p.g[0] + (int64_t)tile * p.P[0] * MSD_WT + j;
-    const cplx* gB = GS ? gsm + p.P[0] * MSD_WT + j : p.g[1] + (int64_t)tile * p.P[1] * MSD_WT + j;
+    const cplx* g0 = GS ? gsm : p.g[0] + (int64_t)tile * p.P[0] * MSD_WT;
+    const cplx* g1 = GS ? gsm + p.P[0] * MSD_WT : p.g[1] + (int64_t)tile * p.P[1] * MSD_WT;
+    const cplx* gA = g0 + j;
+    const cplx* gB = g1 + j;
     if (GS) {
         const cplx* ga = p.g[0] + (int64_t)tile * p.P[0] * MSD_WT;
         const cplx* gb = p.g[1] + (int64_t)tile * p.P[1] * MSD_WT;
@@ -439,40 +489,61 @@ __global__ void __launch_bounds__(NTHR, 1) k_dets_c1(DetsParams p, const WorkIte
                          r0 * (int)gridDim.x < n_items; r0++) {
         if (ii >= n_items) continue;
         const WorkItem it = items[ii];
-        const int E = it.ka * it.ka + it.kb * it.kb;
-        const int nr = (it.det_count + S - 1) / S;
-        for (int r = 0; r < nr; r++) {
-            const int i = r * S + slot;
-            if (i < it.det_count) {
-                switch (it.ka * 5 + it.kb) {
-                    C1_CASE(0, 0) C1_CASE(0, 1) C1_CASE(0, 2) C1_CASE(0, 3) C1_CASE(0, 4)
-                    C1_CASE(1, 0) C1_CASE(1, 1) C1_CASE(1, 2) C1_CASE(1, 3) C1_CASE(1, 4)
-                    C1_CASE(2, 0) C1_CASE(2, 1) C1_CASE(2, 2) C1_CASE(2, 3) C1_CASE(2, 4)
-                    C1_CASE(3, 0) C1_CASE(3, 1) C1_CASE(3, 2) C1_CASE(3, 3) C1_CASE(3, 4)
-                    C1_CASE(4, 0) C1_CASE(4, 1) C1_CASE(4, 2) C1_CASE(4, 3) C1_CASE(4, 4)
-                    default: break;
+        cplx* stage = sR + it.det_count * 2 * MSD_WT;               // [E_staged][det_count][WT]
+        // this group's piece of the entry list; its first 8 entries are requested before pass A
+        const uint2* ent = pull_ent + it.sched_off;
+        const int t0 = __ldg(pull_off + it.pull_off + slot), t1 = __ldg(pull_off + it.pull_off + slot + 1);
+        uint2 nxt = (t0 + j < t1) ? __ldg(ent + t0 + j) : make_uint2(0u, 0u);
+        switch (it.ka * 5 + it.kb) {
+            PULL_CASE(0, 0) PULL_CASE(0, 1) PULL_CASE(0, 2) PULL_CASE(0, 3) PULL_CASE(0, 4)
+            PULL_CASE(1, 0) PULL_CASE(1, 1) PULL_CASE(1, 2) PULL_CASE(1, 3) PULL_CASE(1, 4)
+            PULL_CASE(2, 0) PULL_CASE(2, 1) PULL_CASE(2, 2) PULL_CASE(2, 3) PULL_CASE(2, 4)
+            PULL_CASE(3, 0) PULL_CASE(3, 1) PULL_CASE(3, 2) PULL_CASE(3, 3) PULL_CASE(3, 4)
+            PULL_CASE(4, 0) PULL_CASE(4, 1) PULL_CASE(4, 2) PULL_CASE(4, 3) PULL_CASE(4, 4)
+            default: break;
+        }
+        if (it.ka + it.kb == 0) continue;                           // the reference determinant: W only (uniform over the CTA)
+        __syncthreads();
+        // pass B: branch-free per entry -- value and scale factor are plain shared-memory reads at offsets the setup computed
+        {
+            const unsigned char* sm_j = smem_raw + j * sizeof(cplx);
+            const unsigned char* sr_j = reinterpret_cast<const unsigned char*>(sR) + j * sizeof(cplx);
+            cplx acc = cmake(0.0, 0.0);
+            const unsigned gmask = 0xffu << (threadIdx.x & 24);     // the 8 lanes of this group
+            for (int base = t0; base < t1; base += MSD_WT) {
+                const uint2 mine = nxt;
+                if (base + MSD_WT + j < t1) nxt = __ldg(ent + base + MSD_WT + j);
+                const int n = t1 - base;
+                // four entries at a time: their eight shared-memory reads are issued before any add to the C tile (the compiler
+                // cannot move a load above the conditional store, but the C tile never aliases the operands)
+#pragma unroll
+                for (int i0 = 0; i0 < MSD_WT; i0 += 4) {
+                    uint32_t w0[4];
+                    cplx sv[4], vv[4];
+#pragma unroll
+                    for (int u = 0; u < 4; u++) {
+                        w0[u] = __shfl_sync(gmask, mine.x, i0 + u, MSD_WT);
+                        const uint32_t w1 = __shfl_sync(gmask, mine.y, i0 + u, MSD_WT);
+                        const bool on = i0 + u < n;
+                        sv[u] = *reinterpret_cast<const cplx*>(sr_j + (on ? (w0[u] & 0x3ffu) * 128u : 0u));
+                        vv[u] = *reinterpret_cast<const cplx*>(sm_j + (on ? w1 : 0u));
+                        if (!on) w0[u] = 0u;
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; u++) {
+                        if (i0 + u < n) acc = cfma(vv[u], flip(sv[u], (w0[u] >> 10) & 1u), acc);
+                        if (w0[u] & (1u << 25)) {
+                            cplx* cp = reinterpret_cast<cplx*>(smem_raw + ((w0[u] >> 11) & 0x3fffu) * 128u) + j;
+                            cplx c0 = *cp; c0.x += acc.x; c0.y += acc.y; *cp = c0;
+                            acc = cmake(0.0, 0.0);
+                        }
+                    }
                 }
             }
-            if (E == 0) continue;                                   // uniform over the CTA
-            __syncthreads();
-            // owner phase: slot q adds the entries with x % S == q, in list order
-            const uint32_t* hdr = sched + it.sched_off + (int64_t)r * (HW + (int64_t)S * E);
-            const uint32_t* ent = hdr + HW;
-            const int lo = (int)((__ldg(hdr + (slot >> 1)) >> (16 * (slot & 1))) & 0xffffu);
-            const int hi = (int)((__ldg(hdr + ((slot + 1) >> 1)) >> (16 * ((slot + 1) & 1))) & 0xffffu);
-            for (int t = lo; t < hi; t++) {
-                const uint32_t en = __ldg(ent + t);
-                const int x = (int)(en >> 12), sl = (int)((en >> 5) & 127u), e = (int)(en & 31u);
-                const cplx v = val[(e * S + sl) * MSD_WT + j];
-                cplx cacc = Csm[x * MSD_WT + j];
-                cacc.x += v.x; cacc.y += v.y;
-                Csm[x * MSD_WT + j] = cacc;
-            }
-            __syncthreads();
         }
+        __syncthreads();
     }
     // flush the CTA's C tile into the planar global accumulators
-    __syncthreads();
     for (int e = threadIdx.x; e < PT * MSD_WT; e += NTHR) {
         const cplx v = Csm[e];
         if (v.x == 0.0 && v.y == 0.0) continue;
@@ -1167,18 +1238,28 @@ static cudaError_t launch_persistent(msd_ctx* c, K kernel, int nthr, size_t smem
     return cudaGetLastError();
 }
 
-template <class K>
-static cudaError_t launch_c1(msd_ctx* c, K kernel, int nthr, size_t smem, int n_sm, const DetsParams& p, const WorkItem* items,
-                             int n_items, int ntiles, const uint32_t* sched, cudaStream_t st)
+// closed-form buckets of the force-bias mode by owner pull: one launch per class (larger level <= 3: 512 threads, == 4: 256)
+template <int NTHR, int KLO, int KHI>
+static cudaError_t launch_pull_class(msd_ctx* c, const DetsParams& p, int ntiles, int i0, int i1, cudaStream_t st)
 {
-    if (n_items == 0) return cudaSuccess;
-    cudaError_t e = func_config(c, (const void*)kernel, nthr, smem, nullptr);
+    const int n_items = i1 - i0;
+    if (n_items <= 0) return cudaSuccess;
+    const size_t tile_bytes = (size_t)(p.P[0] + p.P[1]) * MSD_WT * sizeof(cplx);
+    const size_t smem = tile_bytes + 256 + c->pull_pool + (c->pull_gs ? tile_bytes : 0);
+    const void* kern = c->pull_gs ? (const void*)k_dets_pull<NTHR, KLO, KHI, true> : (const void*)k_dets_pull<NTHR, KLO, KHI, false>;
+    cudaError_t e = func_config(c, kern, NTHR, smem, nullptr);
     if (e != cudaSuccess) return e;
-    int workers = (n_sm + 1) / 2;                  // one CTA per SM, about two walker tiles resident at a time
-    if (workers > n_items) workers = n_items;
-    if (ntiles == 1) workers = n_items < n_sm ? n_items : n_sm;
-    dim3 grid(workers, ntiles);
-    kernel<<<grid, nthr, smem, st>>>(p, items, n_items, sched);
+    // one CTA per SM, all resident at once: workers x tiles <= waves x SMs
+    const int waves = (ntiles + c->n_sm - 1) / c->n_sm;
+    int workers = std::max(1, waves * c->n_sm / ntiles);
+    workers = std::min(workers, n_items);
+    if (c->pull_gs)
+        k_dets_pull<NTHR, KLO, KHI, true><<<dim3(workers, ntiles), NTHR, smem, st>>>(p, c->d_items_pull + i0, n_items, c->d_pull_off,
+                                                                                     c->d_pull_ent, (int)c->pull_pool);
+    else
+        k_dets_pull<NTHR, KLO, KHI, false><<<dim3(workers, ntiles), NTHR, smem, st>>>(p, c->d_items_pull + i0, n_items, c->d_pull_off,
+                                                                                      c->d_pull_ent, (int)c->pull_pool);
+    c->launches++;
     return cudaGetLastError();
 }
 
@@ -1222,8 +1303,19 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
         if (e != cudaSuccess) { f.join(); return e; }
         c->launches++;
     }
+    // force bias, closed-form levels: owner-pull kernel (one launch for all buckets) unless the tile does not fit
+    bool cf_done = false;
+    if constexpr (MODE == 1) {
+        if (!no_tiles && c->pull_pool) {
+            cudaError_t e = launch_pull_class<256, 3, 4>(c, p, ntiles, c->pull_class_begin[1], c->pull_class_begin[2], f.stream(li++));
+            if (e == cudaSuccess)
+                e = launch_pull_class<512, -1, 3>(c, p, ntiles, c->pull_class_begin[0], c->pull_class_begin[1], f.stream(li++));
+            if (e != cudaSuccess) { f.join(); return e; }
+            cf_done = true;
+        }
+    }
     // closed-form kernel: three register classes, items sorted by class on the host (msd_api.cu)
-    for (int cl = 2; cl >= 0; cl--) {
+    for (int cl = 2; cl >= 0 && !cf_done; cl--) {
         const int i0 = c->cf_class_begin[cl], i1 = c->cf_class_begin[cl + 1];
         if (i1 == i0) continue;
         cudaError_t e;
@@ -1231,20 +1323,6 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
         // energy mode: one large CTA per SM that also holds Hrot / F of the tile in shared memory (same warps per SM as
         // the 2-3 smaller CTAs of the other modes); falls back to global Hrot / F when the tile does not fit
         bool fhs = false;
-        if constexpr (MODE == 1) {
-            const size_t csm = (size_t)(p.P[0] + p.P[1]) * MSD_WT * sizeof(cplx);
-            const size_t sm1 = csm + (size_t)C1_EMAX[cl] * C1_SLOTS[cl] * MSD_WT * sizeof(cplx);
-            if (sm1 <= 227 * 1024 && c->d_sched && p.P[0] + p.P[1] < 8192 && !no_tiles) {
-                fhs = true;     // handled here
-                const bool gs = sm1 + csm <= 227 * 1024;        // room for the g slices as well
-                if (cl == 0 && gs) e = launch_c1(c, k_dets_c1<-1, 2, 768, true>, 768, sm1 + csm, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
-                else if (cl == 0) e = launch_c1(c, k_dets_c1<-1, 2, 768, false>, 768, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
-                else if (cl == 1 && gs) e = launch_c1(c, k_dets_c1<2, 3, 512, true>, 512, sm1 + csm, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
-                else if (cl == 1) e = launch_c1(c, k_dets_c1<2, 3, 512, false>, 512, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
-                else if (gs) e = launch_c1(c, k_dets_c1<3, 4, 256, true>, 256, sm1 + csm, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
-                else e = launch_c1(c, k_dets_c1<3, 4, 256, false>, 256, sm1, c->n_sm, p, c->d_items_cf + i0, i1 - i0, ntiles, c->d_sched, s);
-            }
-        }
         if constexpr (MODE >= 2) {
             fhs = 3 * gbytes <= 200 * 1024 && !no_tiles;
             if (!fhs) {}

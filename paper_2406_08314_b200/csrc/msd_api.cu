@@ -310,52 +310,123 @@ static int do_setup(msd_ctx* c, std::string* errp, int N, int na, int nb, int n_
         c->gen_group_begin.push_back(i);
         if (g < 10) c->gen_group_elems.push_back(gen_thresholds[g]);
     }
-    // CI-reduction schedules (msd_internal.cuh C1_*): entries of every round grouped by owner slot x % S
+    // Owner-pull lists of the force-bias CI reduction (msd_internal.cuh PULL_*)
     {
+        const int noa = c->sp[0].n_o, nob = c->sp[1].n_o, Pa = c->sp[0].P, PT = c->sp[0].P + c->sp[1].P;
+        // shared memory beside the C tile (and the g tile when it fits as well): scale factors + staged adjugates
+        // layout (bytes from the start of dynamic shared memory): C tile | 16 B holding 1.0 | pool | g tile
+        const size_t tile_bytes = (size_t)PT * MSD_WT * sizeof(cplx), total = 225 * 1024;
+        size_t per_det_max = 256;
+        for (const Bucket& b : c->buckets)
+            if (std::max(b.ka, b.kb) <= MSD_CF_MAX)
+                per_det_max = std::max<size_t>(per_det_max, 256 + (size_t)((b.ka >= 3 ? b.ka * b.ka : 0) + (b.kb >= 3 ? b.kb * b.kb : 0)) * 128);
+        // the g tile must sit in shared memory (level-2 entries address it directly) and every bucket needs >= 16 determinants
+        c->pull_gs = true;
+        c->pull_pool = (2 * tile_bytes + 16 * per_det_max + 256 <= total) ? total - 2 * tile_bytes - 256 : 0;
+        if (PT >= (1 << 14)) c->pull_pool = 0;
         int64_t tab_bytes_all = 0;
         for (const Bucket& b : c->buckets) tab_bytes_all = std::max<int64_t>(tab_bytes_all, b.tab_off + (b.count * b.rs + 15) / 16 * 16);
         std::vector<unsigned char> htab((size_t)std::max<int64_t>(tab_bytes_all, 16));
         CK(cudaMemcpyAsync(htab.data(), c->d_tab, (size_t)tab_bytes_all, cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
-        int64_t words = 0;
-        for (WorkItem& w : c->items_cf) {
-            const int S = C1_SLOTS[cls(w)], E = w.ka * w.ka + w.kb * w.kb;
-            w.sched_off = words;
-            words += (int64_t)((w.det_count + S - 1) / S) * (c1_hdr_words(S) + (int64_t)S * E);
-        }
-        std::vector<uint32_t> sched((size_t)std::max<int64_t>(words, 1), 0u);
-        const int noa = c->sp[0].n_o, nob = c->sp[1].n_o, Pa = c->sp[0].P;
-        std::vector<uint32_t> ent; std::vector<int> cnt;
-        for (const WorkItem& w : c->items_cf) {
-            const int S = C1_SLOTS[cls(w)], ka = w.ka, kb = w.kb, E = ka * ka + kb * kb, HW = c1_hdr_words(S);
-            if (E == 0) { continue; }
-            const int nr = (w.det_count + S - 1) / S;
-            for (int r = 0; r < nr; r++) {
-                uint32_t* hdr = sched.data() + w.sched_off + (int64_t)r * (HW + (int64_t)S * E);
-                uint32_t* out = hdr + HW;
-                const int nd = std::min(S, w.det_count - r * S);
-                ent.clear(); cnt.assign(S + 1, 0);
-                for (int sl = 0; sl < nd; sl++) {
-                    const unsigned char* row = htab.data() + w.tab_off + (int64_t)(r * S + sl) * w.rs;
-                    for (int a = 0; a < ka; a++)
-                        for (int b = 0; b < ka; b++) {
-                            const uint32_t x = (uint32_t)row[ka + b] * noa + row[a];
-                            ent.push_back(x << 12 | (uint32_t)sl << 5 | (uint32_t)(a * ka + b));
-                        }
-                    for (int a = 0; a < kb; a++)
-                        for (int b = 0; b < kb; b++) {
-                            const uint32_t x = (uint32_t)Pa + (uint32_t)row[2 * ka + kb + b] * nob + row[2 * ka + a];
-                            ent.push_back(x << 12 | (uint32_t)sl << 5 | (uint32_t)(ka * ka + a * kb + b));
-                        }
-                }
-                for (uint32_t e : ent) cnt[(e >> 12) % S + 1]++;
-                for (int q = 0; q < S; q++) cnt[q + 1] += cnt[q];
-                for (int q = 0; q <= S; q++) hdr[q >> 1] |= (uint32_t)cnt[q] << (16 * (q & 1));
-                std::vector<int> fill(cnt.begin(), cnt.end() - 1);
-                for (uint32_t e : ent) out[fill[(e >> 12) % S]++] = e;
+        auto pcls = [](const WorkItem& w) { return std::max(w.ka, w.kb) <= 3 ? 0 : 1; };
+        auto estage = [](int ka, int kb) { return (ka >= 3 ? ka * ka : 0) + (kb >= 3 ? kb * kb : 0); };
+        for (int bi = 0; bi < nbk && c->pull_pool; bi++) {
+            const Bucket& b = c->buckets[bi];
+            if (std::max(b.ka, b.kb) > MSD_CF_MAX) continue;
+            const int slots = (std::max(b.ka, b.kb) <= 3 ? 512 : 256) / MSD_WT;
+            int D = (int)std::min<size_t>(PULL_DMAX, c->pull_pool / (256 + (size_t)estage(b.ka, b.kb) * 128));
+            if (D > slots) D = D / slots * slots;                 // whole sweeps of the CTA's determinant slots
+            for (int64_t i0 = 0; i0 < b.count; i0 += D) {
+                WorkItem it;
+                it.bucket = bi; it.ka = b.ka; it.kb = b.kb; it.rs = b.rs;
+                it.det_begin = b.start + i0;
+                it.det_count = (int)std::min<int64_t>(D, b.count - i0);
+                it.tab_off = b.tab_off + i0 * b.rs;
+                it.sched_off = 0; it.pull_off = 0;
+                c->items_pull.push_back(it);
             }
         }
-        CK(upload(&c->d_sched, sched.data(), sched.size(), st));
+        // by class, heaviest chunks first (the persistent CTAs take them in snake order)
+        std::stable_sort(c->items_pull.begin(), c->items_pull.end(), [&](const WorkItem& x, const WorkItem& y) {
+            if (pcls(x) != pcls(y)) return pcls(x) < pcls(y);
+            auto w = [](const WorkItem& t) {
+                auto f = [](int k) { return k <= 1 ? 2.0 : (k == 2 ? 20.0 : (k == 3 ? 160.0 : 600.0)); };
+                return (f(t.ka) + f(t.kb) + 10.0 * (t.ka * t.ka + t.kb * t.kb) + 30.0) * t.det_count;
+            };
+            return w(x) > w(y);
+        });
+        for (int cl = 0; cl <= 2; cl++) {
+            int i = 0;
+            while (i < (int)c->items_pull.size() && pcls(c->items_pull[i]) < cl) i++;
+            c->pull_class_begin[cl] = i;
+        }
+        std::vector<unsigned short> splits;
+        std::vector<uint2> ents;
+        std::vector<uint32_t> cnt((size_t)PT + 1);
+        for (size_t ii = 0; ii < c->items_pull.size(); ii++) {
+            WorkItem& w = c->items_pull[ii];
+            const int G = (pcls(w) == 0 ? 512 : 256) / MSD_WT;
+            w.pull_off = (int64_t)splits.size();
+            w.sched_off = (int64_t)ents.size();
+            const int ka = w.ka, kb = w.kb;
+            const uint32_t one_off = (uint32_t)tile_bytes, pool_off = (uint32_t)tile_bytes + 256u;
+            const uint32_t stage_off = pool_off + (uint32_t)w.det_count * 256u, g_off = pool_off + (uint32_t)c->pull_pool;
+            std::fill(cnt.begin(), cnt.end(), 0u);
+            auto xof = [&](const unsigned char* row, int s, int a, int b) -> uint32_t {
+                return s == 0 ? (uint32_t)row[ka + b] * noa + row[a]
+                              : (uint32_t)Pa + (uint32_t)row[2 * ka + kb + b] * nob + row[2 * ka + a];
+            };
+            for (int d = 0; d < w.det_count; d++) {
+                const unsigned char* row = htab.data() + w.tab_off + (int64_t)d * w.rs;
+                for (int s = 0; s < 2; s++) {
+                    const int k = s ? kb : ka;
+                    for (int a = 0; a < k; a++) for (int b = 0; b < k; b++) cnt[xof(row, s, a, b) + 1]++;
+                }
+            }
+            for (int x = 0; x < PT; x++) cnt[x + 1] += cnt[x];
+            const uint32_t n_ent = cnt[PT];
+            // piece boundaries: the first change of x at or after q * n / G
+            {
+                int x = 0;
+                for (int q = 0; q <= G; q++) {
+                    const uint32_t target = (uint32_t)(((uint64_t)n_ent * q + G - 1) / G);
+                    while (x < PT && cnt[x] < target) x++;
+                    splits.push_back((unsigned short)(q == G ? n_ent : cnt[x]));
+                }
+            }
+            const size_t base = ents.size();
+            ents.resize(base + n_ent);
+            for (int d = 0; d < w.det_count; d++) {
+                const unsigned char* row = htab.data() + w.tab_off + (int64_t)d * w.rs;
+                for (int s = 0; s < 2; s++) {
+                    const int k = s ? kb : ka, no = s ? nob : noa;
+                    const unsigned char* h = row + (s ? 2 * ka : 0);
+                    const unsigned char* pp = h + k;
+                    const int eoff = (s && ka >= 3) ? ka * ka : 0;
+                    for (int a = 0; a < k; a++)
+                        for (int b = 0; b < k; b++) {
+                            const uint32_t x = xof(row, s, a, b);
+                            // w1 = byte offset (walker 0) of the value the entry multiplies: the constant 1.0, an element of the
+                            // g tile, or an element of the staged adjugate (which carries its own sign)
+                            uint32_t w1, sign = (uint32_t)((a + b) & 1);
+                            if (k == 1) { w1 = one_off; sign = 0; }
+                            else if (k == 2) w1 = g_off + ((s ? (uint32_t)Pa : 0u) + (uint32_t)pp[1 - b] * no + h[1 - a]) * 128u;
+                            else { w1 = stage_off + (uint32_t)((eoff + a * k + b) * w.det_count + d) * 128u; sign = 0; }
+                            // w0 = (2 det + spin) [10 bits: byte offset / 128 of the scale factor] | sign << 10 | x << 11 | last << 25
+                            ents[base + cnt[x]++] = make_uint2((uint32_t)(2 * d + s) | sign << 10 | x << 11, w1);
+                        }
+                }
+            }
+            for (uint32_t t = 0; t < n_ent; t++)      // last entry of every x-run
+                if (t + 1 == n_ent || ((ents[base + t].x >> 11) & 0x3fffu) != ((ents[base + t + 1].x >> 11) & 0x3fffu))
+                    ents[base + t].x |= 1u << 25;
+        }
+        if (splits.empty()) splits.push_back(0);
+        if (ents.empty()) ents.push_back(make_uint2(0u, 0u));
+        CK(upload(&c->d_pull_off, splits.data(), splits.size(), st));
+        CK(upload(&c->d_pull_ent, ents.data(), ents.size(), st));
+        CK(upload(&c->d_items_pull, c->items_pull.data(), c->items_pull.size(), st));
         CK(cudaStreamSynchronize(st));
     }
     CK(upload(&c->d_items_cf, c->items_cf.data(), c->items_cf.size(), st));
@@ -447,7 +518,8 @@ extern "C" void msd_destroy(msd_ctx* c)
     for (int s = 0; s < 2; s++) {
         cudaFree(c->sp[s].d_occ_ref); cudaFree(c->sp[s].d_act_v); cudaFree(c->sp[s].d_pos_o); cudaFree(c->sp[s].d_Lsub);
     }
-    cudaFree(c->d_tab); cudaFree(c->d_coef); cudaFree(c->d_items_cf); cudaFree(c->d_items_gen); cudaFree(c->d_sched);
+    cudaFree(c->d_tab); cudaFree(c->d_coef); cudaFree(c->d_items_cf); cudaFree(c->d_items_gen);
+    cudaFree(c->d_items_pull); cudaFree(c->d_pull_off); cudaFree(c->d_pull_ent);
     cudaFree(c->ws.base);
     cudaFree(c->stg_a); cudaFree(c->stg_b); cudaFree(c->stg_out); cudaFree(c->stg_flags);
     for (auto& e : c->ev) if (e) cudaEventDestroy(e);

@@ -99,20 +99,29 @@ struct WorkItem {          // a chunk of one bucket, processed by one CTA per wa
     int64_t det_begin;     // in the sorted list
     int det_count;
     int64_t tab_off;       // byte offset of the chunk's first row
-    int64_t sched_off;     // closed-form items: first word of the item's CI-reduction schedule (see C1_* below)
+    int64_t sched_off;     // pull items (k_dets_pull): first entry of the item's pull list
+    int64_t pull_off;      // pull items: first of the item's G + 1 piece boundaries (uint16, relative to sched_off)
 };
 
-// Force-bias CI reduction without atomics (k_dets_c1, dets.cu).  A CTA of C1_SLOTS[cls] determinant slots x 8 walkers
-// works in rounds of C1_SLOTS determinants: every thread first leaves its c~ R^sbar A[b][a] products in shared memory,
-// then the 8 lanes of slot q add up, in order, exactly the entries whose pair index x satisfies x % C1_SLOTS == q
-// ("owner computes": plain shared-memory read-modify-write, no two threads ever touch the same accumulator).
-// Which entries those are depends only on the excitation table, so the lists are built once at setup:
-//   round r of an item = C1_HDR(S) header words (S+1 uint16 offsets) + S*E entry words, E = ka^2 + kb^2,
-//   entry = x_unified << 12 | slot << 5 | e      (x_unified = x for alpha, P_alpha + x for beta; e = a*k+b, beta after alpha)
-static const int C1_SLOTS[3] = {96, 64, 32};     // register classes: larger level <= 2, == 3, == 4
-static const int C1_EMAX[3] = {8, 18, 32};
-__host__ __device__ constexpr int c1_emax(int cls) { return cls == 0 ? 8 : (cls == 1 ? 18 : 32); }
-__host__ __device__ inline int c1_hdr_words(int S) { return (S + 2) / 2; }
+// Force-bias CI reduction by OWNER PULL (k_dets_pull, dets.cu): nothing is scattered, no atomics.  For every chunk of
+// determinants of one closed-form bucket the setup builds the list of all adjugate entries of the chunk, sorted by the unified
+// pair index x they land on (alpha: x, beta: P_alpha + x),
+//   C^s[x] = sum_{(I, a, b): x_ab(I) = x} c~_I R_I^sbar A_I^s[b][a],
+// and cuts it into G contiguous pieces of (nearly) equal length whose ends fall on changes of x: piece q belongs to lane group q
+// (8 lanes = 8 walkers) of the CTA, so every x has exactly one owner.
+//   pass A  thread = (determinant, walker): R^a, R^b and, for spins of level >= 3, the adjugate by the division-free closed
+//           forms; leaves the scale factors c~ R^b, c~ R^a and the (unscaled) level >= 3 adjugates in shared memory;
+//   pass B  lane group q walks its piece: an entry is either recomputed from the shared-memory g tile (level 1: the scale
+//           itself; level 2: one element of g) or read from the staged adjugate; the running sum of an x-run stays in
+//           registers and is added to the CTA's C tile once per run.
+// List entry (two words), everything pass B needs as ready-made byte offsets so that its inner loop has no branch on the level:
+//   w0 = (2 det_local + spin) [10 bits: offset / 128 of the scale factor] | sign << 10 | x << 11 (14 bits) | last-of-run << 25
+//   w1 = byte offset (walker 0, from the start of dynamic shared memory) of the value the scale multiplies: the constant 1.0
+//        (level 1), one element of the g tile (level 2: the surviving element of the 2x2 minor), or one element of the staged
+//        adjugate (levels 3, 4; it carries its own sign).
+// Shared memory: C tile | 256 B (1.0) | pool = scale factors [D][2][8] + staged adjugates [E'][D][8] | g tile.
+// Chunk sizes follow the pool: 256 B of scale factors per determinant plus 128 B per staged adjugate element.
+#define PULL_DMAX 432      // determinants per chunk (12-bit det_local)
 
 struct Workspace {
     int64_t wc = 0;        // walker capacity of one chunk (multiple of MSD_WT)
@@ -160,9 +169,13 @@ struct msd_ctx {
     unsigned char* d_tab = nullptr;
     double* d_coef = nullptr;
     std::vector<Bucket> buckets;
-    std::vector<WorkItem> items_cf, items_gen;
-    WorkItem* d_items_cf = nullptr; WorkItem* d_items_gen = nullptr;
-    uint32_t* d_sched = nullptr;              // CI-reduction schedules of the closed-form items
+    std::vector<WorkItem> items_cf, items_gen, items_pull;
+    WorkItem* d_items_cf = nullptr; WorkItem* d_items_gen = nullptr; WorkItem* d_items_pull = nullptr;
+    unsigned short* d_pull_off = nullptr;     // per pull item: G + 1 piece boundaries
+    uint2* d_pull_ent = nullptr;              // pull-list entries (see PULL_* above)
+    int pull_class_begin[3] = {0, 0, 0};      // items_pull sorted by class: larger level <= 3 (512 threads), == 4 (256 threads)
+    bool pull_gs = true;                      // the g tile sits in shared memory too
+    size_t pull_pool = 0;                     // bytes of shared memory for scale factors + staged adjugates (0: pull disabled)
     int cf_class_begin[4] = {0, 0, 0, 0};      // items_cf is sorted by register class (larger level <=2, 3, 4)
     std::vector<int> gen_group_begin;         // items_gen is sorted by shared-memory group
     std::vector<int> gen_group_elems;         // ka^2+kb^2 bound of each group (complex elements per thread)

@@ -107,7 +107,7 @@ def main():
         out.update({"ovlp_all": [_c(v) for v in r["ovlp"]], "kappa_all": [float(v) for v in r["kappa"]]})
         print("overlap of all %d walkers: %.0f s" % (x.n_w, time.time() - t), flush=True)
     with open(path, "w") as f:
-        json.dump(out, f, indent=1)
+        json.dump(out, f, separators=(",", ":"))
     print("wrote", path)
 
 
