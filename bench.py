@@ -352,6 +352,29 @@ def main():
                  "unit": "walker*det*step/s", "block_ms": 25.0 * (t_fb + t_ov) + t_e,
                  "energy_share_of_block": t_e / (25.0 * (t_fb + t_ov) + t_e)}
 
+    # ---- one propagation step around the path (force bias, B(x - xbar), new overlap, Eq. 8-12) ----
+    trial.propagator_setup(0.005, 6, inp.h1, inp.L)
+    xf = torch.randn((inp.n_w, inp.n_chol), dtype=torch.float64, device=dev,
+                     generator=torch.Generator(device=dev).manual_seed(1234 + rank))
+    wts = torch.ones(inp.n_w, dtype=torch.float64, device=dev)
+    sout = torch.empty((inp.n_w, 8), dtype=torch.float64, device=dev)
+    pa_w, pb_w = d_a.clone(), d_b.clone()
+    trial.propagate(pa_w, pb_w, xf, weights=wts, out=sout)
+    barrier()
+    pev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in pev:
+        pa_w.copy_(d_a); pb_w.copy_(d_b)          # every timed step starts from the orthonormal walkers
+        flush.zero_()
+        a.record(stream)
+        trial.propagate(pa_w, pb_w, xf, weights=wts, out=sout)
+        b.record(stream)
+    barrier()
+    pms = reduce_max_time(sum(a.elapsed_time(b) for a, b in pev), world, dev) / args.steps
+    propagation = {"call": "msd_propagate: force bias + overlap of the walkers, field matrices (DMMA), orbital update with a "
+                           "6th-order Taylor series, overlap of the new walkers, Eq. 8-12 (dt = 0.005)",
+                   "ms_per_step": pms, "value": total_units(inp.n_w, inp.n_det, 1, world) / (pms * 1e-3),
+                   "unit": "walker*det*step/s", "finite": bool(torch.isfinite(sout).all().item())}
+
     # ---- end to end: the C-ABI *_host calls (pinned HOST buffers; H2D + kernels + D2H inside each call) ----
     def e2e_step():
         trial.force_bias_host(h_a, h_b, out=h_fb)
@@ -473,7 +496,7 @@ def main():
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": n_e2e},
             "gpu_launches": int(launches),
-            "fused": fused, "per_call": per_call, "block_mix": block_mix,
+            "fused": fused, "per_call": per_call, "block_mix": block_mix, "propagation": propagation,
             "roofline": roofline, "roofline_dets": roofline_dets, "roofline_fb_dets": roofline_fb_dets,
             "cpu_baseline": cpu_baseline, "cpu_wick_baseline": cpu_wick, "phases": phases,
             "step_ms": {"min": min(step_ms), "median": statistics.median(step_ms), "max": max(step_ms)}}

@@ -122,6 +122,28 @@ int msd_force_bias_energy(msd_ctx* ctx, int64_t n_w, const void* phi_a, const vo
 int msd_greens(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
                void* G, int32_t* flags, void* stream);
 
+/* One phaseless-AFQMC propagation step around the hot path (Eq. 5, Eq. 7-12).
+ *
+ * msd_propagator_setup fixes the time step dt > 0 and the order n_taylor (1..64) of the Taylor series that applies the field
+ * exponential, builds h' = h - 1/2 sum_g L^g L^g (Eq. 4) and exp(-dt h'/2) on the device (scaling and squaring), and keeps L
+ * with the Cholesky index contiguous (N^2 x n_chol doubles of device memory).  h1, L: the HOST arrays msd_setup was given.
+ * May be called again to change dt.  Synchronises `stream`.
+ *
+ * msd_propagate advances every walker of the batch by one step, IN PLACE:
+ *     v = force bias (as msd_force_bias),  xbar = -i sqrt(dt) v                              Eq. 7 (reading A20)
+ *     psi <- B(x - xbar) psi,  B(y) = exp(-dt h'/2) exp(i sqrt(dt) sum_g y_g L^g) exp(-dt h'/2)     Eq. 5
+ *     S = <Psi_T|psi_new>/<Psi_T|psi_old>,  theta = arg S                                    Eq. 8-9
+ *     I = S exp(x.xbar - xbar.xbar/2),  I_ph = |I| max(0, cos theta),  w <- I_ph w           Eq. 10-12
+ *   phi_a, phi_b  DEVICE walkers as above, overwritten with the propagated (not re-orthonormalised) walkers.
+ *   x        DEVICE [n_w][n_chol] float64: the auxiliary fields, drawn by the caller (standard normal).
+ *   weights  DEVICE [n_w] float64, multiplied by I_ph in place; may be NULL.
+ *   step_out DEVICE [n_w][8] float64: (Re S, Im S, theta, I_ph, Re <Psi_T|psi_new>, Im <Psi_T|psi_new>, Re I, Im I).
+ *   flags    DEVICE [n_w] or NULL: MSD_FLAG_* of the old OR the new walker (NaN outputs for those).
+ * Population control and re-orthogonalisation are the caller's. */
+int msd_propagator_setup(msd_ctx* ctx, double dt, int n_taylor, const double* h1, const double* L, void* stream);
+int msd_propagate(msd_ctx* ctx, int64_t n_w, void* phi_a, void* phi_b, const double* x, double* weights,
+                  double* step_out, int32_t* flags, void* stream);
+
 /* HOST-buffer variants of the hot calls (the end-to-end path: bench.py's "e2e").  phi_a / phi_b / the result /
  * flags are HOST pointers with the same layouts as above (pinned memory makes the copies asynchronous, pageable
  * memory works too).  Each call enqueues on `stream`: host->device copy of the walkers into staging buffers owned by

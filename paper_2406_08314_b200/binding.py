@@ -22,6 +22,7 @@ _CODES = {MSD_EINVAL: "MSD_EINVAL", MSD_ENOMEM: "MSD_ENOMEM", MSD_ECUDA: "MSD_EC
 EXPORTS = ["msd_setup", "msd_setup_from_occ", "msd_overlap", "msd_force_bias", "msd_local_energy", "msd_greens",
            "msd_overlap_host", "msd_force_bias_host", "msd_local_energy_host",
            "msd_force_bias_energy", "msd_force_bias_energy_host",
+           "msd_propagator_setup", "msd_propagate",
            "msd_get_info", "msd_get_packed", "msd_set_workspace_limit", "msd_set_option", "msd_launch_count",
            "msd_set_profiling", "msd_get_phase_ms", "msd_destroy", "msd_last_error"]
 MSD_OPT_NO_SMEM_TILES = 1
@@ -55,6 +56,10 @@ def load_library() -> C.CDLL:
         f = getattr(lib, name)
         f.restype = i32
         f.argtypes = [vp, i64, vp, vp, vp, vp, vp]
+    lib.msd_propagator_setup.restype = i32
+    lib.msd_propagator_setup.argtypes = [vp, dbl, i32, vp, vp, vp]
+    lib.msd_propagate.restype = i32
+    lib.msd_propagate.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp]
     lib.msd_get_info.restype = i32
     lib.msd_get_info.argtypes = [vp, vp]
     lib.msd_get_packed.restype = i32
@@ -182,6 +187,38 @@ class MSDTrial:
         nw = self._walkers(phi_a, phi_b)
         out = torch.empty((nw, 2, self.N, self.N), dtype=torch.complex128, device=phi_a.device) if out is None else out
         return self._call(load_library().msd_greens, phi_a, phi_b, out, flags, stream)
+
+    # -- one propagation step (Eq. 5, 7-12) -------------------------------------------------
+    def propagator_setup(self, dt: float, n_taylor: int, h1, L, stream=None):
+        h1 = _np(h1, np.float64); L = _np(L, np.float64)
+        if h1.shape != (self.N, self.N) or L.shape != (self.n_chol, self.N, self.N):
+            raise ValueError("h1 / L shapes disagree with the trial")
+        self._check(load_library().msd_propagator_setup(self._h, float(dt), int(n_taylor), _ptr(h1), _ptr(L),
+                                                        _stream_ptr(stream)))
+
+    def propagate(self, phi_a, phi_b, x, weights=None, out=None, flags=None, stream=None):
+        """In place on phi_a / phi_b (and weights); returns step_out [n_w][8] float64 (see include/msd.h)."""
+        import torch
+        nw = self._walkers(phi_a, phi_b)
+        dev = phi_a.device
+
+        def f64(t, shape, what):
+            if not (isinstance(t, torch.Tensor) and t.is_cuda and t.device == dev and t.dtype == torch.float64
+                    and t.is_contiguous() and tuple(t.shape) == shape):
+                raise ValueError("%s must be a contiguous CUDA float64 tensor of shape %s" % (what, (shape,)))
+            return t
+        f64(x, (nw, self.n_chol), "x")
+        if weights is not None:
+            f64(weights, (nw,), "weights")
+        out = torch.empty((nw, 8), dtype=torch.float64, device=dev) if out is None else f64(out, (nw, 8), "out")
+        if flags is not None and not (flags.is_cuda and flags.dtype == torch.int32 and flags.is_contiguous()
+                                      and flags.numel() >= nw):
+            raise ValueError("flags must be a contiguous CUDA int32 tensor of at least n_w elements")
+        rc = load_library().msd_propagate(self._h, nw, phi_a.data_ptr(), phi_b.data_ptr(), x.data_ptr(),
+                                          weights.data_ptr() if weights is not None else None, out.data_ptr(),
+                                          flags.data_ptr() if flags is not None else None, _stream_ptr(stream))
+        self._check(rc)
+        return out
 
     # -- HOST-buffer variants (numpy or CPU torch arrays in and out; copies happen inside the C call) ----
     def _call_host(self, fn, phi_a, phi_b, out, flags, stream):

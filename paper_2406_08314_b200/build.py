@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libmsd_b200.so")
-SOURCES = ["msd_api.cu", "pack.cu", "reference.cu", "dets.cu", "dense.cu", "gemm.cu"]
+SOURCES = ["msd_api.cu", "pack.cu", "reference.cu", "dets.cu", "dense.cu", "gemm.cu", "propagate.cu"]
 # bench-side peak probes (FP64 DMMA/DFMA, L2 gather): a separate library that only bench.py loads, not the product ABI
 PROBES_SO = os.path.join(HERE, "libmsd_probes.so")
 PROBES_SRC = "probes.cu"

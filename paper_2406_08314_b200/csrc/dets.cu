@@ -462,7 +462,6 @@ __global__ void __launch_bounds__(NTHR, 1) k_dets_pull(DetsParams p, const WorkI
                                                        const uint2* __restrict__ pull_ent, int pool_bytes)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int G = NTHR / MSD_WT;
     const int PT = p.P[0] + p.P[1];
     cplx* Csm = reinterpret_cast<cplx*>(smem_raw);                  // [(P_a + P_b)][WT]
     cplx* one = Csm + PT * MSD_WT;                                  // 16 walkers' worth of the constant 1.0 (level-1 entries)

@@ -520,6 +520,7 @@ extern "C" void msd_destroy(msd_ctx* c)
     }
     cudaFree(c->d_tab); cudaFree(c->d_coef); cudaFree(c->d_items_cf); cudaFree(c->d_items_gen);
     cudaFree(c->d_items_pull); cudaFree(c->d_pull_off); cudaFree(c->d_pull_ent);
+    cudaFree(c->d_LT); cudaFree(c->d_hp); cudaFree(c->d_E);
     cudaFree(c->ws.base);
     cudaFree(c->stg_a); cudaFree(c->stg_b); cudaFree(c->stg_out); cudaFree(c->stg_flags);
     for (auto& e : c->ev) if (e) cudaEventDestroy(e);
@@ -646,11 +647,11 @@ static size_t carve(const msd_ctx* c, Workspace& ws, char* base, int64_t wc, int
     ws.E2nd = k.take<cplx>(wc);
     ws.E1nd = k.take<cplx>(wc);
     ws.wflags = k.take<int>(wc);
-    if (level >= 3) {
+    if (level == 3) {
         for (int s = 0; s < 2; s++) ws.F[s] = k.take<cplx>((size_t)wc * c->sp[s].P);
         ws.Eacc = k.take<cplx>((size_t)wc * 2);
     }
-    if (level >= 3) ws.X0 = k.take<cplx>((size_t)2 * wc * ng);   // zero for a spin without electrons
+    if (level == 3) ws.X0 = k.take<cplx>((size_t)2 * wc * ng);   // zero for a spin without electrons
     k.off = (k.off + 255) / 256 * 256;
     ws.zero_begin = z0;
     ws.zero_bytes = k.off;
@@ -659,10 +660,18 @@ static size_t carve(const msd_ctx* c, Workspace& ws, char* base, int64_t wc, int
         ws.g[s] = k.take<cplx>((size_t)nt * c->sp[s].P * MSD_WT);
     }
     ws.det0 = k.take<cplx>((size_t)wc * 2);
-    if (level == 2) {
+    if (level == 2 || level == 4) {
         for (int s = 0; s < 2; s++) ws.Gp[s] = k.take<double>((size_t)wc * 2 * c->sp[s].n_r * ldN);
     }
-    if (level >= 3) {
+    if (level == 4) {
+        const int ldg = ng + (ng & 1);
+        ws.fbuf = k.take<cplx>((size_t)wc * ng);
+        ws.Yf = k.take<double>((size_t)2 * wc * ldg);
+        ws.Aw = k.take<cplx>((size_t)wc * N * N);
+        ws.ov_old = k.take<cplx>(wc); ws.ov_new = k.take<cplx>(wc); ws.expo = k.take<cplx>(wc);
+        ws.fl_old = k.take<int>(wc);
+    }
+    if (level == 3) {
         for (int s = 0; s < 2; s++) {
             const auto& sp = c->sp[s];
             ws.thetaT[s] = k.take<double>((size_t)wc * sp.n * 2 * ldN);
@@ -677,7 +686,7 @@ static size_t carve(const msd_ctx* c, Workspace& ws, char* base, int64_t wc, int
     return k.off + 256;
 }
 
-// level: 1 overlap, 2 force bias / greens, 3 energy.  A separate workspace layout per level (the buffers differ);
+// level: 1 overlap, 2 force bias / greens, 3 energy, 4 propagation step.  A separate workspace layout per level (the buffers differ);
 // reallocated only when the level or the walker capacity changes.
 static int ensure_workspace(msd_ctx* c, int level, int64_t nw, std::string* errp)
 {
@@ -716,15 +725,36 @@ static int ensure_workspace(msd_ctx* c, int level, int64_t nw, std::string* errp
 // ---------------------------------------------------------------------------------------------
 // hot calls
 // ---------------------------------------------------------------------------------------------
-enum { CALL_OVERLAP = 1, CALL_FB = 2, CALL_GREENS = 4, CALL_ENERGY = 8, CALL_FB_ENERGY = 16 };
+enum { CALL_OVERLAP = 1, CALL_FB = 2, CALL_GREENS = 4, CALL_ENERGY = 8, CALL_FB_ENERGY = 16, CALL_PROPAGATE = 32 };
 
 static void mark(msd_ctx* c, int i, cudaStream_t st) { if (c->profiling) cudaEventRecord(c->ev[i], st); }
+
+// S6: fb[w][g] += sum_(r,q) L_sub^s[g][(r,q)] G^s_w[(r,q)]  (one spin; fb zeroed by the caller: split-K partial sums meet in RED)
+static cudaError_t launch_fb_gemm(msd_ctx* c, int s, int64_t nw, Workspace& ws, cplx* fb, cudaStream_t st)
+{
+    const auto& sp = c->sp[s];
+    const int N = c->N, ldN = N + (N & 1), ng = c->n_chol;
+    GemmArgs a;
+    a.A = sp.d_Lsub; a.B = ws.Gp[s]; a.C = reinterpret_cast<double*>(fb);
+    a.M = ng; a.N = (int)(2 * nw); a.K = sp.n_r * ldN;
+    a.lda = (int64_t)sp.n_r * ldN; a.ldb = (int64_t)sp.n_r * ldN;
+    a.strideA = 0; a.strideB = 0; a.batch = 1;
+    a.zdiv = 1; a.strideC_hi = 0; a.strideC_lo = 0; a.cs_m = 1; a.cs_j = ng;
+    // skinny output (n_chol x 2 n_w): split K over the SMs, partial sums meet in RED.ADD.F64
+    a.accumulate = 2;
+    const int64_t tiles = (int64_t)((a.M + 63) / 64) * ((a.N + 63) / 64);
+    const int ks = (int)std::max<int64_t>(1, (2 * c->n_sm + tiles - 1) / tiles);
+    a.ksplit = std::min(ks, std::max(1, a.K / 64));
+    cudaError_t e = launch_gemm_tn(c, a, st);
+    c->launches++;
+    return e;
+}
 
 static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, const cplx* phi_a, const cplx* phi_b,
                       cplx* out, int* flags, cudaStream_t st)
 {
     const bool energy_like = (call == CALL_ENERGY || call == CALL_FB_ENERGY);
-    const int level = (call == CALL_OVERLAP) ? 1 : (energy_like ? 3 : 2);
+    const int level = (call == CALL_OVERLAP) ? 1 : (energy_like ? 3 : (call == CALL_PROPAGATE ? 4 : 2));
     if (energy_like && !c->energy_ok) return fail(errp, MSD_EUNSUPPORTED, c->energy_why.c_str());
     int rc = ensure_workspace(c, level, n_w, errp);
     if (rc != MSD_OK) return rc;
@@ -741,7 +771,7 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
         int* fl = flags ? flags + w0 : nullptr;
         CK(cudaMemsetAsync(ws.zero_begin, 0, ws.zero_bytes, st));
         mark(c, 0, st);
-        CK(launch_reference(c, N, ldN, c->dev(0), c->dev(1), nw, pa, pb, ws, level >= 3, st));
+        CK(launch_reference(c, N, ldN, c->dev(0), c->dev(1), nw, pa, pb, ws, level == 3, st));
         c->launches++;
         mark(c, 1, st);
         if (call == CALL_OVERLAP) {
@@ -749,6 +779,33 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
             mark(c, 2, st);
             CK(launch_finish_overlap(c, nw, ws, out + w0, fl, st));
             mark(c, 3, st); mark(c, 4, st); mark(c, 5, st);
+        } else if (call == CALL_PROPAGATE) {
+            // one phaseless-AFQMC step (propagate.cu): force bias and overlap of the walkers as they are, the field
+            // matrices of all walkers as one DMMA contraction, the orbital update in place, the overlap of the new walkers
+            cplx* pa_rw = const_cast<cplx*>(pa); cplx* pb_rw = const_cast<cplx*>(pb);
+            CK(launch_dets(c, 1, nw, ws, st));
+            mark(c, 2, st);
+            CK(launch_green_rows(c, nw, ws, nullptr, st));
+            CK(cudaMemsetAsync(ws.fbuf, 0, sizeof(cplx) * (size_t)nw * ng, st));
+            for (int s = 0; s < 2; s++) {
+                const auto& sp = c->sp[s];
+                if (sp.n_r == 0) continue;
+                CK(launch_fb_gemm(c, s, nw, ws, ws.fbuf, st));
+            }
+            CK(launch_finish_overlap(c, nw, ws, ws.ov_old, ws.fl_old, st));
+            mark(c, 3, st);
+            CK(launch_prop_fields(c, nw, c->prop_x + w0 * (int64_t)ng, ws.fbuf, ws.Yf, ws.expo, st));
+            CK(launch_prop_vhs(c, nw, ws.Yf, ws.Aw, st));
+            CK(launch_prop_orbitals(c, nw, ws.Aw, pa_rw, pb_rw, st));
+            mark(c, 4, st);
+            CK(cudaMemsetAsync(ws.zero_begin, 0, ws.zero_bytes, st));
+            CK(launch_reference(c, N, ldN, c->dev(0), c->dev(1), nw, pa, pb, ws, false, st));
+            c->launches++;
+            CK(launch_dets(c, 0, nw, ws, st));
+            CK(launch_finish_overlap(c, nw, ws, ws.ov_new, fl, st));
+            mark(c, 5, st);
+            CK(launch_prop_finish(c, nw, ws.ov_old, ws.ov_new, ws.expo, c->prop_w ? c->prop_w + w0 : nullptr,
+                                  reinterpret_cast<double*>(out) + w0 * 8, ws.fl_old, fl, st));
         } else if (call == CALL_FB || call == CALL_GREENS) {
             CK(launch_dets(c, 1, nw, ws, st));
             mark(c, 2, st);
@@ -769,21 +826,7 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
                 for (int s = 0; s < 2; s++) {
                     const auto& sp = c->sp[s];
                     if (sp.n_r == 0) continue;
-                    GemmArgs a;
-                    a.A = sp.d_Lsub; a.B = ws.Gp[s]; a.C = reinterpret_cast<double*>(fb);
-                    a.M = ng; a.N = (int)(2 * nw); a.K = sp.n_r * ldN;
-                    a.lda = (int64_t)sp.n_r * ldN; a.ldb = (int64_t)sp.n_r * ldN;
-                    a.strideA = 0; a.strideB = 0; a.batch = 1;
-                    a.zdiv = 1; a.strideC_hi = 0; a.strideC_lo = 0; a.cs_m = 1; a.cs_j = ng;
-                    // skinny output (n_chol x 2 n_w): split K over the SMs, partial sums meet in RED.ADD.F64
-                    a.accumulate = 2;
-                    {
-                        int64_t tiles = (int64_t)((a.M + 63) / 64) * ((a.N + 63) / 64);
-                        int ks = (int)std::max<int64_t>(1, (2 * c->n_sm + tiles - 1) / tiles);
-                        a.ksplit = std::min(ks, std::max(1, a.K / 64));
-                    }
-                    CK(launch_gemm_tn(c, a, st));
-                    c->launches++;
+                    CK(launch_fb_gemm(c, s, nw, ws, fb, st));
                 }
                 mark(c, 3, st);
                 CK(launch_finish_flags(c, nw, ws, fb, ng, fl, st));
@@ -898,6 +941,31 @@ extern "C" int msd_local_energy(msd_ctx* c, int64_t n_w, const void* phi_a, cons
 extern "C" int msd_force_bias_energy(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* out, int32_t* flags,
                                      void* stream)
 { return hot_call(c, CALL_FB_ENERGY, n_w, phi_a, phi_b, out, flags, stream); }
+
+extern "C" int msd_propagator_setup(msd_ctx* c, double dt, int n_taylor, const double* h1, const double* L, void* stream)
+{
+    if (!c) return MSD_EINVAL;
+    if (!(dt > 0.0) || n_taylor < 1 || n_taylor > 64 || !h1 || !L) { c->err = "bad argument"; return MSD_EINVAL; }
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != c->device) { c->err = "context used on another device"; return MSD_EINVAL; }
+    cudaError_t e = prop_setup(c, dt, n_taylor, h1, L, (cudaStream_t)stream);
+    if (e != cudaSuccess) {
+        c->err = std::string("propagator setup failed: ") + cudaGetErrorString(e);
+        cudaGetLastError();
+        return e == cudaErrorMemoryAllocation ? MSD_ENOMEM : MSD_ECUDA;
+    }
+    return MSD_OK;
+}
+
+extern "C" int msd_propagate(msd_ctx* c, int64_t n_w, void* phi_a, void* phi_b, const double* x, double* weights,
+                             double* step_out, int32_t* flags, void* stream)
+{
+    if (!c) return MSD_EINVAL;
+    if (c->prop_dt <= 0.0) { c->err = "msd_propagator_setup has not been called"; return MSD_EINVAL; }
+    if (n_w > 0 && !x) { c->err = "bad argument"; return MSD_EINVAL; }
+    c->prop_x = x; c->prop_w = weights;
+    return hot_call(c, CALL_PROPAGATE, n_w, phi_a, phi_b, step_out, flags, stream);
+}
 
 extern "C" int msd_greens(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* G, int32_t* flags,
                           void* stream)

@@ -126,7 +126,7 @@ struct WorkItem {          // a chunk of one bucket, processed by one CTA per wa
 struct Workspace {
     int64_t wc = 0;        // walker capacity of one chunk (multiple of MSD_WT)
     int64_t want = 0;      // padded n_w the layout was made for
-    int level = 0;         // 1 overlap, 2 force bias/greens, 3 energy : which buffers exist
+    int level = 0;         // 1 overlap, 2 force bias/greens, 3 energy, 4 propagation step : which buffers exist
     char* base = nullptr;  // one cudaMalloc
     size_t bytes = 0;
     // views
@@ -149,6 +149,12 @@ struct Workspace {
     cplx* Hrot[2] = {nullptr, nullptr};       // [wc][P]
     cplx* Eacc = nullptr;                     // [wc][2]: (E1_0, E2_0)  (zeroed)
     cplx* X0 = nullptr;                       // [2][nw][n_chol] tr T^g per spin (zeroed)
+    // propagation step (level 4 = force-bias buffers + these)
+    cplx* fbuf = nullptr;                     // [wc][n_chol] force bias v
+    double* Yf = nullptr;                     // [2 wc][ldg] shifted fields as the GEMM operand
+    cplx* Aw = nullptr;                       // [wc][N][N] field matrices i sqrt(dt) sum_g y_g L^g
+    cplx* ov_old = nullptr; cplx* ov_new = nullptr; cplx* expo = nullptr;     // [wc]
+    int* fl_old = nullptr;                    // [wc]
     char* zero_begin = nullptr;               // region memset to 0 at the start of every chunk
     size_t zero_bytes = 0;
 };
@@ -189,6 +195,12 @@ struct msd_ctx {
     int64_t ws_limit_auto = 0;
     int64_t launches = 0;
     int no_smem_tiles = 0;                    // msd_set_option(MSD_OPT_NO_SMEM_TILES): test hook, see include/msd.h
+    // propagation step (msd_propagator_setup / msd_propagate)
+    double* d_LT = nullptr;                   // [N*N][ldg]  L with the Cholesky index contiguous
+    double* d_hp = nullptr;                   // [N][ld]  h' of Eq. 4
+    double* d_E = nullptr;                    // 3 x [ld][ld]: exp(-dt h'/2), the scaled matrix, scratch
+    double prop_dt = 0.0; int prop_taylor = 0;
+    const double* prop_x = nullptr; double* prop_w = nullptr;      // arguments of the running msd_propagate call
     bool energy_ok = true;                    // the energy calls are supported for this trial (window size, see msd_setup)
     std::string energy_why;
     // launch configurations are fixed by the trial: occupancy per (kernel, block size, dynamic shared memory) is queried
@@ -261,6 +273,14 @@ struct Fork {
     cudaStream_t stream(int i);     // i == 0: the caller's stream; i > 0: a side stream that waits for the fork point
     cudaError_t join();
 };
+
+// propagate.cu
+cudaError_t prop_setup(msd_ctx* c, double dt, int n_taylor, const double* h1, const double* L, cudaStream_t st);
+cudaError_t launch_prop_fields(msd_ctx* c, int64_t nw, const double* x, const cplx* v, double* Y, cplx* expo, cudaStream_t st);
+cudaError_t launch_prop_vhs(msd_ctx* c, int64_t nw, const double* Y, cplx* Aw, cudaStream_t st);
+cudaError_t launch_prop_orbitals(msd_ctx* c, int64_t nw, const cplx* Aw, cplx* phi_a, cplx* phi_b, cudaStream_t st);
+cudaError_t launch_prop_finish(msd_ctx* c, int64_t nw, const cplx* ov_old, const cplx* ov_new, const cplx* expo, double* weights,
+                               double* out, const int* fl_old, int* flags, cudaStream_t st);
 
 // msd_api.cu : opt in to `smem` bytes of dynamic shared memory for `func` on the context's device (raised, never lowered,
 // process-wide per device) and return the resident CTAs per SM for (nthr, smem); cached per context.

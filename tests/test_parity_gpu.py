@@ -608,3 +608,79 @@ def test_binding_validates_outputs_and_limits(torch_cuda):
     ref = o2.run(x, return_G=False)
     assert_parity(dict(fb=fb.cpu().numpy(), E=en.cpu().numpy()), ref, what=("fb", "E"))
     trial.close()
+
+
+# ----------------------------------------------------------------------------------------------
+# one phaseless-AFQMC propagation step (Eq. 5, 7-12) against oracle/propagate.py
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,kw,ws,n_taylor", [("tiny", {}, None, 6), ("open-shell", {}, None, 4), ("small", {}, None, 6),
+                                                 ("cu2o2", {}, [0, 7, 8, 100, 199], 6)])
+def test_propagation_step_against_oracle(torch_cuda, name, kw, ws, n_taylor):
+    """msd_propagate: walkers after B(x - xbar), overlap ratio S (rel 1e-10), phase theta (abs 1e-10), importance function,
+    phaseless weight update -- element by element against the numpy oracle on the same seeded fields; full batch on the
+    GPU, sampled walkers in the oracle at the Cu2O2 size."""
+    from oracle import propagate as op
+    torch = torch_cuda
+    msd = _msd()
+    x = mi.generate(name, **kw)
+    dt = 0.005
+    rng = np.random.default_rng(11)
+    fields = rng.standard_normal((x.n_w, x.n_chol))
+    w0 = rng.uniform(0.5, 1.5, x.n_w)
+    trial = msd.setup_from_inputs(x)
+    with pytest.raises(msd.MSDError):          # no time step yet
+        trial.propagate(torch.tensor(x.phi_a, device="cuda"), torch.tensor(x.phi_b, device="cuda"),
+                        torch.tensor(fields, device="cuda"))
+    trial.propagator_setup(dt, n_taylor, x.h1, x.L)
+    pa = torch.tensor(x.phi_a, device="cuda")
+    pb = torch.tensor(x.phi_b, device="cuda")
+    wt = torch.tensor(w0, device="cuda")
+    fl = torch.full((x.n_w,), -1, dtype=torch.int32, device="cuda")
+    out = trial.propagate(pa, pb, torch.tensor(fields, device="cuda"), weights=wt, flags=fl).cpu().numpy()
+    assert (fl.cpu().numpy() == 0).all()
+    # the propagated walkers are ordinary walkers: the hot calls accept them
+    ov_again = trial.overlap(pa, pb).cpu().numpy()
+    trial.close()
+    ref = op.step(x, fields, dt, weights=w0, n_taylor=n_taylor, walkers=ws)
+    sel = np.arange(x.n_w) if ws is None else np.asarray(ws)
+    pa, pb, wt = pa.cpu().numpy()[sel], pb.cpu().numpy()[sel], wt.cpu().numpy()[sel]
+    out = out[sel]
+    assert np.abs(pa - ref["phi_a"]).max() <= 1e-12 * np.abs(ref["phi_a"]).max()
+    assert np.abs(pb - ref["phi_b"]).max() <= 1e-12 * np.abs(ref["phi_b"]).max()
+    S = out[:, 0] + 1j * out[:, 1]
+    assert (np.abs(S - ref["S"]) / np.abs(ref["S"])).max() <= TOL_REL
+    dth = np.angle(np.exp(1j * (out[:, 2] - ref["theta"])))
+    assert np.abs(dth).max() <= TOL_REL
+    ovn = out[:, 4] + 1j * out[:, 5]
+    assert (np.abs(ovn - ref["ovlp_new"]) / np.abs(ref["ovlp_new"])).max() <= TOL_REL
+    assert (np.abs(ov_again[sel] - ref["ovlp_new"]) / np.abs(ref["ovlp_new"])).max() <= TOL_REL
+    I = out[:, 6] + 1j * out[:, 7]
+    assert (np.abs(I - ref["I"]) / np.abs(ref["I"])).max() <= TOL_REL
+    assert np.abs(out[:, 3] - ref["I_ph"]).max() <= TOL_REL * max(1.0, np.abs(ref["I_ph"]).max())
+    assert np.abs(wt - ref["w"]).max() <= TOL_REL * max(1.0, np.abs(ref["w"]).max())
+
+
+def test_propagation_step_chunked_and_repeated(torch_cuda):
+    """Two steps in a row under a workspace limit that forces walker chunks equal two oracle steps; dt can be changed."""
+    from oracle import propagate as op
+    torch = torch_cuda
+    msd = _msd()
+    x = mi.generate("small", n_w=21, n_det=300)
+    rng = np.random.default_rng(3)
+    f1, f2 = rng.standard_normal((2, x.n_w, x.n_chol))
+    trial = msd.setup_from_inputs(x)
+    trial.set_workspace_limit(600 * 1024)          # one walker tile needs 0.41 MB, two 0.83 MB: three chunks
+    trial.propagator_setup(0.01, 6, x.h1, x.L)
+    trial.propagator_setup(0.004, 6, x.h1, x.L)
+    pa = torch.tensor(x.phi_a, device="cuda")
+    pb = torch.tensor(x.phi_b, device="cuda")
+    wt = torch.ones(x.n_w, dtype=torch.float64, device="cuda")
+    trial.propagate(pa, pb, torch.tensor(f1, device="cuda"), weights=wt)
+    out = trial.propagate(pa, pb, torch.tensor(f2, device="cuda"), weights=wt).cpu().numpy()
+    trial.close()
+    r1 = op.step(x, f1, 0.004)
+    r2 = op.step(x.with_walkers(r1["phi_a"], r1["phi_b"]), f2, 0.004, weights=r1["w"])
+    assert np.abs(pa.cpu().numpy() - r2["phi_a"]).max() <= 1e-11 * np.abs(r2["phi_a"]).max()
+    S = out[:, 0] + 1j * out[:, 1]
+    assert (np.abs(S - r2["S"]) / np.abs(r2["S"])).max() <= TOL_REL
+    assert np.abs(wt.cpu().numpy() - r2["w"]).max() <= TOL_REL * np.abs(r2["w"]).max()
