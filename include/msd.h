@@ -184,8 +184,12 @@ int msd_get_phase_ms(msd_ctx* ctx, float* ms, int n);
  *       only for active windows too wide for shared memory, so that those paths can be parity-tested on small inputs:
  *       1 = a walker tile's CI matrix / Hrot / F do not fit (RED.ADD scatter of C, Hrot / F through L1);
  *       2 = the tile's g slices do not fit either (n_o n_v summed over spins above ~1600: g through L1 as well).
- *       Results are the same.  Unknown option or value: MSD_EINVAL. */
+ *       Results are the same.  Unknown option or value: MSD_EINVAL.
+ *   MSD_OPT_NO_FUSED_S7 (0 / 1; default 0): TEST HOOK.  1 takes the two-kernel form of the half rotation (Lambda = L_sub Theta
+ *       written to memory by the GEMM, dense intermediates by a second kernel) that otherwise only runs for shapes the fused
+ *       kernel does not cover.  Results are the same. */
 #define MSD_OPT_NO_SMEM_TILES 1
+#define MSD_OPT_NO_FUSED_S7 2
 int msd_set_option(msd_ctx* ctx, int option, int64_t value);
 
 void msd_destroy(msd_ctx* ctx);

@@ -26,6 +26,7 @@ EXPORTS = ["msd_setup", "msd_setup_from_occ", "msd_overlap", "msd_force_bias", "
            "msd_get_info", "msd_get_packed", "msd_set_workspace_limit", "msd_set_option", "msd_launch_count",
            "msd_set_profiling", "msd_get_phase_ms", "msd_destroy", "msd_last_error"]
 MSD_OPT_NO_SMEM_TILES = 1
+MSD_OPT_NO_FUSED_S7 = 2
 
 
 class MSDError(RuntimeError):

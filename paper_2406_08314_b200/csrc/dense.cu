@@ -470,6 +470,313 @@ k_energy_dense_mma(int n_chol, int64_t nw, int gchunk, SpinDev sa, SpinDev sb, c
     if (tid == 0) red_add(&Eacc[w * 2 + 1], cscale(-0.5, ex));
 }
 
+// ------------------------------------------------------------------------------------------------
+// S7 fused: the half rotation Lam^g = L_sub^g Theta and everything k_energy_dense_mma derives from it in ONE kernel, so that
+// Lam (1.8 GB at fe2s2) is never written to or read from HBM.  A warp owns slice g of walker w: it computes the n_r x n
+// complex tile Lam^g by FP64 DMMA (MTG x NTG tiles of 8x8, accumulators in registers; its rows of L_sub stream through a
+// per-warp two-stage cp.async buffer, the walker's Theta^T operand sits in shared memory for the whole CTA), drops the tile
+// into its T / Lam_v buffers and carries on with the dense steps of k_energy_dense_mma (X0, Ex0, Bfull, FK) on the same data.
+// When the reference occupies the first n orbitals (n even), Theta[occ rows] is the identity, so the contraction runs over the
+// N - n virtual orbitals only and L_sub[g][r][occ_i] is added as a constant (20 % fewer flops at fe2s2).
+// Shapes: MTG = ceil(n_r / 8) <= 5, NTG = ceil(2 n / 8) <= 6 as template parameters (a predicated-off DMMA costs as much as
+// an executed one, so the tile counts must be compile-time); other shapes take the two-kernel path.
+// ------------------------------------------------------------------------------------------------
+#define FUSE_NWARP 4
+#define FUSE_BK 16
+#define FUSE_LDA 20
+__host__ __device__ inline int fused_ldbs(int Kv) { return (Kv + 15) / 16 * 16 + 4; }
+template <int NWARP, int MTC, int NTC, int MTG, int NTG>
+__global__ void __launch_bounds__(NWARP * 32, NWARP == 8 ? 1 : 2)
+k_energy_fused(int n_chol, int64_t nw, int gchunk, int ldN, int koff, int Kv, SpinDev sa, SpinDev sb,
+               const cplx* __restrict__ theta_a, const cplx* __restrict__ theta_b, const double* __restrict__ thT_a,
+               const double* __restrict__ thT_b, cplx* Bp_a, cplx* Bp_b, cplx* X0 /*[2][nw][n_chol]*/, cplx* F_a, cplx* F_b,
+               cplx* Hrot_a, cplx* Hrot_b, cplx* Eacc, int N)
+{
+    extern __shared__ __align__(16) double smd[];
+    const int s = blockIdx.z;
+    const int64_t w = blockIdx.y;
+    const SpinDev sp = s ? sb : sa;
+    const int n = sp.n, no = sp.n_o, nv = sp.n_v, nr = sp.n_r, P = sp.P;
+    if (n == 0) return;
+    const DenseMmaLayout L(n, nv);
+    const cplx* theta = (s ? theta_b : theta_a) + w * (int64_t)N * n;
+    const double* thT = (s ? thT_b : thT_a) + w * (int64_t)n * 2 * ldN;     // rows (i, c), K = q contiguous
+    const double* Lsub = sp.Lsub;
+    cplx* Bp = (s ? Bp_b : Bp_a) + w * (int64_t)P * n_chol;
+    cplx* F = (s ? F_b : F_a) + w * (int64_t)P;
+    cplx* Hrot = (s ? Hrot_b : Hrot_a) + w * (int64_t)P;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int gq = lane >> 2, tq = lane & 3;
+
+    const int wdoubles = max(L.warp_doubles, 2 * 8 * MTG * FUSE_LDA);     // per-warp buffer: T + Lam_v, aliased by the A stages
+    const int Kvp = (Kv + 3) & ~3;                            // k4-steps; loads beyond Kv are zero-filled
+    const int ldbs = fused_ldbs(Kv);                          // row stride of the Theta^T operand (= 4 mod 16: conflict-free)
+    double* Ap = smd;                                         // [2 half][lda]
+    double* wbase = Ap + 2 * L.half * L.lda;
+    double* wbuf = wbase + wid * wdoubles;
+    double* Tb = wbuf;                                        // [trows][ldt]   (i, c) interleaved
+    double* Lb = wbuf + L.trows * L.ldt;                      // [half][ldb]    Lam_v, then Bfull in place
+    double* Bs = wbase + NWARP * wdoubles;                    // [8 NTG][ldbs]  Theta^T columns (i, c) x virtual orbitals
+    int* pos = reinterpret_cast<int*>(Bs + 8 * NTG * ldbs);   // [16]
+
+    {
+        const int tot = 2 * L.half * L.lda + NWARP * wdoubles + 8 * NTG * ldbs;
+        for (int e = tid; e < tot; e += NWARP * 32) smd[e] = 0.0;
+        if (tid < 16) pos[tid] = tid < no ? sp.pos_o[tid] : 0;
+    }
+    __syncthreads();
+    for (int e = tid; e < nv * n; e += NWARP * 32) {
+        const int r = e / n, l = e - r * n;
+        const cplx t = theta[(int64_t)sp.act_v[r] * n + l];
+        Ap[r * L.lda + 2 * l] = -t.x;            Ap[r * L.lda + 2 * l + 1] = t.y;
+        Ap[(L.half + r) * L.lda + 2 * l] = -t.y; Ap[(L.half + r) * L.lda + 2 * l + 1] = -t.x;
+    }
+    for (int e = tid; e < 2 * n * Kv; e += NWARP * 32) {
+        const int col = e / Kv, k = e - col * Kv;
+        Bs[col * ldbs + k] = (koff + k < ldN) ? thT[(int64_t)col * ldN + koff + k] : 0.0;
+    }
+    __syncthreads();
+
+    const int MT = MTC > 0 ? MTC : 2 * L.half / 8;            // <= 4
+    const int NT = NTC > 0 ? NTC : (n + 7) / 8;
+    const int KS = L.Kp / 4;
+    const int posh[2] = {pos[gq], pos[8 + gq]};
+    const int kc = tq & 1, kl = tq >> 1;
+    double fk[4][2][2];
+#pragma unroll
+    for (int a = 0; a < 4; a++)
+#pragma unroll
+        for (int b = 0; b < 2; b++) { fk[a][b][0] = 0.0; fk[a][b][1] = 0.0; }
+    cplx ex_part = cmake(0.0, 0.0);
+    int a4off[4];
+    long long a4sgn[4];
+#pragma unroll
+    for (int mt = 0; mt < 4; mt++) {
+        const int m = 8 * mt + gq, im = m >= L.half, r = m - im * L.half;
+        a4off[mt] = r * L.ldb + 2 * kl + (kc ^ im);
+        a4sgn[mt] = (!im && kc) ? (long long)0x8000000000000000ull : 0ll;
+    }
+    int ooff[8];
+#pragma unroll
+    for (int t = 0; t < 8; t++) {
+        const int x = tid / NWARP + 32 * t;
+        const int r = x / no, h = x - r * no;
+        ooff[t] = (x < P) ? r * L.ldb + 2 * pos[h] : 0;
+    }
+    const int g_begin = blockIdx.x * gchunk;
+    const int g_end = min(g_begin + gchunk, n_chol + 1);
+    const int nchunk = (Kvp + FUSE_BK - 1) / FUSE_BK;
+    for (int g0 = g_begin; g0 < g_end; g0 += NWARP) {
+        const int g = g0 + wid;
+        const bool live = g < g_end;
+        if (live) {
+            // ---- Lam^g = L_sub^g[:, virtual columns] Theta_V (+ L_sub^g[:, occ columns]) by DMMA, accumulators in registers ----
+            const double* Arow = Lsub + ((int64_t)g * nr) * ldN + koff;
+            double* As = wbuf;                                 // [2][8 MTG][FUSE_LDA]  (aliases Tb / Lb: they are dead here)
+            // lane -> (row lane / 8 + 4 t, 16-byte column lane % 8): plain pointer increments, no per-element index arithmetic
+            const double* asrc = Arow + (int64_t)(lane >> 3) * ldN + (lane & 7) * 2;
+            double* adst = As + (lane >> 3) * FUSE_LDA + (lane & 7) * 2;
+            const int arows = (nr - (lane >> 3) + 3) >> 2;      // rows of this lane: lane / 8, lane / 8 + 4, ...
+            auto load_chunk = [&](int st, int ck) {
+                const int k0 = ck * FUSE_BK;
+                const bool ok = k0 + (lane & 7) * 2 < Kv;
+                const double* sp_ = asrc + k0;
+                double* dp = adst + st * 8 * MTG * FUSE_LDA;
+                for (int t = 0; t < arows; t++) {
+                    cp_async16(dp, ok ? sp_ : Arow, ok ? 16 : 0);
+                    sp_ += 4 * (int64_t)ldN; dp += 4 * FUSE_LDA;
+                }
+            };
+            load_chunk(0, 0);
+            cp_async_commit();
+            // accumulators start from the occupied columns of L_sub (Theta[occ rows] = 1): thread holds (row 8i + gq, column 4j + tq);
+            // these loads are in flight while the first chunk arrives
+            double acc[MTG][NTG][2];
+#pragma unroll
+            for (int i = 0; i < MTG; i++)
+#pragma unroll
+                for (int j = 0; j < NTG; j++) {
+                    const int r = 8 * i + gq, ic = 4 * j + tq;
+                    acc[i][j][0] = (koff && r < nr && ic < n) ? __ldg(Lsub + ((int64_t)g * nr + r) * ldN + ic) : 0.0;
+                    acc[i][j][1] = 0.0;
+                }
+            for (int ck = 0; ck < nchunk; ck++) {
+                if (ck + 1 < nchunk) load_chunk((ck + 1) & 1, ck + 1);
+                cp_async_commit();
+                cp_async_wait<1>();
+                __syncwarp();
+                const double* as = As + (ck & 1) * 8 * MTG * FUSE_LDA + gq * FUSE_LDA + tq;
+                const double* bs = Bs + gq * ldbs + ck * FUSE_BK + tq;
+                auto kstep = [&](int kk) {
+                    double a[MTG], b[NTG];
+#pragma unroll
+                    for (int i = 0; i < MTG; i++) a[i] = as[i * 8 * FUSE_LDA + kk * 4];
+#pragma unroll
+                    for (int j = 0; j < NTG; j++) b[j] = bs[j * 8 * ldbs + kk * 4];
+#pragma unroll
+                    for (int i = 0; i < MTG; i++)
+#pragma unroll
+                        for (int j = 0; j < NTG; j++) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                };
+                const int ksteps = min(FUSE_BK, Kvp - ck * FUSE_BK) / 4;
+                if (ksteps == FUSE_BK / 4) {       // full chunk: straight-line code, fragment loads of step k+1 overlap the DMMAs of step k
+#pragma unroll
+                    for (int kk = 0; kk < FUSE_BK / 4; kk++) kstep(kk);
+                } else {
+#pragma unroll 1
+                    for (int kk = 0; kk < ksteps; kk++) kstep(kk);
+                }
+                __syncwarp();          // the stage is overwritten by the load issued in the next iteration
+            }
+            cp_async_wait<0>();
+            __syncwarp();
+            // accumulators -> T (rows < n) and Lam_v (rows n .. n_r)
+#pragma unroll
+            for (int i = 0; i < MTG; i++) {
+                const int r = 8 * i + gq;
+#pragma unroll
+                for (int j = 0; j < NTG; j++) {
+                    const int ic = 4 * j + tq;
+                    if (r < nr && ic < n) {
+                        double* dst = (r < n) ? Tb + r * L.ldt + 2 * ic : Lb + (r - n) * L.ldb + 2 * ic;
+                        *reinterpret_cast<double2*>(dst) = make_double2(acc[i][j][0], acc[i][j][1]);
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if (live) {
+            // X0 = tr T, Ex0 += sum T[l][i] T[i][l]
+            cplx tr = cmake(0.0, 0.0);
+            for (int l = lane; l < n; l += 32) tr = cadd(tr, cmake(Tb[l * L.ldt + 2 * l], Tb[l * L.ldt + 2 * l + 1]));
+            if (g < n_chol)
+                for (int i = lane; i < n; i += 32) {
+                    int l = i;
+                    cplx e1 = cmake(0.0, 0.0);                 // second chain: the FMA latency is not on the critical path
+                    for (int t = 0; t + 1 < n; t += 2) {
+                        const int l2 = (l + 1 == n) ? 0 : l + 1;
+                        ex_part = cfma(*reinterpret_cast<const cplx*>(Tb + l * L.ldt + 2 * i),
+                                       *reinterpret_cast<const cplx*>(Tb + i * L.ldt + 2 * l), ex_part);
+                        e1 = cfma(*reinterpret_cast<const cplx*>(Tb + l2 * L.ldt + 2 * i),
+                                  *reinterpret_cast<const cplx*>(Tb + i * L.ldt + 2 * l2), e1);
+                        l = (l2 + 1 == n) ? 0 : l2 + 1;
+                    }
+                    if (n & 1)
+                        e1 = cfma(*reinterpret_cast<const cplx*>(Tb + l * L.ldt + 2 * i),
+                                  *reinterpret_cast<const cplx*>(Tb + i * L.ldt + 2 * l), e1);
+                    ex_part = cadd(ex_part, e1);
+                }
+            for (int o = 16; o > 0; o >>= 1) {
+                tr.x += __shfl_down_sync(0xffffffffu, tr.x, o);
+                tr.y += __shfl_down_sync(0xffffffffu, tr.y, o);
+            }
+            if (lane == 0) {
+                if (g < n_chol) X0[((int64_t)s * nw + w) * n_chol + g] = tr;
+                else red_add(&Eacc[w * 2 + 0], tr);
+            }
+            // step 2: Bfull = Lam_v + A' B', n-tiles in chunks of 3
+            for (int nt0 = 0; nt0 < NT; nt0 += 3) {
+                double acc2[4][3][2];
+#pragma unroll
+                for (int mt = 0; mt < 4; mt++) {
+                    const int m = 8 * mt + gq, im = m >= L.half, r = m - im * L.half;
+#pragma unroll
+                    for (int j = 0; j < 3; j++) {
+                        const int i = 8 * (nt0 + j) + 2 * tq;
+                        const bool ok = mt < MT && r < nv;
+                        acc2[mt][j][0] = (ok && i < n) ? Lb[r * L.ldb + 2 * i + im] : 0.0;
+                        acc2[mt][j][1] = (ok && i + 1 < n) ? Lb[r * L.ldb + 2 * i + 2 + im] : 0.0;
+                    }
+                }
+#pragma unroll 2
+                for (int kk = 0; kk < KS; kk++) {
+                    double a[4], b[3];
+#pragma unroll
+                    for (int mt = 0; mt < 4; mt++) a[mt] = mt < MT ? Ap[(8 * mt + gq) * L.lda + 4 * kk + tq] : 0.0;
+#pragma unroll
+                    for (int j = 0; j < 3; j++)
+                        b[j] = (nt0 + j < NT) ? Tb[(2 * kk + kl) * L.ldt + 2 * (8 * (nt0 + j) + gq) + kc] : 0.0;
+#pragma unroll
+                    for (int mt = 0; mt < 4; mt++)
+#pragma unroll
+                        for (int j = 0; j < 3; j++)
+                            if (mt < MT && nt0 + j < NT) dmma884(acc2[mt][j][0], acc2[mt][j][1], a[mt], b[j]);
+                }
+#pragma unroll
+                for (int mt = 0; mt < 4; mt++) {
+                    const int m = 8 * mt + gq, im = m >= L.half, r = m - im * L.half;
+#pragma unroll
+                    for (int j = 0; j < 3; j++) {
+                        const int i = 8 * (nt0 + j) + 2 * tq;
+                        const bool ok = mt < MT && r < nv;
+                        if (ok && i < n) Lb[r * L.ldb + 2 * i + im] = acc2[mt][j][0];
+                        if (ok && i + 1 < n) Lb[r * L.ldb + 2 * i + 2 + im] = acc2[mt][j][1];
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if (live && g < n_chol) {
+            // step 4: FK += A''(Bfull) B''(T[:, pos])
+#pragma unroll 2
+            for (int kk = 0; kk < KS; kk++) {
+                double a[4], b[2];
+#pragma unroll
+                for (int mt = 0; mt < 4; mt++) {
+                    const double v = mt < MT ? Lb[a4off[mt] + 4 * kk] : 0.0;
+                    a[mt] = __longlong_as_double(__double_as_longlong(v) ^ a4sgn[mt]);
+                }
+#pragma unroll
+                for (int j = 0; j < 2; j++) b[j] = Tb[(2 * kk + kl) * L.ldt + 2 * posh[j] + kc];
+#pragma unroll
+                for (int mt = 0; mt < 4; mt++)
+#pragma unroll
+                    for (int j = 0; j < 2; j++)
+                        if (mt < MT) dmma884(fk[mt][j][0], fk[mt][j][1], a[mt], b[j]);
+            }
+        }
+        __syncthreads();
+        {   // cooperative output of the round's slices: thread (x, gi) -> NWARP consecutive slices of one pair index
+            const int gcount = min(NWARP, g_end - g0);
+            const int gi = tid % NWARP;
+#pragma unroll
+            for (int t = 0; t < 8; t++) {
+                const int x = tid / NWARP + 32 * t;
+                if (x >= P || gi >= gcount) continue;
+                const int gg = g0 + gi;
+                const double* lb = wbase + gi * wdoubles + L.trows * L.ldt;
+                const cplx b = cmake(lb[ooff[t]], lb[ooff[t] + 1]);
+                if (gg < n_chol) Bp[(int64_t)x * n_chol + gg] = b;
+                else Hrot[x] = b;
+            }
+        }
+        __syncthreads();
+    }
+
+    // FK: sum the warps' partial tiles, then F -= FK (exchange-like part of F, W9); Ex0
+    double* red = wbase;                                       // aliases the warp buffers (all reads are done)
+#pragma unroll
+    for (int mt = 0; mt < 4; mt++)
+#pragma unroll
+        for (int j = 0; j < 2; j++) {
+            if (mt >= MT) continue;
+            double* dst = red + ((wid * 2 * L.half) + 8 * mt + gq) * 16 + 8 * j + 2 * tq;
+            dst[0] = fk[mt][j][0]; dst[1] = fk[mt][j][1];
+        }
+    __syncthreads();
+    for (int x = tid; x < P; x += NWARP * 32) {
+        const int r = x / no, h = x - r * no;
+        double re = 0.0, im = 0.0;
+        for (int ww = 0; ww < NWARP; ww++) {
+            re += red[((ww * 2 * L.half) + r) * 16 + h];
+            im += red[((ww * 2 * L.half) + L.half + r) * 16 + h];
+        }
+        red_add(&F[x], cmake(-re, -im));
+    }
+    cplx ex = block_sum(ex_part);
+    if (tid == 0) red_add(&Eacc[w * 2 + 1], cscale(-0.5, ex));
+}
+
 // F[x] += sum_g Xt_g B^g[x]  (Coulomb-like part of F, W9);   one warp per x
 __global__ void __launch_bounds__(256)
 k_fx(int n_chol, int64_t nw, int Pa, int Pb, const cplx* __restrict__ X0, const cplx* __restrict__ Bp_a,
@@ -538,6 +845,70 @@ size_t energy_dense_smem(const msd_ctx* c, int GC)
         if (v > smem) smem = v;
     }
     return smem;
+}
+
+template <int NWARP, int MTC, int NTC, int MTG, int NTG>
+static cudaError_t launch_fused_t(msd_ctx* c, int64_t nw, Workspace& ws, int koff, int Kv, cudaStream_t st)
+{
+    const int ldN = c->N + (c->N & 1);
+    size_t smem = 0;
+    for (int s = 0; s < 2; s++) {
+        const auto& sp = c->sp[s];
+        if (sp.n == 0) continue;
+        DenseMmaLayout L(sp.n, sp.n_v);
+        const int wd = std::max(L.warp_doubles, 2 * 8 * MTG * FUSE_LDA);
+        smem = std::max(smem, ((size_t)2 * L.half * L.lda + (size_t)NWARP * wd + (size_t)8 * NTG * fused_ldbs(Kv)) * sizeof(double) + 64);
+    }
+    if (smem > 227 * 1024) return cudaErrorNotSupported;
+    cudaError_t e = func_config(c, (const void*)k_energy_fused<NWARP, MTC, NTC, MTG, NTG>, NWARP * 32, smem, nullptr);
+    if (e != cudaSuccess) return e;
+    const int gchunk = 64;
+    dim3 grid((c->n_chol + 1 + gchunk - 1) / gchunk, (unsigned)nw, 2);
+    k_energy_fused<NWARP, MTC, NTC, MTG, NTG><<<grid, NWARP * 32, smem, st>>>(
+        c->n_chol, nw, gchunk, ldN, koff, Kv, c->dev(0), c->dev(1), ws.theta[0], ws.theta[1], ws.thetaT[0], ws.thetaT[1],
+        ws.Bp[0], ws.Bp[1], ws.X0, ws.F[0], ws.F[1], ws.Hrot[0], ws.Hrot[1], ws.Eacc, c->N);
+    return cudaGetLastError();
+}
+
+// true (and *koff, *Kv set) when the fused S7 kernel covers this trial: both spins with electrons share the tile counts and the
+// shape is one of the instantiated ones
+bool energy_fused_shape(const msd_ctx* c, int* mtc, int* ntc, int* mtg, int* ntg, int* koff, int* Kv)
+{
+    int a = -1, b = -1, m = -1, t = -1;
+    bool contiguous = true;
+    int nn = -1;
+    for (int s = 0; s < 2; s++) {
+        const auto& sp = c->sp[s];
+        if (sp.n == 0) continue;
+        if (sp.n_o > 16 || sp.n_v > 16 || sp.n > 24) return false;
+        const int A = 2 * ((sp.n_v + 7) / 8 * 8) / 8, B = (sp.n + 7) / 8, M = (sp.n_r + 7) / 8, T = (2 * sp.n + 7) / 8;
+        if (a == -1) { a = A; b = B; m = M; t = T; nn = sp.n; }
+        else if (a != A || b != B || m != M || t != T) return false;
+        if (sp.n != nn || (sp.n & 1)) contiguous = false;
+        for (int l = 0; l < sp.n; l++) if (sp.occ_ref[l] != l) contiguous = false;
+    }
+    if (a == -1) return false;
+    const bool have = (a == 4 && b == 3 && m == 5 && t == 5) || (a == 4 && b == 2 && m == 4 && t == 4) ||
+                      (a == 4 && b == 2 && m == 4 && t == 3) || (a == 2 && b == 1 && m == 2 && t == 2);
+    if (!have) return false;
+    const int ldN = c->N + (c->N & 1);
+    *mtc = a; *ntc = b; *mtg = m; *ntg = t;
+    *koff = contiguous ? nn : 0;
+    *Kv = ldN - *koff;
+    return true;
+}
+
+cudaError_t launch_energy_fused(msd_ctx* c, int64_t nw, Workspace& ws, cudaStream_t st)
+{
+    int a, b, m, t, koff, Kv;
+    if (!energy_fused_shape(c, &a, &b, &m, &t, &koff, &Kv)) return cudaErrorNotSupported;
+    cudaError_t e;
+    if (a == 4 && b == 3) e = launch_fused_t<FUSE_NWARP, 4, 3, 5, 5>(c, nw, ws, koff, Kv, st);
+    else if (a == 4 && t == 4) e = launch_fused_t<FUSE_NWARP, 4, 2, 4, 4>(c, nw, ws, koff, Kv, st);
+    else if (a == 4) e = launch_fused_t<FUSE_NWARP, 4, 2, 4, 3>(c, nw, ws, koff, Kv, st);
+    else e = launch_fused_t<FUSE_NWARP, 2, 1, 2, 2>(c, nw, ws, koff, Kv, st);
+    if (e == cudaSuccess) c->launches++;
+    return e;
 }
 
 cudaError_t launch_energy_dense(msd_ctx* c, int64_t nw, Workspace& ws, cudaStream_t st)

@@ -429,6 +429,10 @@ static int do_setup(msd_ctx* c, std::string* errp, int N, int na, int nb, int n_
         CK(upload(&c->d_items_pull, c->items_pull.data(), c->items_pull.size(), st));
         CK(cudaStreamSynchronize(st));
     }
+    {
+        int a, b, m, t, ko, kv;
+        c->need_lam = !energy_fused_shape(c, &a, &b, &m, &t, &ko, &kv);
+    }
     CK(upload(&c->d_items_cf, c->items_cf.data(), c->items_cf.size(), st));
     CK(upload(&c->d_items_gen, c->items_gen.data(), c->items_gen.size(), st));
     CK(cudaStreamSynchronize(st));
@@ -564,6 +568,13 @@ extern "C" int msd_set_option(msd_ctx* c, int option, int64_t value)
 {
     if (!c) return MSD_EINVAL;
     if (option == MSD_OPT_NO_SMEM_TILES && value >= 0 && value <= 2) { c->no_smem_tiles = (int)value; return MSD_OK; }
+    if (option == MSD_OPT_NO_FUSED_S7 && (value == 0 || value == 1)) {
+        c->no_fused = value != 0;
+        int a, b, m, t, ko, kv;
+        c->need_lam = c->no_fused || !energy_fused_shape(c, &a, &b, &m, &t, &ko, &kv);
+        c->ws.want = 0;                  // the workspace layout changes (Lambda buffer)
+        return MSD_OK;
+    }
     c->err = "unknown option or value";
     return MSD_EINVAL;
 }
@@ -675,7 +686,7 @@ static size_t carve(const msd_ctx* c, Workspace& ws, char* base, int64_t wc, int
         for (int s = 0; s < 2; s++) {
             const auto& sp = c->sp[s];
             ws.thetaT[s] = k.take<double>((size_t)wc * sp.n * 2 * ldN);
-            ws.Lam[s] = k.take<cplx>((size_t)(ng + 1) * sp.n_r * wc * sp.n);
+            ws.Lam[s] = c->need_lam ? k.take<cplx>((size_t)(ng + 1) * sp.n_r * wc * sp.n) : nullptr;
             ws.Bp[s] = k.take<cplx>((size_t)wc * sp.P * ng);
             ws.Vss[s] = k.take<cplx>((size_t)nt * sp.P * sp.P * MSD_WT);
             ws.Hrot[s] = k.take<cplx>((size_t)wc * sp.P);
@@ -833,26 +844,30 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
             }
             mark(c, 4, st); mark(c, 5, st);
         } else {   // energy
-            // Lambda = L_sub Theta for every slice (incl. h1), both spins
-            // (independent launches of one phase are forked over the side streams: the last, partly filled wave of one
-            // GEMM overlaps the first wave of the next)
-            Fork fl_(c, st);
-            for (int s = 0; s < 2; s++) {
-                const auto& sp = c->sp[s];
-                if (sp.n == 0 || sp.n_r == 0) continue;
-                GemmArgs a;
-                a.A = sp.d_Lsub; a.B = ws.thetaT[s]; a.C = reinterpret_cast<double*>(ws.Lam[s]);
-                a.M = (ng + 1) * sp.n_r; a.N = (int)(2 * sp.n * nw); a.K = ldN;
-                a.lda = ldN; a.ldb = ldN; a.strideA = 0; a.strideB = 0; a.batch = 1;
-                a.zdiv = 1; a.strideC_hi = 0; a.strideC_lo = 0; a.cs_m = (int64_t)nw * sp.n; a.cs_j = 1;
-                a.accumulate = 0;
-                cudaError_t ge = launch_gemm_tn(c, a, fl_.stream(s));
-                if (ge != cudaSuccess) { fl_.join(); CK(ge); }
-                c->launches++;
-            }
-            CK(fl_.join());
-            mark(c, 2, st);
-            CK(launch_energy_dense(c, nw, ws, st));
+            // S7: Lambda = L_sub Theta and the dense intermediates.  Fused kernel (Lambda never leaves the SM) when the shape is
+            // covered, else the Lambda GEMM + dense kernel pair
+            cudaError_t fe = c->no_fused ? cudaErrorNotSupported : launch_energy_fused(c, nw, ws, st);
+            if (fe != cudaSuccess && fe != cudaErrorNotSupported) CK(fe);
+            if (fe == cudaErrorNotSupported) {
+                cudaGetLastError();
+                Fork fl_(c, st);
+                for (int s = 0; s < 2; s++) {
+                    const auto& sp = c->sp[s];
+                    if (sp.n == 0 || sp.n_r == 0) continue;
+                    GemmArgs a;
+                    a.A = sp.d_Lsub; a.B = ws.thetaT[s]; a.C = reinterpret_cast<double*>(ws.Lam[s]);
+                    a.M = (ng + 1) * sp.n_r; a.N = (int)(2 * sp.n * nw); a.K = ldN;
+                    a.lda = ldN; a.ldb = ldN; a.strideA = 0; a.strideB = 0; a.batch = 1;
+                    a.zdiv = 1; a.strideC_hi = 0; a.strideC_lo = 0; a.cs_m = (int64_t)nw * sp.n; a.cs_j = 1;
+                    a.accumulate = 0;
+                    cudaError_t ge = launch_gemm_tn(c, a, fl_.stream(s));
+                    if (ge != cudaSuccess) { fl_.join(); CK(ge); }
+                    c->launches++;
+                }
+                CK(fl_.join());
+                mark(c, 2, st);
+                CK(launch_energy_dense(c, nw, ws, st));
+            } else mark(c, 2, st);
             mark(c, 3, st);
             // V GEMMs: ab, aa, bb
             Fork fv_(c, st);

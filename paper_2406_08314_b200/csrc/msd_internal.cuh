@@ -201,6 +201,8 @@ struct msd_ctx {
     double* d_E = nullptr;                    // 3 x [ld][ld]: exp(-dt h'/2), the scaled matrix, scratch
     double prop_dt = 0.0; int prop_taylor = 0;
     const double* prop_x = nullptr; double* prop_w = nullptr;      // arguments of the running msd_propagate call
+    bool no_fused = false;                    // MSD_OPT_NO_FUSED_S7: take the Lambda GEMM + dense kernel pair (test hook)
+    bool need_lam = true;                     // the workspace holds the Lambda buffer (two-kernel S7 path)
     bool energy_ok = true;                    // the energy calls are supported for this trial (window size, see msd_setup)
     std::string energy_why;
     // launch configurations are fixed by the trial: occupancy per (kernel, block size, dynamic shared memory) is queried
@@ -258,6 +260,8 @@ cudaError_t launch_dets(msd_ctx* c, int mode, int64_t nw, Workspace& ws, cudaStr
 // dense.cu
 cudaError_t launch_green_rows(msd_ctx* c, int64_t nw, Workspace& ws, cplx* Gfull /*or null*/, cudaStream_t st);
 cudaError_t launch_energy_dense(msd_ctx* c, int64_t nw, Workspace& ws, cudaStream_t st);
+cudaError_t launch_energy_fused(msd_ctx* c, int64_t nw, Workspace& ws, cudaStream_t st);   // cudaErrorNotSupported: use the two-kernel path
+bool energy_fused_shape(const msd_ctx* c, int* mtc, int* ntc, int* mtg, int* ntg, int* koff, int* Kv);
 size_t energy_dense_smem(const msd_ctx* c, int GC);      // shared memory of the scalar S7 kernel with GC slices per CTA
 cudaError_t launch_fx(msd_ctx* c, int64_t nw, Workspace& ws, cudaStream_t st);
 cudaError_t launch_finish_overlap(msd_ctx* c, int64_t nw, Workspace& ws, cplx* ovlp, int* flags, cudaStream_t st);
