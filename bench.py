@@ -420,27 +420,45 @@ def main():
         nr_a = inp.n_alpha + info["n_v_alpha"]
         nr_b = inp.n_beta + info["n_v_beta"]
         ng, nw, N = inp.n_chol, inp.n_w, inp.N
-        # complex MAC = 8 flops; the same-spin products are symmetric: only x <= y is algorithmic work
+        # complex MAC = 8 flops (the method's work; the V kernel executes 6 per complex MAC by the 3-multiplication scheme);
+        # the same-spin products are symmetric: only x <= y is algorithmic work
         flops_v = 8.0 * ng * nw * (Pa * Pb + Pa * (Pa + 1) / 2 + Pb * (Pb + 1) / 2)
-        flops_lam = 4.0 * (ng + 1) * N * nw * (nr_a * inp.n_alpha + nr_b * inp.n_beta)   # real x complex MAC = 4
-        phases = {"energy_ms": {"reference": acc["reference"], "lambda_gemm": acc["p1"], "energy_dense": acc["p2"],
+        # S7 (fused kernel): Lambda = L_sub Theta over the N - n_sigma virtual orbitals when the reference is the first n
+        # orbitals (Theta[occ] = 1), real x complex MAC = 4; dense steps per (walker, slice, spin): Theta_v T (8 n_v n n),
+        # Bfull T[:, pos] (8 n_v n n_o), tr(T T) (8 n^2)
+        contiguous = (list(inp.occ_ref_a) == list(range(inp.n_alpha)) and list(inp.occ_ref_b) == list(range(inp.n_beta))
+                      and inp.n_alpha == inp.n_beta and inp.n_alpha % 2 == 0)
+        kv_a = N - inp.n_alpha if contiguous else N
+        kv_b = N - inp.n_beta if contiguous else N
+        flops_lam = 4.0 * (ng + 1) * nw * (kv_a * nr_a * inp.n_alpha + kv_b * nr_b * inp.n_beta)
+        nva, nvb, noa, nob = info["n_v_alpha"], info["n_v_beta"], info["n_o_alpha"], info["n_o_beta"]
+        flops_dense = 8.0 * ng * nw * (nva * inp.n_alpha * (inp.n_alpha + noa) + inp.n_alpha ** 2
+                                       + nvb * inp.n_beta * (inp.n_beta + nob) + inp.n_beta ** 2)
+        phases = {"energy_ms": {"reference": acc["reference"], "s7_lambda_and_dense": acc["p1"] + acc["p2"],
                                 "v_gemm": acc["p3"], "dets": acc["p4"], "assemble": acc["p5"]},
                   "force_bias_ms": {"reference": fbacc["reference"], "dets": fbacc["p1"], "greens_fb_gemm": fbacc["p2"]}}
-        # dominant DMMA kernel: k_gemm_tn (V and Lambda launches); algorithmic flops / measured duration
-        gemm_ms = acc["p3"] + acc["p1"]
-        achieved = (flops_v + flops_lam) / (gemm_ms * 1e-3) / 1e12
-        roofline = {"kernel": "k_gemm_tn (FP64 DMMA: V and Lambda contractions, %d launches per step)" % 5,
-                    "bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                    "frac": achieved / peak if peak > 0 else None,
-                    "peak_source": "measured live by the bench-side probe (csrc/probes.cu, libmsd_probes.so): register-"
-                                   "resident DMMA m8n8k4 loop; MEASURED_PEAKS.json has no FP64 entry; derived 148 SM x "
-                                   "64 FMA/clk x 1.965 GHz = %.1f" % FP64_PEAK_DERIVED,
-                    "traffic": ncu_traffic("k_gemm_tn")[0],
-                    "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum per launch, mean over the %d k_gemm_tn "
-                                    "launches in profiles/r02_ncu_raw.csv (raw page of one ncu --set full capture of this "
-                                    "command; null when absent)" % ncu_traffic("k_gemm_tn")[1],
-                    "share_of_step": gemm_ms / (sum(step_ms) / len(step_ms)),
-                    "algorithmic_flops_per_step": flops_v + flops_lam}
+        step_mean = sum(step_ms) / len(step_ms)
+        s7_ms, v_ms = acc["p1"] + acc["p2"], acc["p3"]
+        src = ("measured live by the bench-side probe (csrc/probes.cu, libmsd_probes.so): register-resident DMMA m8n8k4 "
+               "loop; MEASURED_PEAKS.json has no FP64 entry; derived 148 SM x 64 FMA/clk x 1.965 GHz = %.1f" % FP64_PEAK_DERIVED)
+
+        def tensor_roofline(kernel, prefix, flops, ms, note):
+            tr, nl = ncu_traffic(prefix)
+            return {"kernel": kernel, "bound": "tensor", "achieved": flops / (ms * 1e-3) / 1e12, "peak": peak,
+                    "unit": "TFLOP/s", "frac": flops / (ms * 1e-3) / 1e12 / peak if peak > 0 else None, "peak_source": src,
+                    "traffic": tr, "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum per launch, mean over the %d "
+                    "launches of this kernel in profiles/r02_ncu_raw.csv (raw page of one ncu --set full capture of this "
+                    "command; null when absent)" % nl, "ms": ms, "share_of_step": ms / step_mean,
+                    "algorithmic_flops_per_step": flops, "note": note}
+        r_s7 = tensor_roofline("k_energy_fused (S7: Lambda = L_sub Theta by FP64 DMMA + dense intermediates, 1 launch)",
+                               "k_energy_fused", flops_lam + flops_dense, s7_ms,
+                               "executes (40/35 padded rows) more DMMA than the algorithmic count")
+        r_v = tensor_roofline("k_vgemm3m (V contractions alpha-beta, alpha-alpha, beta-beta: 3 launches on forked streams)",
+                              "k_vgemm3m", flops_v, v_ms,
+                              "achieved counts 8 flops per complex MAC (the method's work); the kernel executes 6 (3-multiplication "
+                              "scheme), i.e. %.2f TFLOP/s of executed DMMA on 48 x 48 tiles" % (0.75 * flops_v / (v_ms * 1e-3) / 1e12))
+        # the dominant kernel = the one with the larger share of the step
+        roofline, roofline_other = (r_s7, r_v) if s7_ms >= v_ms else (r_v, r_s7)
 
         # energy-mode dets kernels: bound by the L2 -> SM gathers of V / Vbar; algorithmic bytes =
         # 16 B x (ka^2 kb^2 + C(ka,2)^2 + C(kb,2)^2) per walker x determinant, from the level histogram of the inputs
@@ -465,6 +483,7 @@ def main():
     else:
         roofline_dets = None
         roofline_fb_dets = None
+        roofline_other = None
 
     if rank != 0:
         if world > 1:
@@ -497,7 +516,8 @@ def main():
                     "steps": n_e2e},
             "gpu_launches": int(launches),
             "fused": fused, "per_call": per_call, "block_mix": block_mix, "propagation": propagation,
-            "roofline": roofline, "roofline_dets": roofline_dets, "roofline_fb_dets": roofline_fb_dets,
+            "roofline": roofline, "roofline_second_tensor_kernel": roofline_other, "roofline_dets": roofline_dets,
+            "roofline_fb_dets": roofline_fb_dets,
             "cpu_baseline": cpu_baseline, "cpu_wick_baseline": cpu_wick, "phases": phases,
             "step_ms": {"min": min(step_ms), "median": statistics.median(step_ms), "max": max(step_ms)}}
     print(json.dumps(line), flush=True)

@@ -187,9 +187,12 @@ int msd_get_phase_ms(msd_ctx* ctx, float* ms, int n);
  *       Results are the same.  Unknown option or value: MSD_EINVAL.
  *   MSD_OPT_NO_FUSED_S7 (0 / 1; default 0): TEST HOOK.  1 takes the two-kernel form of the half rotation (Lambda = L_sub Theta
  *       written to memory by the GEMM, dense intermediates by a second kernel) that otherwise only runs for shapes the fused
- *       kernel does not cover.  Results are the same. */
+ *       kernel does not cover.  Results are the same.
+ *   MSD_OPT_NO_3M (0 / 1; default 0): TEST HOOK.  1 computes the V contractions with the four-multiplication real form of the
+ *       complex product (k_gemm_tn) instead of the three-multiplication kernel (k_vgemm3m).  Same results to rounding. */
 #define MSD_OPT_NO_SMEM_TILES 1
 #define MSD_OPT_NO_FUSED_S7 2
+#define MSD_OPT_NO_3M 3
 int msd_set_option(msd_ctx* ctx, int option, int64_t value);
 
 void msd_destroy(msd_ctx* ctx);

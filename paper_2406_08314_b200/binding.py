@@ -27,6 +27,7 @@ EXPORTS = ["msd_setup", "msd_setup_from_occ", "msd_overlap", "msd_force_bias", "
            "msd_set_profiling", "msd_get_phase_ms", "msd_destroy", "msd_last_error"]
 MSD_OPT_NO_SMEM_TILES = 1
 MSD_OPT_NO_FUSED_S7 = 2
+MSD_OPT_NO_3M = 3
 
 
 class MSDError(RuntimeError):

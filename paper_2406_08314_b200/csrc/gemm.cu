@@ -193,3 +193,137 @@ cudaError_t launch_gemm_tn(msd_ctx* c, const GemmArgs& a, cudaStream_t st)
     if (best == 1) return launch_cfg<64, 64, 2, 2>(c, a, st);
     return launch_cfg<48, 96, 2, 2>(c, a, st);
 }
+
+// ------------------------------------------------------------------------------------------------
+// Complex bilinear batched product by the 3-multiplication (Karatsuba) scheme, for the V contractions:
+//   C[x][y] = sum_g A[x][g] B[y][g]        A, B complex rows (re, im interleaved, g contiguous), no conjugation
+//   P1 = sum a_r b_r,  P2 = sum a_i b_i,  P3 = sum (a_r + a_i)(b_r + b_i);   C_r = P1 - P2,  C_i = P3 - P1 - P2
+// Three real DMMA products per complex output instead of four (the real form [a_r a_i] x [[b_r b_i], [-b_i b_r]] of
+// k_gemm_tn's expand mode): 25 % fewer tensor-pipe cycles.  One 16-byte shared-memory read yields (a_r, a_i) of a fragment
+// element, the sum a_r + a_i is one DADD (3.5 % of the pipe time of the 27 DMMAs it feeds).  The imaginary part is formed
+// by subtraction: its rounding error is relative to |A||B| instead of |C_i| (bounded by 3 eps sum |a||b|, far inside the
+// 1e-8 Ha energy tolerance).
+// CTA tile 48 rows x 48 complex columns, 4 warps of 24 x 24 (3 x 3 DMMA tiles x 3 products = 27 accumulator tiles),
+// k-tile of 8 gamma (128-byte rows), 4-stage cp.async ring, row stride 24 doubles (conflict-free 16-byte fragment reads).
+// ------------------------------------------------------------------------------------------------
+#define V3_BM 48
+#define V3_BN 48
+#define V3_BG 8          // gamma per k-tile
+#define V3_LD 24         // doubles per staged row: 2 * V3_BG + 8
+#define V3_STAGES 4
+
+__global__ void __launch_bounds__(128, 3) k_vgemm3m(GemmArgs g)
+{
+    extern __shared__ __align__(16) double smem_v3[];
+    double* As = smem_v3;                                     // [STAGES][48][LD]
+    double* Bs = smem_v3 + V3_STAGES * V3_BM * V3_LD;         // [STAGES][48][LD]
+    const int z = blockIdx.z;
+    const int bx = blockIdx.x, by = blockIdx.y;
+    if (g.symmetric && bx < by) return;                       // strictly lower tile (square complex tiles)
+    const int Nc = g.N / 2, ngam = g.K / 2;
+    const double* A = g.A + (int64_t)z * g.strideA;
+    const double* B = g.B + (int64_t)z * g.strideB;
+    const int m0 = by * V3_BM, n0 = bx * V3_BN;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int wm = (wid & 1) * 24, wn = (wid >> 1) * 24;
+    const int gq = lane >> 2, tq = lane & 3;
+    const int KT = (ngam + V3_BG - 1) / V3_BG;
+
+    auto load_tile = [&](int stage, int kt) {
+        const int g0 = kt * V3_BG;
+        double* as = As + stage * V3_BM * V3_LD;
+        double* bs = Bs + stage * V3_BN * V3_LD;
+        // 48 rows x 8 chunks of 16 bytes (one complex each) per operand; 128 threads: 3 chunks of A and 3 of B each
+        for (int c = tid; c < V3_BM * V3_BG; c += 128) {
+            const int r = c >> 3, kc = c & 7;
+            const bool ok = (m0 + r < g.M) && (g0 + kc < ngam);
+            cp_async16(as + r * V3_LD + 2 * kc, ok ? A + (int64_t)(m0 + r) * g.lda + 2 * (g0 + kc) : A, ok ? 16 : 0);
+        }
+        for (int c = tid; c < V3_BN * V3_BG; c += 128) {
+            const int r = c >> 3, kc = c & 7;
+            const bool ok = (n0 + r < Nc) && (g0 + kc < ngam);
+            cp_async16(bs + r * V3_LD + 2 * kc, ok ? B + (int64_t)(n0 + r) * g.ldb + 2 * (g0 + kc) : B, ok ? 16 : 0);
+        }
+    };
+
+    double p1[3][3][2], p2[3][3][2], p3[3][3][2];
+#pragma unroll
+    for (int i = 0; i < 3; i++)
+#pragma unroll
+        for (int j = 0; j < 3; j++)
+#pragma unroll
+            for (int t = 0; t < 2; t++) { p1[i][j][t] = 0.0; p2[i][j][t] = 0.0; p3[i][j][t] = 0.0; }
+
+    for (int s = 0; s < V3_STAGES - 1; s++) {
+        if (s < KT) load_tile(s, s);
+        cp_async_commit();
+    }
+    for (int kt = 0; kt < KT; kt++) {
+        cp_async_wait<V3_STAGES - 2>();
+        __syncthreads();
+        {
+            const int nk = kt + V3_STAGES - 1;
+            if (nk < KT) load_tile(nk % V3_STAGES, nk);
+            cp_async_commit();
+        }
+        const double* as = As + (kt % V3_STAGES) * V3_BM * V3_LD + (wm + gq) * V3_LD + 2 * tq;
+        const double* bs = Bs + (kt % V3_STAGES) * V3_BN * V3_LD + (wn + gq) * V3_LD + 2 * tq;
+#pragma unroll
+        for (int kk = 0; kk < V3_BG / 4; kk++) {
+            double ar[3], ai[3], asum[3], br[3], bi[3], bsum[3];
+#pragma unroll
+            for (int i = 0; i < 3; i++) {
+                const double2 v = *reinterpret_cast<const double2*>(as + i * 8 * V3_LD + kk * 8);
+                ar[i] = v.x; ai[i] = v.y; asum[i] = v.x + v.y;
+            }
+#pragma unroll
+            for (int j = 0; j < 3; j++) {
+                const double2 v = *reinterpret_cast<const double2*>(bs + j * 8 * V3_LD + kk * 8);
+                br[j] = v.x; bi[j] = v.y; bsum[j] = v.x + v.y;
+            }
+#pragma unroll
+            for (int i = 0; i < 3; i++)
+#pragma unroll
+                for (int j = 0; j < 3; j++) {
+                    dmma884(p1[i][j][0], p1[i][j][1], ar[i], br[j]);
+                    dmma884(p2[i][j][0], p2[i][j][1], ai[i], bi[j]);
+                    dmma884(p3[i][j][0], p3[i][j][1], asum[i], bsum[j]);
+                }
+        }
+    }
+    cp_async_wait<0>();
+
+    // epilogue: thread holds rows m = m0 + wm + 8 i + gq, complex columns y = n0 + wn + 8 j + 2 tq (+1)
+    double* Cz = g.C + 2 * ((int64_t)(z / g.zdiv) * g.strideC_hi + (int64_t)(z % g.zdiv) * g.strideC_lo);
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+        const int m = m0 + wm + i * 8 + gq;
+        if (m >= g.M) continue;
+#pragma unroll
+        for (int j = 0; j < 3; j++)
+#pragma unroll
+            for (int t = 0; t < 2; t++) {
+                const int y = n0 + wn + j * 8 + 2 * tq + t;
+                if (y >= Nc) continue;
+                if (g.symmetric && y < m) continue;
+                const double2 v = make_double2(p1[i][j][t] - p2[i][j][t], p3[i][j][t] - p1[i][j][t] - p2[i][j][t]);
+                *reinterpret_cast<double2*>(Cz + 2 * ((int64_t)m * g.cs_m + (int64_t)y * g.cs_j)) = v;
+                if (g.symmetric && y > m) *reinterpret_cast<double2*>(Cz + 2 * ((int64_t)y * g.cs_m + (int64_t)m * g.cs_j)) = v;
+            }
+    }
+}
+
+// A, B: complex rows (g.M rows of A, g.N / 2 rows of B), g.K = 2 x gammas doubles per row; C as in k_gemm_tn
+cudaError_t launch_vgemm3m(msd_ctx* c, const GemmArgs& a, cudaStream_t st)
+{
+    if (a.M <= 0 || a.N <= 0 || a.batch <= 0) return cudaSuccess;
+    if ((a.N & 1) || (a.K & 1) || (a.lda & 1) || (a.ldb & 1) || (a.strideA & 1) || (a.strideB & 1) || a.accumulate || a.ksplit != 1 ||
+        (a.symmetric && a.N != 2 * a.M))
+        return cudaErrorInvalidValue;
+    const size_t smem = (size_t)V3_STAGES * (V3_BM + V3_BN) * V3_LD * sizeof(double);
+    cudaError_t e = func_config(c, (const void*)k_vgemm3m, 128, smem, nullptr);
+    if (e != cudaSuccess) return e;
+    dim3 grid((a.N / 2 + V3_BN - 1) / V3_BN, (a.M + V3_BM - 1) / V3_BM, a.batch);
+    k_vgemm3m<<<grid, 128, smem, st>>>(a);
+    return cudaGetLastError();
+}

@@ -568,6 +568,7 @@ extern "C" int msd_set_option(msd_ctx* c, int option, int64_t value)
 {
     if (!c) return MSD_EINVAL;
     if (option == MSD_OPT_NO_SMEM_TILES && value >= 0 && value <= 2) { c->no_smem_tiles = (int)value; return MSD_OK; }
+    if (option == MSD_OPT_NO_3M && (value == 0 || value == 1)) { c->no_3m = value != 0; return MSD_OK; }
     if (option == MSD_OPT_NO_FUSED_S7 && (value == 0 || value == 1)) {
         c->no_fused = value != 0;
         int a, b, m, t, ko, kv;
@@ -887,7 +888,7 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
                 a.cs_m = (int64_t)B_.P * MSD_WT; a.cs_j = MSD_WT;
                 a.accumulate = 0;
                 a.symmetric = (pr > 0) ? 1 : 0;     // V^{ss}[x][y] = V^{ss}[y][x]
-                cudaError_t ge = launch_gemm_tn(c, a, fv_.stream(pr));
+                cudaError_t ge = c->no_3m ? launch_gemm_tn(c, a, fv_.stream(pr)) : launch_vgemm3m(c, a, fv_.stream(pr));
                 if (ge != cudaSuccess) { fv_.join(); CK(ge); }
                 c->launches++;
             }

@@ -201,6 +201,7 @@ struct msd_ctx {
     double* d_E = nullptr;                    // 3 x [ld][ld]: exp(-dt h'/2), the scaled matrix, scratch
     double prop_dt = 0.0; int prop_taylor = 0;
     const double* prop_x = nullptr; double* prop_w = nullptr;      // arguments of the running msd_propagate call
+    bool no_3m = false;                       // MSD_OPT_NO_3M: V contractions by the 4-multiplication real form (test hook)
     bool no_fused = false;                    // MSD_OPT_NO_FUSED_S7: take the Lambda GEMM + dense kernel pair (test hook)
     bool need_lam = true;                     // the workspace holds the Lambda buffer (two-kernel S7 path)
     bool energy_ok = true;                    // the energy calls are supported for this trial (window size, see msd_setup)
@@ -308,3 +309,4 @@ struct GemmArgs {
                                 //    touch the upper triangle are computed, element (m, j >= m) is also written to (j, m)
 };
 cudaError_t launch_gemm_tn(msd_ctx* c, const GemmArgs& a, cudaStream_t st);
+cudaError_t launch_vgemm3m(msd_ctx* c, const GemmArgs& a, cudaStream_t st);     // complex bilinear product, 3-multiplication scheme

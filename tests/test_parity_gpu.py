@@ -541,6 +541,34 @@ def test_paths_for_windows_too_wide_for_shared_memory_tiles(torch_cuda, level):
         assert_parity(dict(fb=fused[:, :x.n_chol], E=fused[:, x.n_chol:]), ref, walkers=sel, what=("fb", "E"))
 
 
+@pytest.mark.parametrize("name,kw,ws", [("small", {}, None), ("cu2o2", dict(n_w=24), [0, 7, 8, 23]),
+                                        ("sweep", dict(n_det=2000, max_level=5, n_w=16), [0, 15])])
+def test_alternative_dense_paths(torch_cuda, name, kw, ws):
+    """The energy through the non-default dense kernels -- Lambda GEMM + dense kernel pair instead of the fused S7 kernel
+    (MSD_OPT_NO_FUSED_S7), four-multiplication V GEMM instead of the three-multiplication one (MSD_OPT_NO_3M) -- against
+    the oracle, and against the default path."""
+    msd = _msd()
+    torch = torch_cuda
+    x = mi.generate(name, **kw)
+    pa = torch.tensor(x.phi_a, device="cuda")
+    pb = torch.tensor(x.phi_b, device="cuda")
+    ref = o2.run(x, walkers=ws, return_G=False)
+    sel = np.arange(x.n_w) if ws is None else np.asarray(ws)
+    res = {}
+    for opts in ((), (msd.MSD_OPT_NO_FUSED_S7,), (msd.MSD_OPT_NO_3M,), (msd.MSD_OPT_NO_FUSED_S7, msd.MSD_OPT_NO_3M)):
+        trial = msd.setup_from_inputs(x)
+        for o in opts:
+            trial.set_option(o, 1)
+        E = trial.local_energy(pa, pb).cpu().numpy()
+        fused = trial.force_bias_energy(pa, pb).cpu().numpy()
+        trial.close()
+        assert np.abs(E[sel] - ref["E"]).max() <= TOL_E, opts
+        assert np.abs(fused[sel, x.n_chol:] - ref["E"]).max() <= TOL_E, opts
+        res[opts] = E
+    for opts, E in res.items():
+        assert np.abs(E - res[()]).max() <= TOL_E
+
+
 def test_window_wider_than_shared_memory(torch_cuda):
     """An active window of 10 occupied x 100 virtual orbitals per spin (the paper's [Cu2O2]2+ has 16 x 92,
     PAPER.md:L303): 2000 pair indices, so neither the g slices (256 KB per walker tile) nor C / Hrot / F fit in shared
