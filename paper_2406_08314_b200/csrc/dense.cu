@@ -485,7 +485,7 @@ k_energy_dense_mma(int n_chol, int64_t nw, int gchunk, SpinDev sa, SpinDev sb, c
 #define FUSE_BK 16
 #define FUSE_LDA 20
 __host__ __device__ inline int fused_ldbs(int Kv) { return (Kv + 15) / 16 * 16 + 4; }
-template <int NWARP, int MTC, int NTC, int MTG, int NTG>
+template <int NWARP, int MTC, int NTC, int MTG, int NTG, int KSC>
 __global__ void __launch_bounds__(NWARP * 32, NWARP == 8 ? 1 : 2)
 k_energy_fused(int n_chol, int64_t nw, int gchunk, int ldN, int koff, int Kv, SpinDev sa, SpinDev sb,
                const cplx* __restrict__ theta_a, const cplx* __restrict__ theta_b, const double* __restrict__ thT_a,
@@ -539,7 +539,7 @@ k_energy_fused(int n_chol, int64_t nw, int gchunk, int ldN, int koff, int Kv, Sp
 
     const int MT = MTC > 0 ? MTC : 2 * L.half / 8;            // <= 4
     const int NT = NTC > 0 ? NTC : (n + 7) / 8;
-    const int KS = L.Kp / 4;
+    constexpr int KS = KSC;                                   // = Kp / 4 (checked by the launcher)
     const int posh[2] = {pos[gq], pos[8 + gq]};
     const int kc = tq & 1, kl = tq >> 1;
     double fk[4][2][2];
@@ -688,7 +688,7 @@ k_energy_fused(int n_chol, int64_t nw, int gchunk, int ldN, int koff, int Kv, Sp
                         acc2[mt][j][1] = (ok && i + 1 < n) ? Lb[r * L.ldb + 2 * i + 2 + im] : 0.0;
                     }
                 }
-#pragma unroll 2
+#pragma unroll
                 for (int kk = 0; kk < KS; kk++) {
                     double a[4], b[3];
 #pragma unroll
@@ -718,7 +718,7 @@ k_energy_fused(int n_chol, int64_t nw, int gchunk, int ldN, int koff, int Kv, Sp
         __syncwarp();
         if (live && g < n_chol) {
             // step 4: FK += A''(Bfull) B''(T[:, pos])
-#pragma unroll 2
+#pragma unroll
             for (int kk = 0; kk < KS; kk++) {
                 double a[4], b[2];
 #pragma unroll
@@ -847,9 +847,11 @@ size_t energy_dense_smem(const msd_ctx* c, int GC)
     return smem;
 }
 
-template <int NWARP, int MTC, int NTC, int MTG, int NTG>
+template <int NWARP, int MTC, int NTC, int MTG, int NTG, int KSC>
 static cudaError_t launch_fused_t(msd_ctx* c, int64_t nw, Workspace& ws, int koff, int Kv, cudaStream_t st)
 {
+    for (int s = 0; s < 2; s++)
+        if (c->sp[s].n > 0 && DenseMmaLayout(c->sp[s].n, c->sp[s].n_v).Kp / 4 != KSC) return cudaErrorNotSupported;
     const int ldN = c->N + (c->N & 1);
     size_t smem = 0;
     for (int s = 0; s < 2; s++) {
@@ -860,11 +862,11 @@ static cudaError_t launch_fused_t(msd_ctx* c, int64_t nw, Workspace& ws, int kof
         smem = std::max(smem, ((size_t)2 * L.half * L.lda + (size_t)NWARP * wd + (size_t)8 * NTG * fused_ldbs(Kv)) * sizeof(double) + 64);
     }
     if (smem > 227 * 1024) return cudaErrorNotSupported;
-    cudaError_t e = func_config(c, (const void*)k_energy_fused<NWARP, MTC, NTC, MTG, NTG>, NWARP * 32, smem, nullptr);
+    cudaError_t e = func_config(c, (const void*)k_energy_fused<NWARP, MTC, NTC, MTG, NTG, KSC>, NWARP * 32, smem, nullptr);
     if (e != cudaSuccess) return e;
     const int gchunk = 64;
     dim3 grid((c->n_chol + 1 + gchunk - 1) / gchunk, (unsigned)nw, 2);
-    k_energy_fused<NWARP, MTC, NTC, MTG, NTG><<<grid, NWARP * 32, smem, st>>>(
+    k_energy_fused<NWARP, MTC, NTC, MTG, NTG, KSC><<<grid, NWARP * 32, smem, st>>>(
         c->n_chol, nw, gchunk, ldN, koff, Kv, c->dev(0), c->dev(1), ws.theta[0], ws.theta[1], ws.thetaT[0], ws.thetaT[1],
         ws.Bp[0], ws.Bp[1], ws.X0, ws.F[0], ws.F[1], ws.Hrot[0], ws.Hrot[1], ws.Eacc, c->N);
     return cudaGetLastError();
@@ -891,6 +893,9 @@ bool energy_fused_shape(const msd_ctx* c, int* mtc, int* ntc, int* mtg, int* ntg
     const bool have = (a == 4 && b == 3 && m == 5 && t == 5) || (a == 4 && b == 2 && m == 4 && t == 4) ||
                       (a == 4 && b == 2 && m == 4 && t == 3) || (a == 2 && b == 1 && m == 2 && t == 2);
     if (!have) return false;
+    const int ksc = (a == 4 && b == 3) ? 10 : (a == 4 && t == 4) ? 8 : (a == 4) ? 6 : 4;
+    for (int s = 0; s < 2; s++)
+        if (c->sp[s].n > 0 && DenseMmaLayout(c->sp[s].n, c->sp[s].n_v).Kp / 4 != ksc) return false;
     const int ldN = c->N + (c->N & 1);
     *mtc = a; *ntc = b; *mtg = m; *ntg = t;
     *koff = contiguous ? nn : 0;
@@ -903,10 +908,10 @@ cudaError_t launch_energy_fused(msd_ctx* c, int64_t nw, Workspace& ws, cudaStrea
     int a, b, m, t, koff, Kv;
     if (!energy_fused_shape(c, &a, &b, &m, &t, &koff, &Kv)) return cudaErrorNotSupported;
     cudaError_t e;
-    if (a == 4 && b == 3) e = launch_fused_t<FUSE_NWARP, 4, 3, 5, 5>(c, nw, ws, koff, Kv, st);
-    else if (a == 4 && t == 4) e = launch_fused_t<FUSE_NWARP, 4, 2, 4, 4>(c, nw, ws, koff, Kv, st);
-    else if (a == 4) e = launch_fused_t<FUSE_NWARP, 4, 2, 4, 3>(c, nw, ws, koff, Kv, st);
-    else e = launch_fused_t<FUSE_NWARP, 2, 1, 2, 2>(c, nw, ws, koff, Kv, st);
+    if (a == 4 && b == 3) e = launch_fused_t<FUSE_NWARP, 4, 3, 5, 5, 10>(c, nw, ws, koff, Kv, st);          // n = 20 (fe2s2)
+    else if (a == 4 && t == 4) e = launch_fused_t<FUSE_NWARP, 4, 2, 4, 4, 8>(c, nw, ws, koff, Kv, st);      // n = 16 (cu2o2)
+    else if (a == 4) e = launch_fused_t<FUSE_NWARP, 4, 2, 4, 3, 6>(c, nw, ws, koff, Kv, st);                // n = 12 (sweep)
+    else e = launch_fused_t<FUSE_NWARP, 2, 1, 2, 2, 4>(c, nw, ws, koff, Kv, st);                            // n = 8 (small)
     if (e == cudaSuccess) c->launches++;
     return e;
 }
