@@ -229,6 +229,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--n-det", type=int, default=None, help="override the determinant count (kernel sweep, configs[4])")
     ap.add_argument("--max-level", type=int, default=None, help="override the maximum excitation level (kernel sweep)")
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "dets"],
+                    help="N > 1: 'replicas' (default; every rank its own walker batch, no collective, weak scaling) or 'dets' "
+                         "(SURVEY.md 8(f) f4: every rank 1/N of every level bucket of the determinant list and the SAME walkers, "
+                         "one NCCL all-reduce of the partial W / C / E sums per determinant pass, strong scaling)")
     args = ap.parse_args()
     rank, world, local = shard_info(args.gpus)
     if args.impl == "reference":
@@ -257,11 +261,15 @@ def main():
     if args.max_level is not None:
         over["max_level"] = args.max_level
     inp = mi.generate(args.config, **over)
-    if rank > 0:   # replicas: same trial, a different walker batch per rank
+    shard_dets = args.shard == "dets" and world > 1
+    if rank > 0 and not shard_dets:   # replicas: same trial, a different walker batch per rank
         rng = np.random.default_rng(inp.params["seed"] + 7919 * rank)
         inp = inp.with_walkers(mi.walkers_from_rng(rng, inp.n_w, inp.N, inp.n_alpha),
                                mi.walkers_from_rng(rng, inp.n_w, inp.N, inp.n_beta))
-    trial = msd.setup_from_inputs(inp)
+    trial = msd.setup_from_inputs(inp, shard=(rank, world) if shard_dets else (0, 1))
+    if shard_dets:
+        trial.set_allreduce(msd.dist_allreduce())
+    units_world = 1 if shard_dets else world          # determinant shards work on ONE batch together
     info = trial.info()
     stream = torch.cuda.current_stream()
     h_a = torch.from_numpy(inp.phi_a).pin_memory()
@@ -303,7 +311,7 @@ def main():
     clocks = sampler.stop()
     step_ms = [a.elapsed_time(b) for a, b in evs]
     total_ms = reduce_max_time(sum(step_ms), world, dev)
-    value = total_units(inp.n_w, inp.n_det, args.steps, world) / (total_ms * 1e-3)
+    value = total_units(inp.n_w, inp.n_det, args.steps, units_world) / (total_ms * 1e-3)
 
     # ---- the same two outputs from the fused call msd_force_bias_energy (one pass of the determinant kernels) ----
     fused_out = torch.empty((inp.n_w, inp.n_chol + 3), dtype=torch.complex128, device=dev)
@@ -320,7 +328,7 @@ def main():
     fused_ms = reduce_max_time(sum(a.elapsed_time(b) for a, b in fev), world, dev)
     fused = {"call": "msd_force_bias_energy (force bias and local energy of the batch from ONE pass: the energy-mode "
                      "determinant kernels also accumulate C, fb = X0 + C.B/W, SURVEY.md 8(c) W6)",
-             "value": total_units(inp.n_w, inp.n_det, args.steps, world) / (fused_ms * 1e-3), "unit": UNIT,
+             "value": total_units(inp.n_w, inp.n_det, args.steps, units_world) / (fused_ms * 1e-3), "unit": UNIT,
              "ms_per_step": fused_ms / args.steps,
              "max_rel_diff_fb_vs_separate_calls": float(((fused_out[:, :inp.n_chol] - fb).abs().amax(dim=1)
                                                          / fb.abs().amax(dim=1)).max().item()),
@@ -344,11 +352,11 @@ def main():
             b.record(stream)
         barrier()
         cms = reduce_max_time(sum(a.elapsed_time(b) for a, b in cev), world, dev) / args.steps
-        per_call[cname] = {"ms": cms, "value": total_units(inp.n_w, inp.n_det, 1, world) / (cms * 1e-3), "unit": UNIT}
+        per_call[cname] = {"ms": cms, "value": total_units(inp.n_w, inp.n_det, 1, units_world) / (cms * 1e-3), "unit": UNIT}
     t_ov, t_fb, t_e = (per_call[k]["ms"] for k in ("msd_overlap", "msd_force_bias", "msd_local_energy"))
     block_mix = {"definition": "N_w N_d 25 / (25 (t_fb + t_ovlp) + t_E): walker x determinant propagation-step evaluations "
                                "per second in the paper's block of 25 steps + 1 energy estimate (PAPER.md:L303-309)",
-                 "value": total_units(inp.n_w, inp.n_det, 25, world) / ((25.0 * (t_fb + t_ov) + t_e) * 1e-3),
+                 "value": total_units(inp.n_w, inp.n_det, 25, units_world) / ((25.0 * (t_fb + t_ov) + t_e) * 1e-3),
                  "unit": "walker*det*step/s", "block_ms": 25.0 * (t_fb + t_ov) + t_e,
                  "energy_share_of_block": t_e / (25.0 * (t_fb + t_ov) + t_e)}
 
@@ -372,7 +380,7 @@ def main():
     pms = reduce_max_time(sum(a.elapsed_time(b) for a, b in pev), world, dev) / args.steps
     propagation = {"call": "msd_propagate: force bias + overlap of the walkers, field matrices (DMMA), orbital update with a "
                            "6th-order Taylor series, overlap of the new walkers, Eq. 8-12 (dt = 0.005)",
-                   "ms_per_step": pms, "value": total_units(inp.n_w, inp.n_det, 1, world) / (pms * 1e-3),
+                   "ms_per_step": pms, "value": total_units(inp.n_w, inp.n_det, 1, units_world) / (pms * 1e-3),
                    "unit": "walker*det*step/s", "finite": bool(torch.isfinite(sout).all().item())}
 
     # ---- end to end: the C-ABI *_host calls (pinned HOST buffers; H2D + kernels + D2H inside each call) ----
@@ -390,14 +398,15 @@ def main():
     eb.record(stream)
     barrier()
     e2e_ms = reduce_max_time(ea.elapsed_time(eb), world, dev)
-    e2e_val = total_units(inp.n_w, inp.n_det, n_e2e, world) / (e2e_ms * 1e-3)
+    e2e_val = total_units(inp.n_w, inp.n_det, n_e2e, units_world) / (e2e_ms * 1e-3)
     h2d = 2 * (h_a.numel() * 16 + h_b.numel() * 16)      # each of the two host calls copies the walkers in
     d2h = h_fb.numel() * 16 + h_en.numel() * 16
 
     # ---- roofline of the dominant kernel (phase timings from CUDA events inside the library, same stream) ----
     roofline = None
     phases = None
-    if rank == 0:
+    roofline_dets = roofline_fb_dets = roofline_other = None
+    if rank == 0 and not shard_dets:      # (the profiled calls below would be collectives in determinant-shard mode)
         peak = float(probes().msd_probe_fp64_tflops(1, 30.0, None))
         l2_gather = float(probes().msd_probe_l2_gather_gbs(32, 20.0, None))
         trial.set_profiling(True)
@@ -480,10 +489,6 @@ def main():
                             "peak_source": "FP64 pipe (DFMA and DMMA share it): the live DMMA probe",
                             "algorithmic_flops_per_step": fl, "ms": fbacc["p1"],
                             "share_of_step": fbacc["p1"] / (sum(step_ms) / len(step_ms))}
-    else:
-        roofline_dets = None
-        roofline_fb_dets = None
-        roofline_other = None
 
     if rank != 0:
         if world > 1:
@@ -505,12 +510,13 @@ def main():
                     "sample": "all %d walkers x all %d determinants (force bias + local energy in one pass), %.1f s"
                               % (inp.n_w, inp.n_det, sec)}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "strong" if shard_dets else "weak",
             "vs_baseline": None, "dtype": "f64 (complex128)", "data": "synthetic",
             "config": {"workload": args.config, "N": inp.N, "n_alpha": inp.n_alpha, "n_beta": inp.n_beta,
                        "n_chol": inp.n_chol, "n_det": inp.n_det, "n_w": inp.n_w, "active_window": info,
                        "step": "msd_force_bias + msd_local_energy (two calls; the fused one-pass call is reported under 'fused')", "l2": "flushed between timed steps (256 MB write)",
-                       "parallelism": "replicas x%d" % world, "input_sha256": inp.sha256()[:16]},
+                       "parallelism": ("determinant shards x%d (one all-reduce per determinant pass)" if shard_dets else "replicas x%d") % world, "input_sha256": inp.sha256()[:16]},
             "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": n_e2e},

@@ -87,6 +87,26 @@ int msd_setup(msd_ctx** out, int N, int n_alpha, int n_beta, int n_chol, int64_t
               const int64_t* exc_off_b, const int32_t* holes_b, const int32_t* parts_b,
               const double* ci, void* stream);
 
+/* Determinant-sharded multi-GPU (the paper's stated next step).
+ * msd_setup_sharded builds the same trial, but the context evaluates only slice shard_rank of shard_world of every level
+ * bucket of the determinant list (every rank passes the WHOLE trial: active window, table order and introspection are those of
+ * the whole trial; msd_setup = shard 0 of 1).  A hot call on a sharded context needs the partial sums of all ranks:
+ * msd_set_allreduce registers a hook that the call invokes, on the host, once after each determinant pass with
+ *     buf        DEVICE float64 [n]: this rank's partial C^alpha, C^beta, W, E2nd, E1nd of the walker chunk (one contiguous run),
+ *     stream     the stream the call is enqueued on (the library has synchronised it: the partial sums are complete);
+ * the hook must perform, or enqueue on `stream`, an in-place SUM of buf over the ranks (e.g. ncclAllReduce / torch.distributed.all_reduce;
+ * n is about (2 + 2 n_o n_v) complex per walker: 0.7 MB at 100 walkers of a 15 x 15 window) and return.  Every rank must make the
+ * same calls with the same walkers.  Everything that is not a sum over determinants (reference step, dense contractions) is
+ * replicated on every rank.  fn == NULL removes the hook. */
+typedef void (*msd_allreduce_fn)(void* user, void* buf, int64_t n, void* stream);
+int msd_setup_sharded(msd_ctx** out, int N, int n_alpha, int n_beta, int n_chol, int64_t n_det,
+                      const double* h1, const double* L, double e0,
+                      const int32_t* occ_ref_a, const int32_t* occ_ref_b,
+                      const int64_t* exc_off_a, const int32_t* holes_a, const int32_t* parts_a,
+                      const int64_t* exc_off_b, const int32_t* holes_b, const int32_t* parts_b,
+                      const double* ci, int shard_rank, int shard_world, void* stream);
+int msd_set_allreduce(msd_ctx* ctx, msd_allreduce_fn fn, void* user);
+
 /* Convenience for the paper's (coeff, occa, occb) format: occa HOST [n_det][n_alpha],
  * occb HOST [n_det][n_beta] occupation lists (any order inside a row); determinant 0 is the reference. */
 int msd_setup_from_occ(msd_ctx** out, int N, int n_alpha, int n_beta, int n_chol, int64_t n_det,
@@ -159,11 +179,12 @@ int msd_force_bias_energy_host(msd_ctx* ctx, int64_t n_w, const void* phi_a, con
                                void* out, int32_t* flags, void* stream);
 
 /* Introspection of the packed trial (host-side copies made at setup; for tests of the packer).
- * msd_get_info fills info[0..8]: [0]=n_o_alpha, [1]=n_v_alpha, [2]=n_o_beta, [3]=n_v_beta, [4]=number of level
- * buckets, [5]=max level alpha, [6]=max level beta, [7]=walker tile width, [8]=1 if the energy calls are supported.
+ * msd_get_info fills info[0..10]: [0]=n_o_alpha, [1]=n_v_alpha, [2]=n_o_beta, [3]=n_v_beta, [4]=number of level
+ * buckets, [5]=max level alpha, [6]=max level beta, [7]=walker tile width, [8]=1 if the energy calls are supported,
+ * [9]=shard rank, [10]=shard count.
  * msd_get_packed copies, in the packer's sorted order, perm[n_det] (original index of each packed
  * determinant), coef[n_det] (c_I * phase_a * phase_b), level_a[n_det], level_b[n_det]; any may be NULL. HOST. */
-int msd_get_info(const msd_ctx* ctx, int64_t* info9);
+int msd_get_info(const msd_ctx* ctx, int64_t* info11);
 int msd_get_packed(const msd_ctx* ctx, int64_t* perm, double* coef, int32_t* level_a, int32_t* level_b);
 
 /* Set an upper bound (bytes) on the workspace the hot calls may allocate (default: 70 % of free device

@@ -19,7 +19,7 @@ MSD_OK, MSD_EINVAL, MSD_ENOMEM, MSD_ECUDA, MSD_EUNSUPPORTED = 0, -1, -2, -3, -4
 _CODES = {MSD_EINVAL: "MSD_EINVAL", MSD_ENOMEM: "MSD_ENOMEM", MSD_ECUDA: "MSD_ECUDA",
           MSD_EUNSUPPORTED: "MSD_EUNSUPPORTED"}
 
-EXPORTS = ["msd_setup", "msd_setup_from_occ", "msd_overlap", "msd_force_bias", "msd_local_energy", "msd_greens",
+EXPORTS = ["msd_setup", "msd_setup_sharded", "msd_set_allreduce", "msd_setup_from_occ", "msd_overlap", "msd_force_bias", "msd_local_energy", "msd_greens",
            "msd_overlap_host", "msd_force_bias_host", "msd_local_energy_host",
            "msd_force_bias_energy", "msd_force_bias_energy_host",
            "msd_propagator_setup", "msd_propagate",
@@ -51,6 +51,11 @@ def load_library() -> C.CDLL:
     vp, i32, i64, dbl = C.c_void_p, C.c_int, C.c_int64, C.c_double
     lib.msd_setup.restype = i32
     lib.msd_setup.argtypes = [C.POINTER(vp), i32, i32, i32, i32, i64, vp, vp, dbl, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.msd_setup_sharded.restype = i32
+    lib.msd_setup_sharded.argtypes = [C.POINTER(vp), i32, i32, i32, i32, i64, vp, vp, dbl, vp, vp, vp, vp, vp, vp, vp, vp, vp,
+                                      i32, i32, vp]
+    lib.msd_set_allreduce.restype = i32
+    lib.msd_set_allreduce.argtypes = [vp, vp, vp]
     lib.msd_setup_from_occ.restype = i32
     lib.msd_setup_from_occ.argtypes = [C.POINTER(vp), i32, i32, i32, i32, i64, vp, vp, dbl, vp, vp, vp, vp]
     for name in ("msd_overlap", "msd_force_bias", "msd_local_energy", "msd_greens", "msd_force_bias_energy",
@@ -121,6 +126,10 @@ class MSDTrial:
             pass
 
     def _check(self, rc: int):
+        err = getattr(self, "_allreduce_error", None)
+        if err is not None:
+            self._allreduce_error = None
+            raise err
         if rc != MSD_OK:
             msg = load_library().msd_last_error(self._h)
             raise MSDError(rc, msg.decode() if msg else "")
@@ -268,10 +277,10 @@ class MSDTrial:
 
     # -- introspection -------------------------------------------------------------------------
     def info(self) -> dict:
-        a = np.zeros(9, dtype=np.int64)
+        a = np.zeros(11, dtype=np.int64)
         self._check(load_library().msd_get_info(self._h, _ptr(a)))
         keys = ["n_o_alpha", "n_v_alpha", "n_o_beta", "n_v_beta", "n_buckets", "kmax_alpha", "kmax_beta", "walker_tile",
-                "energy_supported"]
+                "energy_supported", "shard_rank", "shard_world"]
         return dict(zip(keys, (int(v) for v in a)))
 
     def packed(self) -> dict:
@@ -284,6 +293,33 @@ class MSDTrial:
 
     def set_workspace_limit(self, nbytes: int):
         self._check(load_library().msd_set_workspace_limit(self._h, int(nbytes)))
+
+    def set_allreduce(self, fn):
+        """Determinant sharding (include/msd.h msd_set_allreduce): fn(t) must sum the CUDA float64 tensor t over the ranks in
+        place, enqueued on the current stream (the binding makes the call's stream current).  None removes the hook."""
+        lib = load_library()
+        if fn is None:
+            self._allreduce_cb = None
+            self._check(lib.msd_set_allreduce(self._h, None, None))
+            return
+        import torch
+
+        class _View:                      # raw device memory as a tensor (no copy): __cuda_array_interface__
+            def __init__(self, ptr, n):
+                self.__cuda_array_interface__ = {"shape": (n,), "typestr": "<f8", "data": (ptr, False), "version": 2}
+
+        def hook(_user, buf, n, stream):
+            try:
+                t = torch.as_tensor(_View(int(buf), int(n)), device=torch.device("cuda", torch.cuda.current_device()))
+                ext = torch.cuda.ExternalStream(int(stream or 0))
+                with torch.cuda.stream(ext):
+                    fn(t)
+                ext.synchronize()         # the kernels the library enqueues next must see the reduced sums
+            except BaseException as e:            # an exception must not cross the C ABI
+                self._allreduce_error = e
+        self._allreduce_error = None
+        self._allreduce_cb = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)(hook)
+        self._check(lib.msd_set_allreduce(self._h, C.cast(self._allreduce_cb, C.c_void_p), None))
 
     def set_option(self, option: int, value: int):
         self._check(load_library().msd_set_option(self._h, int(option), int(value)))
@@ -301,8 +337,8 @@ class MSDTrial:
 
 
 def msd_setup(N, n_alpha, n_beta, n_chol, n_det, h1, L, e0, occ_ref_a, occ_ref_b,
-              exc_off_a, holes_a, parts_a, exc_off_b, holes_b, parts_b, ci, stream=None) -> MSDTrial:
-    """include/msd.h msd_setup: host numpy arrays in, device-resident packed trial out."""
+              exc_off_a, holes_a, parts_a, exc_off_b, holes_b, parts_b, ci, stream=None, shard=(0, 1)) -> MSDTrial:
+    """include/msd.h msd_setup / msd_setup_sharded (shard = (rank, world)): host numpy arrays in, device-resident packed trial out."""
     lib = load_library()
     h1 = _np(h1, np.float64); L = _np(L, np.float64); ci = _np(ci, np.float64)
     ra = _np(occ_ref_a, np.int32); rb = _np(occ_ref_b, np.int32)
@@ -316,9 +352,9 @@ def msd_setup(N, n_alpha, n_beta, n_chol, n_det, h1, L, e0, occ_ref_a, occ_ref_b
     if len(ha) != len(pa) or len(hb) != len(pb) or len(ha) != oa[-1] or len(hb) != ob[-1]:
         raise ValueError("holes / parts lengths disagree with exc_off")
     out = C.c_void_p()
-    rc = lib.msd_setup(C.byref(out), N, n_alpha, n_beta, n_chol, n_det, _ptr(h1), _ptr(L), float(e0),
-                       _ptr(ra), _ptr(rb), _ptr(oa), _ptr(ha), _ptr(pa), _ptr(ob), _ptr(hb), _ptr(pb), _ptr(ci),
-                       _stream_ptr(stream))
+    rc = lib.msd_setup_sharded(C.byref(out), N, n_alpha, n_beta, n_chol, n_det, _ptr(h1), _ptr(L), float(e0),
+                               _ptr(ra), _ptr(rb), _ptr(oa), _ptr(ha), _ptr(pa), _ptr(ob), _ptr(hb), _ptr(pb), _ptr(ci),
+                               int(shard[0]), int(shard[1]), _stream_ptr(stream))
     if rc != MSD_OK:
         msg = lib.msd_last_error(None)
         raise MSDError(rc, msg.decode() if msg else "")
@@ -379,8 +415,17 @@ def msd_local_energy_host(trial: MSDTrial, phi_a, phi_b, out=None, flags=None, s
     return trial.local_energy_host(phi_a, phi_b, out, flags, stream)
 
 
-def setup_from_inputs(inp, stream=None) -> MSDTrial:
-    """Convenience for msd_inputs.MSDInputs (tests / bench)."""
+def setup_from_inputs(inp, stream=None, shard=(0, 1)) -> MSDTrial:
+    """Convenience for msd_inputs.MSDInputs (tests / bench); shard = (rank, world) for determinant sharding."""
     return msd_setup(inp.N, inp.n_alpha, inp.n_beta, inp.n_chol, inp.n_det, inp.h1, inp.L, inp.e0,
                      inp.occ_ref_a, inp.occ_ref_b, inp.exc_off_a, inp.holes_a, inp.parts_a,
-                     inp.exc_off_b, inp.holes_b, inp.parts_b, inp.ci, stream=stream)
+                     inp.exc_off_b, inp.holes_b, inp.parts_b, inp.ci, stream=stream, shard=shard)
+
+
+def dist_allreduce(group=None):
+    """The hook for MSDTrial.set_allreduce under torch.distributed (NCCL over NVLink on GPUs): in-place SUM over the ranks."""
+    import torch.distributed as dist
+
+    def fn(t):
+        dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+    return fn

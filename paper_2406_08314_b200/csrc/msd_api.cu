@@ -65,8 +65,10 @@ static int fail(std::string* errp, int code, const char* msg) { *errp = msg; ret
 static int do_setup(msd_ctx* c, std::string* errp, int N, int na, int nb, int n_chol, int64_t n_det, const double* h1,
                     const double* L, double e0, const int32_t* occ_ref_a, const int32_t* occ_ref_b,
                     const int64_t* off_a, const int32_t* holes_a, const int32_t* parts_a, const int64_t* off_b,
-                    const int32_t* holes_b, const int32_t* parts_b, const double* ci, cudaStream_t st)
+                    const int32_t* holes_b, const int32_t* parts_b, const double* ci, cudaStream_t st, int shard_rank,
+                    int shard_world)
 {
+    if (shard_world < 1 || shard_rank < 0 || shard_rank >= shard_world) return fail(errp, MSD_EINVAL, "bad determinant shard");
     if (!h1 || !L || !off_a || !off_b || !ci || (na > 0 && !occ_ref_a) || (nb > 0 && !occ_ref_b))
         return fail(errp, MSD_EINVAL, "null pointer argument");
     if (N < 1 || na < 0 || nb < 0 || n_chol < 1 || n_det < 1) return fail(errp, MSD_EINVAL, "non-positive size");
@@ -261,6 +263,15 @@ static int do_setup(msd_ctx* c, std::string* errp, int N, int na, int nb, int n_
     // --- work items ---
     for (const Bucket& b : c->buckets)
         if (b.ka * b.ka + b.kb * b.kb > 400) return fail(errp, MSD_EUNSUPPORTED, "k_alpha^2 + k_beta^2 <= 400 required");
+    // Determinant sharding: this context evaluates slice shard_rank of shard_world of EVERY level
+    // bucket (so that all ranks get the same level mix); the window, the table and the introspection stay those of the whole
+    // trial.  `work` are the buckets the work items are cut from.
+    c->shard_rank = shard_rank; c->shard_world = shard_world;
+    std::vector<Bucket> work(c->buckets);
+    for (Bucket& b : work) {
+        const int64_t lo = b.count * shard_rank / shard_world, hi = b.count * (shard_rank + 1) / shard_world;
+        b.start += lo; b.tab_off += lo * b.rs; b.count = hi - lo;
+    }
     auto cost = [](int ka, int kb) {
         double a = ka, b = kb;
         return 1.0 + a * a * a + b * b * b + a * a * b * b;
@@ -273,7 +284,7 @@ static int do_setup(msd_ctx* c, std::string* errp, int N, int na, int nb, int n_
         return g;
     };
     for (int bi = 0; bi < nbk; bi++) {
-        const Bucket& b = c->buckets[bi];
+        const Bucket& b = work[bi];
         const bool gen = std::max(b.ka, b.kb) > MSD_CF_MAX;
         const int m = std::max(b.ka, b.kb);
         int slots = gen ? 128 / MSD_WT : (m <= 3 ? 256 : 128) / MSD_WT;
@@ -332,7 +343,7 @@ static int do_setup(msd_ctx* c, std::string* errp, int N, int na, int nb, int n_
         auto pcls = [](const WorkItem& w) { return std::max(w.ka, w.kb) <= 3 ? 0 : 1; };
         auto estage = [](int ka, int kb) { return (ka >= 3 ? ka * ka : 0) + (kb >= 3 ? kb * kb : 0); };
         for (int bi = 0; bi < nbk && c->pull_pool; bi++) {
-            const Bucket& b = c->buckets[bi];
+            const Bucket& b = work[bi];
             if (std::max(b.ka, b.kb) > MSD_CF_MAX) continue;
             const int slots = (std::max(b.ka, b.kb) <= 3 ? 512 : 256) / MSD_WT;
             int D = (int)std::min<size_t>(PULL_DMAX, c->pull_pool / (256 + (size_t)estage(b.ka, b.kb) * 128));
@@ -450,6 +461,16 @@ extern "C" int msd_setup(msd_ctx** out, int N, int n_alpha, int n_beta, int n_ch
                          const int64_t* exc_off_b, const int32_t* holes_b, const int32_t* parts_b, const double* ci,
                          void* stream)
 {
+    return msd_setup_sharded(out, N, n_alpha, n_beta, n_chol, n_det, h1, L, e0, occ_ref_a, occ_ref_b, exc_off_a, holes_a, parts_a,
+                             exc_off_b, holes_b, parts_b, ci, 0, 1, stream);
+}
+
+extern "C" int msd_setup_sharded(msd_ctx** out, int N, int n_alpha, int n_beta, int n_chol, int64_t n_det, const double* h1,
+                                 const double* L, double e0, const int32_t* occ_ref_a, const int32_t* occ_ref_b,
+                                 const int64_t* exc_off_a, const int32_t* holes_a, const int32_t* parts_a,
+                                 const int64_t* exc_off_b, const int32_t* holes_b, const int32_t* parts_b, const double* ci,
+                                 int shard_rank, int shard_world, void* stream)
+{
     if (!out) { g_setup_error = "out is NULL"; return MSD_EINVAL; }
     *out = nullptr;
     msd_ctx* c = new (std::nothrow) msd_ctx();
@@ -458,7 +479,7 @@ extern "C" int msd_setup(msd_ctx** out, int N, int n_alpha, int n_beta, int n_ch
     int rc;
     try {
         rc = do_setup(c, &err, N, n_alpha, n_beta, n_chol, n_det, h1, L, e0, occ_ref_a, occ_ref_b, exc_off_a, holes_a,
-                      parts_a, exc_off_b, holes_b, parts_b, ci, (cudaStream_t)stream);
+                      parts_a, exc_off_b, holes_b, parts_b, ci, (cudaStream_t)stream, shard_rank, shard_world);
     } catch (const std::bad_alloc&) {
         rc = MSD_ENOMEM; err = "out of host memory";
     }
@@ -543,6 +564,7 @@ extern "C" int msd_get_info(const msd_ctx* c, int64_t* info)
     info[0] = c->sp[0].n_o; info[1] = c->sp[0].n_v; info[2] = c->sp[1].n_o; info[3] = c->sp[1].n_v;
     info[4] = (int64_t)c->buckets.size(); info[5] = c->sp[0].kmax; info[6] = c->sp[1].kmax; info[7] = MSD_WT;
     info[8] = c->energy_ok ? 1 : 0;
+    info[9] = c->shard_rank; info[10] = c->shard_world;
     return MSD_OK;
 }
 
@@ -562,6 +584,12 @@ extern "C" int msd_set_workspace_limit(msd_ctx* c, int64_t bytes)
     c->ws_limit = bytes;
     c->ws_limit_auto = 0;        // re-read the free memory at the next call
     c->ws.want = 0;              // and lay the workspace out again (the fast path of ensure_workspace keys on it)
+    return MSD_OK;
+}
+extern "C" int msd_set_allreduce(msd_ctx* c, msd_allreduce_fn fn, void* user)
+{
+    if (!c) return MSD_EINVAL;
+    c->allreduce = fn; c->allreduce_user = user;
     return MSD_OK;
 }
 extern "C" int msd_set_option(msd_ctx* c, int option, int64_t value)
@@ -741,6 +769,19 @@ enum { CALL_OVERLAP = 1, CALL_FB = 2, CALL_GREENS = 4, CALL_ENERGY = 8, CALL_FB_
 
 static void mark(msd_ctx* c, int i, cudaStream_t st) { if (c->profiling) cudaEventRecord(c->ev[i], st); }
 
+// Determinant sharding: after a determinant pass the per-walker partial sums of this rank -- C^alpha, C^beta, W, E2nd, E1nd,
+// one contiguous run of doubles at the start of the workspace -- are summed over the ranks by the caller's hook (one
+// all-reduce of (2 + 2 n_o n_v ...) complex per walker: SURVEY.md 8(e)(ii)) before anything divides by W.
+static void shard_reduce(msd_ctx* c, Workspace& ws, cudaStream_t st)
+{
+    if (!c->allreduce) return;
+    const int64_t n = (int64_t)((reinterpret_cast<char*>(ws.E1nd + ws.wc) - reinterpret_cast<char*>(ws.C[0])) / sizeof(double));
+    // the partial sums are complete on the device when the hook runs (the determinant kernels ran on forked side streams);
+    // a sharded call is a collective anyway, so the host wait costs nothing that the all-reduce does not
+    cudaStreamSynchronize(st);
+    c->allreduce(c->allreduce_user, ws.C[0], n, (void*)st);
+}
+
 // S6: fb[w][g] += sum_(r,q) L_sub^s[g][(r,q)] G^s_w[(r,q)]  (one spin; fb zeroed by the caller: split-K partial sums meet in RED)
 static cudaError_t launch_fb_gemm(msd_ctx* c, int s, int64_t nw, Workspace& ws, cplx* fb, cudaStream_t st)
 {
@@ -788,6 +829,7 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
         mark(c, 1, st);
         if (call == CALL_OVERLAP) {
             CK(launch_dets(c, 0, nw, ws, st));
+            shard_reduce(c, ws, st);
             mark(c, 2, st);
             CK(launch_finish_overlap(c, nw, ws, out + w0, fl, st));
             mark(c, 3, st); mark(c, 4, st); mark(c, 5, st);
@@ -796,6 +838,7 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
             // matrices of all walkers as one DMMA contraction, the orbital update in place, the overlap of the new walkers
             cplx* pa_rw = const_cast<cplx*>(pa); cplx* pb_rw = const_cast<cplx*>(pb);
             CK(launch_dets(c, 1, nw, ws, st));
+            shard_reduce(c, ws, st);
             mark(c, 2, st);
             CK(launch_green_rows(c, nw, ws, nullptr, st));
             CK(cudaMemsetAsync(ws.fbuf, 0, sizeof(cplx) * (size_t)nw * ng, st));
@@ -814,12 +857,14 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
             CK(launch_reference(c, N, ldN, c->dev(0), c->dev(1), nw, pa, pb, ws, false, st));
             c->launches++;
             CK(launch_dets(c, 0, nw, ws, st));
+            shard_reduce(c, ws, st);
             CK(launch_finish_overlap(c, nw, ws, ws.ov_new, fl, st));
             mark(c, 5, st);
             CK(launch_prop_finish(c, nw, ws.ov_old, ws.ov_new, ws.expo, c->prop_w ? c->prop_w + w0 : nullptr,
                                   reinterpret_cast<double*>(out) + w0 * 8, ws.fl_old, fl, st));
         } else if (call == CALL_FB || call == CALL_GREENS) {
             CK(launch_dets(c, 1, nw, ws, st));
+            shard_reduce(c, ws, st);
             mark(c, 2, st);
             if (call == CALL_GREENS) {
                 cplx* G = out + w0 * (int64_t)2 * N * N;
@@ -903,11 +948,13 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
                 // B^gamma slices that the energy path holds anyway (W6), rows of [n_chol + 3]: fb, then (E, E1, E2)
                 const int64_t stride = (int64_t)ng + 3;
                 CK(launch_dets(c, 3, nw, ws, st));
+                shard_reduce(c, ws, st);
                 mark(c, 5, st);
                 CK(launch_fb_from_cb(c, nw, ws, out + w0 * stride, stride, st));
                 CK(launch_finish_energy(c, nw, ws, out + w0 * stride + ng, stride, fl, st));
             } else {
                 CK(launch_dets(c, 2, nw, ws, st));
+                shard_reduce(c, ws, st);
                 mark(c, 5, st);
                 CK(launch_finish_energy(c, nw, ws, out + w0 * 3, 3, fl, st));
             }

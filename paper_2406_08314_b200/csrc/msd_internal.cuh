@@ -201,6 +201,8 @@ struct msd_ctx {
     double* d_E = nullptr;                    // 3 x [ld][ld]: exp(-dt h'/2), the scaled matrix, scratch
     double prop_dt = 0.0; int prop_taylor = 0;
     const double* prop_x = nullptr; double* prop_w = nullptr;      // arguments of the running msd_propagate call
+    int shard_rank = 0, shard_world = 1;      // determinant sharding (msd_setup_sharded)
+    void (*allreduce)(void*, void*, int64_t, void*) = nullptr; void* allreduce_user = nullptr;     // msd_set_allreduce
     bool no_3m = false;                       // MSD_OPT_NO_3M: V contractions by the 4-multiplication real form (test hook)
     bool no_fused = false;                    // MSD_OPT_NO_FUSED_S7: take the Lambda GEMM + dense kernel pair (test hook)
     bool need_lam = true;                     // the workspace holds the Lambda buffer (two-kernel S7 path)

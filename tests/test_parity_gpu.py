@@ -712,3 +712,86 @@ def test_propagation_step_chunked_and_repeated(torch_cuda):
     S = out[:, 0] + 1j * out[:, 1]
     assert (np.abs(S - r2["S"]) / np.abs(r2["S"])).max() <= TOL_REL
     assert np.abs(wt.cpu().numpy() - r2["w"]).max() <= TOL_REL * np.abs(r2["w"]).max()
+
+
+# ----------------------------------------------------------------------------------------------
+# determinant-sharded contexts; the ranks are emulated ONE AFTER THE OTHER on this GPU
+# ----------------------------------------------------------------------------------------------
+class _EmulatedAllReduce:
+    """Stands in for the all-reduce of `world` ranks that run in turn on one GPU.  Pass p replays the sums of the reductions
+    0..p-1 (captured in earlier passes) and captures the partial buffers of reduction p; after (number of reductions + 1)
+    passes every rank has seen every reduction with the full sum, which is what concurrent ranks see."""
+
+    def __init__(self, world):
+        self.world = world
+        self.partial = {}                         # (reduction index, rank) -> tensor
+        self.rank = 0
+        self.idx = 0
+
+    def begin(self, rank):
+        self.rank, self.idx = rank, 0
+
+    def __call__(self, t):
+        k = self.idx
+        self.idx += 1
+        if all((k, r) in self.partial and self.partial[(k, r)] is not None for r in range(self.world)) and self.sealed > k:
+            t.copy_(sum(self.partial[(k, r)] for r in range(self.world)))
+        else:
+            self.partial[(k, self.rank)] = t.clone()
+
+
+@pytest.mark.parametrize("name,kw,world", [("small", dict(n_w=13), 2), ("sweep", dict(n_det=1500, max_level=6, n_w=9), 3)])
+def test_determinant_sharded_contexts_emulated_ranks(torch_cuda, name, kw, world):
+    """Every rank holds the whole trial but evaluates 1/world of every level bucket; the hook sums the partial W, C, E1nd,
+    E2nd.  Overlap, force bias, energy, the fused call and a propagation step must equal the oracle (and the unsharded
+    library) for every rank."""
+    from oracle import propagate as op
+    torch = torch_cuda
+    msd = _msd()
+    x = mi.generate(name, **kw)
+    ref = o2.run(x, return_G=False)
+    fields = np.random.default_rng(1).standard_normal((x.n_w, x.n_chol))
+    pref = op.step(x, fields, 0.005)
+    trials = [msd.setup_from_inputs(x, shard=(r, world)) for r in range(world)]
+    for r, t in enumerate(trials):
+        info = t.info()
+        assert (info["shard_rank"], info["shard_world"]) == (r, world)
+        t.propagator_setup(0.005, 6, x.h1, x.L)
+    pa0 = torch.tensor(x.phi_a, device="cuda")
+    pb0 = torch.tensor(x.phi_b, device="cuda")
+    xf = torch.tensor(fields, device="cuda")
+
+    def run_all(fn, n_reductions):
+        red = _EmulatedAllReduce(world)
+        outs = None
+        for p in range(n_reductions + 1):
+            red.sealed = p                        # reductions < p are complete and replayed
+            outs = []
+            for r, t in enumerate(trials):
+                t.set_allreduce(red)
+                red.begin(r)
+                outs.append(fn(t))
+            torch.cuda.synchronize()
+        return outs
+
+    for got in run_all(lambda t: t.overlap(pa0, pb0).cpu().numpy(), 1):
+        assert (np.abs(got - ref["ovlp"]) / np.abs(ref["ovlp"])).max() <= TOL_REL
+    for got in run_all(lambda t: t.force_bias(pa0, pb0).cpu().numpy(), 1):
+        assert (np.abs(got - ref["fb"]).max(axis=1) / np.abs(ref["fb"]).max(axis=1)).max() <= TOL_REL
+    for got in run_all(lambda t: t.local_energy(pa0, pb0).cpu().numpy(), 1):
+        assert np.abs(got - ref["E"]).max() <= TOL_E
+    for got in run_all(lambda t: t.force_bias_energy(pa0, pb0).cpu().numpy(), 1):
+        assert np.abs(got[:, x.n_chol:] - ref["E"]).max() <= TOL_E
+        assert (np.abs(got[:, :x.n_chol] - ref["fb"]).max(axis=1) / np.abs(ref["fb"]).max(axis=1)).max() <= TOL_REL
+
+    def prop(t):
+        pa, pb = pa0.clone(), pb0.clone()
+        out = t.propagate(pa, pb, xf).cpu().numpy()
+        return out, pa.cpu().numpy()
+    for out, pa in run_all(prop, 2):
+        S = out[:, 0] + 1j * out[:, 1]
+        assert (np.abs(S - pref["S"]) / np.abs(pref["S"])).max() <= TOL_REL
+        assert np.abs(pa - pref["phi_a"]).max() <= 1e-11 * np.abs(pref["phi_a"]).max()
+    for t in trials:
+        t.set_allreduce(None)
+        t.close()
