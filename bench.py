@@ -481,9 +481,9 @@ def main():
                          "peak_source": "measured live by the bench-side probe (csrc/probes.cu): random 128-byte lines of a "
                                         "32 MB L2-resident buffer, 16 B per lane, 8 independent loads in flight per lane",
                          "algorithmic_l2_bytes_per_step": l2_bytes, "share_of_step": acc["p4"] / (sum(step_ms) / len(step_ms))}
-        # force-bias determinant pass (k_dets_c1 + k_dets_gen<1>): plain FP64 ALU work against the FP64 peak
+        # force-bias determinant pass (k_dets_pull + k_dets_gen<1>): plain FP64 ALU work against the FP64 peak
         fl = fb_dets_flops(ka, kb) * nw
-        roofline_fb_dets = {"kernel": "k_dets_c1 + k_dets_gen<1> (force-bias mode: minors, adjugates, CI reduction)",
+        roofline_fb_dets = {"kernel": "k_dets_pull + k_dets_gen<1> (force-bias mode: minors, adjugates, CI reduction)",
                             "bound": "alu", "achieved": fl / (fbacc["p1"] * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
                             "frac": fl / (fbacc["p1"] * 1e-3) / 1e12 / peak if peak > 0 else None,
                             "peak_source": "FP64 pipe (DFMA and DMMA share it): the live DMMA probe",

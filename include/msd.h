@@ -66,8 +66,10 @@ typedef struct msd_ctx msd_ctx;   /* opaque; owns every device copy made at setu
  *       k_alpha^2 + k_beta^2 <= 400 for every determinant, active window per spin (n_o distinct hole orbitals,
  *       n_v distinct particle orbitals) n_o, n_v <= 255 and n_o*n_v <= 8192.
  *       The energy calls (msd_local_energy, msd_force_bias_energy) additionally need n_o*n_v <= 4096 per spin
- *       (they hold (n_o n_v)^2 two-body tensors per walker): a wider trial still sets up -- overlap, force bias
- *       and Green's function work -- msd_get_info()[8] is 0 and the energy calls return MSD_EUNSUPPORTED.
+ *       (they hold (n_o n_v)^2 two-body tensors per walker) and, for windows wider than 16 x 16, that
+ *       n^2 + 2 n n_v + 2 n_o n_v complex numbers per spin fit in 227 KB of shared memory: a wider trial still sets
+ *       up -- overlap, force bias and Green's function work -- msd_get_info()[8] is 0 and the energy calls return
+ *       MSD_EUNSUPPORTED.
  *   h1   HOST [N][N] row-major, real symmetric.
  *   L    HOST [n_chol][N][N], each slice real symmetric.
  *   e0   constant added to every energy.
