@@ -212,10 +212,15 @@ int msd_get_phase_ms(msd_ctx* ctx, float* ms, int n);
  *       written to memory by the GEMM, dense intermediates by a second kernel) that otherwise only runs for shapes the fused
  *       kernel does not cover.  Results are the same.
  *   MSD_OPT_NO_3M (0 / 1; default 0): TEST HOOK.  1 computes the V contractions with the four-multiplication real form of the
- *       complex product (k_gemm_tn) instead of the three-multiplication kernel (k_vgemm3m).  Same results to rounding. */
+ *       complex product (k_gemm_tn) instead of the three-multiplication kernel (k_vgemm3m).  Same results to rounding.
+ *   MSD_OPT_COOP_MIN_ELEMS (0..200; default 50 for the energy calls, 72 for overlap / force bias): TUNING KNOB / TEST HOOK.  Determinant buckets with an
+ *       excitation level above 4 in either spin and ka^2 + kb^2 above this value run the warp-cooperative kernel (one
+ *       determinant x 8 walkers per warp, 4 helper lanes per walker); the others keep one determinant per thread.  Same
+ *       results to rounding (the two kernels sum the same terms in different orders). */
 #define MSD_OPT_NO_SMEM_TILES 1
 #define MSD_OPT_NO_FUSED_S7 2
 #define MSD_OPT_NO_3M 3
+#define MSD_OPT_COOP_MIN_ELEMS 4
 int msd_set_option(msd_ctx* ctx, int option, int64_t value);
 
 void msd_destroy(msd_ctx* ctx);

@@ -28,6 +28,7 @@ EXPORTS = ["msd_setup", "msd_setup_sharded", "msd_set_allreduce", "msd_setup_fro
 MSD_OPT_NO_SMEM_TILES = 1
 MSD_OPT_NO_FUSED_S7 = 2
 MSD_OPT_NO_3M = 3
+MSD_OPT_COOP_MIN_ELEMS = 4
 
 
 class MSDError(RuntimeError):

@@ -566,9 +566,10 @@ struct SmMat {
     cplx* base; int T;
     __device__ __forceinline__ cplx& at(int e) { return base[e * T]; }
 };
+typedef unsigned short xidx_t;      // a pair index x < n_o n_v <= 8192 (include/msd.h); 16 bits keep the per-thread footprint at 18 B per element
 struct SmIdx {
-    int* base; int T;
-    __device__ __forceinline__ int& at(int e) { return base[e * T]; }
+    xidx_t* base; int T;
+    __device__ __forceinline__ xidx_t& at(int e) { return base[e * T]; }
 };
 
 // in-place Gauss-Jordan inverse with partial pivoting; returns det (0 if an exactly zero pivot appears,
@@ -713,7 +714,7 @@ __device__ __forceinline__ cplx closed_to_smem(SmMat m, SmIdx xs, const unsigned
 //   Ess = (1/R) sum_{a<c} sum_{b<d} (A[b][a] A[d][c] - A[b][c] A[d][a]) Vbar[x_ab][x_cd]        (Jacobi)
 // with columns a and c of A in registers and the C(K,2) loads of one (a,c) pair independent of one another.
 template <int K, int MODE>
-__device__ __noinline__ cplx spin_big(cplx* mbase, int* xbase, int T, const unsigned char* hp, const cplx* __restrict__ g, int no,
+__device__ __noinline__ cplx spin_big(cplx* mbase, xidx_t* xbase, int T, const unsigned char* hp, const cplx* __restrict__ g, int no,
                                       const cplx* __restrict__ Vss, unsigned P, cplx* Ess)
 {
     SmMat m{mbase, T};
@@ -767,7 +768,7 @@ __device__ __noinline__ cplx spin_big(cplx* mbase, int* xbase, int T, const unsi
 }
 
 // any level, runtime k (levels above 8)
-__device__ __noinline__ cplx spin_runtime(cplx* mbase, int* xbase, int T, int k, const unsigned char* hp,
+__device__ __noinline__ cplx spin_runtime(cplx* mbase, xidx_t* xbase, int T, int k, const unsigned char* hp,
                                           const cplx* __restrict__ g, int no, const cplx* __restrict__ Vss, unsigned P, int mode,
                                           cplx* Ess)
 {
@@ -803,7 +804,7 @@ __device__ __noinline__ cplx spin_runtime(cplx* mbase, int* xbase, int T, int k,
 }
 
 template <int MODE>
-__device__ __forceinline__ cplx spin_any(cplx* mbase, int* xbase, int T, int k, const unsigned char* hp, const cplx* __restrict__ g,
+__device__ __forceinline__ cplx spin_any(cplx* mbase, xidx_t* xbase, int T, int k, const unsigned char* hp, const cplx* __restrict__ g,
                                          int no, const cplx* __restrict__ Vss, unsigned P, cplx* Ess)
 {
     SmMat m{mbase, T};
@@ -825,7 +826,7 @@ __device__ __forceinline__ cplx spin_any(cplx* mbase, int* xbase, int T, int k, 
 // opposite-spin second-order sum  sum_v As[v] sum_u Ab[u] Vab[x_u, x_v]:  the K^2 loads of the higher-level spin
 // are unrolled (independent, four accumulators), the other spin's entries are a runtime loop
 template <int K>
-__device__ __noinline__ cplx opp_big(const cplx* mbig, const int* xbig, const cplx* msm, const int* xsm, int T, int ns,
+__device__ __noinline__ cplx opp_big(const cplx* mbig, const xidx_t* xbig, const cplx* msm, const xidx_t* xsm, int T, int ns,
                                      const cplx* __restrict__ V, unsigned sbig, unsigned ssm)
 {
     cplx e = cmake(0.0, 0.0);
@@ -844,7 +845,7 @@ __device__ __noinline__ cplx opp_big(const cplx* mbig, const int* xbig, const cp
     return e;
 }
 
-__device__ __noinline__ cplx opp_runtime(const cplx* mbig, const int* xbig, int nb, const cplx* msm, const int* xsm, int T, int ns,
+__device__ __noinline__ cplx opp_runtime(const cplx* mbig, const xidx_t* xbig, int nb, const cplx* msm, const xidx_t* xsm, int T, int ns,
                                          const cplx* __restrict__ V, unsigned sbig, unsigned ssm)
 {
     cplx e = cmake(0.0, 0.0);
@@ -872,7 +873,7 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
     const int T = blockDim.x;
     unsigned dyn_smem;
     asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn_smem));
-    const int elems_group = (int)(dyn_smem / ((sizeof(cplx) + sizeof(int)) * T));     // (complex + int) per element per thread
+    const int elems_group = (int)(dyn_smem / ((sizeof(cplx) + sizeof(xidx_t)) * T));     // (complex + index) per element per thread
     const cplx* gA = p.g[0] + (int64_t)tile * p.P[0] * MSD_WT + j;      // L1/L2 resident (57 KB per tile)
     const cplx* gB = p.g[1] + (int64_t)tile * p.P[1] * MSD_WT + j;
     double* CA = p.C[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j;
@@ -884,9 +885,12 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
     const cplx* FHB = (M_ENERGY(MODE)) ? p.FH[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j : nullptr;
     cplx Wl = cmake(0.0, 0.0), El = cmake(0.0, 0.0), Hl = cmake(0.0, 0.0);
     // snake order over rounds: items are sorted by descending cost, so alternate the direction to even out
-    for (int r = 0, ii; (ii = r * (int)gridDim.x + ((r & 1) ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x)),
-                        r * (int)gridDim.x < n_items; r++) {
-        if (ii >= n_items) continue;
+    // work items are sized for 128-thread CTAs (msd_api.cu); a smaller CTA takes 1/split of an item at a time
+    const int split = 128 / (int)blockDim.x, n_virt = n_items * split;
+    for (int r = 0, iv; (iv = r * (int)gridDim.x + ((r & 1) ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x)),
+                        r * (int)gridDim.x < n_virt; r++) {
+        if (iv >= n_virt) continue;
+        const int ii = iv / split, part = iv - ii * split;
         const WorkItem it = items[ii];
         const int ka = it.ka, kb = it.kb;
         const int na = ka * ka, nb = kb * kb;
@@ -894,9 +898,9 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
         cplx* mB = mA + na * T;
         // the int region starts at the LAUNCH GROUP's element bound, not at this item's na + nb: warps of a CTA are not
         // synchronised at item boundaries, so an item-dependent split would let one warp's indices alias another's matrix
-        int* xA = reinterpret_cast<int*>(gsm + elems_group * T) + threadIdx.x;
-        int* xB = xA + na * T;
-        for (int i = slot; i < it.det_count; i += nslots) {
+        xidx_t* xA = reinterpret_cast<xidx_t*>(gsm + elems_group * T) + threadIdx.x;
+        xidx_t* xB = xA + na * T;
+        for (int i = part * nslots + slot; i < it.det_count; i += nslots * split) {
             const uint32_t* rp = reinterpret_cast<const uint32_t*>(p.tab + it.tab_off + (int64_t)i * it.rs);
             union { uint32_t w[MSD_MAX_LEVEL]; unsigned char b[4 * MSD_MAX_LEVEL]; } row;
             for (int t = 0; t < it.rs / 4; t++) row.w[t] = __ldg(rp + t);
@@ -910,8 +914,8 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
                 cplx e = cmake(0.0, 0.0);
                 if (na > 0 && nb > 0) {
                     const bool abig = ka >= kb;
-                    const cplx* mb_ = abig ? mA : mB; const int* xb_ = abig ? xA : xB;
-                    const cplx* ms_ = abig ? mB : mA; const int* xs_ = abig ? xB : xA;
+                    const cplx* mb_ = abig ? mA : mB; const xidx_t* xb_ = abig ? xA : xB;
+                    const cplx* ms_ = abig ? mB : mA; const xidx_t* xs_ = abig ? xB : xA;
                     const unsigned sbig = abig ? (unsigned)p.P[1] : 1u, ssm = abig ? 1u : (unsigned)p.P[1];
                     const int ns = abig ? nb : na;
                     switch (abig ? ka : kb) {
@@ -1029,7 +1033,7 @@ __device__ __noinline__ cplx co_gauss_jordan(cplx* mw, int k, int hq)
 // indices (one copy per warp).  On exit mw holds A (entry b*k+a = A[b][a]), xw[b*k+a] = x(a,b); returns R (all helpers);
 // *ess = this helper's share of the same-spin second-order sum.
 template <int MODE>
-__device__ __forceinline__ cplx co_spin(cplx* mw, int* xw, int k, const unsigned char* hp, const cplx* __restrict__ g, int no,
+__device__ __forceinline__ cplx co_spin(cplx* mw, xidx_t* xw, int k, const unsigned char* hp, const cplx* __restrict__ g, int no,
                                         const cplx* __restrict__ Vss, unsigned P, int hq, int j, cplx* ess)
 {
     *ess = cmake(0.0, 0.0);
@@ -1052,7 +1056,7 @@ __device__ __forceinline__ cplx co_spin(cplx* mw, int* xw, int k, const unsigned
     const int lane = hq * 8 + j;
     for (int e = lane; e < k * k; e += 32) {      // pair indices, once per warp
         const int b = e / k, a = e - b * k;
-        xw[e] = (int)hp[k + b] * no + (int)hp[a];
+        xw[e] = (xidx_t)((int)hp[k + b] * no + (int)hp[a]);
     }
     __syncwarp();
     for (int e = hq; e < k * k; e += 4) {         // M[a][b] = g[x(a,b)]; x(a,b) sits at xw[b*k+a]
@@ -1064,24 +1068,27 @@ __device__ __forceinline__ cplx co_spin(cplx* mw, int* xw, int k, const unsigned
     for (int e = hq; e < k * k; e += 4) mw[e * 8] = cmul(R, mw[e * 8]);      // A = R M^-1
     __syncwarp();
     if (M_ENERGY(MODE) && (R.x != 0.0 || R.y != 0.0)) {
-        // T[b,d;a,c] = (A[b][a] A[d][c] - A[b][c] A[d][a]) / R; (a,c) pairs dealt round-robin to the helpers
+        // T[b,d;a,c] = (A[b][a] A[d][c] - A[b][c] A[d][a]) / R; helper hq takes the (a,c) pairs t = hq, hq+4, ... so that
+        // the four helpers of a walker work on four different pairs in the same instruction (all lanes active; dealing
+        // the pairs out by "skip unless t % 4 == hq" ran every pair with 8 of 32 lanes: profiles/r02_probes.md)
         cplx e = cmake(0.0, 0.0);
-        int t = 0;
-        for (int a = 0; a < k; a++)
-            for (int c = a + 1; c < k; c++, t++) {
-                if ((t & 3) != hq) continue;
-                for (int b = 0; b < k; b++) {
-                    const cplx Aba = mw[(b * k + a) * 8], Abc = mw[(b * k + c) * 8];
-                    const unsigned xab = (unsigned)xw[b * k + a] * P;
+        const int npair = k * (k - 1) / 2;
+        for (int t = hq; t < npair; t += 4) {
+            int a = 0, rem = t;
+            while (rem >= k - 1 - a) { rem -= k - 1 - a; a++; }
+            const int c = a + 1 + rem;
+            for (int b = 0; b < k - 1; b++) {
+                const cplx Aba = mw[(b * k + a) * 8], Abc = mw[(b * k + c) * 8];
+                const unsigned xab = (unsigned)xw[b * k + a] * P;
 #pragma unroll 4
-                    for (int d = b + 1; d < k; d++) {
-                        const cplx v = __ldg(&Vss[(xab + (unsigned)xw[d * k + c]) * MSD_WT]);
-                        cplx tt = cmul(Aba, mw[(d * k + c) * 8]);
-                        tt = cfms(Abc, mw[(d * k + a) * 8], tt);
-                        e = cfma(tt, v, e);
-                    }
+                for (int d = b + 1; d < k; d++) {
+                    const cplx v = __ldg(&Vss[(xab + (unsigned)xw[d * k + c]) * MSD_WT]);
+                    cplx tt = cmul(Aba, mw[(d * k + c) * 8]);
+                    tt = cfms(Abc, mw[(d * k + a) * 8], tt);
+                    e = cfma(tt, v, e);
                 }
             }
+        }
         *ess = cmul(e, cinv(R));
     }
     return R;
@@ -1095,7 +1102,7 @@ __global__ void __launch_bounds__(128, 4) k_dets_coop(DetsParams p, const WorkIt
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     const int j = lane & 7, hq = lane >> 3;
     cplx* mwarp = reinterpret_cast<cplx*>(smem_raw) + (size_t)wid * elems * 8;            // [elems][8 walkers]
-    int* xwarp = reinterpret_cast<int*>(reinterpret_cast<cplx*>(smem_raw) + (size_t)nwarps * elems * 8) + wid * elems;
+    xidx_t* xwarp = reinterpret_cast<xidx_t*>(reinterpret_cast<cplx*>(smem_raw) + (size_t)nwarps * elems * 8) + wid * elems;
     const cplx* gA = p.g[0] + (int64_t)tile * p.P[0] * MSD_WT + j;
     const cplx* gB = p.g[1] + (int64_t)tile * p.P[1] * MSD_WT + j;
     double* CA = p.C[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j;
@@ -1114,8 +1121,8 @@ __global__ void __launch_bounds__(128, 4) k_dets_coop(DetsParams p, const WorkIt
         const int na = ka * ka, nb = kb * kb;
         cplx* mA = mwarp + j;
         cplx* mB = mA + na * 8;
-        int* xA = xwarp;
-        int* xB = xwarp + na;
+        xidx_t* xA = xwarp;
+        xidx_t* xB = xwarp + na;
         for (int i = wid; i < it.det_count; i += nwarps) {
             const uint32_t* rp = reinterpret_cast<const uint32_t*>(p.tab + it.tab_off + (int64_t)i * it.rs);
             union { uint32_t w[MSD_MAX_LEVEL]; unsigned char b[4 * MSD_MAX_LEVEL]; } row;
@@ -1222,16 +1229,17 @@ __global__ void k_fh_tile(const cplx* __restrict__ Hrot, const cplx* __restrict_
 // ------------------------------------------------------------------------------------------------
 template <class K>
 static cudaError_t launch_persistent(msd_ctx* c, K kernel, int nthr, size_t smem, int n_sm, const DetsParams& p,
-                                     const WorkItem* items, int n_items, int ntiles, cudaStream_t st)
+                                     const WorkItem* items, int n_items, int ntiles, cudaStream_t st, int vsplit = 1)
 {
     if (n_items == 0) return cudaSuccess;
     int occ = 1;
     cudaError_t e = func_config(c, (const void*)kernel, nthr, smem, &occ);
     if (e != cudaSuccess) return e;
     // about two walker tiles resident at a time (their V slices stay in L2), every SM full
+    const int n_units = n_items * vsplit;      // k_dets_gen with CTAs below 128 threads works on 1/vsplit of an item at a time
     int workers = (n_sm * occ + 1) / 2;
-    if (workers > n_items) workers = n_items;
-    if (ntiles == 1) workers = n_items < n_sm * occ ? n_items : n_sm * occ;
+    if (workers > n_units) workers = n_units;
+    if (ntiles == 1) workers = n_units < n_sm * occ ? n_units : n_sm * occ;
     dim3 grid(workers, ntiles);
     kernel<<<grid, nthr, smem, st>>>(p, items, n_items);
     return cudaGetLastError();
@@ -1278,9 +1286,9 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
     for (size_t gi = c->gen_group_begin.size() - 1; gi-- > 0;) {
         const int i0 = c->gen_group_begin[gi], i1 = c->gen_group_begin[gi + 1];
         if (i1 == i0) continue;
-        if (c->gen_group_elems[gi] > 72) {        // the per-thread form would run with at most 3 warps per SM (measured crossover)
+        if (c->gen_group_elems[gi] > (MODE >= 2 ? c->coop_min_elems : c->coop_min_elems_fb)) {   // measured crossover (MSD_OPT_COOP_MIN_ELEMS)
             const int elems = c->gen_group_elems[gi];
-            const size_t smem = (size_t)4 * elems * (8 * sizeof(cplx) + sizeof(int));
+            const size_t smem = (size_t)4 * elems * (8 * sizeof(cplx) + sizeof(xidx_t));
             auto kern = k_dets_coop<MODE>;
             int occ = 1;
             cudaError_t e = func_config(c, (const void*)kern, 128, smem, &occ);
@@ -1293,12 +1301,15 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
             c->launches++;
             continue;
         }
+        // CTA size: 128 threads unless the group does not fit.  (Smaller CTAs would leave more warps resident -- shared
+        // memory per thread is fixed by the group -- but measured slower: the extra shared memory comes out of the L1 that
+        // holds the walker tile's g / Hrot / F slices.  profiles/r02_probes.md)
+        const size_t per_thread = (size_t)c->gen_group_elems[gi] * (sizeof(cplx) + sizeof(xidx_t));
         int nthr = 128;
-        const size_t per_thread = (size_t)c->gen_group_elems[gi] * (sizeof(cplx) + sizeof(int));
         while (nthr > 32 && per_thread * nthr > 200 * 1024) nthr -= 32;
         size_t smem = per_thread * nthr;
         cudaError_t e = launch_persistent(c, k_dets_gen<MODE>, nthr, smem, c->n_sm, p, c->d_items_gen + i0, i1 - i0, ntiles,
-                                          f.stream(li++));
+                                          f.stream(li++), 128 / nthr);
         if (e != cudaSuccess) { f.join(); return e; }
         c->launches++;
     }

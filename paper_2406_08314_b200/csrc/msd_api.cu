@@ -597,6 +597,7 @@ extern "C" int msd_set_option(msd_ctx* c, int option, int64_t value)
     if (!c) return MSD_EINVAL;
     if (option == MSD_OPT_NO_SMEM_TILES && value >= 0 && value <= 2) { c->no_smem_tiles = (int)value; return MSD_OK; }
     if (option == MSD_OPT_NO_3M && (value == 0 || value == 1)) { c->no_3m = value != 0; return MSD_OK; }
+    if (option == MSD_OPT_COOP_MIN_ELEMS && value >= 0 && value <= 200) { c->coop_min_elems = c->coop_min_elems_fb = (int)value; return MSD_OK; }
     if (option == MSD_OPT_NO_FUSED_S7 && (value == 0 || value == 1)) {
         c->no_fused = value != 0;
         int a, b, m, t, ko, kv;

@@ -203,6 +203,8 @@ struct msd_ctx {
     const double* prop_x = nullptr; double* prop_w = nullptr;      // arguments of the running msd_propagate call
     int shard_rank = 0, shard_world = 1;      // determinant sharding (msd_setup_sharded)
     void (*allreduce)(void*, void*, int64_t, void*) = nullptr; void* allreduce_user = nullptr;     // msd_set_allreduce
+    int coop_min_elems = 50;                  // MSD_OPT_COOP_MIN_ELEMS: groups with ka^2+kb^2 above this run k_dets_coop, the rest k_dets_gen
+    int coop_min_elems_fb = 72;               //   the same for the overlap / force-bias modes (measured crossovers: profiles/r02_sweep.md)
     bool no_3m = false;                       // MSD_OPT_NO_3M: V contractions by the 4-multiplication real form (test hook)
     bool no_fused = false;                    // MSD_OPT_NO_FUSED_S7: take the Lambda GEMM + dense kernel pair (test hook)
     bool need_lam = true;                     // the workspace holds the Lambda buffer (two-kernel S7 path)

@@ -569,6 +569,32 @@ def test_alternative_dense_paths(torch_cuda, name, kw, ws):
         assert np.abs(E - res[()]).max() <= TOL_E
 
 
+@pytest.mark.parametrize("kw,ws", [(dict(n_det=3000, max_level=7, n_w=21), [0, 8, 20]),
+                                   (dict(n_det=1500, max_level=10, n_w=9), [8])])
+def test_high_level_kernels_both_ways(torch_cuda, kw, ws):
+    """MSD_OPT_COOP_MIN_ELEMS: every bucket with a level >= 5 through the warp-cooperative kernel (threshold 0: also the
+    buckets whose other spin is at level 0..4, i.e. its closed-form branch) and through the one-determinant-per-thread
+    kernel (threshold 200: also levels 9-10, its runtime-k branch and CTAs below 128 threads) -- overlap, force bias
+    and energy against the oracle O2, fused call included; ragged last walker tile."""
+    msd = _msd()
+    torch = torch_cuda
+    x = mi.generate("sweep", **kw)
+    pa = torch.tensor(x.phi_a, device="cuda")
+    pb = torch.tensor(x.phi_b, device="cuda")
+    ref = o2.run(x, walkers=ws, return_G=False)
+    for th in (0, 200):
+        trial = msd.setup_from_inputs(x)
+        with pytest.raises(msd.MSDError):
+            trial.set_option(msd.MSD_OPT_COOP_MIN_ELEMS, 201)
+        trial.set_option(msd.MSD_OPT_COOP_MIN_ELEMS, th)
+        got = dict(ovlp=trial.overlap(pa, pb).cpu().numpy(), fb=trial.force_bias(pa, pb).cpu().numpy(),
+                   E=trial.local_energy(pa, pb).cpu().numpy())
+        fused = trial.force_bias_energy(pa, pb).cpu().numpy()
+        trial.close()
+        assert_parity(got, ref, walkers=ws, what=("ovlp", "fb", "E"))
+        assert_parity(dict(fb=fused[:, :x.n_chol], E=fused[:, x.n_chol:]), ref, walkers=ws, what=("fb", "E"))
+
+
 def test_window_wider_than_shared_memory(torch_cuda):
     """An active window of 10 occupied x 100 virtual orbitals per spin (the paper's [Cu2O2]2+ has 16 x 92,
     PAPER.md:L303): 2000 pair indices, so neither the g slices (256 KB per walker tile) nor C / Hrot / F fit in shared
