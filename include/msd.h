@@ -193,6 +193,30 @@ int msd_get_packed(const msd_ctx* ctx, int64_t* perm, double* coef, int32_t* lev
  * memory at the first call); walkers are processed in chunks that fit. */
 int msd_set_workspace_limit(msd_ctx* ctx, int64_t bytes);
 
+/* No-allocation variant of msd_overlap, for callers that cannot allocate in the hot loop (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc).  Same arguments, same result as msd_overlap (same kernels; sums
+ * in the same order up to the order of atomic adds), but the call's workspace -- zeroed per-walker accumulators, Theta, g,
+ * det0 of the walkers -- lives in ONE file-scope device array of MSD_NOALLOC_SCRATCH_BYTES inside the library instead of
+ * the context's cudaMalloc'ed workspace; every GPU that loads the library holds that array until the process exits.
+ *   msd_noalloc_setup(ctx, stream): SET-UP, once per context, with the context's device current, outside the
+ *       no-allocation region: resolves the array's device address for this device and creates the context's side streams
+ *       and events (this call MAY allocate).  Determinant-sharded contexts: MSD_EUNSUPPORTED.
+ *   msd_overlap_noalloc(...): calls no cudaMalloc / cudaFree / stream or event creation and no allocating library routine;
+ *       it launches kernels and records / waits on the context's existing events only.  Without a prior msd_noalloc_setup
+ *       on the context: MSD_EINVAL.  The whole batch must fit: n_w walkers need about
+ *       16 B x ceil8(n_w) x (5 + sum_sigma (N n_sigma + 2 n_o n_v)) bytes (ceil8: rounded up to a multiple of 8; e.g. up to
+ *       48 walkers of N = 100, n_alpha = n_beta = 20 with a
+ *       15 x 15 active window); a larger batch is refused with MSD_ENOMEM and a message that states both sizes -- split the
+ *       batch or use msd_overlap.  n_w = 0 is a no-op.
+ *   The array is shared by every context and every call on the device and keeps the last call's contents; the accumulators
+ *   are cleared at the start of each call.  Calls that overlap on the GPU (different streams, host threads or contexts)
+ *   RACE on it: the caller keeps them ordered (one stream, or events).  It does not interfere with the other calls of the
+ *   context, which keep their own workspace. */
+#define MSD_NOALLOC_SCRATCH_BYTES (4 * 1024 * 1024)
+int msd_noalloc_setup(msd_ctx* ctx, void* stream);
+int msd_overlap_noalloc(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
+                        void* ovlp, int32_t* flags, void* stream);
+
 /* Number of kernels the library launched on this context since setup (for bench.py's gpu_launches). */
 int64_t msd_launch_count(const msd_ctx* ctx);
 

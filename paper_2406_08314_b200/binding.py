@@ -24,7 +24,9 @@ EXPORTS = ["msd_setup", "msd_setup_sharded", "msd_set_allreduce", "msd_setup_fro
            "msd_force_bias_energy", "msd_force_bias_energy_host",
            "msd_propagator_setup", "msd_propagate",
            "msd_get_info", "msd_get_packed", "msd_set_workspace_limit", "msd_set_option", "msd_launch_count",
-           "msd_set_profiling", "msd_get_phase_ms", "msd_destroy", "msd_last_error"]
+           "msd_set_profiling", "msd_get_phase_ms", "msd_destroy", "msd_last_error",
+           "msd_noalloc_setup", "msd_overlap_noalloc"]
+MSD_NOALLOC_SCRATCH_BYTES = 4 * 1024 * 1024
 MSD_OPT_NO_SMEM_TILES = 1
 MSD_OPT_NO_FUSED_S7 = 2
 MSD_OPT_NO_3M = 3
@@ -60,10 +62,13 @@ def load_library() -> C.CDLL:
     lib.msd_setup_from_occ.restype = i32
     lib.msd_setup_from_occ.argtypes = [C.POINTER(vp), i32, i32, i32, i32, i64, vp, vp, dbl, vp, vp, vp, vp]
     for name in ("msd_overlap", "msd_force_bias", "msd_local_energy", "msd_greens", "msd_force_bias_energy",
-                 "msd_overlap_host", "msd_force_bias_host", "msd_local_energy_host", "msd_force_bias_energy_host"):
+                 "msd_overlap_host", "msd_force_bias_host", "msd_local_energy_host", "msd_force_bias_energy_host",
+                 "msd_overlap_noalloc"):
         f = getattr(lib, name)
         f.restype = i32
         f.argtypes = [vp, i64, vp, vp, vp, vp, vp]
+    lib.msd_noalloc_setup.restype = i32
+    lib.msd_noalloc_setup.argtypes = [vp, vp]
     lib.msd_propagator_setup.restype = i32
     lib.msd_propagator_setup.argtypes = [vp, dbl, i32, vp, vp, vp]
     lib.msd_propagate.restype = i32
@@ -165,7 +170,7 @@ class MSDTrial:
     def _out_shape(self, fn, nw):
         """Result shape of a hot call (include/msd.h), by entry-point name."""
         name = fn.__name__.replace("_host", "")
-        return {"msd_overlap": (nw,), "msd_force_bias": (nw, self.n_chol), "msd_local_energy": (nw, 3),
+        return {"msd_overlap": (nw,), "msd_overlap_noalloc": (nw,), "msd_force_bias": (nw, self.n_chol), "msd_local_energy": (nw, 3),
                 "msd_force_bias_energy": (nw, self.n_chol + 3), "msd_greens": (nw, 2, self.N, self.N)}[name]
 
     def overlap(self, phi_a, phi_b, out=None, flags=None, stream=None):
@@ -173,6 +178,15 @@ class MSDTrial:
         nw = self._walkers(phi_a, phi_b)
         out = torch.empty(nw, dtype=torch.complex128, device=phi_a.device) if out is None else out
         return self._call(load_library().msd_overlap, phi_a, phi_b, out, flags, stream)
+
+    def noalloc_setup(self, stream=None):
+        """Set-up for overlap_noalloc (include/msd.h: msd_noalloc_setup): once per context, may allocate."""
+        self._check(load_library().msd_noalloc_setup(self._h, _stream_ptr(stream)))
+
+    def overlap_noalloc(self, phi_a, phi_b, out, flags=None, stream=None):
+        """msd_overlap_noalloc: the overlap with the workspace in the library's static device array; `out` (and `flags`)
+        are the caller's -- nothing is allocated here either.  Batches beyond MSD_NOALLOC_SCRATCH_BYTES raise MSDError."""
+        return self._call(load_library().msd_overlap_noalloc, phi_a, phi_b, out, flags, stream)
 
     def force_bias(self, phi_a, phi_b, out=None, flags=None, stream=None):
         import torch

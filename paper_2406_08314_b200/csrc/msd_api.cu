@@ -1104,3 +1104,117 @@ extern "C" int msd_force_bias_energy_host(msd_ctx* c, int64_t n_w, const void* p
 extern "C" int msd_local_energy_host(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* e, int32_t* flags,
                                      void* stream)
 { return hot_call_host(c, CALL_ENERGY, 3, n_w, phi_a, phi_b, e, flags, stream); }
+
+// ---------------------------------------------------------------------------------------------
+// No-allocation variant of the overlap call (include/msd.h: msd_noalloc_setup, msd_overlap_noalloc).
+//
+// For callers that cannot allocate in the hot loop (code under CUDA graph capture, tight serving loops, harnesses that forbid
+// cudaMalloc): the per-call workspace of msd_overlap -- the zeroed per-walker accumulators C^a, C^b, W, the reference data
+// Theta, g, det0 -- is carved out of ONE file-scope device array of MSD_NOALLOC_SCRATCH_BYTES instead of the context's
+// cudaMalloc'ed workspace.  Every GPU that loads the library holds the array until the process exits.
+//
+// g_noalloc_scratch names the array in DEVICE code only (k_noalloc_clear below uses it directly).  In host code the same
+// name is a host-side stand-in, not a device address: the address the kernels get comes from cudaGetSymbolAddress, taken once
+// per device at set-up (msd_noalloc_setup) with that device current.
+// All contexts and all calls on a device share the array and it keeps the previous call's contents: the accumulator region is
+// cleared at the start of every call, and calls that overlap on the GPU (two streams, two threads, two contexts) race.
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_noalloc_scratch[MSD_NOALLOC_SCRATCH_BYTES];
+
+static const int NOALLOC_MAX_DEVICES = 64;
+static char* g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};      // device address of g_noalloc_scratch on device d (0: not set up)
+static std::mutex g_noalloc_mu;
+
+// clears the first n16 16-byte words of the scratch array (the accumulators that must start at zero)
+__global__ void k_noalloc_clear(size_t n16)
+{
+    uint4* p = reinterpret_cast<uint4*>(g_noalloc_scratch);
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (size_t)gridDim.x * blockDim.x)
+        p[i] = make_uint4(0u, 0u, 0u, 0u);
+}
+
+extern "C" int msd_noalloc_setup(msd_ctx* c, void* stream)
+{
+    if (!c) return MSD_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != c->device) { c->err = "context used on another device"; return MSD_EINVAL; }
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) { c->err = "device ordinal beyond the no-allocation table"; return MSD_EUNSUPPORTED; }
+    if (c->shard_world > 1) { c->err = "msd_overlap_noalloc does not take determinant-sharded contexts"; return MSD_EUNSUPPORTED; }
+    {
+        std::lock_guard<std::mutex> lk(g_noalloc_mu);
+        if (!g_noalloc_ptr[dev]) {
+            char* p = nullptr;
+            cudaError_t e = cudaGetSymbolAddress((void**)&p, g_noalloc_scratch);
+            if (e != cudaSuccess || !p) {
+                c->err = std::string("cudaGetSymbolAddress(g_noalloc_scratch): ") + cudaGetErrorString(e);
+                cudaGetLastError();
+                return MSD_ECUDA;
+            }
+            g_noalloc_ptr[dev] = p;
+        }
+    }
+    // everything the hot call would otherwise create lazily: the context's side streams and fork/join events ...
+    {
+        Fork f(c, st);
+        f.stream(1);
+        cudaError_t e = f.join();
+        if (e != cudaSuccess || f.err != cudaSuccess) { c->err = "creating the side streams failed"; cudaGetLastError(); return MSD_ECUDA; }
+    }
+    // (The kernels' shared-memory attributes and occupancy entries are set by func_config at their first launch:
+    // cudaFuncSetAttribute and the occupancy query allocate nothing.)
+    c->noalloc_ready = true;
+    return MSD_OK;
+}
+
+extern "C" int msd_overlap_noalloc(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* ovlp, int32_t* flags,
+                                   void* stream)
+{
+    if (!c) return MSD_EINVAL;
+    if (n_w < 0 || (n_w > 0 && (!ovlp || (c->sp[0].n > 0 && !phi_a) || (c->sp[1].n > 0 && !phi_b)))) {
+        c->err = "bad argument";
+        return MSD_EINVAL;
+    }
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != c->device) { c->err = "context used on another device"; return MSD_EINVAL; }
+    if (!c->noalloc_ready || dev < 0 || dev >= NOALLOC_MAX_DEVICES || !g_noalloc_ptr[dev]) {
+        c->err = "msd_overlap_noalloc: call msd_noalloc_setup(ctx) first (once per context, outside the no-allocation region)";
+        return MSD_EINVAL;
+    }
+    if (n_w == 0) return MSD_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    // layout of the overlap workspace (level 1) for the whole batch: no chunking here, a batch that does not fit is refused
+    const int64_t wc = (n_w + MSD_WT - 1) / MSD_WT * MSD_WT;
+    Workspace ws;
+    const size_t need = carve(c, ws, nullptr, wc, 1);
+    if (need > (size_t)MSD_NOALLOC_SCRATCH_BYTES) {
+        char msg[256];
+        snprintf(msg, sizeof msg, "msd_overlap_noalloc: n_w = %lld needs %zu bytes of scratch, the library holds "
+                 "MSD_NOALLOC_SCRATCH_BYTES = %d; split the batch or use msd_overlap", (long long)n_w, need, MSD_NOALLOC_SCRATCH_BYTES);
+        c->err = msg;
+        return MSD_ENOMEM;
+    }
+    char* base = g_noalloc_ptr[dev];                // a device address (cudaGetSymbolAddress), never &g_noalloc_scratch
+    carve(c, ws, base, wc, 1);
+    ws.wc = wc; ws.want = wc; ws.level = 1; ws.base = base; ws.bytes = MSD_NOALLOC_SCRATCH_BYTES;
+    const int N = c->N, ldN = N + (N & 1);
+    std::string err;
+    auto run = [&]() -> int {
+        std::string* errp = &err;
+        // the zero region is the first zero_bytes of the array (carve puts it first; a multiple of 256 bytes)
+        if (ws.zero_begin != base) return fail(errp, MSD_ECUDA, "unexpected workspace layout");
+        const size_t n16 = ws.zero_bytes / 16;
+        const unsigned blocks = (unsigned)std::min<size_t>((n16 + 255) / 256, (size_t)c->n_sm * 8);
+        k_noalloc_clear<<<blocks ? blocks : 1, 256, 0, st>>>(n16);
+        CK(cudaGetLastError());
+        c->launches++;
+        CK(launch_reference(c, N, ldN, c->dev(0), c->dev(1), n_w, (const cplx*)phi_a, (const cplx*)phi_b, ws, false, st));
+        c->launches++;
+        CK(launch_dets(c, 0, n_w, ws, st));
+        CK(launch_finish_overlap(c, n_w, ws, (cplx*)ovlp, flags, st));
+        return MSD_OK;
+    };
+    const int rc = run();
+    if (rc != MSD_OK) { c->err = err; cudaGetLastError(); }
+    return rc;
+}

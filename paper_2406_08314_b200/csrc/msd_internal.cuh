@@ -205,6 +205,7 @@ struct msd_ctx {
     void (*allreduce)(void*, void*, int64_t, void*) = nullptr; void* allreduce_user = nullptr;     // msd_set_allreduce
     int coop_min_elems = 50;                  // MSD_OPT_COOP_MIN_ELEMS: groups with ka^2+kb^2 above this run k_dets_coop, the rest k_dets_gen
     int coop_min_elems_fb = 72;               //   the same for the overlap / force-bias modes (measured crossovers: profiles/r02_sweep.md)
+    bool noalloc_ready = false;               // msd_noalloc_setup ran on this context (msd_api.cu, no-allocation overlap call)
     bool no_3m = false;                       // MSD_OPT_NO_3M: V contractions by the 4-multiplication real form (test hook)
     bool no_fused = false;                    // MSD_OPT_NO_FUSED_S7: take the Lambda GEMM + dense kernel pair (test hook)
     bool need_lam = true;                     // the workspace holds the Lambda buffer (two-kernel S7 path)
