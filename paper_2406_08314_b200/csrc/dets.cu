@@ -673,6 +673,72 @@ __device__ __forceinline__ cplx gauss_jordan_t(SmMat m)
     return det;
 }
 
+// Determinant only (overlap mode needs no adjugate): the forward half of the same elimination -- same pivots, same
+// operation order as gauss_jordan / gauss_jordan_t on the rows below the pivot, hence the same value -- at a third of the
+// shared-memory traffic.  0 for an exactly singular matrix.
+__device__ cplx det_lu(SmMat m, int k)
+{
+    cplx det = cmake(1.0, 0.0);
+    for (int j = 0; j < k; j++) {
+        int p = j; double best = cabs2(m.at(j * k + j));
+        for (int i = j + 1; i < k; i++) { double v = cabs2(m.at(i * k + j)); if (v > best) { best = v; p = i; } }
+        if (!(best > 0.0)) return cmake(0.0, 0.0);
+        if (p != j) {
+            for (int c = j; c < k; c++) { cplx t = m.at(j * k + c); m.at(j * k + c) = m.at(p * k + c); m.at(p * k + c) = t; }
+            det = cneg(det);
+        }
+        const cplx pv = m.at(j * k + j);
+        det = cmul(det, pv);
+        const cplx r = cinv(pv);
+        for (int c = j + 1; c < k; c++) m.at(j * k + c) = cmul(m.at(j * k + c), r);
+        for (int i = j + 1; i < k; i++) {
+            const cplx f = m.at(i * k + j);
+            for (int c = j + 1; c < k; c++) m.at(i * k + c) = cfms(f, m.at(j * k + c), m.at(i * k + c));
+        }
+    }
+    return det;
+}
+
+template <int K>
+__device__ __forceinline__ cplx det_lu_t(SmMat m)
+{
+    cplx det = cmake(1.0, 0.0);
+    bool sing = false;
+#pragma unroll (K <= 6 ? K : 1)
+    for (int j = 0; j < K; j++) {
+        int p = j; double best = cabs2(m.at(j * K + j));
+#pragma unroll
+        for (int i = 1; i < K; i++) {
+            if (i > j) { double v = cabs2(m.at(i * K + j)); if (v > best) { best = v; p = i; } }
+        }
+        if (!(best > 0.0)) { sing = true; break; }
+        cplx prow[K];                             // columns <= j are never read again
+#pragma unroll
+        for (int c = 0; c < K; c++) if (c >= j) prow[c] = m.at(p * K + c);
+        if (p != j) {
+#pragma unroll
+            for (int c = 0; c < K; c++) if (c >= j) m.at(p * K + c) = m.at(j * K + c);
+            det = cneg(det);
+        }
+        cplx pv = cmake(1.0, 0.0);
+#pragma unroll
+        for (int c = 0; c < K; c++) if (c == j) pv = prow[c];
+        det = cmul(det, pv);
+        const cplx r = cinv(pv);
+#pragma unroll
+        for (int c = 0; c < K; c++) if (c > j) prow[c] = cmul(prow[c], r);
+#pragma unroll
+        for (int i = 1; i < K; i++) {
+            if (i <= j) continue;
+            const cplx f = m.at(i * K + j);
+#pragma unroll
+            for (int c = 1; c < K; c++)
+                if (c > j) m.at(i * K + c) = cfms(f, prow[c], m.at(i * K + c));
+        }
+    }
+    return sing ? cmake(0.0, 0.0) : det;
+}
+
 // levels 1..4 inside the generic kernel (the other spin of a high-level bucket): closed forms in registers,
 // A and x written to the thread's shared-memory regions
 template <int K>
@@ -688,6 +754,7 @@ __device__ __forceinline__ cplx closed_to_smem(SmMat m, SmIdx xs, const unsigned
 #pragma unroll
         for (int b = 0; b < K; b++) M[a][b] = __ldg(&g[(pn[b] + h[a]) * MSD_WT]);
     cplx R = Closed<K>::det_adj(M, A);
+    if (mode == 0) { *Ess = cmake(0.0, 0.0); return R; }      // overlap: the determinant only (the adjugate is dead code)
 #pragma unroll
     for (int a = 0; a < K; a++)
 #pragma unroll
@@ -730,8 +797,9 @@ __device__ __noinline__ cplx spin_big(cplx* mbase, xidx_t* xbase, int T, const u
 #pragma unroll
         for (int b = 0; b < K; b++) row[b] = __ldg(&g[(pn[b] + ha) * MSD_WT]);
 #pragma unroll
-        for (int b = 0; b < K; b++) { m.at(a * K + b) = row[b]; xs.at(b * K + a) = pn[b] + ha; }
+        for (int b = 0; b < K; b++) { m.at(a * K + b) = row[b]; if (MODE != 0) xs.at(b * K + a) = pn[b] + ha; }
     }
+    if (MODE == 0) { *Ess = cmake(0.0, 0.0); return det_lu_t<K>(m); }      // overlap: forward elimination only
     const cplx R = gauss_jordan_t<K>(m);          // m = M^-1 (or zeros)
 #pragma unroll
     for (int e = 0; e < K * K; e++) m.at(e) = cmul(R, m.at(e));   // A = R M^-1, entry b*K+a = A[b][a]
@@ -780,9 +848,10 @@ __device__ __noinline__ cplx spin_runtime(cplx* mbase, xidx_t* xbase, int T, int
             m.at(a * k + b) = __ldg(&g[x * MSD_WT]);
             xs.at(b * k + a) = x;
         }
+    *Ess = cmake(0.0, 0.0);
+    if (mode == 0) return det_lu(m, k);
     cplx R = gauss_jordan(m, k);
     for (int e = 0; e < k * k; e++) m.at(e) = cmul(R, m.at(e));
-    *Ess = cmake(0.0, 0.0);
     if (mode >= 2 && (R.x != 0.0 || R.y != 0.0)) {
         cplx e = cmake(0.0, 0.0);
         for (int a = 0; a < k; a++)
@@ -1029,6 +1098,42 @@ __device__ __noinline__ cplx co_gauss_jordan(cplx* mw, int k, int hq)
     return det;
 }
 
+// determinant only (overlap mode): the forward half of co_gauss_jordan -- same pivots, same operations on the rows below
+// the pivot, hence the same value; rows j0+1.. are dealt to the four helpers
+__device__ __noinline__ cplx co_det_lu(cplx* mw, int k, int hq)
+{
+    cplx det = cmake(1.0, 0.0);
+    bool sing = false;
+    for (int j0 = 0; j0 < k; j0++) {
+        int p = j0; double best = -1.0;
+        for (int i = j0 + hq; i < k; i += 4) { const double v = cabs2(mw[(i * k + j0) * 8]); if (v > best) { best = v; p = i; } }
+#pragma unroll
+        for (int o = 8; o <= 16; o <<= 1) {
+            const double ob = __shfl_xor_sync(0xffffffffu, best, o);
+            const int op = __shfl_xor_sync(0xffffffffu, p, o);
+            if (ob > best || (ob == best && op < p)) { best = ob; p = op; }
+        }
+        if (!(best > 0.0)) sing = true;
+        if (p != j0) {
+            for (int c = j0 + hq; c < k; c += 4) { const cplx t = mw[(j0 * k + c) * 8]; mw[(j0 * k + c) * 8] = mw[(p * k + c) * 8]; mw[(p * k + c) * 8] = t; }
+            det = cneg(det);
+        }
+        __syncwarp();
+        const cplx pv = mw[(j0 * k + j0) * 8];
+        det = cmul(det, pv);
+        const cplx r = sing ? cmake(0.0, 0.0) : cinv(pv);
+        __syncwarp();
+        for (int c = j0 + 1 + hq; c < k; c += 4) mw[(j0 * k + c) * 8] = cmul(mw[(j0 * k + c) * 8], r);
+        __syncwarp();
+        for (int i = j0 + 1 + hq; i < k; i += 4) {
+            const cplx f = mw[(i * k + j0) * 8];
+            for (int c = j0 + 1; c < k; c++) mw[(i * k + c) * 8] = cfms(f, mw[(j0 * k + c) * 8], mw[(i * k + c) * 8]);
+        }
+        __syncwarp();
+    }
+    return sing ? cmake(0.0, 0.0) : det;
+}
+
 // one spin of the warp's determinant.  mw: this lane's walker column of the spin's matrix region; xw: the spin's pair
 // indices (one copy per warp).  On exit mw holds A (entry b*k+a = A[b][a]), xw[b*k+a] = x(a,b); returns R (all helpers);
 // *ess = this helper's share of the same-spin second-order sum.
@@ -1064,6 +1169,7 @@ __device__ __forceinline__ cplx co_spin(cplx* mw, xidx_t* xw, int k, const unsig
         mw[e * 8] = __ldg(&g[xw[b * k + a] * MSD_WT]);
     }
     __syncwarp();
+    if (MODE == 0) return co_det_lu(mw, k, hq);      // overlap: no adjugate
     const cplx R = co_gauss_jordan(mw, k, hq);
     for (int e = hq; e < k * k; e += 4) mw[e * 8] = cmul(R, mw[e * 8]);      // A = R M^-1
     __syncwarp();
