@@ -263,6 +263,30 @@ def test_walker_equals_reference_exact_singular_minors(torch_cuda, name):
         assert np.abs(got["G"][w] - ref["G"][0]).max() <= TOL_REL
 
 
+@pytest.mark.parametrize("coop_min", [None, 0, 200])
+def test_walker_equals_reference_exact_singular_minors_high_levels(torch_cuda, coop_min):
+    """The same through the level >= 5 kernels (in-shared-memory eliminations: every pivot is exactly zero, so the
+    determinant-only elimination of the overlap call, the Gauss-Jordan inverse of the other calls and their cooperative
+    forms must all return exact zeros, not NaN): N = 12, 6 + 6 electrons, levels up to 6 in each spin; per-thread kernel,
+    cooperative kernel (MSD_OPT_COOP_MIN_ELEMS 0) and the default mix.  Oracle: O0 (seconds at this size)."""
+    msd = _msd()
+    x = mi.generate("sweep", N=12, n_alpha=6, n_beta=6, A=12, n_det=40, max_level=6, n_w=8, n_chol=10)
+    assert max(np.diff(x.exc_off_a).max(), np.diff(x.exc_off_b).max()) >= 5
+    x = _reference_walkers(x, 3)
+    trial = msd.setup_from_inputs(x)
+    if coop_min is not None:
+        trial.set_option(msd.MSD_OPT_COOP_MIN_ELEMS, coop_min)
+    got = gpu_all(torch_cuda, x, trial=trial)
+    trial.close()
+    ref = mo.run(x, "o0", walkers=[0])
+    assert (got["flags"] == 0).all()
+    for w in range(3):
+        assert abs(got["ovlp"][w] - x.ci[0]) <= 1e-15
+        assert np.abs(got["E"][w] - ref["E"][0]).max() <= TOL_E
+        assert np.abs(got["fb"][w] - ref["fb"][0]).max() <= TOL_REL * np.abs(ref["fb"][0]).max()
+        assert np.abs(got["G"][w] - ref["G"][0]).max() <= TOL_REL
+
+
 @pytest.mark.parametrize("eps,K", [(1e-1, 6), (1e-3, 6), (1e-6, 6), (1e-9, 6), (1e-3, 10), (1e-9, 9)])
 def test_near_reference_walkers(torch_cuda, eps, K):
     """P8: psi = QR(D_0 + eps Z): the regime of real AFQMC walkers; stresses det*inverse cofactors (the Jacobi division
