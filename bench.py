@@ -74,7 +74,8 @@ def ncu_traffic(kernel_prefix: str):
     scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
     tot, n = 0.0, 0
     for r in rows[rows.index(hdr) + 2:]:
-        if len(r) > max(k, rd, wr) and r[k].startswith(kernel_prefix):
+        name = r[k][5:] if len(r) > k and r[k].startswith("void ") else (r[k] if len(r) > k else "")   # templated kernels print as "void k<...>"
+        if len(r) > max(k, rd, wr) and name.startswith(kernel_prefix):
             tot += float(r[rd].replace(",", "")) * scale.get(units[rd], 1.0) + \
                    float(r[wr].replace(",", "")) * scale.get(units[wr], 1.0)
             n += 1
@@ -475,7 +476,7 @@ def main():
         kb = np.diff(inp.exc_off_b).astype(np.float64)
         gathers = float(np.sum(ka * ka * kb * kb + (ka * (ka - 1) / 2) ** 2 + (kb * (kb - 1) / 2) ** 2))
         l2_bytes = 16.0 * gathers * nw
-        roofline_dets = {"kernel": "k_dets_cf<2> + k_dets_gen<2> (energy mode, forked over side streams)",
+        roofline_dets = {"kernel": "k_dets_cf<2> + k_dets_gen<2> + k_dets_coop<2> (energy mode, forked over side streams)",
                          "bound": "l2", "achieved": l2_bytes / (acc["p4"] * 1e-3) / 1e9, "peak": l2_gather, "unit": "GB/s",
                          "frac": l2_bytes / (acc["p4"] * 1e-3) / 1e9 / l2_gather if l2_gather > 0 else None,
                          "peak_source": "measured live by the bench-side probe (csrc/probes.cu): random 128-byte lines of a "
