@@ -463,7 +463,8 @@ def main():
         r_s7 = tensor_roofline("k_energy_fused (S7: Lambda = L_sub Theta by FP64 DMMA + dense intermediates, 1 launch)",
                                "k_energy_fused", flops_lam + flops_dense, s7_ms,
                                "executes (40/35 padded rows) more DMMA than the algorithmic count")
-        r_v = tensor_roofline("k_vgemm3m (V contractions alpha-beta, alpha-alpha, beta-beta: 3 launches on forked streams)",
+        r_v = tensor_roofline("k_vgemm3m (V contractions alpha-beta, alpha-alpha, beta-beta: 3 launches on forked streams; the walkers with an "
+                              "ill-conditioned reference block go through the 4-multiplication k_gemm_tn instead: DESIGN.md section 7)",
                               "k_vgemm3m", flops_v, v_ms,
                               "achieved counts 8 flops per complex MAC (the method's work); the kernel executes 6 (3-multiplication "
                               "scheme), i.e. %.2f TFLOP/s of executed DMMA on 48 x 48 tiles" % (0.75 * flops_v / (v_ms * 1e-3) / 1e12))

@@ -237,6 +237,11 @@ int msd_get_phase_ms(msd_ctx* ctx, float* ms, int n);
  *       kernel does not cover.  Results are the same.
  *   MSD_OPT_NO_3M (0 / 1; default 0): TEST HOOK.  1 computes the V contractions with the four-multiplication real form of the
  *       complex product (k_gemm_tn) instead of the three-multiplication kernel (k_vgemm3m).  Same results to rounding.
+ *   MSD_OPT_3M_MAX_COND (value >= 0; default 300): ACCURACY KNOB.  The V contractions of the energy calls use the
+ *       3-multiplication complex product for the walkers whose reference block O0 = psi[occ_ref, :] has
+ *       ||O0||_F ||O0^-1||_F <= value and the 4-multiplication product for the others (chosen per walker on the device; the
+ *       3-multiplication form is 20 % faster but loses 4-15 x more digits on ill-conditioned walkers: DESIGN.md section 7).
+ *       0 = the 4-multiplication product for every walker (same as MSD_OPT_NO_3M = 1); a huge value = always 3 multiplications.
  *   MSD_OPT_COOP_MIN_ELEMS (0..200; default 50 for the energy calls, 72 for overlap / force bias): TUNING KNOB / TEST HOOK.  Determinant buckets with an
  *       excitation level above 4 in either spin and ka^2 + kb^2 above this value run the warp-cooperative kernel (one
  *       determinant x 8 walkers per warp, 4 helper lanes per walker); the others keep one determinant per thread.  Same
@@ -245,6 +250,7 @@ int msd_get_phase_ms(msd_ctx* ctx, float* ms, int n);
 #define MSD_OPT_NO_FUSED_S7 2
 #define MSD_OPT_NO_3M 3
 #define MSD_OPT_COOP_MIN_ELEMS 4
+#define MSD_OPT_3M_MAX_COND 5
 int msd_set_option(msd_ctx* ctx, int option, int64_t value);
 
 void msd_destroy(msd_ctx* ctx);

@@ -31,6 +31,7 @@ MSD_OPT_NO_SMEM_TILES = 1
 MSD_OPT_NO_FUSED_S7 = 2
 MSD_OPT_NO_3M = 3
 MSD_OPT_COOP_MIN_ELEMS = 4
+MSD_OPT_3M_MAX_COND = 5
 
 
 class MSDError(RuntimeError):

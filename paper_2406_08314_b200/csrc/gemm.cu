@@ -27,6 +27,7 @@ k_gemm_tn(GemmArgs g)
     constexpr int BROWS = BX ? BN / 2 : BN;                    // expand mode stages BN/2 complex rows
     double* Bs = smem_gemm + STAGES * BM * LDS_;               // [STAGES][BROWS][LDS_]
     const int z = blockIdx.z / g.ksplit, ks = blockIdx.z - z * g.ksplit;
+    if (g.sel) { const bool hi = !(g.sel[2 * z] <= g.sel_thr) || !(g.sel[2 * z + 1] <= g.sel_thr); if (hi != (g.sel_hi != 0)) return; }
     if (g.symmetric && (int)(blockIdx.x * BN + BN) / 2 - 1 < (int)(blockIdx.y * BM)) return;   // strictly lower tile
     const double* A = g.A + (int64_t)z * g.strideA;
     const double* B = g.B + (int64_t)z * g.strideB;
@@ -218,6 +219,7 @@ __global__ void __launch_bounds__(128, 3) k_vgemm3m(GemmArgs g)
     double* As = smem_v3;                                     // [STAGES][48][LD]
     double* Bs = smem_v3 + V3_STAGES * V3_BM * V3_LD;         // [STAGES][48][LD]
     const int z = blockIdx.z;
+    if (g.sel) { const bool hi = !(g.sel[2 * z] <= g.sel_thr) || !(g.sel[2 * z + 1] <= g.sel_thr); if (hi != (g.sel_hi != 0)) return; }
     const int bx = blockIdx.x, by = blockIdx.y;
     if (g.symmetric && bx < by) return;                       // strictly lower tile (square complex tiles)
     const int Nc = g.N / 2, ngam = g.K / 2;

@@ -597,6 +597,7 @@ extern "C" int msd_set_option(msd_ctx* c, int option, int64_t value)
     if (!c) return MSD_EINVAL;
     if (option == MSD_OPT_NO_SMEM_TILES && value >= 0 && value <= 2) { c->no_smem_tiles = (int)value; return MSD_OK; }
     if (option == MSD_OPT_NO_3M && (value == 0 || value == 1)) { c->no_3m = value != 0; return MSD_OK; }
+    if (option == MSD_OPT_3M_MAX_COND && value >= 0) { c->v3m_max_cond = (double)value; return MSD_OK; }
     if (option == MSD_OPT_COOP_MIN_ELEMS && value >= 0 && value <= 200) { c->coop_min_elems = c->coop_min_elems_fb = (int)value; return MSD_OK; }
     if (option == MSD_OPT_NO_FUSED_S7 && (value == 0 || value == 1)) {
         c->no_fused = value != 0;
@@ -701,6 +702,7 @@ static size_t carve(const msd_ctx* c, Workspace& ws, char* base, int64_t wc, int
         ws.g[s] = k.take<cplx>((size_t)nt * c->sp[s].P * MSD_WT);
     }
     ws.det0 = k.take<cplx>((size_t)wc * 2);
+    ws.kappa2 = (level == 3) ? k.take<double>((size_t)wc * 2) : nullptr;
     if (level == 2 || level == 4) {
         for (int s = 0; s < 2; s++) ws.Gp[s] = k.take<double>((size_t)wc * 2 * c->sp[s].n_r * ldN);
     }
@@ -934,7 +936,15 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
                 a.cs_m = (int64_t)B_.P * MSD_WT; a.cs_j = MSD_WT;
                 a.accumulate = 0;
                 a.symmetric = (pr > 0) ? 1 : 0;     // V^{ss}[x][y] = V^{ss}[y][x]
-                cudaError_t ge = c->no_3m ? launch_gemm_tn(c, a, fv_.stream(pr)) : launch_vgemm3m(c, a, fv_.stream(pr));
+                // 3-multiplication kernel for the well-conditioned walkers, 4-multiplication kernel for the others (both are
+                // launched over the whole batch and skip the walkers of the other kind on the device: no host round trip)
+                cudaError_t ge = cudaSuccess;
+                if (c->no_3m || c->v3m_max_cond <= 0.0) ge = launch_gemm_tn(c, a, fv_.stream(pr));
+                else {
+                    a.sel = ws.kappa2; a.sel_thr = c->v3m_max_cond * c->v3m_max_cond; a.sel_hi = 0;
+                    ge = launch_vgemm3m(c, a, fv_.stream(pr));
+                    if (ge == cudaSuccess) { a.sel_hi = 1; c->launches++; ge = launch_gemm_tn(c, a, fv_.stream(pr)); }
+                }
                 if (ge != cudaSuccess) { fv_.join(); CK(ge); }
                 c->launches++;
             }

@@ -133,6 +133,7 @@ struct Workspace {
     cplx* theta[2] = {nullptr, nullptr};      // [wc][N][n]
     double* thetaT[2] = {nullptr, nullptr};   // [wc][n][2][N]  rows (w,i,c), K = N contiguous
     cplx* det0 = nullptr;                     // [wc][2]
+    double* kappa2 = nullptr;                 // [wc][2]  (||O0||_F ||O0^-1||_F)^2 per walker and spin (energy level only)
     cplx* g[2] = {nullptr, nullptr};          // [nt][P][WT]
     double* C[2] = {nullptr, nullptr};        // [nt][P][2][WT] planar re/im (zeroed every call)
     cplx* Wacc = nullptr;                     // [wc]             (zeroed)
@@ -206,6 +207,8 @@ struct msd_ctx {
     int coop_min_elems = 50;                  // MSD_OPT_COOP_MIN_ELEMS: groups with ka^2+kb^2 above this run k_dets_coop, the rest k_dets_gen
     int coop_min_elems_fb = 72;               //   the same for the overlap / force-bias modes (measured crossovers: profiles/r02_sweep.md)
     bool noalloc_ready = false;               // msd_noalloc_setup ran on this context (msd_api.cu, no-allocation overlap call)
+    double v3m_max_cond = 300.0;              // MSD_OPT_3M_MAX_COND: walkers whose reference block has ||O0||_F ||O0^-1||_F above this take the
+                                              //   4-multiplication V contraction (accuracy: DESIGN.md section 7)
     bool no_3m = false;                       // MSD_OPT_NO_3M: V contractions by the 4-multiplication real form (test hook)
     bool no_fused = false;                    // MSD_OPT_NO_FUSED_S7: take the Lambda GEMM + dense kernel pair (test hook)
     bool need_lam = true;                     // the workspace holds the Lambda buffer (two-kernel S7 path)
@@ -310,6 +313,9 @@ struct GemmArgs {
     int ksplit = 1;             // grid.z = batch * ksplit; slice z % ksplit covers a BK-aligned K range (accumulate == 2)
     int bexpand = 0;            // 1: B holds N/2 COMPLEX rows (re,im interleaved along K); the kernel reads them as the real
                                 //    rows (b_r, -b_i), (b_i, b_r) of a complex product, so that form is never written out
+    // per-batch selection (V contractions): run batch z only if (max(sel[2z], sel[2z+1]) > sel_thr) == (sel_hi != 0);
+    // a NaN counts as above the threshold
+    const double* sel = nullptr; double sel_thr = 0.0; int sel_hi = 0;
     int symmetric = 0;          // 1: C is complex symmetric (M == N/2, A and B describe the same rows): only tiles that
                                 //    touch the upper triangle are computed, element (m, j >= m) is also written to (j, m)
 };

@@ -148,7 +148,9 @@ def test_parity_full_size_against_stored_oracle_values(torch_cuda, name):
     """BASELINE configs[3] (the bench workload, same launch configuration) and configs[2] against oracle values
     stored by tests/golden/make_golden.py (which calls only oracle/): the brute-force oracle needs ~10 minutes per
     walker at the Fe2S2 size.  fe2s2 (SURVEY.md 8(d) plan): overlap of all 100 walkers, force bias (every gamma) of
-    walkers 0..15, energy of walkers 0, 7 | 8 (last lane of tile 0, first lane of tile 1), 57, 99."""
+    walkers 0..15, energy of walkers 0, 7 | 8 (last lane of tile 0, first lane of tile 1), 57, 99 and 34, the walker with
+    the worst-conditioned reference block of the batch (cond 708; cu2o2: walkers 16 and 151, cond 444 and 919), which the
+    V contraction routes to the 4-multiplication kernel."""
     gold = json.load(open(os.path.join(GOLDEN, "%s_seed0.json" % name)))
     x = mi.generate(name)
     assert gold["input_sha256"] == x.sha256()
@@ -163,7 +165,9 @@ def test_parity_full_size_against_stored_oracle_values(torch_cuda, name):
     trial.close()
     if name == "fe2s2":
         assert len(gold["ovlp_all"]) == x.n_w and len(gold["fb_walkers"]) >= 16
-        assert {0, 7, 8, 57, 99} <= set(gold["walkers"])
+        assert {0, 7, 8, 34, 57, 99} <= set(gold["walkers"])
+    else:
+        assert {16, 151} <= set(gold["walkers"])
     _assert_against_golden(gold, ov, fb, E)
 
 
@@ -579,10 +583,12 @@ def test_alternative_dense_paths(torch_cuda, name, kw, ws):
     ref = o2.run(x, walkers=ws, return_G=False)
     sel = np.arange(x.n_w) if ws is None else np.asarray(ws)
     res = {}
-    for opts in ((), (msd.MSD_OPT_NO_FUSED_S7,), (msd.MSD_OPT_NO_3M,), (msd.MSD_OPT_NO_FUSED_S7, msd.MSD_OPT_NO_3M)):
+    pure3m = ((msd.MSD_OPT_3M_MAX_COND, 10 ** 9),)      # the 3-multiplication kernel for every walker, whatever its conditioning
+    for opts in ((), (msd.MSD_OPT_NO_FUSED_S7,), (msd.MSD_OPT_NO_3M,), (msd.MSD_OPT_NO_FUSED_S7, msd.MSD_OPT_NO_3M), pure3m,
+                 ((msd.MSD_OPT_3M_MAX_COND, 0),)):
         trial = msd.setup_from_inputs(x)
         for o in opts:
-            trial.set_option(o, 1)
+            trial.set_option(*(o if isinstance(o, tuple) else (o, 1)))
         E = trial.local_energy(pa, pb).cpu().numpy()
         fused = trial.force_bias_energy(pa, pb).cpu().numpy()
         trial.close()
@@ -590,7 +596,11 @@ def test_alternative_dense_paths(torch_cuda, name, kw, ws):
         assert np.abs(fused[sel, x.n_chol:] - ref["E"]).max() <= TOL_E, opts
         res[opts] = E
     for opts, E in res.items():
-        assert np.abs(E - res[()]).max() <= TOL_E
+        # every walker of the batch, oracle-checked or not.  The pure 3-multiplication path is left out: on walkers with an
+        # ill-conditioned reference block it is 4-15 x less accurate than the others, which is why
+        # the default routes those walkers to the 4-multiplication kernel.
+        if opts != pure3m:
+            assert np.abs(E - res[()]).max() <= TOL_E, opts
 
 
 @pytest.mark.parametrize("kw,ws", [(dict(n_det=3000, max_level=7, n_w=21), [0, 8, 20]),
