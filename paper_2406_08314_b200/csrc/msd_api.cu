@@ -883,10 +883,15 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
                 CK(launch_green_rows(c, nw, ws, nullptr, st));
                 cplx* fb = out + w0 * (int64_t)ng;
                 CK(cudaMemsetAsync(fb, 0, sizeof(cplx) * (size_t)nw * ng, st));
-                for (int s = 0; s < 2; s++) {
-                    const auto& sp = c->sp[s];
-                    if (sp.n_r == 0) continue;
-                    CK(launch_fb_gemm(c, s, nw, ws, fb, st));
+                {   // the two spins' contractions only meet in the RED accumulators of fb: side by side on two streams
+                    Fork ff(c, st);
+                    for (int s = 0; s < 2; s++) {
+                        const auto& sp = c->sp[s];
+                        if (sp.n_r == 0) continue;
+                        cudaError_t ge = launch_fb_gemm(c, s, nw, ws, fb, ff.stream(s));
+                        if (ge != cudaSuccess) { ff.join(); CK(ge); }
+                    }
+                    CK(ff.join());
                 }
                 mark(c, 3, st);
                 CK(launch_finish_flags(c, nw, ws, fb, ng, fl, st));

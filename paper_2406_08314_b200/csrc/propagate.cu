@@ -86,20 +86,118 @@ template <bool CPLX_LEFT>
 __device__ __forceinline__ void prop_matmul(int N, int n, int ldl, const void* left, const cplx* __restrict__ src, cplx* __restrict__ dst,
                                             double scale)
 {
-    for (int e = threadIdx.x; e < N * n; e += blockDim.x) {
+    // four outputs per thread at a time -- column i of rows p, p + G, p + 2G, p + 3G (G = ceil(N / 4)): four independent FMA
+    // chains (one chain of N complex FMAs per output is pure latency) that share every shared-memory read of src;
+    // consecutive threads keep consecutive i (conflict-free shared memory, the row loads broadcast within a warp)
+    const int G = (N + 3) >> 2;
+    for (int e = threadIdx.x; e < G * n; e += blockDim.x) {
         const int p = e / n, i = e - p * n;
-        cplx acc = cmake(0.0, 0.0);
+        int pr[4];
+        cplx acc[4];
+#pragma unroll
+        for (int u = 0; u < 4; u++) { pr[u] = min(p + u * G, N - 1); acc[u] = cmake(0.0, 0.0); }     // clamped duplicates are not stored
         if (CPLX_LEFT) {
-            const cplx* row = reinterpret_cast<const cplx*>(left) + (int64_t)p * N;
-#pragma unroll 4
-            for (int q = 0; q < N; q++) acc = cfma(__ldg(row + q), src[q * n + i], acc);
+            const cplx* L_ = reinterpret_cast<const cplx*>(left);
+#pragma unroll 2
+            for (int q = 0; q < N; q++) {
+                const cplx sv = src[q * n + i];
+#pragma unroll
+                for (int u = 0; u < 4; u++) acc[u] = cfma(__ldg(L_ + (int64_t)pr[u] * N + q), sv, acc[u]);
+            }
         } else {
-            const double* row = reinterpret_cast<const double*>(left) + (int64_t)p * ldl;
-#pragma unroll 4
-            for (int q = 0; q < N; q++) { const double a = __ldg(row + q); const cplx s = src[q * n + i]; acc.x = fma(a, s.x, acc.x); acc.y = fma(a, s.y, acc.y); }
+            const double* L_ = reinterpret_cast<const double*>(left);
+#pragma unroll 2
+            for (int q = 0; q < N; q++) {
+                const cplx sv = src[q * n + i];
+#pragma unroll
+                for (int u = 0; u < 4; u++) {
+                    const double a = __ldg(L_ + (int64_t)pr[u] * ldl + q);
+                    acc[u].x = fma(a, sv.x, acc[u].x); acc[u].y = fma(a, sv.y, acc[u].y);
+                }
+            }
         }
-        dst[e] = cscale(scale, acc);
+#pragma unroll
+        for (int u = 0; u < 4; u++)
+            if (p + u * G < N) dst[(p + u * G) * n + i] = cscale(scale, acc[u]);
     }
+}
+
+// The same product on the FP64 tensor cores (DMMA m8n8k4) for n <= 8 NT columns: a warp owns two 8-row tiles of the result
+// and all NT column tiles; per k-step of 4 it loads its two left-operand fragments from global memory (L1), the NT
+// right-operand fragments from shared memory, and issues 4 (complex left) or 2 (real left) DMMAs per tile:
+//   Cr += Ar Xr - Ai Xi,  Ci += Ar Xi + Ai Xr.
+template <bool CPLX_LEFT, int NT>
+__device__ __forceinline__ void prop_matmul_mma(int N, int n, int ldl, const void* left, const cplx* __restrict__ src,
+                                                cplx* __restrict__ dst, double scale)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    const int g = lane >> 2, t = lane & 3;
+    const int MT = (N + 7) >> 3;
+    for (int mt0 = wid; mt0 < MT; mt0 += 2 * nwarp) {
+        const int mt1 = mt0 + nwarp;
+        const bool two = mt1 < MT;
+        const int p0 = min(mt0 * 8 + g, N - 1), p1 = min(mt1 * 8 + g, N - 1);      // clamped rows are computed and not stored
+        double cr[2][NT][2], ci[2][NT][2];
+#pragma unroll
+        for (int m = 0; m < 2; m++)
+#pragma unroll
+            for (int nt = 0; nt < NT; nt++) { cr[m][nt][0] = cr[m][nt][1] = 0.0; ci[m][nt][0] = ci[m][nt][1] = 0.0; }
+        for (int q0 = 0; q0 < N; q0 += 4) {
+            const int q = q0 + t;
+            const bool qok = q < N;
+            double ar[2], ai[2];
+            if (CPLX_LEFT) {
+                const cplx* L_ = reinterpret_cast<const cplx*>(left);
+                const cplx a0 = qok ? __ldg(L_ + (int64_t)p0 * N + q) : cmake(0.0, 0.0);
+                const cplx a1 = (qok && two) ? __ldg(L_ + (int64_t)p1 * N + q) : cmake(0.0, 0.0);
+                ar[0] = a0.x; ai[0] = a0.y; ar[1] = a1.x; ai[1] = a1.y;
+            } else {
+                const double* L_ = reinterpret_cast<const double*>(left);
+                ar[0] = qok ? __ldg(L_ + (int64_t)p0 * ldl + q) : 0.0;
+                ar[1] = (qok && two) ? __ldg(L_ + (int64_t)p1 * ldl + q) : 0.0;
+                ai[0] = ai[1] = 0.0;
+            }
+#pragma unroll
+            for (int nt = 0; nt < NT; nt++) {
+                const int i = nt * 8 + g;
+                const cplx x = (qok && i < n) ? src[q * n + i] : cmake(0.0, 0.0);
+#pragma unroll
+                for (int m = 0; m < 2; m++) {
+                    if (m == 1 && !two) continue;        // warp-uniform
+                    dmma884(cr[m][nt][0], cr[m][nt][1], ar[m], x.x);
+                    dmma884(ci[m][nt][0], ci[m][nt][1], ar[m], x.y);
+                    if (CPLX_LEFT) {
+                        dmma884(cr[m][nt][0], cr[m][nt][1], -ai[m], x.y);
+                        dmma884(ci[m][nt][0], ci[m][nt][1], ai[m], x.x);
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int m = 0; m < 2; m++) {
+            const int row = (m ? mt1 : mt0) * 8 + g;
+            if ((m == 1 && !two) || row >= N) continue;
+#pragma unroll
+            for (int nt = 0; nt < NT; nt++)
+#pragma unroll
+                for (int k = 0; k < 2; k++) {
+                    const int col = nt * 8 + 2 * t + k;
+                    if (col < n) dst[row * n + col] = cmake(scale * cr[m][nt][k], scale * ci[m][nt][k]);
+                }
+        }
+    }
+}
+
+// dispatch: tensor-core form for n <= 32, the scalar form beyond
+template <bool CPLX_LEFT>
+__device__ __forceinline__ void prop_product(int N, int n, int ldl, const void* left, const cplx* __restrict__ src,
+                                             cplx* __restrict__ dst, double scale)
+{
+    if (n <= 8) prop_matmul_mma<CPLX_LEFT, 1>(N, n, ldl, left, src, dst, scale);
+    else if (n <= 16) prop_matmul_mma<CPLX_LEFT, 2>(N, n, ldl, left, src, dst, scale);
+    else if (n <= 24) prop_matmul_mma<CPLX_LEFT, 3>(N, n, ldl, left, src, dst, scale);
+    else if (n <= 32) prop_matmul_mma<CPLX_LEFT, 4>(N, n, ldl, left, src, dst, scale);
+    else prop_matmul<CPLX_LEFT>(N, n, ldl, left, src, dst, scale);
 }
 
 __global__ void __launch_bounds__(256)
@@ -118,18 +216,18 @@ k_prop_orbitals(int N, int ldN, int na, int nb, int n_taylor, const double* __re
     cplx* sum = t1 + N * n;                              // partial sum of the series
     for (int e = threadIdx.x; e < N * n; e += blockDim.x) t1[e] = phi[e];
     __syncthreads();
-    prop_matmul<false>(N, n, ldN, E, t1, t0, 1.0);       // t0 = E psi
+    prop_product<false>(N, n, ldN, E, t1, t0, 1.0);      // t0 = E psi
     __syncthreads();
     for (int e = threadIdx.x; e < N * n; e += blockDim.x) sum[e] = t0[e];
     __syncthreads();
     for (int k = 1; k <= n_taylor; k++) {
-        prop_matmul<true>(N, n, 0, A, t0, t1, 1.0 / (double)k);       // term_k = A term_{k-1} / k
+        prop_product<true>(N, n, 0, A, t0, t1, 1.0 / (double)k);      // term_k = A term_{k-1} / k
         __syncthreads();
         for (int e = threadIdx.x; e < N * n; e += blockDim.x) { sum[e] = cadd(sum[e], t1[e]); }
         cplx* tmp = t0; t0 = t1; t1 = tmp;
         __syncthreads();
     }
-    prop_matmul<false>(N, n, ldN, E, sum, t1, 1.0);      // psi' = E sum
+    prop_product<false>(N, n, ldN, E, sum, t1, 1.0);     // psi' = E sum
     __syncthreads();
     for (int e = threadIdx.x; e < N * n; e += blockDim.x) phi[e] = t1[e];
 }
