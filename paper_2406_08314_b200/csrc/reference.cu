@@ -1,5 +1,5 @@
 // S1 "reference" (Wick step W1): per (walker, spin)
-//   O0 = psi[occ_ref,:]  (Psi_T^+ phi of PAPER.md Eq. 13 for the reference determinant), pivoted LU,
+//   O0 = psi[occ_ref,:]  (Psi_T^+ phi of PAPER.md Eq. 13 for the reference determinant), row-pivoted Gauss-Jordan inverse,
 //   det0 = det O0 (Eq. 13), Theta = psi O0^-1 (N x n), so that the reference Green's function of Eq. 14
 //   is G0[occ_ref[l], q] = Theta[q, l]; active slice g[h, p] = Theta[p, pos(h)].
 // One CTA per (walker, spin).  complex128 throughout.
