@@ -702,7 +702,11 @@ def test_binding_validates_outputs_and_limits(torch_cuda):
 # one phaseless-AFQMC propagation step (Eq. 5, 7-12) against oracle/propagate.py
 # ----------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("name,kw,ws,n_taylor", [("tiny", {}, None, 6), ("open-shell", {}, None, 4), ("small", {}, None, 6),
-                                                 ("cu2o2", {}, [0, 7, 8, 100, 199], 6)])
+                                                 ("cu2o2", {}, [0, 7, 8, 100, 199], 6),
+                                                 # 34 + 33 electrons: more than 32 columns per walker, the orbital update's
+                                                 # scalar products instead of its tensor-core form (propagate.cu prop_product)
+                                                 ("small", dict(N=72, n_alpha=34, n_beta=33, A=12, n_chol=30, n_det=40, n_w=5,
+                                                                max_level=3), None, 6)])
 def test_propagation_step_against_oracle(torch_cuda, name, kw, ws, n_taylor):
     """msd_propagate: walkers after B(x - xbar), overlap ratio S (rel 1e-10), phase theta (abs 1e-10), importance function,
     phaseless weight update -- element by element against the numpy oracle on the same seeded fields; full batch on the
