@@ -192,11 +192,14 @@ def test_parity_sweep_end_points_against_stored_oracle_values(torch_cuda, n_det,
     _assert_against_golden(gold, ov, fb, E)
 
 
-def test_parity_many_electrons(torch_cuda):
+@pytest.mark.parametrize("kw", [dict(N=72, n_alpha=34, n_beta=33, A=12, n_chol=30, n_det=200, n_w=11, max_level=4),
+                                dict(N=160, n_alpha=30, n_beta=29, A=12, n_chol=20, n_det=120, n_w=9, max_level=3)])
+def test_parity_many_electrons(torch_cuda, kw):
     """34 + 33 electrons in 72 orbitals (more electrons per spin than any BASELINE config: the reference kernel's
     Gauss-Jordan beyond one warp's width of columns, the S7 path for shapes the fused kernel does not instantiate), odd
-    and unequal electron counts; every call on every walker against O2."""
-    x = mi.generate("small", N=72, n_alpha=34, n_beta=33, A=12, n_chol=30, n_det=200, n_w=11, max_level=4)
+    and unequal electron counts; and 30 + 29 electrons in 160 orbitals, a walker block too large for the reference kernel
+    to stage in shared memory (it reads psi from global memory).  Every call on every walker against O2."""
+    x = mi.generate("small", **kw)
     got = gpu_all(torch_cuda, x)
     assert (got["flags"] == 0).all()
     assert_parity(got, o2.run(x))
