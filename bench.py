@@ -340,7 +340,8 @@ def main():
     ov = torch.empty(inp.n_w, dtype=torch.complex128, device=dev)
     calls = {"msd_overlap": lambda: trial.overlap(d_a, d_b, out=ov),
              "msd_force_bias": lambda: trial.force_bias(d_a, d_b, out=fb),
-             "msd_local_energy": lambda: trial.local_energy(d_a, d_b, out=en)}
+             "msd_local_energy": lambda: trial.local_energy(d_a, d_b, out=en),
+             "msd_force_bias_overlap": lambda: trial.force_bias_overlap(d_a, d_b, out=fb, out_ovlp=ov)}
     per_call = {}
     for cname, fn in calls.items():
         fn()
@@ -360,6 +361,12 @@ def main():
                  "value": total_units(inp.n_w, inp.n_det, 25, units_world) / ((25.0 * (t_fb + t_ov) + t_e) * 1e-3),
                  "unit": "walker*det*step/s", "block_ms": 25.0 * (t_fb + t_ov) + t_e,
                  "energy_share_of_block": t_e / (25.0 * (t_fb + t_ov) + t_e)}
+    # the same block when every step takes its force bias and overlap from ONE determinant pass (msd_force_bias_overlap)
+    t_fbo = per_call["msd_force_bias_overlap"]["ms"]
+    block_mix["one_pass"] = {"definition": "N_w N_d 25 / (25 t_fb+ovlp + t_E) with msd_force_bias_overlap (force bias and overlap of "
+                                           "the step's walkers from one determinant pass)",
+                             "value": total_units(inp.n_w, inp.n_det, 25, units_world) / ((25.0 * t_fbo + t_e) * 1e-3),
+                             "unit": "walker*det*step/s", "block_ms": 25.0 * t_fbo + t_e}
 
     # ---- one propagation step around the path (force bias, B(x - xbar), new overlap, Eq. 8-12) ----
     trial.propagator_setup(0.005, 6, inp.h1, inp.L)

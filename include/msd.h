@@ -127,6 +127,12 @@ int msd_overlap(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
 int msd_force_bias(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
                    void* fb, int32_t* flags, void* stream);
 
+/* msd_force_bias with the overlaps of the same walkers from the same determinant pass (the pass forms W = sum_I c_I R_I
+ * and det O0 anyway; a propagation step needs both: PAPER.md Eq. 7 and Eq. 8): fb as in msd_force_bias, ovlp DEVICE [n_w]
+ * as in msd_overlap.  Saves the separate msd_overlap call (0.5 ms of 2.7 ms at the Fe2S2-shaped config). */
+int msd_force_bias_overlap(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
+                           void* fb, void* ovlp, int32_t* flags, void* stream);
+
 /* e DEVICE [n_w][3] complex128 = (E, E1, E2): E = e0 + E1 + E2, E1 one-body, E2 two-body.  S1-S9.
  * Accuracy: everything is expressed through Theta = psi (psi[occ_ref,:])^-1 (Wick's theorem around the reference
  * determinant), so the FP64 error of the energies grows with the conditioning of the walker's reference block O0 =

@@ -25,7 +25,7 @@ EXPORTS = ["msd_setup", "msd_setup_sharded", "msd_set_allreduce", "msd_setup_fro
            "msd_propagator_setup", "msd_propagate",
            "msd_get_info", "msd_get_packed", "msd_set_workspace_limit", "msd_set_option", "msd_launch_count",
            "msd_set_profiling", "msd_get_phase_ms", "msd_destroy", "msd_last_error",
-           "msd_noalloc_setup", "msd_overlap_noalloc"]
+           "msd_noalloc_setup", "msd_overlap_noalloc", "msd_force_bias_overlap"]
 MSD_NOALLOC_SCRATCH_BYTES = 4 * 1024 * 1024
 MSD_OPT_NO_SMEM_TILES = 1
 MSD_OPT_NO_FUSED_S7 = 2
@@ -68,6 +68,8 @@ def load_library() -> C.CDLL:
         f = getattr(lib, name)
         f.restype = i32
         f.argtypes = [vp, i64, vp, vp, vp, vp, vp]
+    lib.msd_force_bias_overlap.restype = i32
+    lib.msd_force_bias_overlap.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp]
     lib.msd_noalloc_setup.restype = i32
     lib.msd_noalloc_setup.argtypes = [vp, vp]
     lib.msd_propagator_setup.restype = i32
@@ -194,6 +196,24 @@ class MSDTrial:
         nw = self._walkers(phi_a, phi_b)
         out = torch.empty((nw, self.n_chol), dtype=torch.complex128, device=phi_a.device) if out is None else out
         return self._call(load_library().msd_force_bias, phi_a, phi_b, out, flags, stream)
+
+    def force_bias_overlap(self, phi_a, phi_b, out=None, out_ovlp=None, flags=None, stream=None):
+        """msd_force_bias_overlap: (fb [n_w][n_chol], ovlp [n_w]) of the same walkers from one determinant pass."""
+        import torch
+        nw = self._walkers(phi_a, phi_b)
+        dev = phi_a.device
+        out = torch.empty((nw, self.n_chol), dtype=torch.complex128, device=dev) if out is None else out
+        out_ovlp = torch.empty(nw, dtype=torch.complex128, device=dev) if out_ovlp is None else out_ovlp
+        if not (isinstance(out_ovlp, torch.Tensor) and out_ovlp.is_cuda and out_ovlp.device == dev
+                and out_ovlp.dtype == torch.complex128 and out_ovlp.is_contiguous() and tuple(out_ovlp.shape) == (nw,)):
+            raise ValueError("out_ovlp must be a contiguous CUDA complex128 tensor of shape (%d,) on the walkers' device" % nw)
+        lib = load_library()
+
+        def fn(h, n, a, b, o, f, st):
+            return lib.msd_force_bias_overlap(h, n, a, b, o, out_ovlp.data_ptr(), f, st)
+        fn.__name__ = "msd_force_bias"
+        self._call(fn, phi_a, phi_b, out, flags, stream)
+        return out, out_ovlp
 
     def local_energy(self, phi_a, phi_b, out=None, flags=None, stream=None):
         import torch

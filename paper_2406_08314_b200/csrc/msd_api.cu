@@ -894,6 +894,8 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
                     CK(ff.join());
                 }
                 mark(c, 3, st);
+                // msd_force_bias_overlap: the pass has W and det0 of every walker anyway (no second determinant pass)
+                if (c->fb_ovlp) CK(launch_finish_overlap(c, nw, ws, c->fb_ovlp + w0, nullptr, st));
                 CK(launch_finish_flags(c, nw, ws, fb, ng, fl, st));
             }
             mark(c, 4, st); mark(c, 5, st);
@@ -1012,6 +1014,17 @@ extern "C" int msd_overlap(msd_ctx* c, int64_t n_w, const void* phi_a, const voi
 extern "C" int msd_force_bias(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* fb, int32_t* flags,
                               void* stream)
 { return hot_call(c, CALL_FB, n_w, phi_a, phi_b, fb, flags, stream); }
+
+extern "C" int msd_force_bias_overlap(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* fb, void* ovlp,
+                                      int32_t* flags, void* stream)
+{
+    if (!c) return MSD_EINVAL;
+    if (n_w > 0 && !ovlp) { c->err = "bad argument"; return MSD_EINVAL; }
+    c->fb_ovlp = (cplx*)ovlp;
+    const int rc = hot_call(c, CALL_FB, n_w, phi_a, phi_b, fb, flags, stream);
+    c->fb_ovlp = nullptr;
+    return rc;
+}
 
 extern "C" int msd_local_energy(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* e, int32_t* flags,
                                 void* stream)

@@ -202,6 +202,7 @@ struct msd_ctx {
     double* d_E = nullptr;                    // 3 x [ld][ld]: exp(-dt h'/2), the scaled matrix, scratch
     double prop_dt = 0.0; int prop_taylor = 0;
     const double* prop_x = nullptr; double* prop_w = nullptr;      // arguments of the running msd_propagate call
+    cplx* fb_ovlp = nullptr;                  // msd_force_bias_overlap: where the running force-bias call also leaves the overlaps
     int shard_rank = 0, shard_world = 1;      // determinant sharding (msd_setup_sharded)
     void (*allreduce)(void*, void*, int64_t, void*) = nullptr; void* allreduce_user = nullptr;     // msd_set_allreduce
     int coop_min_elems = 50;                  // MSD_OPT_COOP_MIN_ELEMS: groups with ka^2+kb^2 above this run k_dets_coop, the rest k_dets_gen

@@ -582,6 +582,37 @@ def test_paths_for_windows_too_wide_for_shared_memory_tiles(torch_cuda, level):
         assert_parity(dict(fb=fused[:, :x.n_chol], E=fused[:, x.n_chol:]), ref, walkers=sel, what=("fb", "E"))
 
 
+@pytest.mark.parametrize("name,kw", [("small", {}), ("open-shell", {}), ("sweep", dict(n_det=3000, max_level=7, n_w=21))])
+def test_force_bias_with_overlap_from_one_pass(torch_cuda, name, kw):
+    """msd_force_bias_overlap: force bias and overlap of the same walkers from one determinant pass against the oracle and
+    against the two separate calls; ragged batch, a chunked workspace (small), flags."""
+    torch = torch_cuda
+    msd = _msd()
+    x = mi.generate(name, **kw)
+    trial = msd.setup_from_inputs(x)
+    pa = torch.tensor(x.phi_a, device="cuda")
+    pb = torch.tensor(x.phi_b, device="cuda")
+    fl = torch.full((x.n_w,), -1, dtype=torch.int32, device="cuda")
+    fb, ov = trial.force_bias_overlap(pa, pb, flags=fl)
+    fb, ov = fb.cpu().numpy(), ov.cpu().numpy()
+    assert (fl.cpu().numpy() == 0).all()
+    ws = list(range(min(x.n_w, 6)))
+    ref = o2.run(x, walkers=ws, want=("ovlp", "greens"), return_G=False)
+    assert_parity(dict(ovlp=ov, fb=fb), ref, walkers=ws, what=("ovlp", "fb"))
+    ov2 = trial.overlap(pa, pb).cpu().numpy()
+    fb2 = trial.force_bias(pa, pb).cpu().numpy()
+    assert (np.abs(ov - ov2) / np.abs(ov2)).max() <= TOL_REL
+    assert (np.abs(fb - fb2).max(axis=1) / np.abs(fb2).max(axis=1)).max() <= TOL_REL
+    if name == "small":
+        trial.set_workspace_limit(600 * 1024)       # one walker tile needs 0.41 MB: several chunks, the overlaps land at their offsets
+        fb3, ov3 = trial.force_bias_overlap(pa, pb)
+        assert (np.abs(ov3.cpu().numpy() - ov2) / np.abs(ov2)).max() <= TOL_REL
+        assert (np.abs(fb3.cpu().numpy() - fb2).max(axis=1) / np.abs(fb2).max(axis=1)).max() <= TOL_REL
+    with pytest.raises(ValueError):
+        trial.force_bias_overlap(pa, pb, out_ovlp=torch.empty(x.n_w + 1, dtype=torch.complex128, device="cuda"))
+    trial.close()
+
+
 @pytest.mark.parametrize("name,kw,ws", [("small", {}, None), ("cu2o2", dict(n_w=24), [0, 7, 8, 23]),
                                         ("sweep", dict(n_det=2000, max_level=5, n_w=16), [0, 15])])
 def test_alternative_dense_paths(torch_cuda, name, kw, ws):
