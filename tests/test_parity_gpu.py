@@ -192,6 +192,30 @@ def test_parity_sweep_end_points_against_stored_oracle_values(torch_cuda, n_det,
     _assert_against_golden(gold, ov, fb, E)
 
 
+@pytest.mark.parametrize("seed", [1, 2, 3, 4])
+@pytest.mark.parametrize("name,kw", [("small", {}), ("sweep", dict(n_det=1500, max_level=7, n_w=19)),
+                                     ("sweep", dict(n_det=800, max_level=10, n_w=9))])
+def test_parity_other_seeds(torch_cuda, name, kw, seed):
+    """Other draws of trial and walkers than the default seed of every other test (the worst reference-block condition
+    numbers of these batches run from 50 to 340): every call, the fused call and the force-bias-with-overlap call, all
+    walkers, against O2."""
+    msd = _msd()
+    torch = torch_cuda
+    x = mi.generate(name, seed=seed, **kw)
+    trial = msd.setup_from_inputs(x)
+    got = gpu_all(torch, x, trial=trial, want_G=False)
+    pa = torch.tensor(x.phi_a, device="cuda")
+    pb = torch.tensor(x.phi_b, device="cuda")
+    fused = trial.force_bias_energy(pa, pb).cpu().numpy()
+    fb2, ov2 = trial.force_bias_overlap(pa, pb)
+    trial.close()
+    ref = o2.run(x, return_G=False)
+    assert (got["flags"] == 0).all()
+    assert_parity(got, ref, what=("ovlp", "fb", "E"))
+    assert_parity(dict(fb=fused[:, :x.n_chol], E=fused[:, x.n_chol:]), ref, what=("fb", "E"))
+    assert_parity(dict(ovlp=ov2.cpu().numpy(), fb=fb2.cpu().numpy()), ref, what=("ovlp", "fb"))
+
+
 @pytest.mark.parametrize("kw", [dict(N=72, n_alpha=34, n_beta=33, A=12, n_chol=30, n_det=200, n_w=11, max_level=4),
                                 dict(N=160, n_alpha=30, n_beta=29, A=12, n_chol=20, n_det=120, n_w=9, max_level=3)])
 def test_parity_many_electrons(torch_cuda, kw):
