@@ -1031,6 +1031,163 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
 }
 
 // ------------------------------------------------------------------------------------------------
+// Level 5 against levels 0..3, overlap and force-bias modes: the whole 5 x 5 Gauss-Jordan inverse in REGISTERS.
+// k_dets_gen keeps one matrix per thread in shared memory and is bound by that traffic (LSU 80 % busy in these groups);
+// here pivoting is a compare-and-swap of whole rows and the column permutation is undone by compare-and-swaps in reverse
+// order, so every index is a compile-time constant and nothing leaves the register file.  A kernel of its own because the
+// 25 complex need a 255-register budget (inside k_dets_gen ptxas puts them in local memory: DESIGN.md section 11).
+// Pivots are the column maxima, as in gauss_jordan_t; exactly singular matrices give R = 0, A = 0 (reading A11).
+// ------------------------------------------------------------------------------------------------
+template <bool WANT_INV>
+__device__ __forceinline__ cplx gj5_reg(cplx (&M)[5][5])
+{
+    constexpr int K = 5;
+    cplx det = cmake(1.0, 0.0);
+    bool sing = false;
+    unsigned swaps = 0u;                       // bit (4 j + i - j - 1): rows j and i were swapped in step j
+#pragma unroll
+    for (int j = 0; j < K; j++) {
+#pragma unroll
+        for (int i = j + 1; i < K; i++) {
+            const bool sw = cabs2(M[i][j]) > cabs2(M[j][j]);
+#pragma unroll
+            for (int c = 0; c < K; c++) {
+                if (!WANT_INV && c < j) continue;
+                const cplx a = M[j][c], b = M[i][c];
+                M[j][c] = sw ? b : a;
+                M[i][c] = sw ? a : b;
+            }
+            if (sw) { det = cneg(det); swaps |= 1u << (4 * j + i - j - 1); }
+        }
+        const cplx pv = M[j][j];
+        if (!(cabs2(pv) > 0.0)) sing = true;
+        det = cmul(det, pv);
+        const cplx r = sing ? cmake(0.0, 0.0) : cinv(pv);
+        if (WANT_INV) M[j][j] = cmake(1.0, 0.0);
+#pragma unroll
+        for (int c = 0; c < K; c++) if (WANT_INV || c > j) M[j][c] = cmul(M[j][c], r);
+#pragma unroll
+        for (int i = 0; i < K; i++) {
+            if (i == j || (!WANT_INV && i < j)) continue;
+            const cplx f = M[i][j];
+            if (WANT_INV) M[i][j] = cmake(0.0, 0.0);
+#pragma unroll
+            for (int c = 0; c < K; c++) if (WANT_INV || c > j) M[i][c] = cfms(f, M[j][c], M[i][c]);
+        }
+    }
+    if (WANT_INV) {
+#pragma unroll
+        for (int j = K - 1; j >= 0; j--)
+#pragma unroll
+            for (int i = K - 1; i > j; i--) {
+                const bool sw = (swaps >> (4 * j + i - j - 1)) & 1u;
+#pragma unroll
+                for (int rr = 0; rr < K; rr++) {
+                    const cplx a = M[rr][j], b = M[rr][i];
+                    M[rr][j] = sw ? b : a;
+                    M[rr][i] = sw ? a : b;
+                }
+            }
+        if (sing) {
+#pragma unroll
+            for (int a = 0; a < K; a++)
+#pragma unroll
+                for (int b = 0; b < K; b++) M[a][b] = cmake(0.0, 0.0);
+        }
+    }
+    return sing ? cmake(0.0, 0.0) : det;
+}
+
+// one bucket (KA, KB) with one spin at level 5 and the other at 0..3
+template <int MODE, int KA, int KB>
+__device__ __forceinline__ void r5_bucket(const DetsParams& p, const WorkItem& it, int slot, int nslots, const cplx* __restrict__ gA,
+                                          const cplx* __restrict__ gB, double* CA, double* CB, cplx& Wl)
+{
+    constexpr int KS = KA == 5 ? KB : KA;               // the small spin's level
+    constexpr int KS1 = KS > 0 ? KS : 1;
+    constexpr bool BIG_A = KA == 5;
+    const cplx* gbig = BIG_A ? gA : gB;
+    const cplx* gsml = BIG_A ? gB : gA;
+    const int nob = BIG_A ? p.no[0] : p.no[1], nos = BIG_A ? p.no[1] : p.no[0];
+    double* Cbig = BIG_A ? CA : CB;
+    double* Csml = BIG_A ? CB : CA;
+    for (int i = slot; i < it.det_count; i += nslots) {
+        const uint32_t* rp = reinterpret_cast<const uint32_t*>(p.tab + it.tab_off + (int64_t)i * it.rs);
+        union { uint32_t w[4]; unsigned char b[16]; } row;        // 2 (KA + KB) <= 16 bytes
+#pragma unroll
+        for (int t = 0; t < 4; t++) row.w[t] = (t < (2 * (KA + KB) + 3) / 4) ? __ldg(rp + t) : 0u;
+        const double cf = __ldg(&p.coef[it.det_begin + i]);
+        const unsigned char* hb = row.b + (BIG_A ? 0 : 2 * KA);
+        const unsigned char* hs = row.b + (BIG_A ? 2 * KA : 0);
+        // small spin first (its adjugate is at most 9 complex)
+        cplx As[KS1][KS1];
+        int xs_h[KS1], xs_p[KS1];
+        cplx Rs = cmake(1.0, 0.0);
+        if (KS > 0) {
+            cplx Ms[KS1][KS1];
+#pragma unroll
+            for (int a = 0; a < KS; a++) { xs_h[a] = (int)hs[a]; xs_p[a] = (int)hs[KS + a] * nos; }
+#pragma unroll
+            for (int a = 0; a < KS; a++)
+#pragma unroll
+                for (int b = 0; b < KS; b++) Ms[a][b] = __ldg(&gsml[(xs_p[b] + xs_h[a]) * MSD_WT]);
+            Rs = Closed<KS>::det_adj(Ms, As);
+        }
+        int hh[5], pp[5];
+#pragma unroll
+        for (int a = 0; a < 5; a++) { hh[a] = (int)hb[a]; pp[a] = (int)hb[5 + a] * nob; }
+        cplx M[5][5];
+#pragma unroll
+        for (int a = 0; a < 5; a++)
+#pragma unroll
+            for (int b = 0; b < 5; b++) M[a][b] = __ldg(&gbig[(pp[b] + hh[a]) * MSD_WT]);
+        const cplx Rb = gj5_reg<MODE == 1>(M);           // M = M^-1 (force-bias mode)
+        const cplx cRb = cscale(cf, Rb), cRs = cscale(cf, Rs);
+        Wl = cfma(cRb, Rs, Wl);
+        if (MODE == 1) {
+            // C^big[x(a,b)] += c Rs A[b][a],  A = Rb M^-1  (entry [b][a] of the inverse belongs to pair (a, b))
+            const cplx sc = cmul(cRs, Rb);
+#pragma unroll
+            for (int a = 0; a < 5; a++)
+#pragma unroll
+                for (int b = 0; b < 5; b++) red_add_planar(Cbig, pp[b] + hh[a], cmul(sc, M[b][a]));
+            if (KS > 0) {
+#pragma unroll
+                for (int a = 0; a < KS; a++)
+#pragma unroll
+                    for (int b = 0; b < KS; b++) red_add_planar(Csml, xs_p[b] + xs_h[a], cmul(cRb, As[b][a]));
+            }
+        }
+    }
+}
+
+#define R5_CASE(KA_, KB_) case KA_ * 8 + KB_: r5_bucket<MODE, KA_, KB_>(p, it, slot, nslots, gA, gB, CA, CB, Wl); break;
+
+template <int MODE>
+__global__ void __launch_bounds__(128, 2) k_dets_r5(DetsParams p, const WorkItem* __restrict__ items, int n_items)
+{
+    const int tile = blockIdx.y;
+    const int j = threadIdx.x & (MSD_WT - 1);
+    const int slot = threadIdx.x / MSD_WT, nslots = blockDim.x / MSD_WT;
+    const cplx* gA = p.g[0] + (int64_t)tile * p.P[0] * MSD_WT + j;
+    const cplx* gB = p.g[1] + (int64_t)tile * p.P[1] * MSD_WT + j;
+    double* CA = p.C[0] + (int64_t)tile * p.P[0] * 2 * MSD_WT + j;
+    double* CB = p.C[1] + (int64_t)tile * p.P[1] * 2 * MSD_WT + j;
+    cplx Wl = cmake(0.0, 0.0);
+    for (int r = 0, ii; (ii = r * (int)gridDim.x + ((r & 1) ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x)),
+                        r * (int)gridDim.x < n_items; r++) {
+        if (ii >= n_items) continue;
+        const WorkItem it = items[ii];
+        switch (it.ka * 8 + it.kb) {
+            R5_CASE(5, 0) R5_CASE(5, 1) R5_CASE(5, 2) R5_CASE(5, 3)
+            R5_CASE(0, 5) R5_CASE(1, 5) R5_CASE(2, 5) R5_CASE(3, 5)
+            default: break;
+        }
+    }
+    flush_walker_sums(p, tile, Wl, cmake(0.0, 0.0), cmake(0.0, 0.0), MODE);
+}
+
+// ------------------------------------------------------------------------------------------------
 // very high levels (ka^2 + kb^2 > 100), cooperative form: a warp = ONE determinant x 8 walkers x 4 helper lanes
 // (lane = helper * 8 + walker).  The four helpers of a (determinant, walker) share its matrices in shared memory
 // (element e of walker j at mw[e * 8 + j]) and split every loop -- pivot search, row updates, the V gathers -- four ways.
@@ -1403,6 +1560,15 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
             if (ntiles == 1) workers = std::min(i1 - i0, c->n_sm * occ);
             kern<<<dim3(workers, ntiles), 128, smem, f.stream(li++)>>>(p, c->d_items_gen + i0, i1 - i0, elems);
             e = cudaGetLastError();
+            if (e != cudaSuccess) { f.join(); return e; }
+            c->launches++;
+            continue;
+        }
+        // groups 0 and 1 (ka^2 + kb^2 <= 34) hold exactly the buckets with one spin at level 5 and the other at 0..3:
+        // overlap and force-bias modes take the register-resident kernel
+        if (MODE <= 1 && gi <= 1 && c->gen_group_elems[gi] <= 34) {
+            cudaError_t e = launch_persistent(c, k_dets_r5<(MODE <= 1 ? MODE : 0)>, 128, 0, c->n_sm, p, c->d_items_gen + i0, i1 - i0, ntiles,
+                                              f.stream(li++));
             if (e != cudaSuccess) { f.join(); return e; }
             c->launches++;
             continue;
