@@ -777,10 +777,71 @@ __device__ __forceinline__ cplx closed_to_smem(SmMat m, SmIdx xs, const unsigned
     return R;
 }
 
+// 5 x 5 Gauss-Jordan in registers (see k_dets_r5 below for the idea): WANT_INV leaves M^-1 in M, else only the determinant
+template <bool WANT_INV>
+__device__ __forceinline__ cplx gj5_reg(cplx (&M)[5][5])
+{
+    constexpr int K = 5;
+    cplx det = cmake(1.0, 0.0);
+    bool sing = false;
+    unsigned swaps = 0u;                       // bit (4 j + i - j - 1): rows j and i were swapped in step j
+#pragma unroll
+    for (int j = 0; j < K; j++) {
+#pragma unroll
+        for (int i = j + 1; i < K; i++) {
+            const bool sw = cabs2(M[i][j]) > cabs2(M[j][j]);
+#pragma unroll
+            for (int c = 0; c < K; c++) {
+                if (!WANT_INV && c < j) continue;
+                const cplx a = M[j][c], b = M[i][c];
+                M[j][c] = sw ? b : a;
+                M[i][c] = sw ? a : b;
+            }
+            if (sw) { det = cneg(det); swaps |= 1u << (4 * j + i - j - 1); }
+        }
+        const cplx pv = M[j][j];
+        if (!(cabs2(pv) > 0.0)) sing = true;
+        det = cmul(det, pv);
+        const cplx r = sing ? cmake(0.0, 0.0) : cinv(pv);
+        if (WANT_INV) M[j][j] = cmake(1.0, 0.0);
+#pragma unroll
+        for (int c = 0; c < K; c++) if (WANT_INV || c > j) M[j][c] = cmul(M[j][c], r);
+#pragma unroll
+        for (int i = 0; i < K; i++) {
+            if (i == j || (!WANT_INV && i < j)) continue;
+            const cplx f = M[i][j];
+            if (WANT_INV) M[i][j] = cmake(0.0, 0.0);
+#pragma unroll
+            for (int c = 0; c < K; c++) if (WANT_INV || c > j) M[i][c] = cfms(f, M[j][c], M[i][c]);
+        }
+    }
+    if (WANT_INV) {
+#pragma unroll
+        for (int j = K - 1; j >= 0; j--)
+#pragma unroll
+            for (int i = K - 1; i > j; i--) {
+                const bool sw = (swaps >> (4 * j + i - j - 1)) & 1u;
+#pragma unroll
+                for (int rr = 0; rr < K; rr++) {
+                    const cplx a = M[rr][j], b = M[rr][i];
+                    M[rr][j] = sw ? b : a;
+                    M[rr][i] = sw ? a : b;
+                }
+            }
+        if (sing) {
+#pragma unroll
+            for (int a = 0; a < K; a++)
+#pragma unroll
+                for (int b = 0; b < K; b++) M[a][b] = cmake(0.0, 0.0);
+        }
+    }
+    return sing ? cmake(0.0, 0.0) : det;
+}
+
 // levels 5..8 with compile-time K: gather, Gauss-Jordan, A = R M^-1, and the same-spin second-order sum
 //   Ess = (1/R) sum_{a<c} sum_{b<d} (A[b][a] A[d][c] - A[b][c] A[d][a]) Vbar[x_ab][x_cd]        (Jacobi)
 // with columns a and c of A in registers and the C(K,2) loads of one (a,c) pair independent of one another.
-template <int K, int MODE>
+template <int K, int MODE, bool R5 = false>
 __device__ __noinline__ cplx spin_big(cplx* mbase, xidx_t* xbase, int T, const unsigned char* hp, const cplx* __restrict__ g, int no,
                                       const cplx* __restrict__ Vss, unsigned P, cplx* Ess)
 {
@@ -800,9 +861,24 @@ __device__ __noinline__ cplx spin_big(cplx* mbase, xidx_t* xbase, int T, const u
         for (int b = 0; b < K; b++) { m.at(a * K + b) = row[b]; if (MODE != 0) xs.at(b * K + a) = pn[b] + ha; }
     }
     if (MODE == 0) { *Ess = cmake(0.0, 0.0); return det_lu_t<K>(m); }      // overlap: forward elimination only
-    const cplx R = gauss_jordan_t<K>(m);          // m = M^-1 (or zeros)
+    cplx R;
+    if constexpr (R5 && K == 5) {
+        // the kernel variant with a 255-register budget: inverse in registers, A written to shared memory once
+        cplx Mr[5][5];
 #pragma unroll
-    for (int e = 0; e < K * K; e++) m.at(e) = cmul(R, m.at(e));   // A = R M^-1, entry b*K+a = A[b][a]
+        for (int a = 0; a < 5; a++)
+#pragma unroll
+            for (int b = 0; b < 5; b++) Mr[a][b] = m.at(a * 5 + b);
+        R = gj5_reg<true>(Mr);
+#pragma unroll
+        for (int a = 0; a < 5; a++)
+#pragma unroll
+            for (int b = 0; b < 5; b++) m.at(a * 5 + b) = cmul(R, Mr[a][b]);
+    } else {
+        R = gauss_jordan_t<K>(m);                 // m = M^-1 (or zeros)
+#pragma unroll
+        for (int e = 0; e < K * K; e++) m.at(e) = cmul(R, m.at(e));   // A = R M^-1, entry b*K+a = A[b][a]
+    }
     *Ess = cmake(0.0, 0.0);
     if (M_ENERGY(MODE) && (R.x != 0.0 || R.y != 0.0)) {
         cplx e2[2] = {cmake(0.0, 0.0), cmake(0.0, 0.0)};      // two chains: the FMA latency is not on the critical path
@@ -872,7 +948,7 @@ __device__ __noinline__ cplx spin_runtime(cplx* mbase, xidx_t* xbase, int T, int
     return R;
 }
 
-template <int MODE>
+template <int MODE, bool R5 = false>
 __device__ __forceinline__ cplx spin_any(cplx* mbase, xidx_t* xbase, int T, int k, const unsigned char* hp, const cplx* __restrict__ g,
                                          int no, const cplx* __restrict__ Vss, unsigned P, cplx* Ess)
 {
@@ -884,7 +960,7 @@ __device__ __forceinline__ cplx spin_any(cplx* mbase, xidx_t* xbase, int T, int 
         case 2: return closed_to_smem<2>(m, xs, hp, g, no, Ess, Vss, P, MODE);
         case 3: return closed_to_smem<3>(m, xs, hp, g, no, Ess, Vss, P, MODE);
         case 4: return closed_to_smem<4>(m, xs, hp, g, no, Ess, Vss, P, MODE);
-        case 5: return spin_big<5, MODE>(mbase, xbase, T, hp, g, no, Vss, P, Ess);
+        case 5: return spin_big<5, MODE, R5>(mbase, xbase, T, hp, g, no, Vss, P, Ess);
         case 6: return spin_big<6, MODE>(mbase, xbase, T, hp, g, no, Vss, P, Ess);
         case 7: return spin_big<7, MODE>(mbase, xbase, T, hp, g, no, Vss, P, Ess);
         case 8: return spin_big<8, MODE>(mbase, xbase, T, hp, g, no, Vss, P, Ess);
@@ -931,8 +1007,10 @@ __device__ __noinline__ cplx opp_runtime(const cplx* mbig, const xidx_t* xbig, i
 
 // Persistent per walker tile like k_dets_cf; shared memory per thread = (ka^2+kb^2) x (complex + int), bounded by the
 // launch group's element count.
-template <int MODE>
-__global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkItem* __restrict__ items, int n_items)
+// R5: the variant for the groups whose high spin is at level 5 (ka^2 + kb^2 <= 34) in the energy modes: 255 registers, the 5 x 5
+// inverse in registers (gj5_reg), the adjugate written to shared memory once for the second-order loops
+template <int MODE, bool R5 = false>
+__global__ void __launch_bounds__(128, R5 ? 2 : 3) k_dets_gen(DetsParams p, const WorkItem* __restrict__ items, int n_items)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx* gsm = reinterpret_cast<cplx*>(smem_raw);
@@ -975,8 +1053,8 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
             for (int t = 0; t < it.rs / 4; t++) row.w[t] = __ldg(rp + t);
             const double cf = __ldg(&p.coef[it.det_begin + i]);
             cplx EssA, EssB;
-            const cplx Ra = spin_any<MODE>(mA, xA, T, ka, row.b, gA, p.no[0], VA, (unsigned)p.P[0], &EssA);
-            const cplx Rb = spin_any<MODE>(mB, xB, T, kb, row.b + 2 * ka, gB, p.no[1], VB, (unsigned)p.P[1], &EssB);
+            const cplx Ra = spin_any<MODE, R5>(mA, xA, T, ka, row.b, gA, p.no[0], VA, (unsigned)p.P[0], &EssA);
+            const cplx Rb = spin_any<MODE, R5>(mB, xB, T, kb, row.b + 2 * ka, gB, p.no[1], VB, (unsigned)p.P[1], &EssB);
             const cplx cRa = cscale(cf, Ra), cRb = cscale(cf, Rb);
             Wl = cfma(cRa, Rb, Wl);
             if (M_ENERGY(MODE)) {
@@ -1038,66 +1116,6 @@ __global__ void __launch_bounds__(128, 3) k_dets_gen(DetsParams p, const WorkIte
 // 25 complex need a 255-register budget (inside k_dets_gen ptxas puts them in local memory: DESIGN.md section 11).
 // Pivots are the column maxima, as in gauss_jordan_t; exactly singular matrices give R = 0, A = 0 (reading A11).
 // ------------------------------------------------------------------------------------------------
-template <bool WANT_INV>
-__device__ __forceinline__ cplx gj5_reg(cplx (&M)[5][5])
-{
-    constexpr int K = 5;
-    cplx det = cmake(1.0, 0.0);
-    bool sing = false;
-    unsigned swaps = 0u;                       // bit (4 j + i - j - 1): rows j and i were swapped in step j
-#pragma unroll
-    for (int j = 0; j < K; j++) {
-#pragma unroll
-        for (int i = j + 1; i < K; i++) {
-            const bool sw = cabs2(M[i][j]) > cabs2(M[j][j]);
-#pragma unroll
-            for (int c = 0; c < K; c++) {
-                if (!WANT_INV && c < j) continue;
-                const cplx a = M[j][c], b = M[i][c];
-                M[j][c] = sw ? b : a;
-                M[i][c] = sw ? a : b;
-            }
-            if (sw) { det = cneg(det); swaps |= 1u << (4 * j + i - j - 1); }
-        }
-        const cplx pv = M[j][j];
-        if (!(cabs2(pv) > 0.0)) sing = true;
-        det = cmul(det, pv);
-        const cplx r = sing ? cmake(0.0, 0.0) : cinv(pv);
-        if (WANT_INV) M[j][j] = cmake(1.0, 0.0);
-#pragma unroll
-        for (int c = 0; c < K; c++) if (WANT_INV || c > j) M[j][c] = cmul(M[j][c], r);
-#pragma unroll
-        for (int i = 0; i < K; i++) {
-            if (i == j || (!WANT_INV && i < j)) continue;
-            const cplx f = M[i][j];
-            if (WANT_INV) M[i][j] = cmake(0.0, 0.0);
-#pragma unroll
-            for (int c = 0; c < K; c++) if (WANT_INV || c > j) M[i][c] = cfms(f, M[j][c], M[i][c]);
-        }
-    }
-    if (WANT_INV) {
-#pragma unroll
-        for (int j = K - 1; j >= 0; j--)
-#pragma unroll
-            for (int i = K - 1; i > j; i--) {
-                const bool sw = (swaps >> (4 * j + i - j - 1)) & 1u;
-#pragma unroll
-                for (int rr = 0; rr < K; rr++) {
-                    const cplx a = M[rr][j], b = M[rr][i];
-                    M[rr][j] = sw ? b : a;
-                    M[rr][i] = sw ? a : b;
-                }
-            }
-        if (sing) {
-#pragma unroll
-            for (int a = 0; a < K; a++)
-#pragma unroll
-                for (int b = 0; b < K; b++) M[a][b] = cmake(0.0, 0.0);
-        }
-    }
-    return sing ? cmake(0.0, 0.0) : det;
-}
-
 // one bucket (KA, KB) with one spin at level 5 and the other at 0..3
 template <int MODE, int KA, int KB>
 __device__ __forceinline__ void r5_bucket(const DetsParams& p, const WorkItem& it, int slot, int nslots, const cplx* __restrict__ gA,
@@ -1580,8 +1598,11 @@ static cudaError_t launch_mode(msd_ctx* c, const DetsParams& p, int ntiles, cuda
         int nthr = 128;
         while (nthr > 32 && per_thread * nthr > 200 * 1024) nthr -= 32;
         size_t smem = per_thread * nthr;
-        cudaError_t e = launch_persistent(c, k_dets_gen<MODE>, nthr, smem, c->n_sm, p, c->d_items_gen + i0, i1 - i0, ntiles,
-                                          f.stream(li++), 128 / nthr);
+        const bool r5 = MODE >= 2 && gi <= 1 && c->gen_group_elems[gi] <= 34 && nthr == 128;
+        cudaError_t e = r5 ? launch_persistent(c, k_dets_gen<MODE, (MODE >= 2)>, nthr, smem, c->n_sm, p, c->d_items_gen + i0, i1 - i0, ntiles,
+                                               f.stream(li++), 1)
+                           : launch_persistent(c, k_dets_gen<MODE>, nthr, smem, c->n_sm, p, c->d_items_gen + i0, i1 - i0, ntiles,
+                                               f.stream(li++), 128 / nthr);
         if (e != cudaSuccess) { f.join(); return e; }
         c->launches++;
     }
