@@ -127,6 +127,12 @@ int msd_overlap(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
 int msd_force_bias(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b,
                    void* fb, int32_t* flags, void* stream);
 
+/* Conditioning of the walkers' reference blocks O0 = psi[occ_ref, :]: cond DEVICE [n_w][2] float64 =
+ * ||O0||_F ||O0^-1||_F per walker and spin (about 2-4 x the 2-norm condition number; inf for a singular block, 0 for a spin
+ * without electrons).  This is the quantity the accuracy of msd_local_energy depends on (see there): walkers beyond
+ * ~2000 carry energy errors above 1e-8 Ha (1e-5 Ha measured at 1e4) and are better re-orthonormalised or evaluated otherwise. */
+int msd_reference_cond(msd_ctx* ctx, int64_t n_w, const void* phi_a, const void* phi_b, double* cond, void* stream);
+
 /* msd_force_bias with the overlaps of the same walkers from the same determinant pass (the pass forms W = sum_I c_I R_I
  * and det O0 anyway; a propagation step needs both: PAPER.md Eq. 7 and Eq. 8): fb as in msd_force_bias, ovlp DEVICE [n_w]
  * as in msd_overlap.  Saves the separate msd_overlap call (0.5 ms of 2.7 ms at the Fe2S2-shaped config). */

@@ -25,7 +25,7 @@ EXPORTS = ["msd_setup", "msd_setup_sharded", "msd_set_allreduce", "msd_setup_fro
            "msd_propagator_setup", "msd_propagate",
            "msd_get_info", "msd_get_packed", "msd_set_workspace_limit", "msd_set_option", "msd_launch_count",
            "msd_set_profiling", "msd_get_phase_ms", "msd_destroy", "msd_last_error",
-           "msd_noalloc_setup", "msd_overlap_noalloc", "msd_force_bias_overlap"]
+           "msd_noalloc_setup", "msd_overlap_noalloc", "msd_force_bias_overlap", "msd_reference_cond"]
 MSD_NOALLOC_SCRATCH_BYTES = 4 * 1024 * 1024
 MSD_OPT_NO_SMEM_TILES = 1
 MSD_OPT_NO_FUSED_S7 = 2
@@ -68,6 +68,8 @@ def load_library() -> C.CDLL:
         f = getattr(lib, name)
         f.restype = i32
         f.argtypes = [vp, i64, vp, vp, vp, vp, vp]
+    lib.msd_reference_cond.restype = i32
+    lib.msd_reference_cond.argtypes = [vp, i64, vp, vp, vp, vp]
     lib.msd_force_bias_overlap.restype = i32
     lib.msd_force_bias_overlap.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp]
     lib.msd_noalloc_setup.restype = i32
@@ -196,6 +198,15 @@ class MSDTrial:
         nw = self._walkers(phi_a, phi_b)
         out = torch.empty((nw, self.n_chol), dtype=torch.complex128, device=phi_a.device) if out is None else out
         return self._call(load_library().msd_force_bias, phi_a, phi_b, out, flags, stream)
+
+    def reference_cond(self, phi_a, phi_b, stream=None):
+        """msd_reference_cond: ||O0||_F ||O0^-1||_F per walker and spin, float64 [n_w][2] on the walkers' device."""
+        import torch
+        nw = self._walkers(phi_a, phi_b)
+        out = torch.empty((nw, 2), dtype=torch.float64, device=phi_a.device)
+        self._check(load_library().msd_reference_cond(self._h, nw, phi_a.data_ptr(), phi_b.data_ptr(), out.data_ptr(),
+                                                      _stream_ptr(stream)))
+        return out
 
     def force_bias_overlap(self, phi_a, phi_b, out=None, out_ovlp=None, flags=None, stream=None):
         """msd_force_bias_overlap: (fb [n_w][n_chol], ovlp [n_w]) of the same walkers from one determinant pass."""

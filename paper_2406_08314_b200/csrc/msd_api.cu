@@ -702,7 +702,7 @@ static size_t carve(const msd_ctx* c, Workspace& ws, char* base, int64_t wc, int
         ws.g[s] = k.take<cplx>((size_t)nt * c->sp[s].P * MSD_WT);
     }
     ws.det0 = k.take<cplx>((size_t)wc * 2);
-    ws.kappa2 = (level == 3) ? k.take<double>((size_t)wc * 2) : nullptr;
+    ws.kappa2 = k.take<double>((size_t)wc * 2);
     if (level == 2 || level == 4) {
         for (int s = 0; s < 2; s++) ws.Gp[s] = k.take<double>((size_t)wc * 2 * c->sp[s].n_r * ldN);
     }
@@ -768,7 +768,14 @@ static int ensure_workspace(msd_ctx* c, int level, int64_t nw, std::string* errp
 // ---------------------------------------------------------------------------------------------
 // hot calls
 // ---------------------------------------------------------------------------------------------
-enum { CALL_OVERLAP = 1, CALL_FB = 2, CALL_GREENS = 4, CALL_ENERGY = 8, CALL_FB_ENERGY = 16, CALL_PROPAGATE = 32 };
+enum { CALL_OVERLAP = 1, CALL_FB = 2, CALL_GREENS = 4, CALL_ENERGY = 8, CALL_FB_ENERGY = 16, CALL_PROPAGATE = 32, CALL_COND = 64 };
+
+// msd_reference_cond: sqrt of the (||O0||_F ||O0^-1||_F)^2 that k_reference leaves per walker and spin
+__global__ void k_cond_out(int64_t n2, const double* __restrict__ kappa2, double* __restrict__ out)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n2) out[i] = sqrt(kappa2[i]);
+}
 
 static void mark(msd_ctx* c, int i, cudaStream_t st) { if (c->profiling) cudaEventRecord(c->ev[i], st); }
 
@@ -810,7 +817,7 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
                       cplx* out, int* flags, cudaStream_t st)
 {
     const bool energy_like = (call == CALL_ENERGY || call == CALL_FB_ENERGY);
-    const int level = (call == CALL_OVERLAP) ? 1 : (energy_like ? 3 : (call == CALL_PROPAGATE ? 4 : 2));
+    const int level = (call == CALL_OVERLAP || call == CALL_COND) ? 1 : (energy_like ? 3 : (call == CALL_PROPAGATE ? 4 : 2));
     if (energy_like && !c->energy_ok) return fail(errp, MSD_EUNSUPPORTED, c->energy_why.c_str());
     int rc = ensure_workspace(c, level, n_w, errp);
     if (rc != MSD_OK) return rc;
@@ -830,7 +837,11 @@ static int run_chunks(msd_ctx* c, std::string* errp, int call, int64_t n_w, cons
         CK(launch_reference(c, N, ldN, c->dev(0), c->dev(1), nw, pa, pb, ws, level == 3, st));
         c->launches++;
         mark(c, 1, st);
-        if (call == CALL_OVERLAP) {
+        if (call == CALL_COND) {
+            k_cond_out<<<(unsigned)((2 * nw + 127) / 128), 128, 0, st>>>(2 * nw, ws.kappa2, reinterpret_cast<double*>(out) + 2 * w0);
+            CK(cudaGetLastError());
+            c->launches++;
+        } else if (call == CALL_OVERLAP) {
             CK(launch_dets(c, 0, nw, ws, st));
             shard_reduce(c, ws, st);
             mark(c, 2, st);
@@ -1014,6 +1025,9 @@ extern "C" int msd_overlap(msd_ctx* c, int64_t n_w, const void* phi_a, const voi
 extern "C" int msd_force_bias(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* fb, int32_t* flags,
                               void* stream)
 { return hot_call(c, CALL_FB, n_w, phi_a, phi_b, fb, flags, stream); }
+
+extern "C" int msd_reference_cond(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, double* cond, void* stream)
+{ return hot_call(c, CALL_COND, n_w, phi_a, phi_b, cond, nullptr, stream); }
 
 extern "C" int msd_force_bias_overlap(msd_ctx* c, int64_t n_w, const void* phi_a, const void* phi_b, void* fb, void* ovlp,
                                       int32_t* flags, void* stream)

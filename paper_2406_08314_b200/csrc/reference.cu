@@ -183,6 +183,6 @@ cudaError_t launch_reference(msd_ctx* c, int N, int ldN, SpinDev sa, SpinDev sb,
     dim3 grid((unsigned)wpad, 2);
     k_reference<<<grid, 256, smem, st>>>(N, ldN, sa, sb, nw, phi_a, phi_b, ws.theta[0], ws.theta[1],
                                          want_thetaT ? ws.thetaT[0] : nullptr, want_thetaT ? ws.thetaT[1] : nullptr,
-                                         ws.det0, ws.g[0], ws.g[1], ws.wflags, stage_psi, want_thetaT ? ws.kappa2 : nullptr);
+                                         ws.det0, ws.g[0], ws.g[1], ws.wflags, stage_psi, ws.kappa2);
     return cudaGetLastError();
 }

@@ -192,6 +192,36 @@ def test_parity_sweep_end_points_against_stored_oracle_values(torch_cuda, n_det,
     _assert_against_golden(gold, ov, fb, E)
 
 
+@pytest.mark.parametrize("name,kw", [("small", {}), ("open-shell", {}), ("cu2o2", dict(n_w=40))])
+def test_reference_block_conditioning(torch_cuda, name, kw):
+    """msd_reference_cond: ||O0||_F ||O0^-1||_F of every walker and spin against numpy (the quantity the energy accuracy
+    depends on and the V contraction is routed by: DESIGN.md section 7); a singular block reads inf; chunked workspace."""
+    torch = torch_cuda
+    msd = _msd()
+    x = mi.generate(name, **kw)
+    pa_h = x.phi_a.copy()
+    pa_h[1][x.occ_ref_a, :] = 0.0                       # walker 1: singular alpha block
+    x = x.with_walkers(pa_h, x.phi_b)
+    trial = msd.setup_from_inputs(x)
+    pa = torch.tensor(x.phi_a, device="cuda")
+    pb = torch.tensor(x.phi_b, device="cuda")
+    want = np.zeros((x.n_w, 2))
+    for w in range(x.n_w):
+        for s_, (phi, occ) in enumerate(((x.phi_a, x.occ_ref_a), (x.phi_b, x.occ_ref_b))):
+            O = phi[w][occ, :]
+            if w == 1 and s_ == 0:
+                want[w, s_] = np.inf
+            elif O.shape[0]:
+                want[w, s_] = np.linalg.norm(O) * np.linalg.norm(np.linalg.inv(O))
+    for limit in (0, 600 * 1024) if name == "small" else (0,):
+        trial.set_workspace_limit(limit)
+        got = trial.reference_cond(pa, pb).cpu().numpy()
+        assert np.isinf(got[1, 0])
+        fin = np.isfinite(want)
+        assert (np.abs(got[fin] - want[fin]) <= 1e-9 * want[fin]).all()
+    trial.close()
+
+
 @pytest.mark.parametrize("seed", [1, 2, 3, 4])
 @pytest.mark.parametrize("name,kw", [("small", {}), ("sweep", dict(n_det=1500, max_level=7, n_w=19)),
                                      ("sweep", dict(n_det=800, max_level=10, n_w=9))])
